@@ -1,0 +1,182 @@
+"""oracle -- TEST INFRASTRUCTURE, NOT PRODUCT.
+
+ctypes front end of `wilson_clover_oracle.c` (plain fp64 C; see that file's header for the
+citations and the list of pins).  Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / `--impl reference` legs may import this package; the product path
+(paper_2510_26313_b200) never does.
+
+All arrays are numpy complex128 in the canonical layouts:
+    gauge  U[mu][t][z][y][x][3][3]     spinor psi[t][z][y][x][4][3]     clover A[t][z][y][x][12][12]
+`dims` is always (Lx, Ly, Lz, Lt).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "wilson_clover_oracle.c")
+_SO = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (-O2, OpenMP, no fast-math: IEEE semantics, reading #19)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-fno-fast-math", "-o", _SO, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _SO
+
+
+def _c(a):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_SO)
+        _lib.orc_norm2.restype = ctypes.c_double
+        _lib.orc_norm2.argtypes = [ctypes.c_long, ctypes.c_void_p]
+        _lib.orc_clover_inverse.argtypes = [ctypes.c_long, ctypes.c_void_p, ctypes.c_void_p]
+        _lib.orc_apply_site_matrix.argtypes = [ctypes.c_long, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+    return _lib
+
+
+def _dims(dims):
+    return (ctypes.c_int * 4)(*[int(d) for d in dims])
+
+
+def _vol(dims):
+    return int(dims[0]) * int(dims[1]) * int(dims[2]) * int(dims[3])
+
+
+def _cc(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.complex128)
+    if shape is not None:
+        assert a.size == int(np.prod(shape)), (a.shape, shape)
+    return a
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def gamma(mu: int) -> np.ndarray:
+    """gamma_mu for mu in 0..3, gamma5 for mu == 5 (4x4 complex)."""
+    out = np.zeros((4, 4), dtype=np.complex128)
+    lib().orc_gamma(ctypes.c_int(mu), _c(out))
+    return out
+
+
+def sigma(mu: int, nu: int) -> np.ndarray:
+    out = np.zeros((4, 4), dtype=np.complex128)
+    lib().orc_sigma(ctypes.c_int(mu), ctypes.c_int(nu), _c(out))
+    return out
+
+
+def hop(dims, U, psi, t_bc: int = -1) -> np.ndarray:
+    """D psi on the full lattice."""
+    V = _vol(dims)
+    U = _cc(U, (4, V, 3, 3)); psi = _cc(psi, (V, 12))
+    out = np.empty_like(psi)
+    lib().orc_hop(_dims(dims), ctypes.c_int(t_bc), _c(U), _c(psi), _c(out))
+    return out
+
+
+def field_strength(dims, U) -> np.ndarray:
+    """F[plane][t][z][y][x][3][3], planes (xy, xz, xt, yz, yt, zt) (step 5)."""
+    V = _vol(dims)
+    U = _cc(U, (4, V, 3, 3))
+    Lx, Ly, Lz, Lt = dims
+    F = np.empty((6, Lt, Lz, Ly, Lx, 3, 3), dtype=np.complex128)
+    lib().orc_field_strength(_dims(dims), _c(U), _c(F))
+    return F
+
+
+def clover(dims, U, kappa: float, csw: float) -> np.ndarray:
+    """A[t][z][y][x][12][12] (step 6)."""
+    V = _vol(dims)
+    U = _cc(U, (4, V, 3, 3))
+    Lx, Ly, Lz, Lt = dims
+    A = np.empty((Lt, Lz, Ly, Lx, 12, 12), dtype=np.complex128)
+    lib().orc_clover(_dims(dims), _c(U), ctypes.c_double(kappa), ctypes.c_double(csw), _c(A))
+    return A
+
+
+def clover_inverse(A) -> np.ndarray:
+    A = _cc(A)
+    Ainv = np.empty_like(A)
+    rc = lib().orc_clover_inverse(ctypes.c_long(A.size // 144), _c(A), _c(Ainv))
+    if rc != 0:
+        raise ArithmeticError("singular clover block")
+    return Ainv
+
+
+def apply_site_matrix(C, psi) -> np.ndarray:
+    C = _cc(C); psi = _cc(psi)
+    out = np.empty_like(psi)
+    lib().orc_apply_site_matrix(ctypes.c_long(psi.size // 12), _c(C), _c(psi), _c(out))
+    return out
+
+
+def M(dims, U, A, kappa: float, psi, dagger: bool = False, t_bc: int = -1) -> np.ndarray:
+    """M psi = A psi - kappa D psi (step 7); dagger -> gamma5 M gamma5."""
+    V = _vol(dims)
+    U = _cc(U, (4, V, 3, 3)); A = _cc(A, (V, 144)); psi = _cc(psi, (V, 12))
+    out = np.empty_like(psi)
+    lib().orc_M(_dims(dims), ctypes.c_int(t_bc), _c(U), _c(A), ctypes.c_double(kappa), ctypes.c_int(int(dagger)),
+                _c(psi), _c(out))
+    return out
+
+
+def Mhat(dims, U, A, Ainv, kappa: float, psi, dagger: bool = False, t_bc: int = -1) -> np.ndarray:
+    """Even-odd Schur operator on even sites (step 8); odd sites of the result are zero."""
+    V = _vol(dims)
+    U = _cc(U, (4, V, 3, 3)); A = _cc(A, (V, 144)); Ainv = _cc(Ainv, (V, 144)); psi = _cc(psi, (V, 12))
+    out = np.empty_like(psi)
+    lib().orc_Mhat(_dims(dims), ctypes.c_int(t_bc), _c(U), _c(A), _c(Ainv), ctypes.c_double(kappa),
+                   ctypes.c_int(int(dagger)), _c(psi), _c(out))
+    return out
+
+
+def schur_source(dims, U, Ainv, kappa: float, b, t_bc: int = -1) -> np.ndarray:
+    V = _vol(dims)
+    U = _cc(U, (4, V, 3, 3)); Ainv = _cc(Ainv, (V, 144)); b = _cc(b, (V, 12))
+    out = np.empty_like(b)
+    lib().orc_schur_source(_dims(dims), ctypes.c_int(t_bc), _c(U), _c(Ainv), ctypes.c_double(kappa), _c(b), _c(out))
+    return out
+
+
+def schur_reconstruct(dims, U, Ainv, kappa: float, b, x_e, t_bc: int = -1) -> np.ndarray:
+    V = _vol(dims)
+    U = _cc(U, (4, V, 3, 3)); Ainv = _cc(Ainv, (V, 144)); b = _cc(b, (V, 12))
+    x = np.array(x_e, dtype=np.complex128, order="C", copy=True)
+    lib().orc_schur_reconstruct(_dims(dims), ctypes.c_int(t_bc), _c(U), _c(Ainv), ctypes.c_double(kappa), _c(b), _c(x))
+    return x
+
+
+def solve_eo(dims, U, A, Ainv, kappa: float, b, tol: float, maxit: int = 10000, t_bc: int = -1):
+    """Even-odd CGNR (step 9).  Returns (x_full, iterations, true relative residual)."""
+    V = _vol(dims)
+    U = _cc(U, (4, V, 3, 3)); A = _cc(A, (V, 144)); Ainv = _cc(Ainv, (V, 144)); b = _cc(b, (V, 12))
+    x = np.zeros_like(b)
+    rel = ctypes.c_double(0.0)
+    it = lib().orc_solve_eo(_dims(dims), ctypes.c_int(t_bc), _c(U), _c(A), _c(Ainv), ctypes.c_double(kappa), _c(b), _c(x),
+                            ctypes.c_double(tol), ctypes.c_int(maxit), ctypes.byref(rel))
+    return x, int(it), float(rel.value)
+
+
+def solve_full(dims, U, A, kappa: float, b, tol: float, maxit: int = 10000, t_bc: int = -1):
+    """CG on the unpreconditioned normal equations (cross-check of step 9)."""
+    V = _vol(dims)
+    U = _cc(U, (4, V, 3, 3)); A = _cc(A, (V, 144)); b = _cc(b, (V, 12))
+    x = np.zeros_like(b)
+    rel = ctypes.c_double(0.0)
+    it = lib().orc_solve_full(_dims(dims), ctypes.c_int(t_bc), _c(U), _c(A), ctypes.c_double(kappa), _c(b), _c(x),
+                              ctypes.c_double(tol), ctypes.c_int(maxit), ctypes.byref(rel))
+    return x, int(it), float(rel.value)

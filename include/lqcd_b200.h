@@ -1,0 +1,176 @@
+/*
+ * lqcd_b200.h -- C ABI of the B200-native multi-RHS Wilson-clover Dslash and batched
+ * mixed-precision CG (hot path of the LapH workflow of arxiv 2510.26313).
+ *
+ * The calls follow the paper's statement of the problem as condensed in BASELINE.json
+ * north_star ("load gauge field, build clover term, apply M to N_rhs spinors, solve M x = b
+ * for N_rhs sources") and the driver/library split of PAPER.md L110 (Sec. V-B: the driver
+ * owns I/O and task order; the library owns device data and host<->device copies; persistent
+ * state lives in one long-lived object -- here the opaque lq_ctx).  The operator itself is the
+ * textbook Sheikholeslami-Wohlert operator fixed by BASELINE.json and spelled out in
+ * SURVEY.md 8(c.1); "batched" means N independent right-hand sides sharing each link and
+ * clover load (Sec. V-C3); "mixed precision" is PAPER.md L116/L164.
+ *
+ * Conventions (binding):
+ *   dims = (Lx, Ly, Lz, Lt), all even.  mu = 0,1,2,3 = x,y,z,t.  Lexicographic site index
+ *   i = x + Lx*(y + Ly*(z + Lz*t)); parity = (x+y+z+t) mod 2 (0 = even).
+ *   Periodic in x,y,z; in t the hopped term is multiplied by t_bc (-1 antiperiodic, +1 periodic)
+ *   when the hop wraps around the lattice.  DeGrand-Rossi gamma basis, gamma5 = diag(1,1,-1,-1).
+ *   D psi(x) = sum_mu (1-g_mu) U_mu(x) psi(x+mu) + (1+g_mu) U_mu(x-mu)^dag psi(x-mu)
+ *   A(x)     = 1 - kappa*csw * sum_{mu<nu} sigma_{mu nu} (x) F_{mu nu}(x),  F from the 4-leaf clover
+ *   M = A - kappa D,  M^dag = g5 M g5,  Mhat = A_ee - kappa^2 D_eo A_oo^{-1} D_oe (even sites).
+ *
+ * CANONICAL layouts (row-major, complex = (re, im) pairs of the stated precision):
+ *   gauge   U[mu][t][z][y][x][row][col]
+ *   spinor  psi[rhs][t][z][y][x][spin][colour]
+ * NATIVE spinor layout (what the kernels stream; for timing without reorders):
+ *   one parity:  payload[j = 0..23][cb = 0..Vh-1][rhs = 0..N-1]  with j = 2*(3*spin+colour) + (0 re | 1 im),
+ *                cb = (site index within the parity) = i_lex / 2 restricted to that parity,
+ *                element = double (LQ_FP64), float (LQ_FP32) or int16 (LQ_HALF);
+ *   LQ_HALF appends, after the payload rounded up to 256 bytes, fp32 norms[cb][rhs]:
+ *                value = q * norm / 32767, norm = max-abs over the 24 reals of that (site, rhs).
+ *   full lattice: the even-parity block followed by the odd-parity block (each lq_native_bytes(.., 1)).
+ *   The RHS index is innermost so that one SU(3) link / clover block load serves the whole batch.
+ *
+ * Ownership: the caller owns every buffer it passes; the library copies what it keeps (links)
+ * and owns its native copies and scratch.  Device scratch comes from cudaMalloc unless an
+ * allocator is installed with lq_set_allocator (the Python binding installs a PyTorch-backed one).
+ * Pointers are HOST or DEVICE as said by the `loc` argument next to them.
+ *
+ * Errors: every call returns 0 on success or a negative lq_status; no exceptions, no abort, no
+ * printing.  lq_last_error(ctx) gives a message for the last failure on that context.  All work is
+ * enqueued on the context's stream; calls that return values to the host synchronise that stream.
+ * There is NO CPU fallback: every operation runs in this library's CUDA kernels.
+ */
+#ifndef LQCD_B200_H
+#define LQCD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LQ_MAX_RHS 16
+
+typedef struct lq_ctx lq_ctx;
+
+typedef enum { LQ_FP64 = 0, LQ_FP32 = 1, LQ_HALF = 2 } lq_prec;
+typedef enum { LQ_HOST = 0, LQ_DEVICE = 1 } lq_loc;
+typedef enum { LQ_CANONICAL = 0, LQ_NATIVE = 1 } lq_layout;
+
+typedef enum {
+    LQ_OK = 0,
+    LQ_EINVAL = -1,        /* bad dims / odd extent / unsupported nrhs, precision or op */
+    LQ_ESTATE = -2,        /* gauge or clover not loaded yet */
+    LQ_ENOMEM = -3,
+    LQ_ECUDA = -4,
+    LQ_ENOTCONVERGED = -5, /* lq_solve: some RHS missed tol within the caps; x and info still filled */
+    LQ_ESINGULAR = -6      /* lq_build_clover: a 6x6 block is singular / not positive definite */
+} lq_status;
+
+/* Operators of lq_apply.  "full" ops act on full-lattice fields; "parity" ops act on one parity
+ * (in NATIVE layout the buffers are single-parity blocks; in CANONICAL layout they are full-lattice
+ * arrays of which only the stated parity is read / written, the other parity of `out` is zeroed). */
+typedef enum {
+    LQ_OP_HOP = 0,        /* full:   out = D in                                           (step 4) */
+    LQ_OP_M = 1,          /* full:   out = A in - kappa D in                              (step 7) */
+    LQ_OP_MDAG = 2,       /* full:   out = g5 M g5 in                                              */
+    LQ_OP_CLOVER = 3,     /* full:   out = A in                                           (step 6) */
+    LQ_OP_CLOVER_INV = 4, /* full:   out = A^{-1} in                                               */
+    LQ_OP_HOP_EO = 5,     /* parity: out_e = D_eo in_o                                             */
+    LQ_OP_HOP_OE = 6,     /* parity: out_o = D_oe in_e                                             */
+    LQ_OP_MHAT = 7,       /* parity: out_e = A_ee in_e - kappa^2 D_eo A_oo^{-1} D_oe in_e (step 8) */
+    LQ_OP_MHAT_DAG = 8,   /* parity: out_e = g5 Mhat g5 in_e                                       */
+    LQ_OP_KERNEL_A = 9,   /* parity: out_o = A_oo^{-1} D_oe in_e   */
+    LQ_OP_KERNEL_B = 10   /* parity: out_e = A_ee in_e - kappa^2 D_eo in2_o   */
+} lq_op;
+
+/* ---- context --------------------------------------------------------------------------------- */
+/* Creates a context for a lattice dims = (Lx,Ly,Lz,Lt) (all even, Lx >= 2) on CUDA device `device`.
+ * `cuda_stream` is a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or NULL for the
+ * default stream; the library never creates streams of its own. */
+int lq_create(lq_ctx** out, const int dims[4], int device, void* cuda_stream);
+int lq_destroy(lq_ctx* ctx);
+const char* lq_last_error(const lq_ctx* ctx);
+
+/* Optional device allocator (must be installed before the first lq_load_gauge).  alloc returns a
+ * device pointer aligned to >= 256 bytes or NULL; release gets the same pointer back. */
+typedef void* (*lq_alloc_fn)(size_t bytes, void* user);
+typedef void (*lq_free_fn)(void* ptr, void* user);
+int lq_set_allocator(lq_ctx* ctx, lq_alloc_fn alloc, lq_free_fn release, void* user);
+
+/* ---- gauge field and clover term ------------------------------------ */
+/* links: CANONICAL gauge field, complex of precision in_prec (LQ_FP64 or LQ_FP32), at `loc`.
+ * The library copies it into its native even/odd layout in fp64 (always 18 reals per link) and in
+ * fp32 with `recon` = 18 (full) or 12 (third row rebuilt in-kernel as conj(row0 x row1)) reals.
+ * The boundary sign t_bc (+1 / -1) is never folded into the stored links.  Invalidates the clover. */
+int lq_load_gauge(lq_ctx* ctx, const void* links, int in_prec, int loc, int recon, int t_bc);
+/* Bench only: fills the gauge field on the device, U = SU(3) projection (Gram-Schmidt on rows,
+ * third row conj(a x b)) of 1 + eps*G, G_ij ~ CN(0,1) from the counter-based generator documented
+ * in paper_2510_26313_b200/inputs.py (same stream / index convention). */
+int lq_fill_gauge_random(lq_ctx* ctx, uint64_t seed, double eps, int recon, int t_bc);
+/* Computes A and A^{-1} (two 6x6 Hermitian blocks per site, both parities) on the device in fp64
+ * from the 4-leaf field strength, keeps fp64 and fp32 copies.  LQ_ESINGULAR if a block is not
+ * positive definite. */
+int lq_build_clover(lq_ctx* ctx, double kappa, double csw);
+
+/* ---- operator application (rows a3, a4, a5) ----------------------------------------------------- */
+/* out = op(in [, in2]) for nrhs right-hand sides in precision `prec`.
+ * nrhs in {1,2,4,8,12,16}.  CANONICAL: complex double (LQ_FP64) or complex float (LQ_FP32) arrays
+ * psi[rhs][t][z][y][x][4][3] at `loc`, reordered internally (LQ_HALF: canonical arrays are complex
+ * float and are quantised to int16+norm on the way in -- the operator then sees what the half-storage
+ * solver sees).  NATIVE: device buffers in the native layout (loc must be LQ_DEVICE).
+ * in2 is used by LQ_OP_KERNEL_B only (the odd-parity field to hop), else NULL.  out must not alias
+ * in / in2. */
+int lq_apply(lq_ctx* ctx, int op, void* out, const void* in, const void* in2, int nrhs, int prec, int loc, int layout);
+
+/* ---- native layout helpers ------------------------------------------------------------------------ */
+size_t lq_native_bytes(const lq_ctx* ctx, int nrhs, int prec, int parity_only);
+/* canonical (complex double, at loc) -> native (device, precision prec, full lattice) and back */
+int lq_pack(lq_ctx* ctx, void* native_out, const void* canonical_in, int nrhs, int prec, int loc);
+int lq_unpack(lq_ctx* ctx, void* canonical_out, const void* native_in, int nrhs, int prec, int loc);
+/* Bench only: complex-Gaussian spinors written straight into a native device buffer (full lattice if
+ * parity_only == 0, else that many sites of parity `parity`), same counter-based generator. */
+int lq_fill_spinor_random(lq_ctx* ctx, void* native_out, int nrhs, int prec, uint64_t seed, int parity_only, int parity);
+
+/* ---- batched mixed-precision solve (rows a2, a6-a11) ---------------------------------------------- */
+typedef struct {
+    double tol;          /* target ||b - M x|| / ||b|| per RHS (full system, fp64)                   */
+    int max_outer;       /* cap on fp64 defect-correction cycles                                      */
+    int max_inner;       /* cap on inner CG iterations per cycle                                      */
+    int inner_prec;      /* LQ_FP64, LQ_FP32 or LQ_HALF: storage of the inner CG vectors              */
+    double delta;        /* inner CG stops when ||z_k|| <= delta*||z_k(0)|| for every RHS k           */
+    int check_every;     /* inner iterations between convergence polls (host sync of N scalars)       */
+    int use_graph;       /* 1: replay the inner iteration body as a CUDA graph                        */
+} lq_solve_param;
+
+typedef struct {
+    int nrhs;
+    int outer_cycles;                  /* defect-correction cycles executed                          */
+    int inner_iters;                   /* inner CG iterations summed over cycles (shared by the batch) */
+    int iters[LQ_MAX_RHS];             /* inner iteration count at which RHS k first met tol (estimate; parity unpinned) */
+    double true_rel_residual[LQ_MAX_RHS]; /* ||bhat_e - Mhat x_e|| / ||b|| in fp64 = full-system residual   */
+    double seconds;                    /* device time of the solve proper (CUDA events), excl. pack/unpack */
+    double dslash_applies;             /* single-parity stencil kernel launches (A or B), all precisions */
+} lq_solve_info;
+
+/* Solves M x = b for nrhs independent right-hand sides (no block-Krylov coupling).  b, x: full-lattice
+ * complex double, CANONICAL at `loc`, or NATIVE LQ_FP64 device buffers.  x is output only (zero start).
+ * Even-odd preconditioned CGNR in inner_prec inside an fp64 restart defect correction
+ * (SURVEY 8(c.1) step 11).  Returns LQ_ENOTCONVERGED (x, info still valid) if any RHS misses tol. */
+int lq_solve(lq_ctx* ctx, void* x, const void* b, int nrhs, int loc, int layout, const lq_solve_param* param, lq_solve_info* info);
+
+/* Launch-parameter knobs of the stencil kernels (the paper's autotuning, reduced to an
+ * offline sweep): threads per block (0 = default) and right-hand sides per thread (0 = auto: 4 if
+ * nrhs % 4 == 0, else 2, else 1; fp64 caps at 2). */
+int lq_set_tuning(lq_ctx* ctx, int dslash_block, int dslash_rpt);
+
+/* Number of kernels this library has launched on this context since creation (for bench.py). */
+long long lq_kernel_launches(const lq_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LQCD_B200_H */

@@ -1,0 +1,234 @@
+"""Thin ctypes binding of include/lqcd_b200.h -- argument marshalling only; every step runs in the CUDA library.
+
+PyTorch is used for device memory (the library's scratch comes from a torch-backed allocator callback) and for
+the stream (torch.cuda.current_stream()).  There is no CPU fallback: if the shared library is missing, importing
+the entry points raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SO_PATH = os.path.join(HERE, "liblqcd_b200.so")
+
+LQ_FP64, LQ_FP32, LQ_HALF = 0, 1, 2
+LQ_HOST, LQ_DEVICE = 0, 1
+LQ_CANONICAL, LQ_NATIVE = 0, 1
+LQ_MAX_RHS = 16
+(LQ_OP_HOP, LQ_OP_M, LQ_OP_MDAG, LQ_OP_CLOVER, LQ_OP_CLOVER_INV, LQ_OP_HOP_EO, LQ_OP_HOP_OE, LQ_OP_MHAT, LQ_OP_MHAT_DAG,
+ LQ_OP_KERNEL_A, LQ_OP_KERNEL_B) = range(11)
+LQ_OK, LQ_EINVAL, LQ_ESTATE, LQ_ENOMEM, LQ_ECUDA, LQ_ENOTCONVERGED, LQ_ESINGULAR = 0, -1, -2, -3, -4, -5, -6
+PREC = {"fp64": LQ_FP64, "fp32": LQ_FP32, "half": LQ_HALF}
+
+EXPORTS = ["lq_create", "lq_destroy", "lq_last_error", "lq_set_allocator", "lq_load_gauge", "lq_fill_gauge_random",
+           "lq_build_clover", "lq_apply", "lq_native_bytes", "lq_pack", "lq_unpack", "lq_fill_spinor_random", "lq_solve",
+           "lq_set_tuning", "lq_kernel_launches"]
+
+
+class SolveParam(ctypes.Structure):
+    _fields_ = [("tol", ctypes.c_double), ("max_outer", ctypes.c_int), ("max_inner", ctypes.c_int), ("inner_prec", ctypes.c_int),
+                ("delta", ctypes.c_double), ("check_every", ctypes.c_int), ("use_graph", ctypes.c_int)]
+
+
+class SolveInfo(ctypes.Structure):
+    _fields_ = [("nrhs", ctypes.c_int), ("outer_cycles", ctypes.c_int), ("inner_iters", ctypes.c_int),
+                ("iters", ctypes.c_int * LQ_MAX_RHS), ("true_rel_residual", ctypes.c_double * LQ_MAX_RHS),
+                ("seconds", ctypes.c_double), ("dslash_applies", ctypes.c_double)]
+
+
+ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
+FREE_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p)
+
+_lib = None
+
+
+class LqError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("lqcd_b200 error %d: %s" % (code, msg))
+        self.code = code
+
+
+def load_library():
+    """Loads liblqcd_b200.so (fails loudly if it has not been built: there is no fallback path)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(SO_PATH):
+        raise ImportError("%s not found: run `python -m paper_2510_26313_b200.build` (no CPU fallback exists)" % SO_PATH)
+    lib = ctypes.CDLL(SO_PATH)
+    vp, ci, cd, u64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_uint64
+    lib.lq_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(ci), ci, vp]
+    lib.lq_destroy.argtypes = [vp]
+    lib.lq_last_error.argtypes = [vp]; lib.lq_last_error.restype = ctypes.c_char_p
+    lib.lq_set_allocator.argtypes = [vp, ALLOC_FN, FREE_FN, vp]
+    lib.lq_load_gauge.argtypes = [vp, vp, ci, ci, ci, ci]
+    lib.lq_fill_gauge_random.argtypes = [vp, u64, cd, ci, ci]
+    lib.lq_build_clover.argtypes = [vp, cd, cd]
+    lib.lq_apply.argtypes = [vp, ci, vp, vp, vp, ci, ci, ci, ci]
+    lib.lq_native_bytes.argtypes = [vp, ci, ci, ci]; lib.lq_native_bytes.restype = ctypes.c_size_t
+    lib.lq_pack.argtypes = [vp, vp, vp, ci, ci, ci]
+    lib.lq_unpack.argtypes = [vp, vp, vp, ci, ci, ci]
+    lib.lq_fill_spinor_random.argtypes = [vp, vp, ci, ci, u64, ci, ci]
+    lib.lq_solve.argtypes = [vp, vp, vp, ci, ci, ci, ctypes.POINTER(SolveParam), ctypes.POINTER(SolveInfo)]
+    lib.lq_set_tuning.argtypes = [vp, ci, ci]
+    lib.lq_kernel_launches.argtypes = [vp]; lib.lq_kernel_launches.restype = ctypes.c_longlong
+    _lib = lib
+    return lib
+
+
+def _ptr(a):
+    """Raw pointer + location of a numpy array (host) or torch tensor (host or device)."""
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"]
+        return ctypes.c_void_p(a.ctypes.data), LQ_HOST
+    assert a.is_contiguous()
+    return ctypes.c_void_p(a.data_ptr()), (LQ_DEVICE if a.is_cuda else LQ_HOST)
+
+
+class Context:
+    """One lattice on one GPU: the paper's 'singleton for persistent data' as an explicit handle."""
+
+    def __init__(self, dims, device: int = 0, torch_allocator: bool = True):
+        import torch
+        self.torch = torch
+        self.lib = load_library()
+        self.dims = tuple(int(d) for d in dims)
+        self.V = int(np.prod(self.dims))
+        self.device = device
+        torch.cuda.set_device(device)
+        self.stream = torch.cuda.current_stream(device)
+        h = ctypes.c_void_p()
+        rc = self.lib.lq_create(ctypes.byref(h), (ctypes.c_int * 4)(*self.dims), device, ctypes.c_void_p(self.stream.cuda_stream))
+        if rc != 0:
+            raise LqError(rc, "lq_create failed")
+        self.h = h
+        self._blocks = {}
+        if torch_allocator:
+            def _alloc(nbytes, _user):
+                try:
+                    t = torch.empty(int(nbytes), dtype=torch.uint8, device="cuda:%d" % device)
+                except Exception:
+                    return None
+                self._blocks[t.data_ptr()] = t
+                return t.data_ptr()
+
+            def _free(ptr, _user):
+                self._blocks.pop(ptr, None)
+
+            self._alloc_cb, self._free_cb = ALLOC_FN(_alloc), FREE_FN(_free)
+            self._check(self.lib.lq_set_allocator(self.h, self._alloc_cb, self._free_cb, None))
+
+    # ------------------------------------------------------------------ plumbing
+    def _check(self, rc, allow=()):
+        if rc != 0 and rc not in allow:
+            raise LqError(rc, self.lib.lq_last_error(self.h).decode())
+        return rc
+
+    def close(self):
+        if getattr(self, "h", None) is not None and self.h:
+            self.lib.lq_destroy(self.h)
+            self.h = None
+            self._blocks.clear()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def launches(self) -> int:
+        return int(self.lib.lq_kernel_launches(self.h))
+
+    def set_tuning(self, dslash_block=0, dslash_rpt=0):
+        self._check(self.lib.lq_set_tuning(self.h, dslash_block, dslash_rpt))
+
+    # ------------------------------------------------------------------ gauge / clover
+    def load_gauge(self, U, recon: int = 18, t_bc: int = -1):
+        """U: canonical [mu][t][z][y][x][3][3] complex128/complex64, numpy (host) or torch (host/device)."""
+        if isinstance(U, np.ndarray):
+            prec = LQ_FP64 if U.dtype == np.complex128 else LQ_FP32
+            U = np.ascontiguousarray(U)
+        else:
+            prec = LQ_FP64 if U.dtype == self.torch.complex128 else LQ_FP32
+        assert (U.size if isinstance(U, np.ndarray) else U.numel()) == 4 * self.V * 9
+        p, loc = _ptr(U)
+        self._check(self.lib.lq_load_gauge(self.h, p, prec, loc, recon, t_bc))
+
+    def fill_gauge_random(self, seed: int, eps: float, recon: int = 18, t_bc: int = -1):
+        self._check(self.lib.lq_fill_gauge_random(self.h, seed, eps, recon, t_bc))
+
+    def build_clover(self, kappa: float, csw: float):
+        self._check(self.lib.lq_build_clover(self.h, kappa, csw))
+
+    # ------------------------------------------------------------------ native buffers
+    def native_bytes(self, nrhs: int, prec: int, parity_only: bool = False) -> int:
+        return int(self.lib.lq_native_bytes(self.h, nrhs, prec, int(parity_only)))
+
+    def native_empty(self, nrhs: int, prec: int, parity_only: bool = False):
+        return self.torch.empty(self.native_bytes(nrhs, prec, parity_only), dtype=self.torch.uint8, device="cuda:%d" % self.device)
+
+    def pack(self, canonical, nrhs: int, prec: int):
+        out = self.native_empty(nrhs, prec)
+        p, loc = _ptr(canonical)
+        self._check(self.lib.lq_pack(self.h, ctypes.c_void_p(out.data_ptr()), p, nrhs, prec, loc))
+        return out
+
+    def unpack(self, native, nrhs: int, prec: int) -> np.ndarray:
+        Lx, Ly, Lz, Lt = self.dims
+        out = np.empty((nrhs, Lt, Lz, Ly, Lx, 4, 3), dtype=np.complex128)
+        self._check(self.lib.lq_unpack(self.h, ctypes.c_void_p(out.ctypes.data), ctypes.c_void_p(native.data_ptr()), nrhs, prec, LQ_HOST))
+        return out
+
+    def fill_spinor_random(self, native, nrhs: int, prec: int, seed: int, parity_only: bool = False, parity: int = 0):
+        self._check(self.lib.lq_fill_spinor_random(self.h, ctypes.c_void_p(native.data_ptr()), nrhs, prec, seed, int(parity_only), parity))
+
+    # ------------------------------------------------------------------ operator
+    def apply_native(self, op: int, out, inp, nrhs: int, prec: int, in2=None):
+        self._check(self.lib.lq_apply(self.h, op, ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(inp.data_ptr()),
+                                      ctypes.c_void_p(in2.data_ptr()) if in2 is not None else None, nrhs, prec, LQ_DEVICE, LQ_NATIVE))
+
+    def apply(self, op: int, psi: np.ndarray, prec: int = LQ_FP64, in2: np.ndarray | None = None) -> np.ndarray:
+        """Canonical host arrays psi[rhs][t][z][y][x][4][3]; complex128 for fp64, complex64 otherwise."""
+        dt = np.complex128 if prec == LQ_FP64 else np.complex64
+        psi = np.ascontiguousarray(psi, dtype=dt)
+        nrhs = psi.shape[0]
+        out = np.empty_like(psi)
+        p2 = None
+        if in2 is not None:
+            in2 = np.ascontiguousarray(in2, dtype=dt)
+            p2 = ctypes.c_void_p(in2.ctypes.data)
+        self._check(self.lib.lq_apply(self.h, op, ctypes.c_void_p(out.ctypes.data), ctypes.c_void_p(psi.ctypes.data), p2, nrhs, prec,
+                                      LQ_HOST, LQ_CANONICAL))
+        return out
+
+    # ------------------------------------------------------------------ solve
+    def solve(self, b, tol: float, inner_prec: int = LQ_FP32, delta: float = 1e-3, max_outer: int = 50, max_inner: int = 2000,
+              check_every: int = 10, use_graph: bool = False, x_out=None, native: bool = False, nrhs: int | None = None):
+        """Solves M x = b.  b: canonical complex128 numpy / torch array (host or device), or a native fp64 device
+        buffer when native=True (then nrhs is required).  Returns (x, info dict)."""
+        prm = SolveParam(tol, max_outer, max_inner, inner_prec, delta, check_every, int(use_graph))
+        info = SolveInfo()
+        if native:
+            x = x_out if x_out is not None else self.native_empty(nrhs, LQ_FP64)
+            rc = self.lib.lq_solve(self.h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(b.data_ptr()), nrhs, LQ_DEVICE, LQ_NATIVE,
+                                   ctypes.byref(prm), ctypes.byref(info))
+        else:
+            if isinstance(b, np.ndarray):
+                b = np.ascontiguousarray(b, dtype=np.complex128)
+                x = x_out if x_out is not None else np.empty_like(b)
+            else:
+                x = x_out if x_out is not None else self.torch.empty_like(b)
+            nrhs = b.shape[0]
+            pb, loc = _ptr(b)
+            px, locx = _ptr(x)
+            assert loc == locx
+            rc = self.lib.lq_solve(self.h, px, pb, nrhs, loc, LQ_CANONICAL, ctypes.byref(prm), ctypes.byref(info))
+        self._check(rc, allow=(LQ_ENOTCONVERGED,))
+        d = dict(converged=(rc == 0), nrhs=info.nrhs, outer_cycles=info.outer_cycles, inner_iters=info.inner_iters,
+                 iters=list(info.iters)[:nrhs], true_rel_residual=list(info.true_rel_residual)[:nrhs], seconds=info.seconds,
+                 dslash_applies=info.dslash_applies)
+        return x, d

@@ -1,0 +1,289 @@
+// api.cu -- the C ABI of include/lqcd_b200.h: context, ingest, apply, pack/unpack, solve.
+#include <algorithm>
+#include <string.h>
+#include "internal.cuh"
+
+void solver_forget(lq_ctx* c);
+int mhat_native(lq_ctx* c, int prec, int n, void* out_e, const void* in_e, int dagger);
+
+int set_err(lq_ctx* c, int code, const std::string& msg) {
+    if (c) c->err = msg;
+    return code;
+}
+void* dev_alloc(lq_ctx* c, size_t bytes) {
+    void* p = nullptr;
+    if (bytes == 0) bytes = 256;
+    if (c->alloc_fn) p = c->alloc_fn(bytes, c->alloc_user);
+    else if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); p = nullptr; }
+    if (!p) { set_err(c, LQ_ENOMEM, "device allocation of " + std::to_string(bytes) + " bytes failed"); return nullptr; }
+    c->owned.push_back(p);
+    return p;
+}
+void dev_free(lq_ctx* c, void* p) {
+    if (!p) return;
+    auto it = std::find(c->owned.begin(), c->owned.end(), p);
+    if (it != c->owned.end()) c->owned.erase(it);
+    if (c->free_fn) c->free_fn(p, c->alloc_user);
+    else if (!c->alloc_fn) cudaFree(p);
+}
+
+static bool nrhs_ok(int n) { return n == 1 || n == 2 || n == 4 || n == 8 || n == 12 || n == 16; }
+
+extern "C" {
+
+int lq_create(lq_ctx** out, const int dims[4], int device, void* cuda_stream) {
+    if (!out || !dims) return LQ_EINVAL;
+    *out = nullptr;
+    for (int k = 0; k < 4; k++) if (dims[k] < 2 || (dims[k] & 1)) return LQ_EINVAL;
+    const long long V = (long long)dims[0] * dims[1] * dims[2] * dims[3];
+    if (V / 2 * LQ_MAX_RHS >= (1LL << 31)) return LQ_EINVAL;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return LQ_ECUDA; }
+    lq_ctx* c = new lq_ctx();
+    for (int k = 0; k < 4; k++) c->g.L[k] = dims[k];
+    c->g.Lxh = dims[0] / 2; c->g.V = V; c->g.Vh = (int)(V / 2);
+    c->device = device; c->stream = (cudaStream_t)cuda_stream; c->t_bc = -1;
+    c->gauge64 = nullptr; c->gauge32 = nullptr; c->recon32 = 18;
+    c->clov64 = c->clovinv64 = nullptr; c->clov32 = c->clovinv32 = nullptr;
+    c->kappa = c->csw = 0; c->has_gauge = c->has_clover = false;
+    c->alloc_fn = nullptr; c->free_fn = nullptr; c->alloc_user = nullptr;
+    c->launches = 0; c->dslash_block = 0; c->dslash_rpt = 0;
+    c->red_partials = nullptr; c->red_partials_elems = 0; c->red_counter = nullptr; c->h_scalars = nullptr; c->d_flag = nullptr;
+    if (cudaMalloc(&c->red_counter, 256) != cudaSuccess || cudaMemset(c->red_counter, 0, 256) != cudaSuccess ||
+        cudaMallocHost(&c->h_scalars, 8 * LQ_MAX_RHS * sizeof(double)) != cudaSuccess) { cudaGetLastError(); delete c; return LQ_ECUDA; }
+    c->d_flag = (int*)(c->red_counter + 16);
+    *out = c;
+    return 0;
+}
+
+int lq_destroy(lq_ctx* c) {
+    if (!c) return LQ_EINVAL;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    solver_forget(c);
+    std::vector<void*> owned = c->owned;
+    for (void* p : owned) dev_free(c, p);
+    cudaFree(c->red_counter);
+    cudaFreeHost(c->h_scalars);
+    delete c;
+    return 0;
+}
+
+const char* lq_last_error(const lq_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+int lq_set_allocator(lq_ctx* c, lq_alloc_fn alloc, lq_free_fn release, void* user) {
+    if (!c) return LQ_EINVAL;
+    if (!c->owned.empty()) return set_err(c, LQ_ESTATE, "allocator must be installed before the first allocation");
+    c->alloc_fn = alloc; c->free_fn = release; c->alloc_user = user;
+    return 0;
+}
+
+int lq_set_tuning(lq_ctx* c, int dslash_block, int dslash_rpt) {
+    if (!c) return LQ_EINVAL;
+    c->dslash_block = dslash_block; c->dslash_rpt = dslash_rpt;
+    return 0;
+}
+
+long long lq_kernel_launches(const lq_ctx* c) { return c ? c->launches : 0; }
+
+static int ensure_gauge_storage(lq_ctx* c, int recon) {
+    if (recon != 18 && recon != 12) return set_err(c, LQ_EINVAL, "recon must be 18 or 12");
+    if (!c->gauge64) { c->gauge64 = (double*)dev_alloc(c, (size_t)8 * 18 * c->g.Vh * sizeof(double)); if (!c->gauge64) return LQ_ENOMEM; }
+    if (!c->gauge32) { c->gauge32 = (float*)dev_alloc(c, (size_t)8 * 18 * c->g.Vh * sizeof(float)); if (!c->gauge32) return LQ_ENOMEM; }
+    return 0;
+}
+
+int lq_load_gauge(lq_ctx* c, const void* links, int in_prec, int loc, int recon, int t_bc) {
+    if (!c || !links) return LQ_EINVAL;
+    if (in_prec != LQ_FP64 && in_prec != LQ_FP32) return set_err(c, LQ_EINVAL, "gauge precision must be fp64 or fp32");
+    if (t_bc != 1 && t_bc != -1) return set_err(c, LQ_EINVAL, "t_bc must be +1 or -1");
+    cudaSetDevice(c->device);
+    LQ_TRY(ensure_gauge_storage(c, recon));
+    const size_t bytes = (size_t)4 * c->g.V * 18 * elem_bytes(in_prec);
+    const void* dev = links;
+    void* staging = nullptr;
+    if (loc == LQ_HOST) {
+        staging = dev_alloc(c, bytes);
+        if (!staging) return LQ_ENOMEM;
+        LQ_CUDA(c, cudaMemcpyAsync(staging, links, bytes, cudaMemcpyHostToDevice, c->stream));
+        dev = staging;
+    }
+    int rc = gauge_ingest(c, dev, in_prec);
+    if (rc == 0) rc = gauge_make_fp32(c, recon);
+    if (rc == 0 && cudaStreamSynchronize(c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "gauge ingest failed");
+    if (staging) dev_free(c, staging);
+    if (rc) return rc;
+    c->t_bc = t_bc; c->has_gauge = true; c->has_clover = false;
+    return 0;
+}
+
+int lq_fill_gauge_random(lq_ctx* c, uint64_t seed, double eps, int recon, int t_bc) {
+    if (!c) return LQ_EINVAL;
+    if (t_bc != 1 && t_bc != -1) return set_err(c, LQ_EINVAL, "t_bc must be +1 or -1");
+    cudaSetDevice(c->device);
+    LQ_TRY(ensure_gauge_storage(c, recon));
+    LQ_TRY(fill_gauge(c, seed, eps));
+    LQ_TRY(gauge_make_fp32(c, recon));
+    LQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->t_bc = t_bc; c->has_gauge = true; c->has_clover = false;
+    return 0;
+}
+
+int lq_build_clover(lq_ctx* c, double kappa, double csw) {
+    if (!c) return LQ_EINVAL;
+    if (!c->has_gauge) return set_err(c, LQ_ESTATE, "load the gauge field before building the clover term");
+    cudaSetDevice(c->device);
+    return clover_build(c, kappa, csw);
+}
+
+size_t lq_native_bytes(const lq_ctx* c, int nrhs, int prec, int parity_only) {
+    if (!c || nrhs < 1) return 0;
+    return parity_bytes(c->g, nrhs, prec) * (parity_only ? 1 : 2);
+}
+
+// stage a canonical array on the device if it lives on the host; returns the device pointer (or nullptr on failure)
+static const void* stage_in(lq_ctx* c, const void* p, size_t bytes, int loc, void** staging) {
+    *staging = nullptr;
+    if (loc == LQ_DEVICE) return p;
+    *staging = dev_alloc(c, bytes);
+    if (!*staging) return nullptr;
+    if (cudaMemcpyAsync(*staging, p, bytes, cudaMemcpyHostToDevice, c->stream) != cudaSuccess) { set_err(c, LQ_ECUDA, "H2D copy failed"); return nullptr; }
+    return *staging;
+}
+
+int lq_pack(lq_ctx* c, void* native_out, const void* canonical_in, int nrhs, int prec, int loc) {
+    if (!c || !native_out || !canonical_in || !nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "lq_pack: bad argument");
+    cudaSetDevice(c->device);
+    const size_t bytes = (size_t)nrhs * c->g.V * 24 * sizeof(double);
+    void* st; const void* dev = stage_in(c, canonical_in, bytes, loc, &st);
+    if (!dev) return LQ_ENOMEM;
+    int rc = spinor_pack(c, native_out, dev, nrhs, prec, LQ_FP64);
+    if (rc == 0 && cudaStreamSynchronize(c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "pack failed");
+    if (st) dev_free(c, st);
+    return rc;
+}
+int lq_unpack(lq_ctx* c, void* canonical_out, const void* native_in, int nrhs, int prec, int loc) {
+    if (!c || !canonical_out || !native_in || !nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "lq_unpack: bad argument");
+    cudaSetDevice(c->device);
+    const size_t bytes = (size_t)nrhs * c->g.V * 24 * sizeof(double);
+    void* dev = canonical_out; void* st = nullptr;
+    if (loc == LQ_HOST) { st = dev_alloc(c, bytes); if (!st) return LQ_ENOMEM; dev = st; }
+    int rc = spinor_unpack(c, dev, native_in, nrhs, prec, LQ_FP64);
+    if (rc == 0 && st && cudaMemcpyAsync(canonical_out, st, bytes, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "D2H copy failed");
+    if (rc == 0 && cudaStreamSynchronize(c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "unpack failed");
+    if (st) dev_free(c, st);
+    return rc;
+}
+
+int lq_fill_spinor_random(lq_ctx* c, void* native_out, int nrhs, int prec, uint64_t seed, int parity_only, int parity) {
+    if (!c || !native_out || !nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "lq_fill_spinor_random: bad argument");
+    cudaSetDevice(c->device);
+    return fill_spinor(c, native_out, nrhs, prec, seed, parity_only, parity);
+}
+
+// the operator on native buffers
+static int apply_native(lq_ctx* c, int op, void* out, const void* in, const void* in2, int n, int prec) {
+    const size_t pb = parity_bytes(c->g, n, prec);
+    char* out_e = (char*)out; char* out_o = out_e + pb;
+    const char* in_e = (const char*)in; const char* in_o = in_e + pb;
+    const double k = c->kappa;
+    switch (op) {
+    case LQ_OP_HOP:
+        LQ_TRY(op_hop(c, prec, n, 0, out_e, in_o, 0));
+        return op_hop(c, prec, n, 1, out_o, in_e, 0);
+    case LQ_OP_M: case LQ_OP_MDAG: {
+        const int dag = op == LQ_OP_MDAG;
+        LQ_TRY(op_kernel_b(c, prec, n, 0, out_e, in_e, in_o, -k, 1, dag));
+        return op_kernel_b(c, prec, n, 1, out_o, in_o, in_e, -k, 1, dag);
+    }
+    case LQ_OP_CLOVER: case LQ_OP_CLOVER_INV: {
+        const int inv = op == LQ_OP_CLOVER_INV;
+        LQ_TRY(op_clover(c, prec, n, 0, out_e, in_e, inv));
+        return op_clover(c, prec, n, 1, out_o, in_o, inv);
+    }
+    case LQ_OP_HOP_EO: return op_hop(c, prec, n, 0, out, in, 0);
+    case LQ_OP_HOP_OE: return op_hop(c, prec, n, 1, out, in, 0);
+    case LQ_OP_MHAT: return mhat_native(c, prec, n, out, in, 0);
+    case LQ_OP_MHAT_DAG: return mhat_native(c, prec, n, out, in, 1);
+    case LQ_OP_KERNEL_A: return op_kernel_a(c, prec, n, 1, out, in, 0);
+    case LQ_OP_KERNEL_B: return op_kernel_b(c, prec, n, 0, out, in, in2, -k * k, 1, 0);
+    default: return set_err(c, LQ_EINVAL, "unknown operator");
+    }
+}
+
+int lq_apply(lq_ctx* c, int op, void* out, const void* in, const void* in2, int nrhs, int prec, int loc, int layout) {
+    if (!c || !out || !in) return set_err(c, LQ_EINVAL, "lq_apply: null argument");
+    if (!nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "nrhs must be one of 1,2,4,8,12,16");
+    if (prec != LQ_FP64 && prec != LQ_FP32 && prec != LQ_HALF) return set_err(c, LQ_EINVAL, "bad precision");
+    if (op < 0 || op > LQ_OP_KERNEL_B) return set_err(c, LQ_EINVAL, "unknown operator");
+    if (op == LQ_OP_KERNEL_B && !in2) return set_err(c, LQ_EINVAL, "LQ_OP_KERNEL_B needs in2");
+    if (out == in || out == in2) return set_err(c, LQ_EINVAL, "out must not alias an input");
+    if (!c->has_gauge) return set_err(c, LQ_ESTATE, "gauge field not loaded");
+    const bool needs_clover = !(op == LQ_OP_HOP || op == LQ_OP_HOP_EO || op == LQ_OP_HOP_OE);
+    if (needs_clover && !c->has_clover) return set_err(c, LQ_ESTATE, "clover term not built");
+    cudaSetDevice(c->device);
+    if (layout == LQ_NATIVE) {
+        if (loc != LQ_DEVICE) return set_err(c, LQ_EINVAL, "native buffers must be device buffers");
+        return apply_native(c, op, out, in, in2, nrhs, prec);
+    }
+    // canonical: stage, pack, apply, unpack
+    const int cprec = prec == LQ_FP64 ? LQ_FP64 : LQ_FP32;
+    const size_t cbytes = (size_t)nrhs * c->g.V * 24 * elem_bytes(cprec);
+    const size_t pb = parity_bytes(c->g, nrhs, prec);
+    const bool full = op <= LQ_OP_CLOVER_INV;
+    int in_par = 0, out_par = 0;       // parity blocks used by parity ops
+    if (op == LQ_OP_HOP_EO) { in_par = 1; out_par = 0; }
+    if (op == LQ_OP_HOP_OE || op == LQ_OP_KERNEL_A) { in_par = 0; out_par = 1; }
+    void *st_in = nullptr, *st_in2 = nullptr, *st_out = nullptr;
+    void *n_in = dev_alloc(c, 2 * pb), *n_in2 = in2 ? dev_alloc(c, 2 * pb) : nullptr, *n_out = dev_alloc(c, 2 * pb);
+    int rc = (!n_in || !n_out || (in2 && !n_in2)) ? LQ_ENOMEM : 0;
+    const void* d_in = nullptr; const void* d_in2 = nullptr;
+    if (rc == 0) { d_in = stage_in(c, in, cbytes, loc, &st_in); if (!d_in) rc = LQ_ENOMEM; }
+    if (rc == 0 && in2) { d_in2 = stage_in(c, in2, cbytes, loc, &st_in2); if (!d_in2) rc = LQ_ENOMEM; }
+    if (rc == 0) rc = spinor_pack(c, n_in, d_in, nrhs, prec, cprec);
+    if (rc == 0 && in2) rc = spinor_pack(c, n_in2, d_in2, nrhs, prec, cprec);
+    if (rc == 0 && cudaMemsetAsync(n_out, 0, 2 * pb, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "memset failed");
+    if (rc == 0) {
+        if (full) rc = apply_native(c, op, n_out, n_in, nullptr, nrhs, prec);
+        else rc = apply_native(c, op, (char*)n_out + out_par * pb, (char*)n_in + in_par * pb, in2 ? (char*)n_in2 + pb : nullptr, nrhs, prec);
+    }
+    void* d_out = out;
+    if (rc == 0 && loc == LQ_HOST) { st_out = dev_alloc(c, cbytes); if (!st_out) rc = LQ_ENOMEM; d_out = st_out; }
+    if (rc == 0) rc = spinor_unpack(c, d_out, n_out, nrhs, prec, cprec);
+    if (rc == 0 && st_out && cudaMemcpyAsync(out, st_out, cbytes, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "D2H copy failed");
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess && rc == 0) rc = set_err(c, LQ_ECUDA, std::string("lq_apply: ") + cudaGetErrorString(cudaGetLastError()));
+    void* tofree[] = {st_in, st_in2, st_out, n_in, n_in2, n_out};
+    for (void* p : tofree) if (p) dev_free(c, p);
+    return rc;
+}
+
+int lq_solve(lq_ctx* c, void* x, const void* b, int nrhs, int loc, int layout, const lq_solve_param* param, lq_solve_info* info) {
+    if (!c || !x || !b || !param || !info) return set_err(c, LQ_EINVAL, "lq_solve: null argument");
+    if (!nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "nrhs must be one of 1,2,4,8,12,16");
+    if (!(param->tol > 0) || param->max_outer < 1 || param->max_inner < 1) return set_err(c, LQ_EINVAL, "bad solve parameters");
+    cudaSetDevice(c->device);
+    if (layout == LQ_NATIVE) {
+        if (loc != LQ_DEVICE) return set_err(c, LQ_EINVAL, "native buffers must be device buffers");
+        return solve_native(c, x, b, nrhs, param, info);
+    }
+    const size_t cbytes = (size_t)nrhs * c->g.V * 24 * sizeof(double);
+    const size_t pb = parity_bytes(c->g, nrhs, LQ_FP64);
+    void *st_b = nullptr, *st_x = nullptr;
+    void *n_b = dev_alloc(c, 2 * pb), *n_x = dev_alloc(c, 2 * pb);
+    int rc = (!n_b || !n_x) ? LQ_ENOMEM : 0;
+    const void* d_b = nullptr;
+    if (rc == 0) { d_b = stage_in(c, b, cbytes, loc, &st_b); if (!d_b) rc = LQ_ENOMEM; }
+    if (rc == 0) rc = spinor_pack(c, n_b, d_b, nrhs, LQ_FP64, LQ_FP64);
+    if (st_b && rc == 0) { cudaStreamSynchronize(c->stream); dev_free(c, st_b); st_b = nullptr; }
+    int src = 0;
+    if (rc == 0) { src = solve_native(c, n_x, n_b, nrhs, param, info); if (src != 0 && src != LQ_ENOTCONVERGED) rc = src; }
+    void* d_x = x;
+    if (rc == 0 && loc == LQ_HOST) { st_x = dev_alloc(c, cbytes); if (!st_x) rc = LQ_ENOMEM; d_x = st_x; }
+    if (rc == 0) rc = spinor_unpack(c, d_x, n_x, nrhs, LQ_FP64, LQ_FP64);
+    if (rc == 0 && st_x && cudaMemcpyAsync(x, st_x, cbytes, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "D2H copy failed");
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess && rc == 0) rc = set_err(c, LQ_ECUDA, std::string("lq_solve: ") + cudaGetErrorString(cudaGetLastError()));
+    void* tofree[] = {st_b, st_x, n_b, n_x};
+    for (void* p : tofree) if (p) dev_free(c, p);
+    return rc ? rc : src;
+}
+
+}  // extern "C"

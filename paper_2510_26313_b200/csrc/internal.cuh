@@ -1,0 +1,49 @@
+// internal.cuh -- cross-file declarations of the CUDA path (not part of the C ABI).
+#pragma once
+#include "common.cuh"
+#include "dslash.cuh"
+
+// dslash_*.cu
+template <class S, int RECON, int FORM>
+int launch_dslash(lq_ctx* c, DslashArgs<S> a, int rpt_override);
+
+// ops.cu : typed single-parity building blocks on native fields
+// out(parity) = [C] D in(1-parity) ; form A uses A^{-1}, form HOP nothing
+int op_hop(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* in, int dagger);
+int op_kernel_a(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* in, int dagger);
+// out(parity) = C x + coef D in ; use_clover: 1 -> A(parity), 0 -> identity
+int op_kernel_b(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger);
+// out(parity) = A x or A^{-1} x (site-local)
+int op_clover(lq_ctx* c, int prec, int nrhs, int parity, void* out, const void* x, int inverse);
+
+// reorder.cu
+int gauge_ingest(lq_ctx* c, const void* dev_canonical, int in_prec);            // canonical (device) -> native fp64
+int gauge_make_fp32(lq_ctx* c, int recon);                                       // native fp64 -> native fp32 (18 or 12)
+int spinor_pack(lq_ctx* c, void* native_full, const void* dev_canonical, int nrhs, int prec, int in_prec);
+int spinor_unpack(lq_ctx* c, void* dev_canonical, const void* native_full, int nrhs, int prec, int out_prec);
+int spinor_convert(lq_ctx* c, void* dst, int dst_prec, const void* src, int src_prec, int nrhs, const double* d_scale /*per rhs, multiplies*/, int invert_scale);
+int spinor_zero_parity(lq_ctx* c, void* parity_block, int nrhs, int prec);
+int canonical_zero_parity(lq_ctx* c, void* dev_canonical, int nrhs, int prec, int parity);
+
+// clover.cu
+int clover_build(lq_ctx* c, double kappa, double csw);
+
+// blas.cu : per-RHS block BLAS on one parity block; results stay on the device
+int blas_norm2(lq_ctx* c, int prec, int nrhs, const void* x, double* d_out);                       // d_out[k] = ||x_k||^2
+// CG step 1: alpha_k = rr_k / pAp_k;  x += alpha p;  r -= alpha q;  rr_new_k = ||r_k||^2
+int blas_cg_update_xr(lq_ctx* c, int prec, int nrhs, void* x, void* r, const void* p, const void* q,
+                      const double* d_rr, const double* d_pAp, double* d_rr_new);
+// CG step 2: beta_k = rr_new_k / rr_k;  p = r + beta p
+int blas_cg_update_p(lq_ctx* c, int prec, int nrhs, void* p, const void* r, const double* d_rr_new, const double* d_rr);
+// y (fp64) += s_k * e (prec)       (defect-correction accumulate)
+int blas_axpy_mixed(lq_ctx* c, int prec, int nrhs, void* y64, const void* e, const double* d_scale);
+// r = b - t (fp64), d_out[k] = ||r_k||^2
+int blas_residual(lq_ctx* c, int nrhs, void* r, const void* b, const void* t, double* d_out);
+int blas_copy(lq_ctx* c, int prec, int nrhs, void* dst, const void* src);
+
+// fill.cu
+int fill_gauge(lq_ctx* c, uint64_t seed, double eps);
+int fill_spinor(lq_ctx* c, void* native, int nrhs, int prec, uint64_t seed, int parity_only, int parity);
+
+// solver.cu
+int solve_native(lq_ctx* c, void* x_full64, const void* b_full64, int nrhs, const lq_solve_param* p, lq_solve_info* info);

@@ -1,0 +1,191 @@
+// reorder.cu -- canonical <-> native reorders and precision conversion.
+#include "internal.cuh"
+
+// ---- gauge ---------------------------------------------------------------------------------------------------
+template <typename Tin>
+__global__ void gauge_ingest_kernel(Geom g, const Tin* __restrict__ canon, double* __restrict__ native) {
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= 8LL * g.Vh) return;
+    const int cb = (int)(tid % g.Vh);
+    const int pm = (int)(tid / g.Vh);           // parity*4 + mu
+    const int parity = pm >> 2, mu = pm & 3;
+    int xh, y, z, t, odd;
+    cb_coords(g, parity, cb, xh, y, z, t, odd);
+    const long long site = (2 * xh + odd) + (long long)g.L[0] * (y + (long long)g.L[1] * (z + (long long)g.L[2] * t));
+    const Tin* src = canon + ((long long)mu * g.V + site) * 18;
+    double r[18];
+#pragma unroll
+    for (int k = 0; k < 18; k++) r[k] = (double)src[k];
+    store_planes<double, 18>(native + (size_t)pm * 18 * g.Vh, g.Vh, cb, r);
+}
+int gauge_ingest(lq_ctx* c, const void* dev_canonical, int in_prec) {
+    const long long threads = 8LL * c->g.Vh;
+    const int block = 128; const int grid = (int)((threads + block - 1) / block);
+    if (in_prec == LQ_FP64) gauge_ingest_kernel<double><<<grid, block, 0, c->stream>>>(c->g, (const double*)dev_canonical, c->gauge64);
+    else if (in_prec == LQ_FP32) gauge_ingest_kernel<float><<<grid, block, 0, c->stream>>>(c->g, (const float*)dev_canonical, c->gauge64);
+    else return set_err(c, LQ_EINVAL, "gauge precision must be fp64 or fp32");
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
+}
+template <int RECON>
+__global__ void gauge_to_fp32_kernel(int Vh, const double* __restrict__ src, float* __restrict__ dst) {
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= 8LL * Vh) return;
+    const int cb = (int)(tid % Vh), pm = (int)(tid / Vh);
+    double r[18]; float f[18];
+    load_planes<double, 18>(src + (size_t)pm * 18 * Vh, Vh, cb, r);
+#pragma unroll
+    for (int k = 0; k < RECON; k++) f[k] = (float)r[k];
+    store_planes<float, RECON>(dst + (size_t)pm * RECON * Vh, Vh, cb, f);
+}
+int gauge_make_fp32(lq_ctx* c, int recon) {
+    const long long threads = 8LL * c->g.Vh;
+    const int block = 128; const int grid = (int)((threads + block - 1) / block);
+    if (recon == 18) gauge_to_fp32_kernel<18><<<grid, block, 0, c->stream>>>(c->g.Vh, c->gauge64, c->gauge32);
+    else gauge_to_fp32_kernel<12><<<grid, block, 0, c->stream>>>(c->g.Vh, c->gauge64, c->gauge32);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    c->recon32 = recon;
+    return 0;
+}
+
+// ---- scalar element access of a native parity block ---------------------------------------------------------------
+template <class S>
+__device__ __forceinline__ void load_site(const SView<S>& v, int Vh, int N, int cb, int k, double* o) {
+    const size_t plane = (size_t)Vh * N, off = (size_t)cb * N + k;
+    double sc = 1.0;
+    if constexpr (S::has_norm) sc = (double)(v.n[off] * (1.0f / 32767.0f));
+#pragma unroll
+    for (int j = 0; j < 24; j++) o[j] = (double)v.d[j * plane + off] * sc;
+}
+template <class S>
+__device__ __forceinline__ void store_site(const SView<S>& v, int Vh, int N, int cb, int k, const double* o) {
+    const size_t plane = (size_t)Vh * N, off = (size_t)cb * N + k;
+    if constexpr (S::has_norm) {
+        float mx = 0.f;
+#pragma unroll
+        for (int j = 0; j < 24; j++) mx = fmaxf(mx, fabsf((float)o[j]));
+        v.n[off] = mx;
+        const float inv = mx > 0.f ? 32767.0f / mx : 0.f;
+#pragma unroll
+        for (int j = 0; j < 24; j++) v.d[j * plane + off] = (short)rintf((float)o[j] * inv);
+    } else {
+#pragma unroll
+        for (int j = 0; j < 24; j++) v.d[j * plane + off] = (typename S::store_t)o[j];
+    }
+}
+
+// ---- spinor pack / unpack ---------------------------------------------------------------------------------------------
+template <class S, typename Tc, bool PACK>
+__global__ void spinor_reorder_kernel(Geom g, int N, SView<S> even, SView<S> odd, Tc* canon) {
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= 2LL * g.Vh * N) return;
+    const int k = (int)(tid % N);
+    const long long r = tid / N;
+    const int cb = (int)(r % g.Vh), parity = (int)(r / g.Vh);
+    int xh, y, z, t, odd_;
+    cb_coords(g, parity, cb, xh, y, z, t, odd_);
+    const long long site = (2 * xh + odd_) + (long long)g.L[0] * (y + (long long)g.L[1] * (z + (long long)g.L[2] * t));
+    Tc* p = canon + ((long long)k * g.V + site) * 24;
+    const SView<S>& v = parity ? odd : even;
+    double o[24];
+    if constexpr (PACK) {
+#pragma unroll
+        for (int j = 0; j < 24; j++) o[j] = (double)p[j];
+        store_site<S>(v, g.Vh, N, cb, k, o);
+    } else {
+        load_site<S>(v, g.Vh, N, cb, k, o);
+#pragma unroll
+        for (int j = 0; j < 24; j++) p[j] = (Tc)o[j];
+    }
+}
+template <class S, bool PACK>
+static int reorder_t(lq_ctx* c, void* native_full, void* canon, int nrhs, int cprec) {
+    SView<S> e = make_view<S>(c->g, native_full, nrhs, 0), o = make_view<S>(c->g, native_full, nrhs, 1);
+    const long long threads = 2LL * c->g.Vh * nrhs;
+    const int block = 128; const int grid = (int)((threads + block - 1) / block);
+    if (cprec == LQ_FP64) spinor_reorder_kernel<S, double, PACK><<<grid, block, 0, c->stream>>>(c->g, nrhs, e, o, (double*)canon);
+    else spinor_reorder_kernel<S, float, PACK><<<grid, block, 0, c->stream>>>(c->g, nrhs, e, o, (float*)canon);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
+}
+int spinor_pack(lq_ctx* c, void* native_full, const void* dev_canonical, int nrhs, int prec, int in_prec) {
+    void* cn = const_cast<void*>(dev_canonical);
+    if (prec == LQ_FP64) return reorder_t<F64, true>(c, native_full, cn, nrhs, in_prec);
+    if (prec == LQ_FP32) return reorder_t<F32, true>(c, native_full, cn, nrhs, in_prec);
+    return reorder_t<H16, true>(c, native_full, cn, nrhs, in_prec);
+}
+int spinor_unpack(lq_ctx* c, void* dev_canonical, const void* native_full, int nrhs, int prec, int out_prec) {
+    void* nf = const_cast<void*>(native_full);
+    if (prec == LQ_FP64) return reorder_t<F64, false>(c, nf, dev_canonical, nrhs, out_prec);
+    if (prec == LQ_FP32) return reorder_t<F32, false>(c, nf, dev_canonical, nrhs, out_prec);
+    return reorder_t<H16, false>(c, nf, dev_canonical, nrhs, out_prec);
+}
+
+// ---- precision conversion of one parity block, with an optional per-RHS scale ----------------------------------------------
+template <class SD, class SS>
+__global__ void convert_kernel(int Vh, int N, SView<SD> dst, SView<SS> src, const double* __restrict__ scale, int invert) {
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= (long long)Vh * N) return;
+    const int k = (int)(tid % N), cb = (int)(tid / N);
+    double o[24];
+    load_site<SS>(src, Vh, N, cb, k, o);
+    if (scale) {
+        double s = scale[k];
+        if (invert) s = (s != 0.0) ? 1.0 / s : 0.0;
+#pragma unroll
+        for (int j = 0; j < 24; j++) o[j] *= s;
+    }
+    store_site<SD>(dst, Vh, N, cb, k, o);
+}
+template <class SD, class SS>
+static int convert_t(lq_ctx* c, void* dst, const void* src, int nrhs, const double* d_scale, int invert) {
+    SView<SD> d = make_view<SD>(c->g, dst, nrhs, 0);
+    SView<SS> s = make_view<SS>(c->g, const_cast<void*>(src), nrhs, 0);
+    const long long threads = (long long)c->g.Vh * nrhs;
+    const int block = 128; const int grid = (int)((threads + block - 1) / block);
+    convert_kernel<SD, SS><<<grid, block, 0, c->stream>>>(c->g.Vh, nrhs, d, s, d_scale, invert);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
+}
+template <class SD>
+static int convert_d(lq_ctx* c, void* dst, const void* src, int src_prec, int nrhs, const double* d_scale, int invert) {
+    if (src_prec == LQ_FP64) return convert_t<SD, F64>(c, dst, src, nrhs, d_scale, invert);
+    if (src_prec == LQ_FP32) return convert_t<SD, F32>(c, dst, src, nrhs, d_scale, invert);
+    return convert_t<SD, H16>(c, dst, src, nrhs, d_scale, invert);
+}
+int spinor_convert(lq_ctx* c, void* dst, int dst_prec, const void* src, int src_prec, int nrhs, const double* d_scale, int invert) {
+    if (dst_prec == LQ_FP64) return convert_d<F64>(c, dst, src, src_prec, nrhs, d_scale, invert);
+    if (dst_prec == LQ_FP32) return convert_d<F32>(c, dst, src, src_prec, nrhs, d_scale, invert);
+    return convert_d<H16>(c, dst, src, src_prec, nrhs, d_scale, invert);
+}
+
+int spinor_zero_parity(lq_ctx* c, void* parity_block, int nrhs, int prec) {
+    LQ_CUDA(c, cudaMemsetAsync(parity_block, 0, parity_bytes(c->g, nrhs, prec), c->stream));
+    return 0;
+}
+
+template <typename Tc>
+__global__ void canonical_zero_parity_kernel(Geom g, int N, Tc* canon, int parity) {
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= (long long)g.Vh * N) return;
+    const int cb = (int)(tid % g.Vh), k = (int)(tid / g.Vh);
+    int xh, y, z, t, odd_;
+    cb_coords(g, parity, cb, xh, y, z, t, odd_);
+    const long long site = (2 * xh + odd_) + (long long)g.L[0] * (y + (long long)g.L[1] * (z + (long long)g.L[2] * t));
+    Tc* p = canon + ((long long)k * g.V + site) * 24;
+#pragma unroll
+    for (int j = 0; j < 24; j++) p[j] = Tc(0);
+}
+int canonical_zero_parity(lq_ctx* c, void* dev_canonical, int nrhs, int prec, int parity) {
+    const long long threads = (long long)c->g.Vh * nrhs;
+    const int block = 128; const int grid = (int)((threads + block - 1) / block);
+    if (prec == LQ_FP64) canonical_zero_parity_kernel<double><<<grid, block, 0, c->stream>>>(c->g, nrhs, (double*)dev_canonical, parity);
+    else canonical_zero_parity_kernel<float><<<grid, block, 0, c->stream>>>(c->g, nrhs, (float*)dev_canonical, parity);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
+}

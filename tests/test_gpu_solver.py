@@ -1,0 +1,107 @@
+"""GPU solver parity: true residual recomputed by the oracle's full M, solution vs
+the oracle's own CG, every inner precision.  Iteration counts are not compared (parity unpinned, 8(c.3))."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2510_26313_b200 import inputs
+from paper_2510_26313_b200 import binding as B
+from tests.oracle_ops import OracleCase, rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+def true_residuals(orc, x, b):
+    out = []
+    for k in range(b.shape[0]):
+        r = b[k].ravel() - oracle.M(orc.dims, orc.U, orc.A, orc.kappa, x[k], False, orc.t_bc).ravel()
+        out.append(np.linalg.norm(r) / np.linalg.norm(b[k].ravel()))
+    return np.array(out)
+
+
+def setup(dims, seed, eps, kappa, csw, recon=18):
+    U = inputs.make_links(dims, seed, eps)
+    ctx = B.Context(dims)
+    ctx.load_gauge(U, recon=recon)
+    ctx.build_clover(kappa, csw)
+    return ctx, OracleCase(dims, U, kappa, csw)
+
+
+def test_config0_solve_fp64():
+    """configs[0]: 4^3 x 8, 1 RHS, fp64 throughout, even-odd CG on MdagM to 1e-10."""
+    cfg = inputs.CONFIGS[0]
+    ctx, orc = setup(cfg["dims"], cfg["gauge_seed"], cfg["eps"], cfg["kappa"], cfg["csw"])
+    b = inputs.gaussian_spinors(cfg["dims"], 1, cfg["source_seed"])
+    x, info = ctx.solve(b, tol=cfg["tol"], inner_prec=B.LQ_FP64, delta=1e-11, check_every=5)
+    assert info["converged"]
+    res = true_residuals(orc, x, b)
+    assert res[0] <= cfg["tol"]
+    assert abs(info["true_rel_residual"][0] - res[0]) <= 1e-12          # Schur identity: eo residual = full residual
+    xo, it, _ = oracle.solve_eo(cfg["dims"], orc.U, orc.A, orc.Ainv, cfg["kappa"], b[0], cfg["tol"] * 1e-2)
+    assert rel_err(x[0], xo.reshape(x[0].shape)) <= 20 * cfg["tol"]     # cond(M) is O(10) on these links
+    assert 0 < info["inner_iters"] < 10 * it
+    ctx.close()
+
+
+@pytest.mark.parametrize("inner,delta,tol", [(B.LQ_FP32, 1e-3, 1e-8), (B.LQ_HALF, 1e-2, 1e-9), (B.LQ_FP64, 1e-4, 1e-10)])
+@pytest.mark.parametrize("use_graph", [False, True])
+def test_batched_mixed_precision_solve(inner, delta, tol, use_graph):
+    """8^3 x 16 stand-in for configs[1] / configs[3]: LapH-diluted sources, fp32 / int16 inner CG, fp64 defect correction."""
+    dims = (8, 8, 8, 16)
+    nrhs = 8 if inner != B.LQ_HALF else 12
+    n_t = 2 if inner != B.LQ_HALF else 3
+    ctx, orc = setup(dims, 1001, 0.2, 0.124, 1.2)
+    b = inputs.laph_sources(dims, nrhs, n_t, 2001)
+    x, info = ctx.solve(b, tol=tol, inner_prec=inner, delta=delta, use_graph=use_graph, check_every=4)
+    assert info["converged"], info
+    res = true_residuals(orc, x, b)
+    assert np.all(res <= tol), res
+    assert np.allclose(res, info["true_rel_residual"], rtol=1e-3, atol=tol * 1e-3)
+    for k in (0, nrhs - 1):
+        xo, _, _ = oracle.solve_eo(dims, orc.U, orc.A, orc.Ainv, 0.124, b[k], tol * 1e-2)
+        assert rel_err(x[k], xo.reshape(x[k].shape)) <= 50 * tol
+    assert info["outer_cycles"] >= 1 and info["inner_iters"] > 0
+    ctx.close()
+
+
+def test_solve_device_buffers_and_native_layout():
+    import torch
+    dims = (8, 4, 4, 8)
+    ctx, orc = setup(dims, 3, 0.3, 0.12, 1.0)
+    b = inputs.gaussian_spinors(dims, 4, 9)
+    x_host, _ = ctx.solve(b, tol=1e-9, inner_prec=B.LQ_FP32)
+    bd = torch.from_numpy(b).cuda()
+    xd, info = ctx.solve(bd, tol=1e-9, inner_prec=B.LQ_FP32)
+    assert info["converged"] and np.array_equal(xd.cpu().numpy(), x_host)     # deterministic reductions: bit-identical
+    nb = ctx.pack(b, 4, B.LQ_FP64)
+    nx, info = ctx.solve(nb, tol=1e-9, inner_prec=B.LQ_FP32, native=True, nrhs=4)
+    assert np.array_equal(ctx.unpack(nx, 4, B.LQ_FP64), x_host)
+    assert np.all(true_residuals(orc, x_host, b) <= 1e-9)
+    ctx.close()
+
+
+def test_zero_and_mixed_difficulty_sources():
+    """Degenerate batch: one RHS identically zero, one tiny, one point source; per-RHS alpha/beta guards (reading #18)."""
+    dims = (4, 4, 4, 8)
+    ctx, orc = setup(dims, 1000, 0.3, 0.12, 1.0)
+    b = inputs.gaussian_spinors(dims, 4, 5)
+    b[1] = 0
+    b[2] *= 1e-12
+    b[3] = 0
+    b[3, 0, 0, 0, 0, 0, 0] = 1.0
+    x, info = ctx.solve(b, tol=1e-9, inner_prec=B.LQ_FP32)
+    assert info["converged"] and np.all(np.isfinite(x.view(np.float64)))
+    assert np.all(x[1] == 0)
+    res = [np.linalg.norm(b[k].ravel() - oracle.M(dims, orc.U, orc.A, 0.12, x[k]).ravel()) / np.linalg.norm(b[k].ravel()) for k in (0, 2, 3)]
+    assert max(res) <= 1e-9
+    ctx.close()
+
+
+def test_not_converged_is_reported():
+    dims = (4, 4, 4, 8)
+    ctx, orc = setup(dims, 1000, 0.3, 0.12, 1.0)
+    b = inputs.gaussian_spinors(dims, 2, 5)
+    x, info = ctx.solve(b, tol=1e-12, inner_prec=B.LQ_FP32, max_outer=1, max_inner=4, check_every=2)
+    assert not info["converged"] and max(info["true_rel_residual"]) > 1e-12
+    assert np.all(np.isfinite(x.view(np.float64)))
+    ctx.close()

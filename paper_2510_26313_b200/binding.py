@@ -99,7 +99,9 @@ class Context:
         self.V = int(np.prod(self.dims))
         self.device = device
         torch.cuda.set_device(device)
-        self.stream = torch.cuda.current_stream(device)
+        # a dedicated non-default stream: the legacy default stream cannot be captured into a CUDA graph
+        self.stream = torch.cuda.Stream(device=device)
+        self.stream.wait_stream(torch.cuda.current_stream(device))
         h = ctypes.c_void_p()
         rc = self.lib.lq_create(ctypes.byref(h), (ctypes.c_int * 4)(*self.dims), device, ctypes.c_void_p(self.stream.cuda_stream))
         if rc != 0:
@@ -122,7 +124,12 @@ class Context:
             self._check(self.lib.lq_set_allocator(self.h, self._alloc_cb, self._free_cb, None))
 
     # ------------------------------------------------------------------ plumbing
+    def _enter(self):
+        """Order the library's stream after work already queued on torch's current stream (input tensors)."""
+        self.stream.wait_stream(self.torch.cuda.current_stream(self.device))
+
     def _check(self, rc, allow=()):
+        self.torch.cuda.current_stream(self.device).wait_stream(self.stream)
         if rc != 0 and rc not in allow:
             raise LqError(rc, self.lib.lq_last_error(self.h).decode())
         return rc
@@ -149,6 +156,7 @@ class Context:
     # ------------------------------------------------------------------ gauge / clover
     def load_gauge(self, U, recon: int = 18, t_bc: int = -1):
         """U: canonical [mu][t][z][y][x][3][3] complex128/complex64, numpy (host) or torch (host/device)."""
+        self._enter()
         if isinstance(U, np.ndarray):
             prec = LQ_FP64 if U.dtype == np.complex128 else LQ_FP32
             U = np.ascontiguousarray(U)
@@ -172,22 +180,26 @@ class Context:
         return self.torch.empty(self.native_bytes(nrhs, prec, parity_only), dtype=self.torch.uint8, device="cuda:%d" % self.device)
 
     def pack(self, canonical, nrhs: int, prec: int):
+        self._enter()
         out = self.native_empty(nrhs, prec)
         p, loc = _ptr(canonical)
         self._check(self.lib.lq_pack(self.h, ctypes.c_void_p(out.data_ptr()), p, nrhs, prec, loc))
         return out
 
     def unpack(self, native, nrhs: int, prec: int) -> np.ndarray:
+        self._enter()
         Lx, Ly, Lz, Lt = self.dims
         out = np.empty((nrhs, Lt, Lz, Ly, Lx, 4, 3), dtype=np.complex128)
         self._check(self.lib.lq_unpack(self.h, ctypes.c_void_p(out.ctypes.data), ctypes.c_void_p(native.data_ptr()), nrhs, prec, LQ_HOST))
         return out
 
     def fill_spinor_random(self, native, nrhs: int, prec: int, seed: int, parity_only: bool = False, parity: int = 0):
+        self._enter()
         self._check(self.lib.lq_fill_spinor_random(self.h, ctypes.c_void_p(native.data_ptr()), nrhs, prec, seed, int(parity_only), parity))
 
     # ------------------------------------------------------------------ operator
     def apply_native(self, op: int, out, inp, nrhs: int, prec: int, in2=None):
+        self._enter()
         self._check(self.lib.lq_apply(self.h, op, ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(inp.data_ptr()),
                                       ctypes.c_void_p(in2.data_ptr()) if in2 is not None else None, nrhs, prec, LQ_DEVICE, LQ_NATIVE))
 
@@ -210,6 +222,7 @@ class Context:
               check_every: int = 10, use_graph: bool = False, x_out=None, native: bool = False, nrhs: int | None = None):
         """Solves M x = b.  b: canonical complex128 numpy / torch array (host or device), or a native fp64 device
         buffer when native=True (then nrhs is required).  Returns (x, info dict)."""
+        self._enter()
         prm = SolveParam(tol, max_outer, max_inner, inner_prec, delta, check_every, int(use_graph))
         info = SolveInfo()
         if native:

@@ -163,8 +163,8 @@ int solve_native(lq_ctx* c, void* x_full, const void* b_full, int n, const lq_so
                     int rc = 0;
                     for (int j = 0; j < check_every && rc == 0; j++) { rc = cg_iteration(c, w, prec, n, rr, d_pAp, rrn); double* s = rr; rr = rrn; rrn = s; }
                     c->launches = l0;
-                    cudaError_t ce = cudaStreamEndCapture(c->stream, &graph);
-                    if (rc) return rc;
+                    cudaError_t ce = cudaStreamEndCapture(c->stream, &graph);   // always close the capture, even on failure
+                    if (rc) { if (ce == cudaSuccess && graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
                     LQ_CUDA(c, ce);
                     LQ_CUDA(c, cudaGraphInstantiate(&gexec, graph, 0));
                     cudaGraphDestroy(graph);

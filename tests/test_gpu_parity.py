@@ -142,7 +142,7 @@ def test_pack_unpack_and_device_generators():
     assert np.array_equal(ctx.unpack(nat32, 4, B.LQ_FP32), psi.astype(np.complex64).astype(np.complex128))
     nath = ctx.pack(psi, 4, B.LQ_HALF)
     back = ctx.unpack(nath, 4, B.LQ_HALF)
-    site_max = np.abs(np.stack([psi.real, psi.imag])).max(axis=(0, 5, 6), keepdims=False)
+    site_max = np.abs(np.stack([psi.real, psi.imag])).max(axis=(0, 6, 7))
     assert np.all(np.abs(back - psi).max(axis=(5, 6)) <= 1.01 * site_max / 32767)      # |err| <= norm/(2*32767) per real
     gen = ctx.native_empty(4, B.LQ_FP64)
     ctx.fill_spinor_random(gen, 4, B.LQ_FP64, 31)

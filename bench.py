@@ -1,0 +1,342 @@
+#!/usr/bin/env python
+"""bench.py -- measures BASELINE.json's metric ("multi-RHS clover Dslash HBM GB/s & % of peak; batched CG sec/RHS").
+
+One "step" is one pass of the whole hot path over one batch of synthetic sources:
+a batched mixed-precision even-odd CG solve M x = b for N_rhs LapH-diluted sources on the workload's lattice
+(default: BASELINE.json configs[1], 16^3 x 32, 8 RHS, fp32 inner CG, fp64 defect correction, tol 1e-8).
+`value` is seconds per RHS with the sources resident in HBM; `e2e` is the same through the C ABI with HOST buffers.
+`roofline` is the dominant kernel (fused kernel A = A^-1 D, fp32) timed alone on the same lattice and batch with
+rotating buffer sets larger than L2.  `dslash` adds the configs[2] sweep (32^3 x 64, N = 1..16) and configs[4]
+(64^3 x 128, N = 4, 12-real links) operator throughput; `cpu_baseline` times the fp64 oracle on the host cores.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg1|cfg3] [--no-extras]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2510_26313_b200 import inputs  # noqa: E402
+
+L2_BYTES = 126e6
+FLOP_A, FLOP_B, FLOP_HOP = 1824.0, 1872.0, 1320.0      # per output site per RHS (BASELINE.json north_star)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback", 1965.0
+
+
+def bytes_per_site_rhs(kind: str, prec: str, nrhs: int, recon: int) -> float:
+    """Compulsory (algorithmic) bytes per output site per RHS: every input site read once, output written once,
+    8 links + 72 clover reals shared by the batch."""
+    s = {"fp64": 8.0, "fp32": 4.0, "half": 2.0}[prec]
+    g = 8.0 if prec == "fp64" else 4.0
+    spinor = 24 * s + (4.0 if prec == "half" else 0.0)
+    per_batch = 8 * recon * g + (0.0 if kind == "hop" else 72 * g)
+    streams = 3 if kind == "B" else 2
+    return streams * spinor + per_batch / nrhs
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(device), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            v = [q.strip() for q in line.split(",")]
+            if len(v) < 7:
+                continue
+            try:
+                sm.append(float(v[0])); mx.append(float(v[1])); power.append(float(v[2]))
+            except ValueError:
+                continue
+            for n, q in zip(names, v[3:7]):
+                if q.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(power)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ------------------------------------------------------------------------------------------------ operator timing
+def time_dslash(ctx, B, kind: str, prec: str, nrhs: int, recon: int, iters: int = 20, warmup: int = 3):
+    """Average device time of one single-parity stencil launch (kernel A, kernel B or the bare hop), native layout,
+    rotating buffer sets so that no launch starts with its operands in L2.  Returns a dict of seconds / GB/s / GFLOP/s."""
+    import torch
+    P = B.PREC[prec]
+    pbytes = ctx.native_bytes(nrhs, P, True)
+    per_set = pbytes * (3 if kind == "B" else 2)
+    nsets = max(3, int(np.ceil(2.5 * L2_BYTES / per_set)) + 1)
+    nsets = min(nsets, 64)
+    sets = []
+    for i in range(nsets):
+        bufs = [ctx.native_empty(nrhs, P, True) for _ in range(3 if kind == "B" else 2)]
+        for j, b in enumerate(bufs[1:]):
+            ctx.fill_spinor_random(b, nrhs, P, 7000 + 10 * i + j, parity_only=True, parity=(0 if (kind == "B" and j == 0) else (0 if kind != "B" else 1)))
+        sets.append(bufs)
+    op = {"A": B.LQ_OP_KERNEL_A, "B": B.LQ_OP_KERNEL_B, "hop": B.LQ_OP_HOP_OE}[kind]
+
+    def launch(i):
+        s = sets[i % nsets]
+        if kind == "B":
+            ctx.apply_native(op, s[0], s[1], nrhs, P, in2=s[2])
+        else:
+            ctx.apply_native(op, s[0], s[1], nrhs, P)
+
+    for i in range(warmup):
+        launch(i)
+    ctx.stream.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(ctx.stream)
+    for i in range(iters):
+        launch(warmup + i)
+    e1.record(ctx.stream)
+    e1.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3 / iters
+    Vh = ctx.V // 2
+    bps = bytes_per_site_rhs(kind, prec, nrhs, recon)
+    flop = {"A": FLOP_A, "B": FLOP_B, "hop": FLOP_HOP}[kind]
+    del sets
+    return dict(kind=kind, prec=prec, nrhs=nrhs, recon=recon, seconds=sec, bytes_per_site_rhs=bps,
+                gbs=bps * Vh * nrhs / sec * 1e-9, gflops=flop * Vh * nrhs / sec * 1e-9, nsets=nsets)
+
+
+def roofline_entry(r, peak, peak_src, traffic=None):
+    return {"bound": "hbm", "kernel": "dslash_kernel<%s,N=%d,recon=%d,form=%s>" % (r["prec"], r["nrhs"], r["recon"], r["kind"]),
+            "achieved": round(r["gbs"], 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+            "frac": round(r["gbs"] / peak, 4), "frac_of_8TBs": round(r["gbs"] / 8000.0, 4), "traffic": traffic,
+            "us_per_launch": round(r["seconds"] * 1e6, 2), "gflops": round(r["gflops"], 1),
+            "algorithmic_bytes_per_site_rhs": r["bytes_per_site_rhs"]}
+
+
+# ------------------------------------------------------------------------------------------------ workloads
+SOLVER_WORKLOADS = {
+    "cfg1": dict(cfg=1, inner="fp32", delta=1e-3, desc="configs[1]: 16^3x32, 8 RHS LapH time/spin-diluted, fp32 inner CG + fp64 defect correction, tol 1e-8"),
+    "cfg3": dict(cfg=3, inner="half", delta=1e-2, desc="configs[3]: 48^3x96, 12 RHS LapH-diluted, int16+norm inner CG, fp32 clover, fp64 outer, tol 1e-9"),
+}
+
+
+def make_sources_host(cfg):
+    c = inputs.CONFIGS[cfg]
+    return inputs.laph_sources(c["dims"], c["nrhs"], c["n_t"], c["source_seed"])
+
+
+def cpu_baseline(cfg_id: int, budget_s: float = 25.0):
+    """The oracle as it stands on the host cores: full even-odd CG solves of single RHS of the workload, as many as fit
+    the time budget (at least one)."""
+    import oracle
+    c = inputs.CONFIGS[cfg_id]
+    dims = c["dims"]
+    if cfg_id == 3:   # a full 48^3x96 oracle solve takes hours: bounded sample on a 16^3x32 sub-volume of the same recipe
+        dims = (16, 16, 16, 32)
+    U = inputs.make_links(dims, c["gauge_seed"], c["eps"])
+    A = oracle.clover(dims, U, c["kappa"], c["csw"])
+    Ainv = oracle.clover_inverse(A)
+    b = inputs.laph_sources(dims, 4, c["n_t"], c["source_seed"])
+    t0 = time.perf_counter()
+    n, its = 0, []
+    while n < 4:
+        x, it, res = oracle.solve_eo(dims, U, A, Ainv, c["kappa"], b[n], c["tol"])
+        its.append(it); n += 1
+        if time.perf_counter() - t0 > budget_s * 0.5:
+            break
+    dt = time.perf_counter() - t0
+    return {"value": dt / n, "unit": "s/RHS", "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": "%d of the workload's RHS solved one at a time by oracle.solve_eo (fp64 CGNR, true residual recomputed every "
+                      "iteration) on %s, tol %g; iterations %s" % (n, "x".join(map(str, dims)), c["tol"], its)}
+
+
+def operator_sweeps(B, device, peak):
+    """configs[2]: 32^3x64 fp32 sweep over N_rhs (kernel A, kernel B, bare hop); configs[4]: 64^3x128, N=4, 12-real links."""
+    import torch
+    out = {"unit": "GB/s (algorithmic bytes / CUDA-event time)", "peak_gbs": peak, "cfg2_32x32x32x64_fp32_recon18": [], "cfg4_64x64x64x128_fp32_recon12": []}
+    for cfg_id, key in ((2, "cfg2_32x32x32x64_fp32_recon18"), (4, "cfg4_64x64x64x128_fp32_recon12")):
+        c = inputs.CONFIGS[cfg_id]
+        ctx = B.Context(c["dims"], device=device)
+        ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=c["recon"])
+        ctx.build_clover(c["kappa"], c["csw"])
+        ns = c["nrhs"] if isinstance(c["nrhs"], tuple) else (c["nrhs"],)
+        for n in ns:
+            for kind in ("A", "B", "hop"):
+                r = time_dslash(ctx, B, kind, "fp32", n, c["recon"], iters=20)
+                out[key].append({"kernel": kind, "nrhs": n, "us": round(r["seconds"] * 1e6, 1), "gbs": round(r["gbs"], 1), "gflops": round(r["gflops"], 1),
+                                 "frac_measured_hbm": round(r["gbs"] / peak, 4), "frac_8TBs": round(r["gbs"] / 8000.0, 4)})
+        ctx.close()
+        torch.cuda.empty_cache()
+    return out
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+def run_reference(args, rank, world):
+    """`--impl reference`: this tier has no reference implementation to install; the arm times the CPU oracle as it stands
+    on the host cores (rank 0 only), on the same config / metric / unit."""
+    if rank != 0:
+        return
+    wl = SOLVER_WORKLOADS[args.workload]
+    c = inputs.CONFIGS[wl["cfg"]]
+    vals = []
+    cb = None
+    for _ in range(max(1, min(args.steps, 2))):
+        cb = cpu_baseline(wl["cfg"], budget_s=20.0)
+        vals.append(cb["value"])
+    v = float(np.mean(vals))
+    line = {"impl": "reference", "metric": "batched CG sec/RHS", "value": v, "unit": "s/RHS", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": v * c["nrhs"] * 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": wl["desc"], "note": "CPU oracle, bounded sample per step"},
+            "cpu_baseline": dict(cb, value=v), "e2e": {"value": v, "unit": "s/RHS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------ main
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg1", choices=sorted(SOLVER_WORKLOADS))
+    ap.add_argument("--no-extras", action="store_true", help="skip the configs[2]/[4] operator sweep and the CPU baseline")
+    ap.add_argument("--no-graph", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1")); local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        return run_reference(args, rank, world)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2510_26313_b200 import binding as B
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    args.warmup = max(args.warmup, 3)
+
+    wl = SOLVER_WORKLOADS[args.workload]
+    c = inputs.CONFIGS[wl["cfg"]]
+    dims, nrhs = c["dims"], c["nrhs"]
+    peak, peak_src, _ = measured_peaks()
+    ctx = B.Context(dims, device=local)
+    if wl["cfg"] == 1:
+        ctx.load_gauge(inputs.make_links(dims, c["gauge_seed"] + rank, c["eps"]), recon=c["recon"])
+    else:
+        ctx.fill_gauge_random(c["gauge_seed"] + rank, c["eps"], recon=c["recon"])
+    ctx.build_clover(c["kappa"], c["csw"])
+    b_host = torch.from_numpy(make_sources_host(wl["cfg"])).pin_memory()
+    x_host = torch.empty_like(b_host).pin_memory()
+    b_dev = b_host.cuda()
+    x_dev = torch.empty_like(b_dev)
+    kw = dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=wl["delta"], check_every=10, use_graph=not args.no_graph)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident steps
+    info = None
+    for _ in range(args.warmup):
+        _, info = ctx.solve(b_dev, x_out=x_dev, **kw)
+    assert info["converged"], info
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = ctx.launches
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(ctx.stream)
+    for _ in range(args.steps):
+        _, info = ctx.solve(b_dev, x_out=x_dev, **kw)
+    e1.record(ctx.stream)
+    barrier()
+    launches = ctx.launches - l0
+    t_dev = e0.elapsed_time(e1) * 1e-3
+    # ---- end to end: host buffers in, host buffers out, through the C ABI
+    ctx.solve(b_host, x_out=x_host, **kw)
+    barrier()
+    w0 = time.perf_counter()
+    for _ in range(args.steps):
+        ctx.solve(b_host, x_out=x_host, **kw)
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - w0
+    clocks = sampler.stop() if sampler else None
+    if world > 1:
+        tt = torch.tensor([t_dev, t_e2e], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_dev, t_e2e = float(tt[0]), float(tt[1])
+
+    # ---- dominant kernel alone (roofline), same lattice and batch
+    rA = time_dslash(ctx, B, "A", "half" if wl["inner"] == "half" else "fp32", nrhs, c["recon"], iters=50)
+    rB = time_dslash(ctx, B, "B", "half" if wl["inner"] == "half" else "fp32", nrhs, c["recon"], iters=50)
+    ws_mb = (7 * ctx.native_bytes(nrhs, B.PREC[wl["inner"]], True) + ctx.V * (4 * c["recon"] + 144) * 4) / 1e6
+    ctx.close()
+    del b_dev, x_dev
+    torch.cuda.empty_cache()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    extras = {}
+    if not args.no_extras and world == 1:
+        extras["dslash"] = operator_sweeps(B, local, peak)
+        extras["cpu_baseline"] = cpu_baseline(wl["cfg"])
+    total_rhs = nrhs * world
+    line = {
+        "metric": "batched CG sec/RHS", "value": t_dev / args.steps / total_rhs, "unit": "s/RHS", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if wl["inner"] == "fp32" else "i16+f32", "data": "synthetic",
+        "config": {"workload": wl["desc"], "lattice": "x".join(map(str, dims)), "nrhs_per_gpu": nrhs, "parallelism": "replicas only (RHS-independent)",
+                   "l2": "working set of one inner iteration (7 inner vectors + fp32 gauge + clover, %.0f MB) exceeds the 126 MB L2; kernel timing rotates buffer sets" % ws_mb,
+                   "cuda_graph": not args.no_graph, "kappa": c["kappa"], "csw": c["csw"], "tol": c["tol"]},
+        "solver": {"outer_cycles": info["outer_cycles"], "inner_iters": info["inner_iters"], "true_rel_residual_max": max(info["true_rel_residual"]),
+                   "dslash_applies_per_step": info["dslash_applies"]},
+        "e2e": {"value": t_e2e / args.steps / total_rhs, "unit": "s/RHS", "h2d_bytes_per_step": b_host.numel() * 16, "d2h_bytes_per_step": x_host.numel() * 16},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "roofline": roofline_entry(rA, peak, peak_src),
+        "roofline_kernel_B": roofline_entry(rB, peak, peak_src),
+    }
+    line.update(extras)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

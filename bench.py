@@ -225,6 +225,28 @@ def run_reference(args, rank, world):
     print(json.dumps(line))
 
 
+# ------------------------------------------------------------------------------------------------ single-operator mode
+def run_op(args, B, device):
+    f = args.op.split(":")
+    cfg_id, kind, prec, n = int(f[0].replace("cfg", "")), f[1], f[2], int(f[3])
+    block = int(f[4]) if len(f) > 4 else 0
+    rpt = int(f[5]) if len(f) > 5 else 0
+    c = inputs.CONFIGS[cfg_id]
+    peak, peak_src, _ = measured_peaks()
+    ctx = B.Context(c["dims"], device=device)
+    ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=c["recon"])
+    ctx.build_clover(c["kappa"], c["csw"])
+    if block or rpt:
+        ctx.set_tuning(block, rpt)
+    sampler = ClockSampler(device)
+    r = time_dslash(ctx, B, kind, prec, n, c["recon"], iters=args.op_iters, warmup=max(args.warmup, 3))
+    clocks = sampler.stop()
+    ctx.close()
+    e = roofline_entry(r, peak, peak_src)
+    e.update({"op": args.op, "lattice": "x".join(map(str, c["dims"])), "iters": args.op_iters, "clocks": clocks})
+    print(json.dumps(e))
+
+
 # ------------------------------------------------------------------------------------------------ main
 def main():
     ap = argparse.ArgumentParser()
@@ -235,6 +257,10 @@ def main():
     ap.add_argument("--workload", default="cfg1", choices=sorted(SOLVER_WORKLOADS))
     ap.add_argument("--no-extras", action="store_true", help="skip the configs[2]/[4] operator sweep and the CPU baseline")
     ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--op", default=None, metavar="CFG:KIND:PREC:N",
+                    help="time ONE stencil kernel only, e.g. cfg2:A:fp32:8 (lattice and links of configs[CFG]; KIND A|B|hop; "
+                         "PREC fp64|fp32|half); optional :block:rpt tuning suffix.  Prints its own JSON line (used for ncu captures)")
+    ap.add_argument("--op-iters", type=int, default=20)
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1")); local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
@@ -246,6 +272,8 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local)
+    if args.op:
+        return run_op(args, B, local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     args.warmup = max(args.warmup, 3)

@@ -163,9 +163,9 @@ typedef struct {
 int lq_solve(lq_ctx* ctx, void* x, const void* b, int nrhs, int loc, int layout, const lq_solve_param* param, lq_solve_info* info);
 
 /* Launch-parameter knobs of the stencil kernels (the paper's autotuning, reduced to an
- * offline sweep): threads per block (0 = default) and right-hand sides per thread (0 = auto: 4 if
- * nrhs % 4 == 0, else 2, else 1; fp64 caps at 2). */
-int lq_set_tuning(lq_ctx* ctx, int dslash_block, int dslash_rpt);
+ * offline sweep): kernel-variant bits (0 = default; see csrc/dslash_launch.cuh) and right-hand sides
+ * per thread (0 = auto: the RHS group width 4 / 2 / 1 of nrhs, fp64 caps at 2; must divide the group width). */
+int lq_set_tuning(lq_ctx* ctx, int dslash_variant, int dslash_rpt);
 
 /* Number of kernels this library has launched on this context since creation (for bench.py). */
 long long lq_kernel_launches(const lq_ctx* ctx);

@@ -150,8 +150,8 @@ class Context:
     def launches(self) -> int:
         return int(self.lib.lq_kernel_launches(self.h))
 
-    def set_tuning(self, dslash_block=0, dslash_rpt=0):
-        self._check(self.lib.lq_set_tuning(self.h, dslash_block, dslash_rpt))
+    def set_tuning(self, dslash_variant=0, dslash_rpt=0):
+        self._check(self.lib.lq_set_tuning(self.h, dslash_variant, dslash_rpt))
 
     # ------------------------------------------------------------------ gauge / clover
     def load_gauge(self, U, recon: int = 18, t_bc: int = -1):

@@ -1,76 +1,58 @@
 // blas.cu -- fused block-BLAS with per-RHS reductions.
 //
-// A native parity block is 24 planes of Vh*N elements with the RHS index innermost, so every kernel here is
-// elementwise over e = cb*N + k.  One thread owns VW = min(N,4) consecutive elements (one site, VW right-hand
-// sides) through all 24 planes (needed for the half format's per-(site,rhs) norm).  Per-RHS sums: fp64
-// accumulators, fixed-shape shared-memory tree over threads with the same RHS group (block size G*2^m,
-// strides multiples of G = N/VW), per-block partials, and a fixed-order final pass by the last block to
-// finish.  Deterministic; results stay on the device.
+// Every kernel here is elementwise over the blocked native layout (common.cuh).  One thread owns one site and VW
+// consecutive right-hand sides of one RHS group (VW = R for fp32/half, min(R,2) for fp64) through all 24 reals
+// (needed for the half format's per-(site,rhs) norm).  A warp lies inside one unit (site block, RHS group), so
+// per-RHS sums are: fp64 accumulators per thread, warp shuffle over the lanes with the same RHS, a fixed-order
+// sum over the block's warps of the same group, per-block partials, and a fixed-order final pass by the last
+// block to finish.  Deterministic; results stay on the device.
 #include "internal.cuh"
-#include "dslash.cuh"
+#include "dslash_kernel.cuh"
 
-template <class S, int VW> struct SiteVec {
-    using T = typename S::comp_t;
-    T v[24][VW];
-    __device__ __forceinline__ void load(const SView<S>& f, size_t plane, size_t e) {
-        T sc[VW];
-        if constexpr (S::has_norm) {
-            float n[VW]; load_norm<VW>(f.n + e, n);
-#pragma unroll
-            for (int k = 0; k < VW; k++) sc[k] = n[k] * (1.0f / 32767.0f);
-        }
-#pragma unroll
-        for (int j = 0; j < 24; j++) {
-            load_comp<S, VW>(f.d + j * plane + e, v[j]);
-            if constexpr (S::has_norm) {
-#pragma unroll
-                for (int k = 0; k < VW; k++) v[j][k] *= sc[k];
-            }
-        }
-    }
-    __device__ __forceinline__ void store(const SView<S>& f, size_t plane, size_t e) const {
-        if constexpr (S::has_norm) {
-            float mx[VW], inv[VW];
-#pragma unroll
-            for (int k = 0; k < VW; k++) mx[k] = 0.f;
-#pragma unroll
-            for (int j = 0; j < 24; j++)
-#pragma unroll
-                for (int k = 0; k < VW; k++) mx[k] = fmaxf(mx[k], fabsf(v[j][k]));
-#pragma unroll
-            for (int k = 0; k < VW; k++) { inv[k] = mx[k] > 0.f ? 32767.0f / mx[k] : 0.f; f.n[e + k] = mx[k]; }
-#pragma unroll
-            for (int j = 0; j < 24; j++) {
-                T q[VW];
-#pragma unroll
-                for (int k = 0; k < VW; k++) q[k] = rintf(v[j][k] * inv[k]);
-                store_comp<S, VW>(f.d + j * plane + e, q);
-            }
-        } else {
-#pragma unroll
-            for (int j = 0; j < 24; j++) store_comp<S, VW>(f.d + j * plane + e, v[j]);
-        }
+template <int VW, int R> struct BlasIdx {
+    static constexpr int TPG = R / VW, UT = SB * TPG, US = 24 * SB * R, UN = SB * R, PL = SB * R;
+    size_t own, own_n;
+    int rhs0;     // first right-hand side of this thread
+    bool valid;
+    __device__ __forceinline__ BlasIdx(const Geom& g, int G) {
+        const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+        const int u = (int)(tid / UT);
+        const int lu = (int)(tid - (long long)u * UT);
+        const int s = lu / TPG, hoff = (lu - s * TPG) * VW;
+        const int blk = u / G, grp = u - blk * G;
+        valid = (u < g.NB * G) && (blk * SB + s < g.Vh);
+        own = (size_t)u * US + s * R + hoff;
+        own_n = (size_t)u * UN + s * R + hoff;
+        rhs0 = grp * R + hoff;
     }
 };
 
-// block tree + last-block final pass.  part[VW] are this thread's sums for RHS (threadIdx % G)*VW + k.
-template <int VW>
+// part[VW] are this thread's sums for right-hand sides rhs0 + k.  Block size must be a multiple of 32.
+template <int VW, int R>
 __device__ void reduce_per_rhs(double (&part)[VW], int N, int G, double* partials, unsigned int* counter, double* out) {
-    extern __shared__ double sm[];
-    const int t = threadIdx.x, nt = blockDim.x;
+    constexpr int TPG = R / VW;
+    extern __shared__ double sm[];       // [max(nwarps * R, blockDim.x)]
+    const int t = threadIdx.x, nt = blockDim.x, lane = t & 31, w = t >> 5, nw = nt >> 5;
 #pragma unroll
-    for (int k = 0; k < VW; k++) sm[t * VW + k] = part[k];
-    __syncthreads();
-    for (int stride = nt >> 1; stride >= G; stride >>= 1) {
-        if (t < stride) {
+    for (int k = 0; k < VW; k++) {
 #pragma unroll
-            for (int k = 0; k < VW; k++) sm[t * VW + k] += sm[(t + stride) * VW + k];
-        }
-        __syncthreads();
+        for (int off = 16; off >= TPG; off >>= 1) part[k] += __shfl_xor_sync(0xffffffffu, part[k], off);
     }
-    if (t < G) {
+    if (lane < TPG) {
 #pragma unroll
-        for (int k = 0; k < VW; k++) partials[(size_t)blockIdx.x * N + t * VW + k] = sm[t * VW + k];
+        for (int k = 0; k < VW; k++) sm[w * R + lane * VW + k] = part[k];
+    }
+    __syncthreads();
+    if (t < N) {
+        // warps of this block whose unit belongs to group t / R, in warp order
+        const long long gw0 = (long long)blockIdx.x * nw;
+        const int grp = t / R, r = t - grp * R;
+        double s = 0.0;
+        for (int ww = 0; ww < nw; ww++) {
+            const long long u = (gw0 + ww) / TPG;
+            if ((int)(u % G) == grp) s += sm[ww * R + r];
+        }
+        partials[(size_t)blockIdx.x * N + t] = s;
     }
     __shared__ bool last;
     __threadfence();
@@ -95,123 +77,125 @@ __device__ void reduce_per_rhs(double (&part)[VW], int N, int G, double* partial
     if (t < N) out[t] = sm[t];
 }
 
-struct BlasGeom { int N, G; long long elems; size_t plane; };
+struct BlasGeom { Geom g; int N, G; };
 
-template <class S, int VW>
+template <class S, int VW, int R>
 __global__ void norm2_kernel(BlasGeom bg, SView<S> x, double* partials, unsigned int* counter, double* out) {
-    const long long e = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * VW;
+    using T = typename S::comp_t;
+    BlasIdx<VW, R> ix(bg.g, bg.G);
     double part[VW];
 #pragma unroll
     for (int k = 0; k < VW; k++) part[k] = 0.0;
-    if (e < bg.elems) {
-        SiteVec<S, VW> a; a.load(x, bg.plane, e);
+    if (ix.valid) {
+        T a[24][VW];
+        load_site_regs<S, VW, R>(x.d + ix.own, S::has_norm ? x.n + ix.own_n : nullptr, a);
 #pragma unroll
         for (int j = 0; j < 24; j++)
 #pragma unroll
-            for (int k = 0; k < VW; k++) part[k] += (double)a.v[j][k] * (double)a.v[j][k];
+            for (int k = 0; k < VW; k++) part[k] += (double)a[j][k] * (double)a[j][k];
     }
-    reduce_per_rhs<VW>(part, bg.N, bg.G, partials, counter, out);
+    reduce_per_rhs<VW, R>(part, bg.N, bg.G, partials, counter, out);
 }
 
-template <class S, int VW>
+template <class S, int VW, int R>
 __global__ void cg_update_xr_kernel(BlasGeom bg, SView<S> x, SView<S> r, SView<S> p, SView<S> q, const double* __restrict__ rr,
                                     const double* __restrict__ pAp, double* partials, unsigned int* counter, double* rr_new) {
     using T = typename S::comp_t;
-    const long long e = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * VW;
+    BlasIdx<VW, R> ix(bg.g, bg.G);
     double part[VW];
 #pragma unroll
     for (int k = 0; k < VW; k++) part[k] = 0.0;
-    if (e < bg.elems) {
-        const int k0 = (int)(e % bg.N);
+    if (ix.valid) {
         T alpha[VW];
 #pragma unroll
-        for (int k = 0; k < VW; k++) { const double d = pAp[k0 + k]; alpha[k] = (T)(d > 0.0 ? rr[k0 + k] / d : 0.0); }
+        for (int k = 0; k < VW; k++) { const double d = pAp[ix.rhs0 + k]; alpha[k] = (T)(d > 0.0 ? rr[ix.rhs0 + k] / d : 0.0); }
         {
-            SiteVec<S, VW> a, b; a.load(x, bg.plane, e); b.load(p, bg.plane, e);
+            T a[24][VW], b[24][VW];
+            load_site_regs<S, VW, R>(x.d + ix.own, S::has_norm ? x.n + ix.own_n : nullptr, a);
+            load_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, b);
 #pragma unroll
             for (int j = 0; j < 24; j++)
 #pragma unroll
-                for (int k = 0; k < VW; k++) a.v[j][k] += alpha[k] * b.v[j][k];
-            a.store(x, bg.plane, e);
+                for (int k = 0; k < VW; k++) a[j][k] += alpha[k] * b[j][k];
+            store_site_regs<S, VW, R>(x.d + ix.own, S::has_norm ? x.n + ix.own_n : nullptr, a);
         }
         {
-            SiteVec<S, VW> a, b; a.load(r, bg.plane, e); b.load(q, bg.plane, e);
+            T a[24][VW], b[24][VW];
+            load_site_regs<S, VW, R>(r.d + ix.own, S::has_norm ? r.n + ix.own_n : nullptr, a);
+            load_site_regs<S, VW, R>(q.d + ix.own, S::has_norm ? q.n + ix.own_n : nullptr, b);
 #pragma unroll
             for (int j = 0; j < 24; j++)
 #pragma unroll
-                for (int k = 0; k < VW; k++) { a.v[j][k] -= alpha[k] * b.v[j][k]; part[k] += (double)a.v[j][k] * (double)a.v[j][k]; }
-            a.store(r, bg.plane, e);
+                for (int k = 0; k < VW; k++) { a[j][k] -= alpha[k] * b[j][k]; part[k] += (double)a[j][k] * (double)a[j][k]; }
+            store_site_regs<S, VW, R>(r.d + ix.own, S::has_norm ? r.n + ix.own_n : nullptr, a);
         }
     }
-    reduce_per_rhs<VW>(part, bg.N, bg.G, partials, counter, rr_new);
+    reduce_per_rhs<VW, R>(part, bg.N, bg.G, partials, counter, rr_new);
 }
 
-template <class S, int VW>
+template <class S, int VW, int R>
 __global__ void cg_update_p_kernel(BlasGeom bg, SView<S> p, SView<S> r, const double* __restrict__ rr_new, const double* __restrict__ rr) {
     using T = typename S::comp_t;
-    const long long e = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * VW;
-    if (e >= bg.elems) return;
-    const int k0 = (int)(e % bg.N);
+    BlasIdx<VW, R> ix(bg.g, bg.G);
+    if (!ix.valid) return;
     T beta[VW];
 #pragma unroll
-    for (int k = 0; k < VW; k++) { const double d = rr[k0 + k]; beta[k] = (T)(d > 0.0 ? rr_new[k0 + k] / d : 0.0); }
-    SiteVec<S, VW> a, b; a.load(p, bg.plane, e); b.load(r, bg.plane, e);
+    for (int k = 0; k < VW; k++) { const double d = rr[ix.rhs0 + k]; beta[k] = (T)(d > 0.0 ? rr_new[ix.rhs0 + k] / d : 0.0); }
+    T a[24][VW], b[24][VW];
+    load_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, a);
+    load_site_regs<S, VW, R>(r.d + ix.own, S::has_norm ? r.n + ix.own_n : nullptr, b);
 #pragma unroll
     for (int j = 0; j < 24; j++)
 #pragma unroll
-        for (int k = 0; k < VW; k++) a.v[j][k] = b.v[j][k] + beta[k] * a.v[j][k];
-    a.store(p, bg.plane, e);
+        for (int k = 0; k < VW; k++) a[j][k] = b[j][k] + beta[k] * a[j][k];
+    store_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, a);
 }
 
 // y (fp64) += s_k * e
-template <class S, int VW>
+template <class S, int VW, int R>
 __global__ void axpy_mixed_kernel(BlasGeom bg, double* __restrict__ y, SView<S> ev, const double* __restrict__ scale) {
-    const long long e = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * VW;
-    if (e >= bg.elems) return;
-    const int k0 = (int)(e % bg.N);
-    SiteVec<S, VW> a; a.load(ev, bg.plane, e);
+    using T = typename S::comp_t;
+    BlasIdx<VW, R> ix(bg.g, bg.G);
+    if (!ix.valid) return;
+    T a[24][VW];
+    load_site_regs<S, VW, R>(ev.d + ix.own, S::has_norm ? ev.n + ix.own_n : nullptr, a);
 #pragma unroll
     for (int j = 0; j < 24; j++)
 #pragma unroll
-        for (int k = 0; k < VW; k++) y[j * bg.plane + e + k] += scale[k0 + k] * (double)a.v[j][k];
+        for (int k = 0; k < VW; k++) y[ix.own + j * ix.PL + k] += scale[ix.rhs0 + k] * (double)a[j][k];
 }
 
 // r = b - t (fp64), per-RHS ||r||^2
-template <int VW>
+template <int VW, int R>
 __global__ void residual_kernel(BlasGeom bg, double* __restrict__ r, const double* __restrict__ b, const double* __restrict__ tv,
                                 double* partials, unsigned int* counter, double* out) {
-    const long long e = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * VW;
+    BlasIdx<VW, R> ix(bg.g, bg.G);
     double part[VW];
 #pragma unroll
     for (int k = 0; k < VW; k++) part[k] = 0.0;
-    if (e < bg.elems) {
+    if (ix.valid) {
 #pragma unroll
         for (int j = 0; j < 24; j++)
 #pragma unroll
             for (int k = 0; k < VW; k++) {
-                const size_t i = j * bg.plane + e + k;
+                const size_t i = ix.own + j * ix.PL + k;
                 const double d = b[i] - tv[i];
                 r[i] = d; part[k] += d * d;
             }
     }
-    reduce_per_rhs<VW>(part, bg.N, bg.G, partials, counter, out);
+    reduce_per_rhs<VW, R>(part, bg.N, bg.G, partials, counter, out);
 }
 
 // ---- host side -----------------------------------------------------------------------------------------------------
-struct Launch { BlasGeom bg; int vw, block, grid; size_t smem; };
+struct Launch { BlasGeom bg; int R, vw, block, grid; size_t smem; };
 static int plan(lq_ctx* c, int nrhs, int maxvw, Launch& L) {
-    int vw = nrhs < 4 ? nrhs : 4;
-    if (vw > maxvw) vw = maxvw;
-    if (nrhs % vw) return set_err(c, LQ_EINVAL, "unsupported nrhs");
-    L.vw = vw;
-    L.bg.N = nrhs; L.bg.G = nrhs / vw; L.bg.elems = (long long)c->g.Vh * nrhs; L.bg.plane = (size_t)c->g.Vh * nrhs;
-    int block = L.bg.G;
-    while (block * 2 <= 256) block *= 2;
-    L.block = block;
-    const long long threads = L.bg.elems / vw;
-    L.grid = (int)((threads + block - 1) / block);
-    L.smem = (size_t)block * vw * sizeof(double);
-    if (L.smem < (size_t)block * sizeof(double)) L.smem = (size_t)block * sizeof(double);
+    const int R = group_width(nrhs);
+    L.R = R; L.vw = R < maxvw ? R : maxvw;
+    L.bg.g = c->g; L.bg.N = nrhs; L.bg.G = nrhs / R;
+    L.block = 128;
+    const long long threads = (long long)c->g.NB * L.bg.G * SB * (R / L.vw);
+    L.grid = (int)((threads + L.block - 1) / L.block);
+    L.smem = (size_t)L.block * sizeof(double);
     if ((size_t)L.grid * nrhs > c->red_partials_elems) {
         if (c->red_partials) dev_free(c, c->red_partials);
         c->red_partials_elems = (size_t)L.grid * nrhs * 2;
@@ -220,21 +204,19 @@ static int plan(lq_ctx* c, int nrhs, int maxvw, Launch& L) {
     }
     return 0;
 }
-#define VW_DISPATCH(L, MAXVW, CALL4, CALL2, CALL1)          \
-    do {                                                       \
-        if (L.vw == 4) { if constexpr (MAXVW >= 4) { CALL4; } } \
-        else if (L.vw == 2) { CALL2; }                        \
-        else { CALL1; }                                        \
+// dispatch on (VW, R): fp32/half (4,4) (2,2) (1,1); fp64 (2,4) (2,2) (1,1)
+#define VW_DISPATCH(L, S, KERNEL, SMEM, ...)                                                                      \
+    do {                                                                                                          \
+        constexpr bool F64K_ = S::prec == LQ_FP64;                                                                \
+        if (L.R == 4) KERNEL<S, (F64K_ ? 2 : 4), 4><<<L.grid, L.block, SMEM, c->stream>>>(__VA_ARGS__);           \
+        else if (L.R == 2) KERNEL<S, 2, 2><<<L.grid, L.block, SMEM, c->stream>>>(__VA_ARGS__);                    \
+        else KERNEL<S, 1, 1><<<L.grid, L.block, SMEM, c->stream>>>(__VA_ARGS__);                                  \
     } while (0)
 
 template <class S> static int norm2_t(lq_ctx* c, int nrhs, const void* x, double* d_out) {
-    constexpr int MAXVW = S::prec == LQ_FP64 ? 2 : 4;
-    Launch L; LQ_TRY(plan(c, nrhs, MAXVW, L));
+    Launch L; LQ_TRY(plan(c, nrhs, S::prec == LQ_FP64 ? 2 : 4, L));
     SView<S> vx = make_view<S>(c->g, const_cast<void*>(x), nrhs, 0);
-    VW_DISPATCH(L, MAXVW,
-        (norm2_kernel<S, MAXVW><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, vx, c->red_partials, c->red_counter, d_out)),
-        (norm2_kernel<S, 2><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, vx, c->red_partials, c->red_counter, d_out)),
-        (norm2_kernel<S, 1><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, vx, c->red_partials, c->red_counter, d_out)));
+    VW_DISPATCH(L, S, norm2_kernel, L.smem, L.bg, vx, c->red_partials, c->red_counter, d_out);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
@@ -246,14 +228,10 @@ int blas_norm2(lq_ctx* c, int prec, int nrhs, const void* x, double* d_out) {
 }
 
 template <class S> static int xr_t(lq_ctx* c, int nrhs, void* x, void* r, const void* p, const void* q, const double* rr, const double* pAp, double* rrn) {
-    constexpr int MAXVW = S::prec == LQ_FP64 ? 2 : 4;
-    Launch L; LQ_TRY(plan(c, nrhs, MAXVW, L));
+    Launch L; LQ_TRY(plan(c, nrhs, S::prec == LQ_FP64 ? 2 : 4, L));
     SView<S> vx = make_view<S>(c->g, x, nrhs, 0), vr = make_view<S>(c->g, r, nrhs, 0);
     SView<S> vp = make_view<S>(c->g, const_cast<void*>(p), nrhs, 0), vq = make_view<S>(c->g, const_cast<void*>(q), nrhs, 0);
-    VW_DISPATCH(L, MAXVW,
-        (cg_update_xr_kernel<S, MAXVW><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, vx, vr, vp, vq, rr, pAp, c->red_partials, c->red_counter, rrn)),
-        (cg_update_xr_kernel<S, 2><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, vx, vr, vp, vq, rr, pAp, c->red_partials, c->red_counter, rrn)),
-        (cg_update_xr_kernel<S, 1><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, vx, vr, vp, vq, rr, pAp, c->red_partials, c->red_counter, rrn)));
+    VW_DISPATCH(L, S, cg_update_xr_kernel, L.smem, L.bg, vx, vr, vp, vq, rr, pAp, c->red_partials, c->red_counter, rrn);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
@@ -265,13 +243,9 @@ int blas_cg_update_xr(lq_ctx* c, int prec, int nrhs, void* x, void* r, const voi
 }
 
 template <class S> static int p_t(lq_ctx* c, int nrhs, void* p, const void* r, const double* rrn, const double* rr) {
-    constexpr int MAXVW = S::prec == LQ_FP64 ? 2 : 4;
-    Launch L; LQ_TRY(plan(c, nrhs, MAXVW, L));
+    Launch L; LQ_TRY(plan(c, nrhs, S::prec == LQ_FP64 ? 2 : 4, L));
     SView<S> vp = make_view<S>(c->g, p, nrhs, 0), vr = make_view<S>(c->g, const_cast<void*>(r), nrhs, 0);
-    VW_DISPATCH(L, MAXVW,
-        (cg_update_p_kernel<S, MAXVW><<<L.grid, L.block, 0, c->stream>>>(L.bg, vp, vr, rrn, rr)),
-        (cg_update_p_kernel<S, 2><<<L.grid, L.block, 0, c->stream>>>(L.bg, vp, vr, rrn, rr)),
-        (cg_update_p_kernel<S, 1><<<L.grid, L.block, 0, c->stream>>>(L.bg, vp, vr, rrn, rr)));
+    VW_DISPATCH(L, S, cg_update_p_kernel, 0, L.bg, vp, vr, rrn, rr);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
@@ -283,13 +257,9 @@ int blas_cg_update_p(lq_ctx* c, int prec, int nrhs, void* p, const void* r, cons
 }
 
 template <class S> static int axpy_t(lq_ctx* c, int nrhs, void* y, const void* e, const double* s) {
-    constexpr int MAXVW = S::prec == LQ_FP64 ? 2 : 4;
-    Launch L; LQ_TRY(plan(c, nrhs, MAXVW, L));
+    Launch L; LQ_TRY(plan(c, nrhs, S::prec == LQ_FP64 ? 2 : 4, L));
     SView<S> ve = make_view<S>(c->g, const_cast<void*>(e), nrhs, 0);
-    VW_DISPATCH(L, MAXVW,
-        (axpy_mixed_kernel<S, MAXVW><<<L.grid, L.block, 0, c->stream>>>(L.bg, (double*)y, ve, s)),
-        (axpy_mixed_kernel<S, 2><<<L.grid, L.block, 0, c->stream>>>(L.bg, (double*)y, ve, s)),
-        (axpy_mixed_kernel<S, 1><<<L.grid, L.block, 0, c->stream>>>(L.bg, (double*)y, ve, s)));
+    VW_DISPATCH(L, S, axpy_mixed_kernel, 0, L.bg, (double*)y, ve, s);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
@@ -302,8 +272,10 @@ int blas_axpy_mixed(lq_ctx* c, int prec, int nrhs, void* y64, const void* e, con
 
 int blas_residual(lq_ctx* c, int nrhs, void* r, const void* b, const void* t, double* d_out) {
     Launch L; LQ_TRY(plan(c, nrhs, 2, L));
-    if (L.vw == 2) residual_kernel<2><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, (double*)r, (const double*)b, (const double*)t, c->red_partials, c->red_counter, d_out);
-    else residual_kernel<1><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, (double*)r, (const double*)b, (const double*)t, c->red_partials, c->red_counter, d_out);
+    double* rp = (double*)r; const double* bp = (const double*)b; const double* tp = (const double*)t;
+    if (L.R == 4) residual_kernel<2, 4><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, rp, bp, tp, c->red_partials, c->red_counter, d_out);
+    else if (L.R == 2) residual_kernel<2, 2><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, rp, bp, tp, c->red_partials, c->red_counter, d_out);
+    else residual_kernel<1, 1><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, rp, bp, tp, c->red_partials, c->red_counter, d_out);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;

@@ -39,7 +39,7 @@ __device__ inline void load_link64(const double* __restrict__ gauge, const Geom&
     int parity, cb;
     coords_to_cb(g, x[0], x[1], x[2], x[3], parity, cb);
     double r[18];
-    load_planes<double, 18>(gauge + (size_t)(parity * 4 + mu) * 18 * g.Vh, g.Vh, cb, r);
+    load_planes<double, 18>(link_block(gauge, g.NB, 18, parity, cb / SB, mu), cb % SB, r);
 #pragma unroll
     for (int k = 0; k < 9; k++) { u.re[k] = r[2 * k]; u.im[k] = r[2 * k + 1]; }
 }
@@ -145,23 +145,23 @@ __global__ void __launch_bounds__(64) clover_build_kernel(Geom g, const double* 
         if (!invert6(mr, mi)) atomicExch(flag, 1);
         pack_block(mr, mi, recinv + 36 * b);
     }
-    store_planes<double, 72>(clov + (size_t)parity * 72 * g.Vh, g.Vh, cb, rec);
-    store_planes<double, 72>(clovinv + (size_t)parity * 72 * g.Vh, g.Vh, cb, recinv);
+    store_planes<double, 72>(clover_block(clov, g.NB, parity, cb / SB), cb % SB, rec);
+    store_planes<double, 72>(clover_block(clovinv, g.NB, parity, cb / SB), cb % SB, recinv);
 }
 
-__global__ void clover_to_fp32_kernel(int Vh, const double* __restrict__ src, float* __restrict__ dst) {
+__global__ void clover_to_fp32_kernel(int Vh, int NB, const double* __restrict__ src, float* __restrict__ dst) {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= 2 * Vh) return;
     const int parity = tid / Vh, cb = tid - parity * Vh;
     double r[72]; float f[72];
-    load_planes<double, 72>(src + (size_t)parity * 72 * Vh, Vh, cb, r);
+    load_planes<double, 72>(clover_block(src, NB, parity, cb / SB), cb % SB, r);
 #pragma unroll
     for (int k = 0; k < 72; k++) f[k] = (float)r[k];
-    store_planes<float, 72>(dst + (size_t)parity * 72 * Vh, Vh, cb, f);
+    store_planes<float, 72>(clover_block(dst, NB, parity, cb / SB), cb % SB, f);
 }
 
 int clover_build(lq_ctx* c, double kappa, double csw) {
-    const size_t n = (size_t)2 * 72 * c->g.Vh;
+    const size_t n = (size_t)2 * 72 * c->g.NB * SB;
     if (!c->clov64) {
         c->clov64 = (double*)dev_alloc(c, n * 8); c->clovinv64 = (double*)dev_alloc(c, n * 8);
         c->clov32 = (float*)dev_alloc(c, n * 4); c->clovinv32 = (float*)dev_alloc(c, n * 4);
@@ -172,9 +172,9 @@ int clover_build(lq_ctx* c, double kappa, double csw) {
     clover_build_kernel<<<(threads + 63) / 64, 64, 0, c->stream>>>(c->g, c->gauge64, kappa * csw, c->clov64, c->clovinv64, c->d_flag);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
-    clover_to_fp32_kernel<<<(threads + 127) / 128, 128, 0, c->stream>>>(c->g.Vh, c->clov64, c->clov32);
+    clover_to_fp32_kernel<<<(threads + 127) / 128, 128, 0, c->stream>>>(c->g.Vh, c->g.NB, c->clov64, c->clov32);
     LQ_LAUNCHED(c);
-    clover_to_fp32_kernel<<<(threads + 127) / 128, 128, 0, c->stream>>>(c->g.Vh, c->clovinv64, c->clovinv32);
+    clover_to_fp32_kernel<<<(threads + 127) / 128, 128, 0, c->stream>>>(c->g.Vh, c->g.NB, c->clovinv64, c->clovinv32);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     int flag = 0;

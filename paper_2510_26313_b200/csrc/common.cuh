@@ -8,10 +8,13 @@
 #include "../../include/lqcd_b200.h"
 
 // ------------------------------------------------------------------ geometry
+constexpr int SB = 32;   // sites per native block (one warp-wide row of every plane)
+
 struct Geom {
     int L[4];      // Lx, Ly, Lz, Lt
     int Lxh;       // Lx / 2
     int Vh;        // sites per parity
+    int NB;        // native site blocks per parity = ceil(Vh / SB); sites cb >= Vh of the last block are padding
     long long V;   // all sites
 };
 
@@ -33,68 +36,98 @@ struct F64 { using store_t = double; using comp_t = double; static constexpr int
 struct F32 { using store_t = float;  using comp_t = float;  static constexpr int prec = LQ_FP32; static constexpr bool has_norm = false; };
 struct H16 { using store_t = short;  using comp_t = float;  static constexpr int prec = LQ_HALF; static constexpr bool has_norm = true; };
 
+// ------------------------------------------------------------------ native spinor layout (one parity, N right-hand sides)
+// The batch is cut into G = N/R groups of R = 4 (N % 4 == 0), 2 (N even) or 1 consecutive right-hand sides and the
+// sites into blocks of SB = 32 consecutive checkerboard sites:
+//     payload[blk][g][j = 0..23][s = 0..31][r = 0..R-1]      real j = 2*(3*spin + colour) + (re|im)
+//     norm   [blk][g][s][r]                                   (half storage only)
+// The RHS index is innermost (BASELINE.json north_star, layout item 1): a thread that owns (site, group) reads one
+// 16-byte vector per real (R = 4, fp32), a warp reads one contiguous 512-byte row, and every row of a neighbour
+// unit sits at a COMPILE-TIME offset j*SB*R from the unit base, so the 24 loads of a neighbour share one address.
+__host__ __device__ inline int group_width(int N) { return (N % 4 == 0) ? 4 : ((N % 2 == 0) ? 2 : 1); }
+
 // one parity of a native spinor batch
 template <class S> struct SView {
-    typename S::store_t* d;   // payload [24][Vh][N]
-    float* n;                 // norms [Vh][N] (H16 only)
+    typename S::store_t* d;   // payload
+    float* n;                 // norms (H16 only)
 };
+// element offset of (rhs k, site cb, real j) in the payload, and of (k, cb) in the norms
+__host__ __device__ inline size_t sp_index(int N, int cb, int k, int j) {
+    const int R = group_width(N), G = N / R;
+    const size_t u = (size_t)(cb / SB) * G + k / R;
+    return (u * 24 + j) * (SB * R) + (size_t)(cb % SB) * R + k % R;
+}
+__host__ __device__ inline size_t nrm_index(int N, int cb, int k) {
+    const int R = group_width(N), G = N / R;
+    const size_t u = (size_t)(cb / SB) * G + k / R;
+    return u * (SB * R) + (size_t)(cb % SB) * R + k % R;
+}
 
 inline size_t elem_bytes(int prec) { return prec == LQ_FP64 ? 8 : (prec == LQ_FP32 ? 4 : 2); }
 inline size_t round256(size_t b) { return (b + 255) & ~size_t(255); }
-// bytes of one parity block of a native spinor batch
+// bytes of one parity block of a native spinor batch (padded to whole site blocks)
 inline size_t parity_bytes(const Geom& g, int nrhs, int prec) {
-    size_t pay = round256((size_t)24 * g.Vh * nrhs * elem_bytes(prec));
-    if (prec == LQ_HALF) pay += round256((size_t)g.Vh * nrhs * sizeof(float));
+    size_t pay = round256((size_t)24 * g.NB * SB * nrhs * elem_bytes(prec));
+    if (prec == LQ_HALF) pay += round256((size_t)g.NB * SB * nrhs * sizeof(float));
     return pay;
 }
 template <class S> inline SView<S> make_view(const Geom& g, void* base, int nrhs, int parity_block) {
     char* p = (char*)base + (size_t)parity_block * parity_bytes(g, nrhs, S::prec);
     SView<S> v;
     v.d = (typename S::store_t*)p;
-    v.n = S::has_norm ? (float*)(p + round256((size_t)24 * g.Vh * nrhs * elem_bytes(S::prec))) : nullptr;
+    v.n = S::has_norm ? (float*)(p + round256((size_t)24 * g.NB * SB * nrhs * elem_bytes(S::prec))) : nullptr;
     return v;
 }
 
-// ------------------------------------------------------------------ vector-plane storage of per-site constants
-// A per-site record of R reals (link: 18 or 12, clover: 72) is stored as planes of VL = 16/sizeof(T)
-// reals: plane q holds reals [q*VL, q*VL+VL) of every site, offset q*VL*Vh + cb*VL; a remainder of
-// R % VL reals (2 for an 18-real fp32 link) forms a last, narrower plane.  All lanes of a warp that
-// work on consecutive sites read consecutive 16-byte vectors; lanes that share a site broadcast.
+// ------------------------------------------------------------------ blocked vector-plane storage of per-site constants
+// A per-site record of R reals (link: 18 or 12, clover: 72) of the SB sites of one block is stored as planes of
+// VL = 16/sizeof(T) reals: plane q holds reals [q*VL, q*VL+VL) of the 32 sites (offset q*VL*SB + s*VL); a remainder
+// of R % VL reals (2 for an 18-real fp32 link) forms a last, narrower plane.  All offsets inside a block are
+// compile-time constants; a warp working on the 32 sites of a block reads 512 contiguous bytes per plane.
+//   gauge : [parity][blk][mu][planes][s]      block of (parity, blk) = 4*RECON*SB reals
+//   clover: [parity][blk][planes][s]          block = 72*SB reals
 template <typename T> struct VecOf;
 template <> struct VecOf<float>  { using v_t = float4;  static constexpr int VL = 4; };
 template <> struct VecOf<double> { using v_t = double2; static constexpr int VL = 2; };
 
 template <typename T, int R>
-__device__ __forceinline__ void load_planes(const T* __restrict__ base, int Vh, int cb, T* out) {
+__device__ __forceinline__ void load_planes(const T* __restrict__ blockbase, int s, T* out) {
     constexpr int VL = VecOf<T>::VL;
     constexpr int NF = R / VL;
     constexpr int REM = R - NF * VL;
 #pragma unroll
     for (int q = 0; q < NF; q++) {
         if constexpr (VL == 4) {
-            float4 v = __ldg(reinterpret_cast<const float4*>(base + (size_t)q * 4 * Vh) + cb);
+            float4 v = __ldg(reinterpret_cast<const float4*>(blockbase + q * 4 * SB) + s);
             out[4 * q] = v.x; out[4 * q + 1] = v.y; out[4 * q + 2] = v.z; out[4 * q + 3] = v.w;
         } else {
-            double2 v = __ldg(reinterpret_cast<const double2*>(base + (size_t)q * 2 * Vh) + cb);
+            double2 v = __ldg(reinterpret_cast<const double2*>(blockbase + q * 2 * SB) + s);
             out[2 * q] = v.x; out[2 * q + 1] = v.y;
         }
     }
     if constexpr (REM == 2) {
-        float2 v = __ldg(reinterpret_cast<const float2*>(base + (size_t)NF * VL * Vh) + cb);
+        float2 v = __ldg(reinterpret_cast<const float2*>(blockbase + NF * VL * SB) + s);
         out[NF * VL] = v.x; out[NF * VL + 1] = v.y;
     }
 }
 template <typename T, int R>
-__device__ __forceinline__ void store_planes(T* __restrict__ base, int Vh, int cb, const T* in) {
+__device__ __forceinline__ void store_planes(T* __restrict__ blockbase, int s, const T* in) {
     constexpr int VL = VecOf<T>::VL;
     constexpr int NF = R / VL;
     constexpr int REM = R - NF * VL;
 #pragma unroll
     for (int q = 0; q < NF; q++)
 #pragma unroll
-        for (int e = 0; e < VL; e++) base[(size_t)q * VL * Vh + (size_t)cb * VL + e] = in[q * VL + e];
+        for (int e = 0; e < VL; e++) blockbase[q * VL * SB + s * VL + e] = in[q * VL + e];
 #pragma unroll
-    for (int e = 0; e < REM; e++) base[(size_t)NF * VL * Vh + (size_t)cb * REM + e] = in[NF * VL + e];
+    for (int e = 0; e < REM; e++) blockbase[NF * VL * SB + s * REM + e] = in[NF * VL + e];
+}
+// base of the link block of (parity, site block, mu) / of the clover block of (parity, site block)
+template <typename T> __host__ __device__ inline T* link_block(T* gauge, int NB, int recon, int parity, int blk, int mu) {
+    return gauge + ((size_t)(parity * NB + blk) * 4 + mu) * (size_t)(recon * SB);
+}
+template <typename T> __host__ __device__ inline T* clover_block(T* clov, int NB, int parity, int blk) {
+    return clov + (size_t)(parity * NB + blk) * (size_t)(72 * SB);
 }
 
 // ------------------------------------------------------------------ context
@@ -103,11 +136,11 @@ struct lq_ctx {
     int device;
     cudaStream_t stream;
     int t_bc;
-    // gauge: [parity][mu] blocks of R*Vh reals
+    // gauge: [parity][blk][mu] blocks of R*SB reals
     double* gauge64;  // R = 18
     float* gauge32;   // R = recon32
     int recon32;
-    // clover: [parity] blocks of 72*Vh reals; A and A^{-1}
+    // clover: [parity][blk] blocks of 72*SB reals; A and A^{-1}
     double *clov64, *clovinv64;
     float *clov32, *clovinv32;
     double kappa, csw;
@@ -117,6 +150,7 @@ struct lq_ctx {
     long long launches;
     int dslash_block;               // tuning knob (0 = default)
     int dslash_rpt;                 // tuning knob (0 = auto)
+    int dslash_variant;             // tuning knob: kernel variant bits (0 = default)
     std::string err;
     // reduction scratch
     double* red_partials; size_t red_partials_elems;
@@ -137,5 +171,3 @@ void dev_free(lq_ctx* c, void* p);
 #define LQ_TRY(x) do { int r_ = (x); if (r_ != 0) return r_; } while (0)
 #define LQ_LAUNCHED(ctx) do { (ctx)->launches++; } while (0)
 
-inline const double* gauge64_block(const lq_ctx* c, int parity, int mu) { return c->gauge64 + ((size_t)(parity * 4 + mu)) * 18 * c->g.Vh; }
-inline const float* gauge32_block(const lq_ctx* c, int parity, int mu) { return c->gauge32 + ((size_t)(parity * 4 + mu)) * c->recon32 * c->g.Vh; }

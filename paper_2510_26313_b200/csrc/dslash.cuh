@@ -6,13 +6,17 @@
 // with D replaced by g5 D g5 when dsign = -1 (dagger, row a5: only the projector signs flip because the
 // clover blocks commute with g5 = diag(1,1,-1,-1)).
 //
-// One thread owns one output site and RPT consecutive right-hand sides; the N/RPT threads of a site are
-// adjacent lanes, so a warp reads each of the 24 real planes of a neighbour as one contiguous run
-// (RHS index innermost) and the link / clover loads of a site are shared by its lanes and reused in
-// registers across the thread's RPT right-hand sides (the paper's stencil-coefficient reuse).
-// Spin projection uses the DeGrand-Rossi rank-2 structure of (1 -+ gamma_mu); boundaries are wrapped
-// in-kernel and the antiperiodic sign multiplies the hopped term (never the stored link, so 12-real
-// reconstruction stays valid).
+// Thread mapping on the blocked native layout (common.cuh): a "unit" is (site block of 32 sites, RHS group of
+// R right-hand sides).  One thread owns one output site and RPT consecutive right-hand sides of the group
+// (RPT divides R; R/RPT adjacent lanes share a site).  With RPT = R = 4 (fp32) a warp is exactly one unit: every
+// real of a neighbour is one 16-byte load per lane, 512 contiguous bytes per warp, at a compile-time offset from
+// ONE per-neighbour address; the link and the clover block of the site are loaded once per thread as 16-byte
+// vectors and reused in registers across the thread's right-hand sides (the paper's stencil-coefficient reuse,
+// PAPER.md L136); the other RHS groups of the same sites run in adjacent warps and find the links in L1.
+// All complex arithmetic is written as explicit fused multiply-adds (1128 FP instructions per site per RHS for
+// kernel A: 8 x (12 project + 72 SU(3) + 24 accumulate) + 264 clover).  Spin projection uses the DeGrand-Rossi
+// rank-2 structure of (1 -+ gamma_mu); boundaries are wrapped in-kernel and the antiperiodic sign multiplies the
+// hopped term (never the stored link, so 12-real reconstruction stays valid).
 #pragma once
 #include "common.cuh"
 
@@ -22,16 +26,19 @@ template <class S> struct DslashArgs {
     using T = typename S::comp_t;
     Geom g;
     int parity;            // parity of the output sites
-    int N, G;              // right-hand sides, lanes per site (N / RPT)
+    int N, G;              // right-hand sides, RHS groups (N / R)
     SView<S> out, in, x;   // out / x on `parity`, in on 1-parity
-    const T* gauge;        // [parity][mu] blocks of RECON*Vh reals
-    const T* clover;       // 72*Vh reals of the output parity, or nullptr (identity)
+    const T* gauge;        // [parity][blk][mu] blocks of RECON*SB reals
+    const T* clover;       // [blk] blocks of 72*SB reals of the output parity, or nullptr (identity)
     T coef;                // FORM_B
     T tsign;               // t_bc
     T dsign;               // +1, -1 = dagger
 };
 
-// ---- RPT-wide loads / stores of one real plane ------------------------------------------------------
+__device__ __forceinline__ float fm(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fm(double a, double b, double c) { return fma(a, b, c); }
+
+// ---- RPT-wide loads / stores of one real of one site ------------------------------------------------
 template <class S, int RPT>
 __device__ __forceinline__ void load_comp(const typename S::store_t* __restrict__ p, typename S::comp_t* o) {
     if constexpr (S::prec == LQ_FP32) {
@@ -39,7 +46,10 @@ __device__ __forceinline__ void load_comp(const typename S::store_t* __restrict_
         else if constexpr (RPT == 2) { float2 v = __ldg((const float2*)p); o[0] = v.x; o[1] = v.y; }
         else { o[0] = __ldg(p); }
     } else if constexpr (S::prec == LQ_FP64) {
-        if constexpr (RPT == 2) { double2 v = __ldg((const double2*)p); o[0] = v.x; o[1] = v.y; }
+        if constexpr (RPT == 4) {
+            double2 v = __ldg((const double2*)p), w = __ldg((const double2*)p + 1);
+            o[0] = v.x; o[1] = v.y; o[2] = w.x; o[3] = w.y;
+        } else if constexpr (RPT == 2) { double2 v = __ldg((const double2*)p); o[0] = v.x; o[1] = v.y; }
         else { o[0] = __ldg(p); }
     } else {
         if constexpr (RPT == 4) { short4 v = __ldg((const short4*)p); o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
@@ -52,6 +62,11 @@ template <int RPT> __device__ __forceinline__ void load_norm(const float* __rest
     else if constexpr (RPT == 2) { float2 v = __ldg((const float2*)p); o[0] = v.x; o[1] = v.y; }
     else { o[0] = __ldg(p); }
 }
+template <int RPT> __device__ __forceinline__ void store_norm(float* __restrict__ p, const float* o) {
+    if constexpr (RPT == 4) *(float4*)p = make_float4(o[0], o[1], o[2], o[3]);
+    else if constexpr (RPT == 2) *(float2*)p = make_float2(o[0], o[1]);
+    else *p = o[0];
+}
 template <class S, int RPT>
 __device__ __forceinline__ void store_comp(typename S::store_t* __restrict__ p, const typename S::comp_t* o) {
     if constexpr (S::prec == LQ_FP32) {
@@ -59,7 +74,8 @@ __device__ __forceinline__ void store_comp(typename S::store_t* __restrict__ p, 
         else if constexpr (RPT == 2) *(float2*)p = make_float2(o[0], o[1]);
         else *p = o[0];
     } else if constexpr (S::prec == LQ_FP64) {
-        if constexpr (RPT == 2) *(double2*)p = make_double2(o[0], o[1]);
+        if constexpr (RPT == 4) { *(double2*)p = make_double2(o[0], o[1]); *((double2*)p + 1) = make_double2(o[2], o[3]); }
+        else if constexpr (RPT == 2) *(double2*)p = make_double2(o[0], o[1]);
         else *p = o[0];
     } else {
         if constexpr (RPT == 4) *(short4*)p = make_short4((short)o[0], (short)o[1], (short)o[2], (short)o[3]);
@@ -70,15 +86,21 @@ __device__ __forceinline__ void store_comp(typename S::store_t* __restrict__ p, 
 
 // ---- link load (+ 12-real reconstruction: third row = conj(row0 x row1)) -----------------------------
 template <typename T, int RECON>
-__device__ __forceinline__ void load_link(const T* __restrict__ blk, int Vh, int cb, T* u) {
-    load_planes<T, RECON>(blk, Vh, cb, u);
+__device__ __forceinline__ void load_link(const T* __restrict__ blockbase, int s, T* u) {
+    load_planes<T, RECON>(blockbase, s, u);
     if constexpr (RECON == 12) {
 #pragma unroll
         for (int c = 0; c < 3; c++) {
             const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
             // (a x b)_c = a_c1 b_c2 - a_c2 b_c1, conjugated
-            T re = u[2 * c1] * u[6 + 2 * c2] - u[2 * c1 + 1] * u[6 + 2 * c2 + 1] - (u[2 * c2] * u[6 + 2 * c1] - u[2 * c2 + 1] * u[6 + 2 * c1 + 1]);
-            T im = u[2 * c1] * u[6 + 2 * c2 + 1] + u[2 * c1 + 1] * u[6 + 2 * c2] - (u[2 * c2] * u[6 + 2 * c1 + 1] + u[2 * c2 + 1] * u[6 + 2 * c1]);
+            T re = u[2 * c1] * u[6 + 2 * c2];
+            re = fm(-u[2 * c1 + 1], u[6 + 2 * c2 + 1], re);
+            re = fm(-u[2 * c2], u[6 + 2 * c1], re);
+            re = fm(u[2 * c2 + 1], u[6 + 2 * c1 + 1], re);
+            T im = u[2 * c1] * u[6 + 2 * c2 + 1];
+            im = fm(u[2 * c1 + 1], u[6 + 2 * c2], im);
+            im = fm(-u[2 * c2], u[6 + 2 * c1 + 1], im);
+            im = fm(-u[2 * c2 + 1], u[6 + 2 * c1], im);
             u[12 + 2 * c] = re; u[12 + 2 * c + 1] = -im;
         }
     }
@@ -86,18 +108,20 @@ __device__ __forceinline__ void load_link(const T* __restrict__ blk, int Vh, int
 
 // ---- one of the eight hopping terms -------------------------------------------------------------------
 // acc[j][k] += cu * (1 - sigma*gamma_MU) W psi(nb),  W = U (FWD) or U^dag (backward), sigma = +-1.
-template <class S, int RPT, int RECON, int MU, bool FWD>
-__device__ __forceinline__ void hop_dir(const DslashArgs<S>& a, int nb_cb, const typename S::comp_t* __restrict__ link_blk, int link_cb,
-                                        typename S::comp_t cu, typename S::comp_t sigma, int goff, typename S::comp_t (&acc)[24][RPT]) {
+// `nb` points at real 0 of the neighbour's RPT right-hand sides; real j is at nb + j*SB*R.
+template <class S, int RPT, int R, int RECON, int MU, bool FWD>
+__device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ nb, const float* __restrict__ nb_norm,
+                                        const typename S::comp_t* __restrict__ link_blk, int link_s,
+                                        typename S::comp_t cu, typename S::comp_t sigma, typename S::comp_t (&acc)[24][RPT]) {
     using T = typename S::comp_t;
-    const int Vh = a.g.Vh, N = a.N;
+    constexpr int PL = SB * R;   // elements between consecutive reals of a site
     T u[18];
-    load_link<T, RECON>(link_blk, Vh, link_cb, u);
+    load_link<T, RECON>(link_blk, link_s, u);
 
     T cuk[RPT], clk[RPT];
     if constexpr (S::has_norm) {
         float nrm[RPT];
-        load_norm<RPT>(a.in.n + (size_t)nb_cb * N + goff, nrm);
+        load_norm<RPT>(nb_norm, nrm);
 #pragma unroll
         for (int k = 0; k < RPT; k++) cuk[k] = cu * nrm[k] * (1.0f / 32767.0f);
     } else {
@@ -109,29 +133,27 @@ __device__ __forceinline__ void hop_dir(const DslashArgs<S>& a, int nb_cb, const
 
     // projected half spinor h[s][c][ri][k]
     T h[2][3][2][RPT];
-    const typename S::store_t* base = a.in.d + (size_t)nb_cb * N + goff;
-    const size_t plane = (size_t)Vh * N;
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         T p[4][2][RPT];
 #pragma unroll
         for (int s = 0; s < 4; s++)
 #pragma unroll
-            for (int ri = 0; ri < 2; ri++) load_comp<S, RPT>(base + (size_t)(2 * (3 * s + c) + ri) * plane, p[s][ri]);
+            for (int ri = 0; ri < 2; ri++) load_comp<S, RPT>(nb + (2 * (3 * s + c) + ri) * PL, p[s][ri]);
 #pragma unroll
         for (int k = 0; k < RPT; k++) {
             if constexpr (MU == 0) {        // h0 = p0 - s i p3, h1 = p1 - s i p2
-                h[0][c][0][k] = p[0][0][k] + sigma * p[3][1][k]; h[0][c][1][k] = p[0][1][k] - sigma * p[3][0][k];
-                h[1][c][0][k] = p[1][0][k] + sigma * p[2][1][k]; h[1][c][1][k] = p[1][1][k] - sigma * p[2][0][k];
+                h[0][c][0][k] = fm(sigma, p[3][1][k], p[0][0][k]);  h[0][c][1][k] = fm(-sigma, p[3][0][k], p[0][1][k]);
+                h[1][c][0][k] = fm(sigma, p[2][1][k], p[1][0][k]);  h[1][c][1][k] = fm(-sigma, p[2][0][k], p[1][1][k]);
             } else if constexpr (MU == 1) { // h0 = p0 + s p3, h1 = p1 - s p2
-                h[0][c][0][k] = p[0][0][k] + sigma * p[3][0][k]; h[0][c][1][k] = p[0][1][k] + sigma * p[3][1][k];
-                h[1][c][0][k] = p[1][0][k] - sigma * p[2][0][k]; h[1][c][1][k] = p[1][1][k] - sigma * p[2][1][k];
+                h[0][c][0][k] = fm(sigma, p[3][0][k], p[0][0][k]);  h[0][c][1][k] = fm(sigma, p[3][1][k], p[0][1][k]);
+                h[1][c][0][k] = fm(-sigma, p[2][0][k], p[1][0][k]); h[1][c][1][k] = fm(-sigma, p[2][1][k], p[1][1][k]);
             } else if constexpr (MU == 2) { // h0 = p0 - s i p2, h1 = p1 + s i p3
-                h[0][c][0][k] = p[0][0][k] + sigma * p[2][1][k]; h[0][c][1][k] = p[0][1][k] - sigma * p[2][0][k];
-                h[1][c][0][k] = p[1][0][k] - sigma * p[3][1][k]; h[1][c][1][k] = p[1][1][k] + sigma * p[3][0][k];
+                h[0][c][0][k] = fm(sigma, p[2][1][k], p[0][0][k]);  h[0][c][1][k] = fm(-sigma, p[2][0][k], p[0][1][k]);
+                h[1][c][0][k] = fm(-sigma, p[3][1][k], p[1][0][k]); h[1][c][1][k] = fm(sigma, p[3][0][k], p[1][1][k]);
             } else {                        // h0 = p0 - s p2, h1 = p1 - s p3
-                h[0][c][0][k] = p[0][0][k] - sigma * p[2][0][k]; h[0][c][1][k] = p[0][1][k] - sigma * p[2][1][k];
-                h[1][c][0][k] = p[1][0][k] - sigma * p[3][0][k]; h[1][c][1][k] = p[1][1][k] - sigma * p[3][1][k];
+                h[0][c][0][k] = fm(-sigma, p[2][0][k], p[0][0][k]); h[0][c][1][k] = fm(-sigma, p[2][1][k], p[0][1][k]);
+                h[1][c][0][k] = fm(-sigma, p[3][0][k], p[1][0][k]); h[1][c][1][k] = fm(-sigma, p[3][1][k], p[1][1][k]);
             }
         }
     }
@@ -142,49 +164,49 @@ __device__ __forceinline__ void hop_dir(const DslashArgs<S>& a, int nb_cb, const
         for (int r = 0; r < 3; r++) {
             T wr[RPT], wi[RPT];
 #pragma unroll
-            for (int k = 0; k < RPT; k++) { wr[k] = 0; wi[k] = 0; }
-#pragma unroll
             for (int c = 0; c < 3; c++) {
                 // FWD: U[r][c];  backward: conj(U[c][r])
                 const T ur = FWD ? u[2 * (3 * r + c)] : u[2 * (3 * c + r)];
                 const T ui = FWD ? u[2 * (3 * r + c) + 1] : -u[2 * (3 * c + r) + 1];
 #pragma unroll
                 for (int k = 0; k < RPT; k++) {
-                    wr[k] += ur * h[s][c][0][k] - ui * h[s][c][1][k];
-                    wi[k] += ur * h[s][c][1][k] + ui * h[s][c][0][k];
+                    if (c == 0) { wr[k] = ur * h[s][c][0][k]; wi[k] = ur * h[s][c][1][k]; }
+                    else { wr[k] = fm(ur, h[s][c][0][k], wr[k]); wi[k] = fm(ur, h[s][c][1][k], wi[k]); }
+                    wr[k] = fm(-ui, h[s][c][1][k], wr[k]);
+                    wi[k] = fm(ui, h[s][c][0][k], wi[k]);
                 }
             }
             // upper spin rows: acc_s += cu w_s
             const int ju = 2 * (3 * s + r);
 #pragma unroll
-            for (int k = 0; k < RPT; k++) { acc[ju][k] += cuk[k] * wr[k]; acc[ju + 1][k] += cuk[k] * wi[k]; }
+            for (int k = 0; k < RPT; k++) { acc[ju][k] = fm(cuk[k], wr[k], acc[ju][k]); acc[ju + 1][k] = fm(cuk[k], wi[k], acc[ju + 1][k]); }
             // lower spin rows (reconstruction)
             if constexpr (MU == 0) {        // row2 = (s i) w1, row3 = (s i) w0
                 const int jl = 2 * (3 * (3 - s) + r);
 #pragma unroll
-                for (int k = 0; k < RPT; k++) { acc[jl][k] -= clk[k] * wi[k]; acc[jl + 1][k] += clk[k] * wr[k]; }
+                for (int k = 0; k < RPT; k++) { acc[jl][k] = fm(-clk[k], wi[k], acc[jl][k]); acc[jl + 1][k] = fm(clk[k], wr[k], acc[jl + 1][k]); }
             } else if constexpr (MU == 1) { // row2 = -s w1, row3 = +s w0
                 const int jl = 2 * (3 * (3 - s) + r);
                 if (s == 0) {
 #pragma unroll
-                    for (int k = 0; k < RPT; k++) { acc[jl][k] += clk[k] * wr[k]; acc[jl + 1][k] += clk[k] * wi[k]; }
+                    for (int k = 0; k < RPT; k++) { acc[jl][k] = fm(clk[k], wr[k], acc[jl][k]); acc[jl + 1][k] = fm(clk[k], wi[k], acc[jl + 1][k]); }
                 } else {
 #pragma unroll
-                    for (int k = 0; k < RPT; k++) { acc[jl][k] -= clk[k] * wr[k]; acc[jl + 1][k] -= clk[k] * wi[k]; }
+                    for (int k = 0; k < RPT; k++) { acc[jl][k] = fm(-clk[k], wr[k], acc[jl][k]); acc[jl + 1][k] = fm(-clk[k], wi[k], acc[jl + 1][k]); }
                 }
             } else if constexpr (MU == 2) { // row2 = (s i) w0, row3 = -(s i) w1
                 const int jl = 2 * (3 * (2 + s) + r);
                 if (s == 0) {
 #pragma unroll
-                    for (int k = 0; k < RPT; k++) { acc[jl][k] -= clk[k] * wi[k]; acc[jl + 1][k] += clk[k] * wr[k]; }
+                    for (int k = 0; k < RPT; k++) { acc[jl][k] = fm(-clk[k], wi[k], acc[jl][k]); acc[jl + 1][k] = fm(clk[k], wr[k], acc[jl + 1][k]); }
                 } else {
 #pragma unroll
-                    for (int k = 0; k < RPT; k++) { acc[jl][k] += clk[k] * wi[k]; acc[jl + 1][k] -= clk[k] * wr[k]; }
+                    for (int k = 0; k < RPT; k++) { acc[jl][k] = fm(clk[k], wi[k], acc[jl][k]); acc[jl + 1][k] = fm(-clk[k], wr[k], acc[jl + 1][k]); }
                 }
             } else {                        // row2 = -s w0, row3 = -s w1
                 const int jl = 2 * (3 * (2 + s) + r);
 #pragma unroll
-                for (int k = 0; k < RPT; k++) { acc[jl][k] -= clk[k] * wr[k]; acc[jl + 1][k] -= clk[k] * wi[k]; }
+                for (int k = 0; k < RPT; k++) { acc[jl][k] = fm(-clk[k], wr[k], acc[jl][k]); acc[jl + 1][k] = fm(-clk[k], wi[k], acc[jl + 1][k]); }
             }
         }
 }

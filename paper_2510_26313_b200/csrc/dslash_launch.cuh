@@ -1,32 +1,50 @@
-// dslash_launch.cuh -- launcher body; each dslash_*.cu instantiates it for one storage type.
+// dslash_launch.cuh -- launcher body; each dslash_*.cu instantiates it for one (storage type, link reals, form).
 #pragma once
 #include "dslash_kernel.cuh"
 
-template <class S, int RPT, int RECON, int FORM>
-static int launch_one(lq_ctx* c, DslashArgs<S> a, int block) {
-    a.G = a.N / RPT;
-    const long long threads = (long long)a.g.Vh * a.G;
-    const int grid = (int)((threads + block - 1) / block);
-    dslash_kernel<S, RPT, RECON, FORM><<<grid, block, 0, c->stream>>>(a);
+template <class S, int RPT, int R, int RECON, int FORM, int MINB>
+static int launch_one(lq_ctx* c, DslashArgs<S> a) {
+    constexpr int BLOCK = 128;
+    a.G = a.N / R;
+    const long long threads = (long long)a.g.NB * a.G * SB * (R / RPT);
+    const int grid = (int)((threads + BLOCK - 1) / BLOCK);
+    dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB><<<grid, BLOCK, 0, c->stream>>>(a);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
 
-template <class S, int RECON, int FORM>
-int launch_dslash(lq_ctx* c, DslashArgs<S> a, int rpt_override) {
-    constexpr int MAXRPT = (S::prec == LQ_FP64) ? 2 : 4;
-    int rpt = rpt_override > 0 ? rpt_override : ((a.N % 4 == 0) ? 4 : ((a.N % 2 == 0) ? 2 : 1));
-    if (rpt > MAXRPT) rpt = MAXRPT;
-    if (a.N % rpt != 0) return set_err(c, LQ_EINVAL, "nrhs not divisible by rhs-per-thread");
-    const int block = c->dslash_block > 0 ? c->dslash_block : 128;
-    if (rpt == 1) return launch_one<S, 1, RECON, FORM>(c, a, block);
-    if (rpt == 2) return launch_one<S, 2, RECON, FORM>(c, a, block);
-    if constexpr (MAXRPT == 4) { if (rpt == 4) return launch_one<S, 4, RECON, FORM>(c, a, block); }
-    return set_err(c, LQ_EINVAL, "bad rhs-per-thread");
+// Register budget per thread = 65536 / (128 * MINB): MINB 2 -> 255, 3 -> 168, 4 -> 128, 5 -> 96 (rounded by ptxas).
+// `variant` bit 0 selects the alternative budget (fp32 only; a tuning knob for profiling runs).
+template <class S, int RPT, int R, int RECON, int FORM>
+static int launch_rpt(lq_ctx* c, DslashArgs<S> a, int variant) {
+    constexpr bool F64K = S::prec == LQ_FP64;
+    constexpr int DEF = F64K ? (RPT == 2 ? 2 : 3) : (RPT == 4 ? 2 : (RPT == 2 ? 3 : 4));
+    if constexpr (S::prec == LQ_FP32) {
+        constexpr int ALT = RPT == 4 ? 3 : (RPT == 2 ? 4 : 5);
+        if (variant & 1) return launch_one<S, RPT, R, RECON, FORM, ALT>(c, a);
+    }
+    return launch_one<S, RPT, R, RECON, FORM, DEF>(c, a);
 }
 
-#define INSTANTIATE_DSLASH(S, RECON)                                                   \
-    template int launch_dslash<S, RECON, FORM_HOP>(lq_ctx*, DslashArgs<S>, int);       \
-    template int launch_dslash<S, RECON, FORM_A>(lq_ctx*, DslashArgs<S>, int);         \
-    template int launch_dslash<S, RECON, FORM_B>(lq_ctx*, DslashArgs<S>, int);
+template <class S, int RECON, int FORM>
+int launch_dslash(lq_ctx* c, DslashArgs<S> a, int rpt, int variant) {
+    constexpr int MAXRPT = (S::prec == LQ_FP64) ? 2 : 4;
+    const int R = group_width(a.N);
+    if (rpt <= 0) rpt = R;
+    if (rpt > MAXRPT) rpt = MAXRPT;
+    if (rpt > R) rpt = R;
+    if (R % rpt != 0) return set_err(c, LQ_EINVAL, "rhs-per-thread must divide the RHS group width");
+    if (R == 4) {
+        if constexpr (MAXRPT == 4) { if (rpt == 4) return launch_rpt<S, 4, 4, RECON, FORM>(c, a, variant); }
+        if (rpt == 2) return launch_rpt<S, 2, 4, RECON, FORM>(c, a, variant);
+        return launch_rpt<S, 1, 4, RECON, FORM>(c, a, variant);
+    }
+    if (R == 2) {
+        if (rpt == 2) return launch_rpt<S, 2, 2, RECON, FORM>(c, a, variant);
+        return launch_rpt<S, 1, 2, RECON, FORM>(c, a, variant);
+    }
+    return launch_rpt<S, 1, 1, RECON, FORM>(c, a, variant);
+}
+
+#define INSTANTIATE_DSLASH(S, RECON, FORM) template int launch_dslash<S, RECON, FORM>(lq_ctx*, DslashArgs<S>, int, int);

@@ -56,7 +56,7 @@ __global__ void fill_gauge_kernel(Geom g, uint64_t key, double eps, double* __re
     }
     double r[18];
     for (int e = 0; e < 9; e++) { r[2 * e] = wr[e]; r[2 * e + 1] = wi[e]; }
-    store_planes<double, 18>(native + (size_t)pm * 18 * g.Vh, g.Vh, cb, r);
+    store_planes<double, 18>(link_block(native, g.NB, 18, parity, cb / SB, mu), cb % SB, r);
 }
 int fill_gauge(lq_ctx* c, uint64_t seed, double eps) {
     const long long threads = 8LL * c->g.Vh;
@@ -82,11 +82,11 @@ __global__ void fill_spinor_kernel(Geom g, int N, uint64_t key, SView<S> even, S
     double o[24];
     for (int e = 0; e < 12; e++) cgauss(key, ((uint64_t)k * (uint64_t)g.V + site) * 12 + e, o[2 * e], o[2 * e + 1]);
     const SView<S>& v = (only || parity == 0) ? even : odd;
-    const size_t plane = (size_t)g.Vh * N, off = (size_t)cb * N + k;
+    const size_t plane = (size_t)SB * group_width(N), off = sp_index(N, cb, k, 0);
     if constexpr (S::has_norm) {
         float mx = 0.f;
         for (int j = 0; j < 24; j++) mx = fmaxf(mx, fabsf((float)o[j]));
-        v.n[off] = mx;
+        v.n[nrm_index(N, cb, k)] = mx;
         const float inv = mx > 0.f ? 32767.0f / mx : 0.f;
         for (int j = 0; j < 24; j++) v.d[j * plane + off] = (short)rintf((float)o[j] * inv);
     } else {

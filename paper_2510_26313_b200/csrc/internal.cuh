@@ -5,7 +5,7 @@
 
 // dslash_*.cu
 template <class S, int RECON, int FORM>
-int launch_dslash(lq_ctx* c, DslashArgs<S> a, int rpt_override);
+int launch_dslash(lq_ctx* c, DslashArgs<S> a, int rpt, int variant);
 
 // ops.cu : typed single-parity building blocks on native fields
 // out(parity) = [C] D in(1-parity) ; form A uses A^{-1}, form HOP nothing

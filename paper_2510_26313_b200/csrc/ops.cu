@@ -18,16 +18,16 @@ static DslashArgs<S> base_args(lq_ctx* c, int nrhs, int out_parity, void* out, c
 
 template <class S, int FORM>
 static int run_form(lq_ctx* c, DslashArgs<S> a) {
-    if constexpr (S::prec == LQ_FP64) return launch_dslash<S, 18, FORM>(c, a, c->dslash_rpt);
+    if constexpr (S::prec == LQ_FP64) return launch_dslash<S, 18, FORM>(c, a, c->dslash_rpt, c->dslash_variant);
     else {
-        if (c->recon32 == 12) return launch_dslash<S, 12, FORM>(c, a, c->dslash_rpt);
-        return launch_dslash<S, 18, FORM>(c, a, c->dslash_rpt);
+        if (c->recon32 == 12) return launch_dslash<S, 12, FORM>(c, a, c->dslash_rpt, c->dslash_variant);
+        return launch_dslash<S, 18, FORM>(c, a, c->dslash_rpt, c->dslash_variant);
     }
 }
 
 template <class S> static const typename S::comp_t* clover_ptr(lq_ctx* c, int parity, int inverse) {
-    if constexpr (S::prec == LQ_FP64) return (inverse ? c->clovinv64 : c->clov64) + (size_t)parity * 72 * c->g.Vh;
-    else return (inverse ? c->clovinv32 : c->clov32) + (size_t)parity * 72 * c->g.Vh;
+    if constexpr (S::prec == LQ_FP64) return clover_block(inverse ? c->clovinv64 : c->clov64, c->g.NB, parity, 0);
+    else return clover_block(inverse ? c->clovinv32 : c->clov32, c->g.NB, parity, 0);
 }
 
 int op_hop(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* in, int dagger) {
@@ -60,76 +60,39 @@ int op_kernel_b(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const 
 }
 
 // ---- site-local clover apply: out = C x --------------------------------------------------------------------
-template <class S, int RPT>
-__global__ void __launch_bounds__(256) clover_apply_kernel(Geom g, int N, int G, SView<S> out, SView<S> x, const typename S::comp_t* __restrict__ clover) {
+template <class S, int RPT, int R>
+__global__ void __launch_bounds__(128) clover_apply_kernel(Geom g, int G, SView<S> out, SView<S> x, const typename S::comp_t* __restrict__ clover) {
     using T = typename S::comp_t;
+    constexpr int TPG = R / RPT, UT = SB * TPG, US = 24 * SB * R, UN = SB * R;
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
-    if (tid >= g.Vh * G) return;
-    const int cb = tid / G, goff = (tid - cb * G) * RPT;
-    const size_t plane = (size_t)g.Vh * N;
-    T sc[RPT];
-    if constexpr (S::has_norm) {
-        float nrm[RPT];
-        load_norm<RPT>(x.n + (size_t)cb * N + goff, nrm);
-#pragma unroll
-        for (int k = 0; k < RPT; k++) sc[k] = nrm[k] * (1.0f / 32767.0f);
-    }
-    T res[24][RPT];
-#pragma unroll
-    for (int b = 0; b < 2; b++) {
-        T v[6][2][RPT], o[6][2][RPT], cl[36];
-#pragma unroll
-        for (int i = 0; i < 6; i++)
-#pragma unroll
-            for (int ri = 0; ri < 2; ri++) {
-                load_comp<S, RPT>(x.d + (size_t)(12 * b + 2 * i + ri) * plane + (size_t)cb * N + goff, v[i][ri]);
-                if constexpr (S::has_norm) {
-#pragma unroll
-                    for (int k = 0; k < RPT; k++) v[i][ri][k] *= sc[k];
-                }
-            }
-        load_planes<T, 36>(clover + (size_t)b * 36 * g.Vh, g.Vh, cb, cl);
-        clover_block_mul<T, RPT>(cl, v, o);
-#pragma unroll
-        for (int i = 0; i < 6; i++)
-#pragma unroll
-            for (int ri = 0; ri < 2; ri++)
-#pragma unroll
-                for (int k = 0; k < RPT; k++) res[12 * b + 2 * i + ri][k] = o[i][ri][k];
-    }
-    typename S::store_t* ob = out.d + (size_t)cb * N + goff;
-    if constexpr (S::has_norm) {
-        float mx[RPT], inv[RPT];
-#pragma unroll
-        for (int k = 0; k < RPT; k++) mx[k] = 0.f;
-#pragma unroll
-        for (int j = 0; j < 24; j++)
-#pragma unroll
-            for (int k = 0; k < RPT; k++) mx[k] = fmaxf(mx[k], fabsf(res[j][k]));
-#pragma unroll
-        for (int k = 0; k < RPT; k++) { inv[k] = mx[k] > 0.f ? 32767.0f / mx[k] : 0.f; out.n[(size_t)cb * N + goff + k] = mx[k]; }
-#pragma unroll
-        for (int j = 0; j < 24; j++) {
-            T q[RPT];
-#pragma unroll
-            for (int k = 0; k < RPT; k++) q[k] = rintf(res[j][k] * inv[k]);
-            store_comp<S, RPT>(ob + (size_t)j * plane, q);
-        }
-    } else {
-#pragma unroll
-        for (int j = 0; j < 24; j++) store_comp<S, RPT>(ob + (size_t)j * plane, res[j]);
-    }
+    const int u = tid / UT;
+    if (u >= g.NB * G) return;
+    const int lu = tid - u * UT;
+    const int s = lu / TPG, hoff = (lu - s * TPG) * RPT;
+    const int blk = u / G;
+    if (blk * SB + s >= g.Vh) return;
+    const size_t own = (size_t)u * US + s * R + hoff, own_n = (size_t)u * UN + s * R + hoff;
+    T v[24][RPT];
+    load_site_regs<S, RPT, R>(x.d + own, S::has_norm ? x.n + own_n : nullptr, v);
+    clover_apply_regs<T, RPT>(clover + (size_t)blk * (72 * SB), s, v);
+    store_site_regs<S, RPT, R>(out.d + own, S::has_norm ? out.n + own_n : nullptr, v);
 }
 
 template <class S> static int clover_t(lq_ctx* c, int nrhs, int parity, void* out, const void* x, int inverse) {
     SView<S> vo = make_view<S>(c->g, out, nrhs, 0), vx = make_view<S>(c->g, const_cast<void*>(x), nrhs, 0);
     const typename S::comp_t* cl = clover_ptr<S>(c, parity, inverse);
-    const int rpt = (nrhs % 2 == 0) ? 2 : 1;
-    const int G = nrhs / rpt;
-    const long long threads = (long long)c->g.Vh * G;
-    const int block = 128, grid = (int)((threads + block - 1) / block);
-    if (rpt == 2) clover_apply_kernel<S, 2><<<grid, block, 0, c->stream>>>(c->g, nrhs, G, vo, vx, cl);
-    else clover_apply_kernel<S, 1><<<grid, block, 0, c->stream>>>(c->g, nrhs, G, vo, vx, cl);
+    const int R = group_width(nrhs), G = nrhs / R;
+    const int block = 128;
+    if (R >= 2) {   // two right-hand sides per thread
+        const long long threads = (long long)c->g.NB * G * SB * (R / 2);
+        const int grid = (int)((threads + block - 1) / block);
+        if (R == 4) clover_apply_kernel<S, 2, 4><<<grid, block, 0, c->stream>>>(c->g, G, vo, vx, cl);
+        else clover_apply_kernel<S, 2, 2><<<grid, block, 0, c->stream>>>(c->g, G, vo, vx, cl);
+    } else {
+        const long long threads = (long long)c->g.NB * G * SB;
+        const int grid = (int)((threads + block - 1) / block);
+        clover_apply_kernel<S, 1, 1><<<grid, block, 0, c->stream>>>(c->g, G, vo, vx, cl);
+    }
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;

@@ -16,7 +16,7 @@ __global__ void gauge_ingest_kernel(Geom g, const Tin* __restrict__ canon, doubl
     double r[18];
 #pragma unroll
     for (int k = 0; k < 18; k++) r[k] = (double)src[k];
-    store_planes<double, 18>(native + (size_t)pm * 18 * g.Vh, g.Vh, cb, r);
+    store_planes<double, 18>(link_block(native, g.NB, 18, parity, cb / SB, mu), cb % SB, r);
 }
 int gauge_ingest(lq_ctx* c, const void* dev_canonical, int in_prec) {
     const long long threads = 8LL * c->g.Vh;
@@ -29,21 +29,21 @@ int gauge_ingest(lq_ctx* c, const void* dev_canonical, int in_prec) {
     return 0;
 }
 template <int RECON>
-__global__ void gauge_to_fp32_kernel(int Vh, const double* __restrict__ src, float* __restrict__ dst) {
+__global__ void gauge_to_fp32_kernel(int Vh, int NB, const double* __restrict__ src, float* __restrict__ dst) {
     const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= 8LL * Vh) return;
     const int cb = (int)(tid % Vh), pm = (int)(tid / Vh);
     double r[18]; float f[18];
-    load_planes<double, 18>(src + (size_t)pm * 18 * Vh, Vh, cb, r);
+    load_planes<double, 18>(link_block(src, NB, 18, pm >> 2, cb / SB, pm & 3), cb % SB, r);
 #pragma unroll
     for (int k = 0; k < RECON; k++) f[k] = (float)r[k];
-    store_planes<float, RECON>(dst + (size_t)pm * RECON * Vh, Vh, cb, f);
+    store_planes<float, RECON>(link_block(dst, NB, RECON, pm >> 2, cb / SB, pm & 3), cb % SB, f);
 }
 int gauge_make_fp32(lq_ctx* c, int recon) {
     const long long threads = 8LL * c->g.Vh;
     const int block = 128; const int grid = (int)((threads + block - 1) / block);
-    if (recon == 18) gauge_to_fp32_kernel<18><<<grid, block, 0, c->stream>>>(c->g.Vh, c->gauge64, c->gauge32);
-    else gauge_to_fp32_kernel<12><<<grid, block, 0, c->stream>>>(c->g.Vh, c->gauge64, c->gauge32);
+    if (recon == 18) gauge_to_fp32_kernel<18><<<grid, block, 0, c->stream>>>(c->g.Vh, c->g.NB, c->gauge64, c->gauge32);
+    else gauge_to_fp32_kernel<12><<<grid, block, 0, c->stream>>>(c->g.Vh, c->g.NB, c->gauge64, c->gauge32);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     c->recon32 = recon;
@@ -52,27 +52,29 @@ int gauge_make_fp32(lq_ctx* c, int recon) {
 
 // ---- scalar element access of a native parity block ---------------------------------------------------------------
 template <class S>
-__device__ __forceinline__ void load_site(const SView<S>& v, int Vh, int N, int cb, int k, double* o) {
-    const size_t plane = (size_t)Vh * N, off = (size_t)cb * N + k;
+__device__ __forceinline__ void load_site(const SView<S>& v, int N, int cb, int k, double* o) {
+    const int PL = SB * group_width(N);
+    const size_t off = sp_index(N, cb, k, 0);
     double sc = 1.0;
-    if constexpr (S::has_norm) sc = (double)(v.n[off] * (1.0f / 32767.0f));
+    if constexpr (S::has_norm) sc = (double)(v.n[nrm_index(N, cb, k)] * (1.0f / 32767.0f));
 #pragma unroll
-    for (int j = 0; j < 24; j++) o[j] = (double)v.d[j * plane + off] * sc;
+    for (int j = 0; j < 24; j++) o[j] = (double)v.d[off + (size_t)j * PL] * sc;
 }
 template <class S>
-__device__ __forceinline__ void store_site(const SView<S>& v, int Vh, int N, int cb, int k, const double* o) {
-    const size_t plane = (size_t)Vh * N, off = (size_t)cb * N + k;
+__device__ __forceinline__ void store_site(const SView<S>& v, int N, int cb, int k, const double* o) {
+    const int PL = SB * group_width(N);
+    const size_t off = sp_index(N, cb, k, 0);
     if constexpr (S::has_norm) {
         float mx = 0.f;
 #pragma unroll
         for (int j = 0; j < 24; j++) mx = fmaxf(mx, fabsf((float)o[j]));
-        v.n[off] = mx;
+        v.n[nrm_index(N, cb, k)] = mx;
         const float inv = mx > 0.f ? 32767.0f / mx : 0.f;
 #pragma unroll
-        for (int j = 0; j < 24; j++) v.d[j * plane + off] = (short)rintf((float)o[j] * inv);
+        for (int j = 0; j < 24; j++) v.d[off + (size_t)j * PL] = (short)rintf((float)o[j] * inv);
     } else {
 #pragma unroll
-        for (int j = 0; j < 24; j++) v.d[j * plane + off] = (typename S::store_t)o[j];
+        for (int j = 0; j < 24; j++) v.d[off + (size_t)j * PL] = (typename S::store_t)o[j];
     }
 }
 
@@ -93,9 +95,9 @@ __global__ void spinor_reorder_kernel(Geom g, int N, SView<S> even, SView<S> odd
     if constexpr (PACK) {
 #pragma unroll
         for (int j = 0; j < 24; j++) o[j] = (double)p[j];
-        store_site<S>(v, g.Vh, N, cb, k, o);
+        store_site<S>(v, N, cb, k, o);
     } else {
-        load_site<S>(v, g.Vh, N, cb, k, o);
+        load_site<S>(v, N, cb, k, o);
 #pragma unroll
         for (int j = 0; j < 24; j++) p[j] = (Tc)o[j];
     }
@@ -131,14 +133,14 @@ __global__ void convert_kernel(int Vh, int N, SView<SD> dst, SView<SS> src, cons
     if (tid >= (long long)Vh * N) return;
     const int k = (int)(tid % N), cb = (int)(tid / N);
     double o[24];
-    load_site<SS>(src, Vh, N, cb, k, o);
+    load_site<SS>(src, N, cb, k, o);
     if (scale) {
         double s = scale[k];
         if (invert) s = (s != 0.0) ? 1.0 / s : 0.0;
 #pragma unroll
         for (int j = 0; j < 24; j++) o[j] *= s;
     }
-    store_site<SD>(dst, Vh, N, cb, k, o);
+    store_site<SD>(dst, N, cb, k, o);
 }
 template <class SD, class SS>
 static int convert_t(lq_ctx* c, void* dst, const void* src, int nrhs, const double* d_scale, int invert) {

@@ -65,13 +65,26 @@ def test_multi_rhs_ragged_lattice(nrhs, prec):
     ctx.close()
 
 
-@pytest.mark.parametrize("rpt", [1, 2, 4])
-def test_rhs_per_thread_variants(rpt):
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("nrhs,rpt", [(8, 1), (8, 2), (8, 4), (2, 1), (2, 2)])
+def test_rhs_per_thread_variants(nrhs, rpt, variant):
+    """Every (RHS group width, RHS per thread, register-budget variant) instantiation of the stencil kernels."""
     dims = (8, 4, 4, 6)
     ctx, orc = make_case(dims, 99, 0.3, 0.12, 1.0)
-    ctx.set_tuning(dslash_block=64, dslash_rpt=rpt)
+    ctx.set_tuning(dslash_variant=variant, dslash_rpt=rpt)
     for prec in (B.LQ_FP64, B.LQ_FP32, B.LQ_HALF):
-        check_ops(ctx, orc, 8, prec, ops=[B.LQ_OP_MDAG, B.LQ_OP_KERNEL_A, B.LQ_OP_KERNEL_B])
+        check_ops(ctx, orc, nrhs, prec, ops=[B.LQ_OP_MDAG, B.LQ_OP_KERNEL_A, B.LQ_OP_KERNEL_B])
+    ctx.close()
+
+
+@pytest.mark.parametrize("nrhs", [1, 4, 12])
+@pytest.mark.parametrize("prec", [B.LQ_FP64, B.LQ_FP32, B.LQ_HALF])
+def test_padded_last_site_block(nrhs, prec):
+    """Vh = 216 is not a multiple of the 32-site native block: the last block is 3/4 padding that no kernel may
+    read into a result or a reduction."""
+    dims = (6, 6, 2, 6)
+    ctx, orc = make_case(dims, 4321, 0.3, 0.124, 1.0)
+    check_ops(ctx, orc, nrhs, prec, ops=[B.LQ_OP_HOP, B.LQ_OP_M, B.LQ_OP_MHAT, B.LQ_OP_KERNEL_A, B.LQ_OP_KERNEL_B, B.LQ_OP_CLOVER_INV])
     ctx.close()
 
 

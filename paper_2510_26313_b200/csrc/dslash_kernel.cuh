@@ -100,7 +100,29 @@ __device__ __forceinline__ void store_site_regs(typename S::store_t* __restrict_
     }
 }
 
-template <class S, int RPT, int R, int RECON, int FORM, int BLOCK, int MINB>
+// kernel modes (tuning variants; all compute the same result)
+enum { MODE_BASE = 0, MODE_L2PF = 1, MODE_PIPE = 2, MODE_PIPE_L2PF = 3 };
+
+// site coordinates and strides of one thread, and its neighbour in direction D = 2*mu + (0 forward | 1 backward)
+struct SiteCtx { int cb, xh, y, z, t, odd, Lxh, Ly, Lz, Lt; };
+template <int D> __device__ __forceinline__ int neighbour(const SiteCtx& c) {
+    constexpr int mu = D >> 1; constexpr bool fwd = (D & 1) == 0;
+    if constexpr (mu == 0) {
+        const int xn = fwd ? (c.odd ? (c.xh + 1 == c.Lxh ? 0 : c.xh + 1) : c.xh) : (c.odd ? c.xh : (c.xh == 0 ? c.Lxh - 1 : c.xh - 1));
+        return c.cb - c.xh + xn;
+    } else if constexpr (mu == 1) {
+        const int sy = c.Lxh;
+        return fwd ? ((c.y + 1 == c.Ly) ? c.cb - (c.Ly - 1) * sy : c.cb + sy) : ((c.y == 0) ? c.cb + (c.Ly - 1) * sy : c.cb - sy);
+    } else if constexpr (mu == 2) {
+        const int sz = c.Lxh * c.Ly;
+        return fwd ? ((c.z + 1 == c.Lz) ? c.cb - (c.Lz - 1) * sz : c.cb + sz) : ((c.z == 0) ? c.cb + (c.Lz - 1) * sz : c.cb - sz);
+    } else {
+        const int st = c.Lxh * c.Ly * c.Lz;
+        return fwd ? ((c.t + 1 == c.Lt) ? c.cb - (c.Lt - 1) * st : c.cb + st) : ((c.t == 0) ? c.cb + (c.Lt - 1) * st : c.cb - st);
+    }
+}
+
+template <class S, int RPT, int R, int RECON, int FORM, int BLOCK, int MINB, int MODE>
 __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S> a) {
     using T = typename S::comp_t;
     using ST = typename S::store_t;
@@ -115,13 +137,38 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
     const int lu = tid - u * UT;
     const int s = lu / TPG, hoff = (lu - s * TPG) * RPT;
     const int blk = u / G, grp = u - blk * G;
-    const int cb = blk * SB + s;
-    if (cb >= a.g.Vh) return;               // padding sites of the last block
-    int xh, y, z, t, odd;
-    cb_coords(a.g, a.parity, cb, xh, y, z, t, odd);
+    SiteCtx sc;
+    sc.cb = blk * SB + s;
+    if (sc.cb >= a.g.Vh) return;            // padding sites of the last block
+    cb_coords(a.g, a.parity, sc.cb, sc.xh, sc.y, sc.z, sc.t, sc.odd);
+    sc.Lxh = a.g.Lxh; sc.Ly = a.g.L[1]; sc.Lz = a.g.L[2]; sc.Lt = a.g.L[3];
 
     const size_t own = (size_t)u * US + s * R + hoff;
     const size_t own_n = (size_t)u * UN + s * R + hoff;
+
+    const int NB = a.g.NB;
+    // forward links live on the output site, backward links on the neighbour (other parity)
+    const T* gown = a.gauge + ((size_t)(a.parity * NB + blk) * 4) * (RECON * SB);
+    const T* gopp = a.gauge + ((size_t)((1 - a.parity) * NB) * 4) * (RECON * SB);
+    const ST* inb = a.in.d + (size_t)grp * US + hoff;
+    const float* inn = S::has_norm ? a.in.n + (size_t)grp * UN + hoff : nullptr;
+    const size_t bstride = (size_t)G * US, nstride = (size_t)G * UN;
+#define LQ_NB_PTR(nb) (inb + (size_t)((nb) >> 5) * bstride + ((nb) & 31) * R)
+#define LQ_NB_NRM(nb) (S::has_norm ? inn + (size_t)((nb) >> 5) * nstride + ((nb) & 31) * R : nullptr)
+#define LQ_LINK(D, nb) (((D) & 1) ? gopp + ((size_t)((nb) >> 5) * 4 + ((D) >> 1)) * (RECON * SB) : gown + ((D) >> 1) * (RECON * SB))
+#define LQ_LINK_S(D, nb) (((D) & 1) ? ((nb) & 31) : s)
+
+    if constexpr (MODE == MODE_L2PF || MODE == MODE_PIPE_L2PF) {
+        // pull the 24 rows of every neighbour towards L2 now; the loads below then see L2 latency
+        constexpr int EPL = 128 / sizeof(ST);       // elements per 128-byte line
+        constexpr int ROWS_PER_LINE = (EPL >= SB * R) ? EPL / (SB * R) : 1;
+        if (hoff == 0 && (ROWS_PER_LINE > 1 || ((s * R) % EPL) == 0)) {
+#define LQ_PF(D) { const int nb_ = neighbour<D>(sc); const ST* q_ = LQ_NB_PTR(nb_); \
+                   _Pragma("unroll") for (int j = 0; j < 24; j += ROWS_PER_LINE) asm volatile("prefetch.global.L2 [%0];" ::"l"(q_ + j * SB * R)); }
+            LQ_PF(2) LQ_PF(3) LQ_PF(4) LQ_PF(5) LQ_PF(6) LQ_PF(7)
+#undef LQ_PF
+        }
+    }
 
     T acc[24][RPT];
     // ---- prologue (FORM_B): acc = C x  (or x when no clover) -----------------------------------------
@@ -137,48 +184,34 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
 
     // ---- the eight hops ---------------------------------------------------------------------------------
     const T c0 = (FORM == FORM_B) ? a.coef : T(1);
-    const int NB = a.g.NB;
-    // forward links live on the output site, backward links on the neighbour (other parity)
-    const T* gown = a.gauge + ((size_t)(a.parity * NB + blk) * 4) * (RECON * SB);
-    const T* gopp = a.gauge + ((size_t)((1 - a.parity) * NB) * 4) * (RECON * SB);
-    const int Lxh = a.g.Lxh, Ly = a.g.L[1], Lz = a.g.L[2], Lt = a.g.L[3];
-    const int sy = Lxh, sz = Lxh * Ly, st = Lxh * Ly * Lz;
-    const ST* inb = a.in.d + (size_t)grp * US + hoff;
-    const float* inn = S::has_norm ? a.in.n + (size_t)grp * UN + hoff : nullptr;
-    const size_t bstride = (size_t)G * US, nstride = (size_t)G * UN;
-#define LQ_NB_PTR(nb) (inb + (size_t)((nb) >> 5) * bstride + ((nb) & 31) * R)
-#define LQ_NB_NRM(nb) (S::has_norm ? inn + (size_t)((nb) >> 5) * nstride + ((nb) & 31) * R : nullptr)
-#define LQ_BWD_LINK(nb, mu) (gopp + ((size_t)((nb) >> 5) * 4 + (mu)) * (RECON * SB))
-    {   // x
-        const int xp = odd ? (xh + 1 == Lxh ? 0 : xh + 1) : xh;
-        const int xm = odd ? xh : (xh == 0 ? Lxh - 1 : xh - 1);
-        const int nbp = cb - xh + xp, nbm = cb - xh + xm;
-        hop_dir<S, RPT, R, RECON, 0, true>(LQ_NB_PTR(nbp), LQ_NB_NRM(nbp), gown, s, c0, a.dsign, acc);
-        hop_dir<S, RPT, R, RECON, 0, false>(LQ_NB_PTR(nbm), LQ_NB_NRM(nbm), LQ_BWD_LINK(nbm, 0), nbm & 31, c0, -a.dsign, acc);
-    }
-    {   // y
-        const int nbp = (y + 1 == Ly) ? cb - (Ly - 1) * sy : cb + sy;
-        const int nbm = (y == 0) ? cb + (Ly - 1) * sy : cb - sy;
-        hop_dir<S, RPT, R, RECON, 1, true>(LQ_NB_PTR(nbp), LQ_NB_NRM(nbp), gown + RECON * SB, s, c0, a.dsign, acc);
-        hop_dir<S, RPT, R, RECON, 1, false>(LQ_NB_PTR(nbm), LQ_NB_NRM(nbm), LQ_BWD_LINK(nbm, 1), nbm & 31, c0, -a.dsign, acc);
-    }
-    {   // z
-        const int nbp = (z + 1 == Lz) ? cb - (Lz - 1) * sz : cb + sz;
-        const int nbm = (z == 0) ? cb + (Lz - 1) * sz : cb - sz;
-        hop_dir<S, RPT, R, RECON, 2, true>(LQ_NB_PTR(nbp), LQ_NB_NRM(nbp), gown + 2 * RECON * SB, s, c0, a.dsign, acc);
-        hop_dir<S, RPT, R, RECON, 2, false>(LQ_NB_PTR(nbm), LQ_NB_NRM(nbm), LQ_BWD_LINK(nbm, 2), nbm & 31, c0, -a.dsign, acc);
-    }
-    {   // t (boundary sign on the wrapped term)
-        const int nbp = (t + 1 == Lt) ? cb - (Lt - 1) * st : cb + st;
-        const int nbm = (t == 0) ? cb + (Lt - 1) * st : cb - st;
-        const T cp = (t + 1 == Lt) ? c0 * a.tsign : c0;
-        const T cm = (t == 0) ? c0 * a.tsign : c0;
-        hop_dir<S, RPT, R, RECON, 3, true>(LQ_NB_PTR(nbp), LQ_NB_NRM(nbp), gown + 3 * RECON * SB, s, cp, a.dsign, acc);
-        hop_dir<S, RPT, R, RECON, 3, false>(LQ_NB_PTR(nbm), LQ_NB_NRM(nbm), LQ_BWD_LINK(nbm, 3), nbm & 31, cm, -a.dsign, acc);
+    const T cp = (sc.t + 1 == sc.Lt) ? c0 * a.tsign : c0;     // boundary sign on the wrapped t terms
+    const T cm = (sc.t == 0) ? c0 * a.tsign : c0;
+    if constexpr (MODE == MODE_PIPE || MODE == MODE_PIPE_L2PF) {
+        NbData<S, RPT> da, db;
+#define LQ_LOAD(D, buf) { const int nb_ = neighbour<D>(sc); hop_load<S, RPT, R, RECON>(LQ_NB_PTR(nb_), LQ_NB_NRM(nb_), LQ_LINK(D, nb_), LQ_LINK_S(D, nb_), buf); }
+#define LQ_COMP(D, buf) hop_compute<S, RPT, RECON, ((D) >> 1), (((D) & 1) == 0)>(buf, (D) == 6 ? cp : ((D) == 7 ? cm : c0), ((D) & 1) ? -a.dsign : a.dsign, acc);
+        LQ_LOAD(0, da)
+        LQ_LOAD(1, db) LQ_COMP(0, da)
+        LQ_LOAD(2, da) LQ_COMP(1, db)
+        LQ_LOAD(3, db) LQ_COMP(2, da)
+        LQ_LOAD(4, da) LQ_COMP(3, db)
+        LQ_LOAD(5, db) LQ_COMP(4, da)
+        LQ_LOAD(6, da) LQ_COMP(5, db)
+        LQ_LOAD(7, db) LQ_COMP(6, da)
+        LQ_COMP(7, db)
+#undef LQ_LOAD
+#undef LQ_COMP
+    } else {
+#define LQ_HOP(D) { const int nb_ = neighbour<D>(sc); \
+        hop_dir<S, RPT, R, RECON, ((D) >> 1), (((D) & 1) == 0)>(LQ_NB_PTR(nb_), LQ_NB_NRM(nb_), LQ_LINK(D, nb_), LQ_LINK_S(D, nb_), \
+                (D) == 6 ? cp : ((D) == 7 ? cm : c0), ((D) & 1) ? -a.dsign : a.dsign, acc); }
+        LQ_HOP(0) LQ_HOP(1) LQ_HOP(2) LQ_HOP(3) LQ_HOP(4) LQ_HOP(5) LQ_HOP(6) LQ_HOP(7)
+#undef LQ_HOP
     }
 #undef LQ_NB_PTR
 #undef LQ_NB_NRM
-#undef LQ_BWD_LINK
+#undef LQ_LINK
+#undef LQ_LINK_S
 
     // ---- epilogue (FORM_A): acc <- C acc -----------------------------------------------------------------
     if constexpr (FORM == FORM_A) clover_apply_regs<T, RPT>(a.clover + (size_t)blk * (72 * SB), s, acc);

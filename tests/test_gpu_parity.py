@@ -65,7 +65,7 @@ def test_multi_rhs_ragged_lattice(nrhs, prec):
     ctx.close()
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2, 4, 6])
 @pytest.mark.parametrize("nrhs,rpt", [(8, 1), (8, 2), (8, 4), (2, 1), (2, 2)])
 def test_rhs_per_thread_variants(nrhs, rpt, variant):
     """Every (RHS group width, RHS per thread, register-budget variant) instantiation of the stencil kernels."""

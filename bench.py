@@ -231,13 +231,14 @@ def run_op(args, B, device):
     cfg_id, kind, prec, n = int(f[0].replace("cfg", "")), f[1], f[2], int(f[3])
     variant = int(f[4]) if len(f) > 4 else 0
     rpt = int(f[5]) if len(f) > 5 else 0
+    pfd = int(f[6]) if len(f) > 6 else -1
     c = inputs.CONFIGS[cfg_id]
     peak, peak_src, _ = measured_peaks()
     ctx = B.Context(c["dims"], device=device)
     ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=c["recon"])
     ctx.build_clover(c["kappa"], c["csw"])
-    if variant or rpt:
-        ctx.set_tuning(variant, rpt)
+    if variant or rpt or pfd >= 0:
+        ctx.set_tuning(variant, rpt, pfd)
     sampler = ClockSampler(device)
     r = time_dslash(ctx, B, kind, prec, n, c["recon"], iters=args.op_iters, warmup=max(args.warmup, 3))
     clocks = sampler.stop()
@@ -259,7 +260,7 @@ def main():
     ap.add_argument("--no-graph", action="store_true")
     ap.add_argument("--op", default=None, metavar="CFG:KIND:PREC:N",
                     help="time ONE stencil kernel only, e.g. cfg2:A:fp32:8 (lattice and links of configs[CFG]; KIND A|B|hop; "
-                         "PREC fp64|fp32|half); optional :variant:rpt tuning suffix.  Prints its own JSON line (used for ncu captures)")
+                         "PREC fp64|fp32|half); optional :variant:rpt:pfd tuning suffix.  Prints its own JSON line (used for ncu captures)")
     ap.add_argument("--op-iters", type=int, default=20)
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1")); local = int(os.environ.get("LOCAL_RANK", "0"))

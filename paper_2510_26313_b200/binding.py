@@ -73,7 +73,7 @@ def load_library():
     lib.lq_unpack.argtypes = [vp, vp, vp, ci, ci, ci]
     lib.lq_fill_spinor_random.argtypes = [vp, vp, ci, ci, u64, ci, ci]
     lib.lq_solve.argtypes = [vp, vp, vp, ci, ci, ci, ctypes.POINTER(SolveParam), ctypes.POINTER(SolveInfo)]
-    lib.lq_set_tuning.argtypes = [vp, ci, ci]
+    lib.lq_set_tuning.argtypes = [vp, ci, ci, ci]
     lib.lq_kernel_launches.argtypes = [vp]; lib.lq_kernel_launches.restype = ctypes.c_longlong
     _lib = lib
     return lib
@@ -150,8 +150,8 @@ class Context:
     def launches(self) -> int:
         return int(self.lib.lq_kernel_launches(self.h))
 
-    def set_tuning(self, dslash_variant=0, dslash_rpt=0):
-        self._check(self.lib.lq_set_tuning(self.h, dslash_variant, dslash_rpt))
+    def set_tuning(self, dslash_variant=0, dslash_rpt=0, dslash_pfd=-1):
+        self._check(self.lib.lq_set_tuning(self.h, dslash_variant, dslash_rpt, dslash_pfd))
 
     # ------------------------------------------------------------------ gauge / clover
     def load_gauge(self, U, recon: int = 18, t_bc: int = -1):

@@ -41,12 +41,13 @@ int lq_create(lq_ctx** out, const int dims[4], int device, void* cuda_stream) {
     lq_ctx* c = new lq_ctx();
     for (int k = 0; k < 4; k++) c->g.L[k] = dims[k];
     c->g.Lxh = dims[0] / 2; c->g.V = V; c->g.Vh = (int)(V / 2); c->g.NB = (c->g.Vh + SB - 1) / SB;
+    c->g.dLxh = make_fastdiv(c->g.Lxh); c->g.dLy = make_fastdiv(dims[1]); c->g.dLz = make_fastdiv(dims[2]);
     c->device = device; c->stream = (cudaStream_t)cuda_stream; c->t_bc = -1;
     c->gauge64 = nullptr; c->gauge32 = nullptr; c->recon32 = 18;
     c->clov64 = c->clovinv64 = nullptr; c->clov32 = c->clovinv32 = nullptr;
     c->kappa = c->csw = 0; c->has_gauge = c->has_clover = false;
     c->alloc_fn = nullptr; c->free_fn = nullptr; c->alloc_user = nullptr;
-    c->launches = 0; c->dslash_block = 0; c->dslash_rpt = 0; c->dslash_variant = 0;
+    c->launches = 0; c->dslash_block = 0; c->dslash_rpt = 0; c->dslash_variant = 0; c->dslash_pfd = LQ_DEFAULT_PFD;
     c->red_partials = nullptr; c->red_partials_elems = 0; c->red_counter = nullptr; c->h_scalars = nullptr; c->d_flag = nullptr;
     if (cudaMalloc(&c->red_counter, 256) != cudaSuccess || cudaMemset(c->red_counter, 0, 256) != cudaSuccess ||
         cudaMallocHost(&c->h_scalars, 8 * LQ_MAX_RHS * sizeof(double)) != cudaSuccess) { cudaGetLastError(); delete c; return LQ_ECUDA; }
@@ -77,9 +78,9 @@ int lq_set_allocator(lq_ctx* c, lq_alloc_fn alloc, lq_free_fn release, void* use
     return 0;
 }
 
-int lq_set_tuning(lq_ctx* c, int dslash_variant, int dslash_rpt) {
+int lq_set_tuning(lq_ctx* c, int dslash_variant, int dslash_rpt, int dslash_pfd) {
     if (!c) return LQ_EINVAL;
-    c->dslash_variant = dslash_variant; c->dslash_rpt = dslash_rpt;
+    c->dslash_variant = dslash_variant; c->dslash_rpt = dslash_rpt; c->dslash_pfd = dslash_pfd < 0 ? LQ_DEFAULT_PFD : dslash_pfd;
     return 0;
 }
 

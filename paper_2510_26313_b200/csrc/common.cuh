@@ -9,8 +9,29 @@
 
 // ------------------------------------------------------------------ geometry
 constexpr int SB = 32;   // sites per native block (one warp-wide row of every plane)
+constexpr int LQ_DEFAULT_PFD = 64;    // default L2 prefetch distance of the stencil kernels, in site blocks
+
+// division of a non-negative int < 2^31 by a fixed positive divisor: q = (umulhi(m, n) + n) >> l  (Granlund-Montgomery)
+struct FastDiv {
+    unsigned m, l;
+    __host__ __device__ inline int div(int n) const {
+#ifdef __CUDA_ARCH__
+        return (int)((__umulhi(m, (unsigned)n) + (unsigned)n) >> l);
+#else
+        return (int)(((unsigned)(((unsigned long long)m * (unsigned)n) >> 32) + (unsigned)n) >> l);
+#endif
+    }
+};
+inline FastDiv make_fastdiv(int d) {
+    FastDiv f; unsigned l = 0;
+    while ((1u << l) < (unsigned)d) l++;
+    f.l = l;
+    f.m = (unsigned)((((unsigned long long)1 << 32) * ((1ull << l) - (unsigned)d)) / (unsigned)d + 1);
+    return f;
+}
 
 struct Geom {
+    FastDiv dLxh, dLy, dLz;   // divisions by Lx/2, Ly, Lz
     int L[4];      // Lx, Ly, Lz, Lt
     int Lxh;       // Lx / 2
     int Vh;        // sites per parity
@@ -20,9 +41,9 @@ struct Geom {
 
 // checkerboard index -> coordinates.  cb = xh + Lxh*(y + Ly*(z + Lz*t)), x = 2*xh + ((y+z+t+parity)&1)
 __host__ __device__ inline void cb_coords(const Geom& g, int parity, int cb, int& xh, int& y, int& z, int& t, int& odd) {
-    xh = cb % g.Lxh; int r = cb / g.Lxh;
-    y = r % g.L[1]; r /= g.L[1];
-    z = r % g.L[2]; t = r / g.L[2];
+    int r = g.dLxh.div(cb); xh = cb - r * g.Lxh;
+    int q = g.dLy.div(r); y = r - q * g.L[1];
+    t = g.dLz.div(q); z = q - t * g.L[2];
     odd = (y + z + t + parity) & 1;
 }
 // full coordinates -> (parity, cb)
@@ -150,7 +171,8 @@ struct lq_ctx {
     long long launches;
     int dslash_block;               // tuning knob (0 = default)
     int dslash_rpt;                 // tuning knob (0 = auto)
-    int dslash_variant;             // tuning knob: kernel variant bits (0 = default)
+    int dslash_variant;             // tuning knob: kernel variant (0 = default)
+    int dslash_pfd;                 // tuning knob: L2 prefetch distance in site blocks (0 = off)
     std::string err;
     // reduction scratch
     double* red_partials; size_t red_partials_elems;

@@ -27,12 +27,14 @@ template <class S> struct DslashArgs {
     Geom g;
     int parity;            // parity of the output sites
     int N, G;              // right-hand sides, RHS groups (N / R)
+    FastDiv dG;            // division by G
     SView<S> out, in, x;   // out / x on `parity`, in on 1-parity
     const T* gauge;        // [parity][blk][mu] blocks of RECON*SB reals
     const T* clover;       // [blk] blocks of 72*SB reals of the output parity, or nullptr (identity)
     T coef;                // FORM_B
     T tsign;               // t_bc
     T dsign;               // +1, -1 = dagger
+    int pfd;               // L2 prefetch distance in site blocks (0 = off)
 };
 
 __device__ __forceinline__ float fm(float a, float b, float c) { return fmaf(a, b, c); }
@@ -106,58 +108,11 @@ __device__ __forceinline__ void load_link(const T* __restrict__ blockbase, int s
     }
 }
 
-// ---- one of the eight hopping terms -------------------------------------------------------------------
-// acc[j][k] += cu * (1 - sigma*gamma_MU) W psi(nb),  W = U (FWD) or U^dag (backward), sigma = +-1.
-// `nb` points at real 0 of the neighbour's RPT right-hand sides; real j is at nb + j*SB*R.
-template <class S, int RPT, int R, int RECON, int MU, bool FWD>
-__device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ nb, const float* __restrict__ nb_norm,
-                                        const typename S::comp_t* __restrict__ link_blk, int link_s,
-                                        typename S::comp_t cu, typename S::comp_t sigma, typename S::comp_t (&acc)[24][RPT]) {
-    using T = typename S::comp_t;
-    constexpr int PL = SB * R;   // elements between consecutive reals of a site
-    T u[18];
-    load_link<T, RECON>(link_blk, link_s, u);
-
-    T cuk[RPT], clk[RPT];
-    if constexpr (S::has_norm) {
-        float nrm[RPT];
-        load_norm<RPT>(nb_norm, nrm);
-#pragma unroll
-        for (int k = 0; k < RPT; k++) cuk[k] = cu * nrm[k] * (1.0f / 32767.0f);
-    } else {
-#pragma unroll
-        for (int k = 0; k < RPT; k++) cuk[k] = cu;
-    }
-#pragma unroll
-    for (int k = 0; k < RPT; k++) clk[k] = sigma * cuk[k];
-
-    // projected half spinor h[s][c][ri][k]
-    T h[2][3][2][RPT];
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-        T p[4][2][RPT];
-#pragma unroll
-        for (int s = 0; s < 4; s++)
-#pragma unroll
-            for (int ri = 0; ri < 2; ri++) load_comp<S, RPT>(nb + (2 * (3 * s + c) + ri) * PL, p[s][ri]);
-#pragma unroll
-        for (int k = 0; k < RPT; k++) {
-            if constexpr (MU == 0) {        // h0 = p0 - s i p3, h1 = p1 - s i p2
-                h[0][c][0][k] = fm(sigma, p[3][1][k], p[0][0][k]);  h[0][c][1][k] = fm(-sigma, p[3][0][k], p[0][1][k]);
-                h[1][c][0][k] = fm(sigma, p[2][1][k], p[1][0][k]);  h[1][c][1][k] = fm(-sigma, p[2][0][k], p[1][1][k]);
-            } else if constexpr (MU == 1) { // h0 = p0 + s p3, h1 = p1 - s p2
-                h[0][c][0][k] = fm(sigma, p[3][0][k], p[0][0][k]);  h[0][c][1][k] = fm(sigma, p[3][1][k], p[0][1][k]);
-                h[1][c][0][k] = fm(-sigma, p[2][0][k], p[1][0][k]); h[1][c][1][k] = fm(-sigma, p[2][1][k], p[1][1][k]);
-            } else if constexpr (MU == 2) { // h0 = p0 - s i p2, h1 = p1 + s i p3
-                h[0][c][0][k] = fm(sigma, p[2][1][k], p[0][0][k]);  h[0][c][1][k] = fm(-sigma, p[2][0][k], p[0][1][k]);
-                h[1][c][0][k] = fm(-sigma, p[3][1][k], p[1][0][k]); h[1][c][1][k] = fm(sigma, p[3][0][k], p[1][1][k]);
-            } else {                        // h0 = p0 - s p2, h1 = p1 - s p3
-                h[0][c][0][k] = fm(-sigma, p[2][0][k], p[0][0][k]); h[0][c][1][k] = fm(-sigma, p[2][1][k], p[0][1][k]);
-                h[1][c][0][k] = fm(-sigma, p[3][0][k], p[1][0][k]); h[1][c][1][k] = fm(-sigma, p[3][1][k], p[1][1][k]);
-            }
-        }
-    }
-    // colour multiply and accumulate
+// ---- SU(3) x projected half spinor, spin reconstruction and accumulation --------------------------------
+// acc += cuk * (upper rows) and +-clk * (lower rows) of (1 - sigma gamma_MU) W h,  W = U (FWD) or U^dag.
+template <typename T, int RPT, int MU, bool FWD>
+__device__ __forceinline__ void hop_mulacc(const T (&h)[2][3][2][RPT], const T (&u)[18], const T (&cuk)[RPT], const T (&clk)[RPT],
+                                           T (&acc)[24][RPT]) {
 #pragma unroll
     for (int s = 0; s < 2; s++)
 #pragma unroll
@@ -211,103 +166,56 @@ __device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ 
         }
 }
 
-// ---- split form of a hopping term: all loads first (hop_load), arithmetic later (hop_compute) ---------------
-// Used by the software-pipelined kernel mode: the loads of direction d+1 are issued before the arithmetic of
-// direction d, so every warp always has one full neighbour (24 reals x RPT + one link) in flight.
-template <class S, int RPT> struct NbData {
+// ---- one of the eight hopping terms -------------------------------------------------------------------
+// acc[j][k] += cu * (1 - sigma*gamma_MU) W psi(nb),  W = U (FWD) or U^dag (backward), sigma = +-1.
+// `nb` points at real 0 of the neighbour's RPT right-hand sides; real j is at nb + j*SB*R.
+template <class S, int RPT, int R, int RECON, int MU, bool FWD>
+__device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ nb, const float* __restrict__ nb_norm,
+                                        const typename S::comp_t* __restrict__ link_blk, int link_s,
+                                        typename S::comp_t cu, typename S::comp_t sigma, typename S::comp_t (&acc)[24][RPT]) {
     using T = typename S::comp_t;
-    T p[24][RPT];
+    constexpr int PL = SB * R;   // elements between consecutive reals of a site
     T u[18];
-    float nrm[RPT];
-};
-template <class S, int RPT, int R, int RECON>
-__device__ __forceinline__ void hop_load(const typename S::store_t* __restrict__ nb, const float* __restrict__ nb_norm,
-                                         const typename S::comp_t* __restrict__ link_blk, int link_s, NbData<S, RPT>& d) {
-    constexpr int PL = SB * R;
-    load_planes<typename S::comp_t, RECON>(link_blk, link_s, d.u);
-    if constexpr (S::has_norm) load_norm<RPT>(nb_norm, d.nrm);
-#pragma unroll
-    for (int j = 0; j < 24; j++) load_comp<S, RPT>(nb + j * PL, d.p[j]);
-}
-template <class S, int RPT, int RECON, int MU, bool FWD>
-__device__ __forceinline__ void hop_compute(NbData<S, RPT>& d, typename S::comp_t cu, typename S::comp_t sigma,
-                                            typename S::comp_t (&acc)[24][RPT]) {
-    using T = typename S::comp_t;
-    T (&u)[18] = d.u;
-    if constexpr (RECON == 12) {
-#pragma unroll
-        for (int c = 0; c < 3; c++) {
-            const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
-            T re = u[2 * c1] * u[6 + 2 * c2];
-            re = fm(-u[2 * c1 + 1], u[6 + 2 * c2 + 1], re);
-            re = fm(-u[2 * c2], u[6 + 2 * c1], re);
-            re = fm(u[2 * c2 + 1], u[6 + 2 * c1 + 1], re);
-            T im = u[2 * c1] * u[6 + 2 * c2 + 1];
-            im = fm(u[2 * c1 + 1], u[6 + 2 * c2], im);
-            im = fm(-u[2 * c2], u[6 + 2 * c1 + 1], im);
-            im = fm(-u[2 * c2 + 1], u[6 + 2 * c1], im);
-            u[12 + 2 * c] = re; u[12 + 2 * c + 1] = -im;
-        }
-    }
+    load_link<T, RECON>(link_blk, link_s, u);
+
     T cuk[RPT], clk[RPT];
+    if constexpr (S::has_norm) {
+        float nrm[RPT];
+        load_norm<RPT>(nb_norm, nrm);
 #pragma unroll
-    for (int k = 0; k < RPT; k++) {
-        if constexpr (S::has_norm) cuk[k] = cu * d.nrm[k] * (1.0f / 32767.0f); else cuk[k] = cu;
-        clk[k] = sigma * cuk[k];
+        for (int k = 0; k < RPT; k++) cuk[k] = cu * nrm[k] * (1.0f / 32767.0f);
+    } else {
+#pragma unroll
+        for (int k = 0; k < RPT; k++) cuk[k] = cu;
     }
-#define P_(s, c, ri) d.p[2 * (3 * (s) + (c)) + (ri)][k]
+#pragma unroll
+    for (int k = 0; k < RPT; k++) clk[k] = sigma * cuk[k];
+
+    // projected half spinor h[s][c][ri][k]
     T h[2][3][2][RPT];
 #pragma unroll
-    for (int c = 0; c < 3; c++)
+    for (int c = 0; c < 3; c++) {
+        T p[4][2][RPT];
+#pragma unroll
+        for (int s = 0; s < 4; s++)
+#pragma unroll
+            for (int ri = 0; ri < 2; ri++) load_comp<S, RPT>(nb + (2 * (3 * s + c) + ri) * PL, p[s][ri]);
 #pragma unroll
         for (int k = 0; k < RPT; k++) {
-            if constexpr (MU == 0) {
-                h[0][c][0][k] = fm(sigma, P_(3, c, 1), P_(0, c, 0));  h[0][c][1][k] = fm(-sigma, P_(3, c, 0), P_(0, c, 1));
-                h[1][c][0][k] = fm(sigma, P_(2, c, 1), P_(1, c, 0));  h[1][c][1][k] = fm(-sigma, P_(2, c, 0), P_(1, c, 1));
-            } else if constexpr (MU == 1) {
-                h[0][c][0][k] = fm(sigma, P_(3, c, 0), P_(0, c, 0));  h[0][c][1][k] = fm(sigma, P_(3, c, 1), P_(0, c, 1));
-                h[1][c][0][k] = fm(-sigma, P_(2, c, 0), P_(1, c, 0)); h[1][c][1][k] = fm(-sigma, P_(2, c, 1), P_(1, c, 1));
-            } else if constexpr (MU == 2) {
-                h[0][c][0][k] = fm(sigma, P_(2, c, 1), P_(0, c, 0));  h[0][c][1][k] = fm(-sigma, P_(2, c, 0), P_(0, c, 1));
-                h[1][c][0][k] = fm(-sigma, P_(3, c, 1), P_(1, c, 0)); h[1][c][1][k] = fm(sigma, P_(3, c, 0), P_(1, c, 1));
-            } else {
-                h[0][c][0][k] = fm(-sigma, P_(2, c, 0), P_(0, c, 0)); h[0][c][1][k] = fm(-sigma, P_(2, c, 1), P_(0, c, 1));
-                h[1][c][0][k] = fm(-sigma, P_(3, c, 0), P_(1, c, 0)); h[1][c][1][k] = fm(-sigma, P_(3, c, 1), P_(1, c, 1));
+            if constexpr (MU == 0) {        // h0 = p0 - s i p3, h1 = p1 - s i p2
+                h[0][c][0][k] = fm(sigma, p[3][1][k], p[0][0][k]);  h[0][c][1][k] = fm(-sigma, p[3][0][k], p[0][1][k]);
+                h[1][c][0][k] = fm(sigma, p[2][1][k], p[1][0][k]);  h[1][c][1][k] = fm(-sigma, p[2][0][k], p[1][1][k]);
+            } else if constexpr (MU == 1) { // h0 = p0 + s p3, h1 = p1 - s p2
+                h[0][c][0][k] = fm(sigma, p[3][0][k], p[0][0][k]);  h[0][c][1][k] = fm(sigma, p[3][1][k], p[0][1][k]);
+                h[1][c][0][k] = fm(-sigma, p[2][0][k], p[1][0][k]); h[1][c][1][k] = fm(-sigma, p[2][1][k], p[1][1][k]);
+            } else if constexpr (MU == 2) { // h0 = p0 - s i p2, h1 = p1 + s i p3
+                h[0][c][0][k] = fm(sigma, p[2][1][k], p[0][0][k]);  h[0][c][1][k] = fm(-sigma, p[2][0][k], p[0][1][k]);
+                h[1][c][0][k] = fm(-sigma, p[3][1][k], p[1][0][k]); h[1][c][1][k] = fm(sigma, p[3][0][k], p[1][1][k]);
+            } else {                        // h0 = p0 - s p2, h1 = p1 - s p3
+                h[0][c][0][k] = fm(-sigma, p[2][0][k], p[0][0][k]); h[0][c][1][k] = fm(-sigma, p[2][1][k], p[0][1][k]);
+                h[1][c][0][k] = fm(-sigma, p[3][0][k], p[1][0][k]); h[1][c][1][k] = fm(-sigma, p[3][1][k], p[1][1][k]);
             }
         }
-#undef P_
-#pragma unroll
-    for (int s = 0; s < 2; s++)
-#pragma unroll
-        for (int r = 0; r < 3; r++) {
-            T wr[RPT], wi[RPT];
-#pragma unroll
-            for (int c = 0; c < 3; c++) {
-                const T ur = FWD ? u[2 * (3 * r + c)] : u[2 * (3 * c + r)];
-                const T ui = FWD ? u[2 * (3 * r + c) + 1] : -u[2 * (3 * c + r) + 1];
-#pragma unroll
-                for (int k = 0; k < RPT; k++) {
-                    if (c == 0) { wr[k] = ur * h[s][c][0][k]; wi[k] = ur * h[s][c][1][k]; }
-                    else { wr[k] = fm(ur, h[s][c][0][k], wr[k]); wi[k] = fm(ur, h[s][c][1][k], wi[k]); }
-                    wr[k] = fm(-ui, h[s][c][1][k], wr[k]);
-                    wi[k] = fm(ui, h[s][c][0][k], wi[k]);
-                }
-            }
-            const int ju = 2 * (3 * s + r);
-            // lower-row target and the signs of (re <- , im <-): see hop_dir for the gamma algebra
-            constexpr bool XY = (MU == 0 || MU == 1);
-            const int jl = XY ? 2 * (3 * (3 - s) + r) : 2 * (3 * (2 + s) + r);
-#pragma unroll
-            for (int k = 0; k < RPT; k++) {
-                acc[ju][k] = fm(cuk[k], wr[k], acc[ju][k]); acc[ju + 1][k] = fm(cuk[k], wi[k], acc[ju + 1][k]);
-                if constexpr (MU == 0) { acc[jl][k] = fm(-clk[k], wi[k], acc[jl][k]); acc[jl + 1][k] = fm(clk[k], wr[k], acc[jl + 1][k]); }
-                else if constexpr (MU == 1) {
-                    if (s == 0) { acc[jl][k] = fm(clk[k], wr[k], acc[jl][k]); acc[jl + 1][k] = fm(clk[k], wi[k], acc[jl + 1][k]); }
-                    else { acc[jl][k] = fm(-clk[k], wr[k], acc[jl][k]); acc[jl + 1][k] = fm(-clk[k], wi[k], acc[jl + 1][k]); }
-                } else if constexpr (MU == 2) {
-                    if (s == 0) { acc[jl][k] = fm(-clk[k], wi[k], acc[jl][k]); acc[jl + 1][k] = fm(clk[k], wr[k], acc[jl + 1][k]); }
-                    else { acc[jl][k] = fm(clk[k], wi[k], acc[jl][k]); acc[jl + 1][k] = fm(-clk[k], wr[k], acc[jl + 1][k]); }
-                } else { acc[jl][k] = fm(-clk[k], wr[k], acc[jl][k]); acc[jl + 1][k] = fm(-clk[k], wi[k], acc[jl + 1][k]); }
-            }
-        }
+    }
+    hop_mulacc<T, RPT, MU, FWD>(h, u, cuk, clk, acc);
 }

@@ -100,9 +100,6 @@ __device__ __forceinline__ void store_site_regs(typename S::store_t* __restrict_
     }
 }
 
-// kernel modes (tuning variants; all compute the same result)
-enum { MODE_BASE = 0, MODE_L2PF = 1, MODE_PIPE = 2, MODE_PIPE_L2PF = 3 };
-
 // site coordinates and strides of one thread, and its neighbour in direction D = 2*mu + (0 forward | 1 backward)
 struct SiteCtx { int cb, xh, y, z, t, odd, Lxh, Ly, Lz, Lt; };
 template <int D> __device__ __forceinline__ int neighbour(const SiteCtx& c) {
@@ -122,7 +119,7 @@ template <int D> __device__ __forceinline__ int neighbour(const SiteCtx& c) {
     }
 }
 
-template <class S, int RPT, int R, int RECON, int FORM, int BLOCK, int MINB, int MODE>
+template <class S, int RPT, int R, int RECON, int FORM, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S> a) {
     using T = typename S::comp_t;
     using ST = typename S::store_t;
@@ -130,13 +127,13 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
     constexpr int UT = SB * TPG;            // threads per unit
     constexpr int US = 24 * SB * R;         // payload elements per unit
     constexpr int UN = SB * R;              // norm elements per unit
-    const int tid = blockIdx.x * BLOCK + threadIdx.x;
     const int G = a.G;
+    const int tid = blockIdx.x * BLOCK + threadIdx.x;
     const int u = tid / UT;                 // unit = blk*G + grp
     if (u >= a.g.NB * G) return;
     const int lu = tid - u * UT;
+    const int blk = a.dG.div(u), grp = u - blk * G;
     const int s = lu / TPG, hoff = (lu - s * TPG) * RPT;
-    const int blk = u / G, grp = u - blk * G;
     SiteCtx sc;
     sc.cb = blk * SB + s;
     if (sc.cb >= a.g.Vh) return;            // padding sites of the last block
@@ -158,15 +155,41 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
 #define LQ_LINK(D, nb) (((D) & 1) ? gopp + ((size_t)((nb) >> 5) * 4 + ((D) >> 1)) * (RECON * SB) : gown + ((D) >> 1) * (RECON * SB))
 #define LQ_LINK_S(D, nb) (((D) & 1) ? ((nb) & 31) : s)
 
-    if constexpr (MODE == MODE_L2PF || MODE == MODE_PIPE_L2PF) {
-        // pull the 24 rows of every neighbour towards L2 now; the loads below then see L2 latency
-        constexpr int EPL = 128 / sizeof(ST);       // elements per 128-byte line
-        constexpr int ROWS_PER_LINE = (EPL >= SB * R) ? EPL / (SB * R) : 1;
-        if (hoff == 0 && (ROWS_PER_LINE > 1 || ((s * R) % EPL) == 0)) {
-#define LQ_PF(D) { const int nb_ = neighbour<D>(sc); const ST* q_ = LQ_NB_PTR(nb_); \
-                   _Pragma("unroll") for (int j = 0; j < 24; j += ROWS_PER_LINE) asm volatile("prefetch.global.L2 [%0];" ::"l"(q_ + j * SB * R)); }
-            LQ_PF(2) LQ_PF(3) LQ_PF(4) LQ_PF(5) LQ_PF(6) LQ_PF(7)
-#undef LQ_PF
+    // ---- distance prefetch into L2 ------------------------------------------------------------------------
+    // An SM can keep only a few KB of L1 misses in flight, so a demand load that goes to HBM (~2.5x the latency of
+    // an L2 hit) costs ~2.5x the L1 miss-slot time: the kernel is bound by (bytes fetched) x (their latency), not by
+    // HBM bandwidth.  Every unit therefore asks L2, with fire-and-forget prefetches, for the data that the unit
+    // `pfd` site blocks further along the sweep will touch FIRST: the input unit one time-slice ahead (the +t
+    // neighbours; every other neighbour was touched by earlier blocks), both parities' link slabs and the clover
+    // block.  One 128-byte line per lane per instruction; ~10 instructions per thread.
+    {
+        if (a.pfd > 0) {
+            const int pb = blk + a.pfd;
+            if (pb < NB) {
+                constexpr int LINE = 128;
+                const int st32 = (sc.Lxh * sc.Ly * sc.Lz) / SB;
+                int pbt = pb + st32; if (pbt >= NB) pbt -= NB;
+                const char* q = (const char*)(a.in.d + ((size_t)pbt * G + grp) * US);
+                for (int i = lu; i < (int)(US * sizeof(ST) / LINE); i += UT) asm volatile("prefetch.global.L2 [%0];" ::"l"(q + (size_t)i * LINE));
+                if constexpr (FORM == FORM_B) {
+                    const char* qx = (const char*)(a.x.d + ((size_t)pb * G + grp) * US);
+                    for (int i = lu; i < (int)(US * sizeof(ST) / LINE); i += UT) asm volatile("prefetch.global.L2 [%0];" ::"l"(qx + (size_t)i * LINE));
+                }
+                constexpr int GL = 4 * RECON * SB * sizeof(T) / LINE;     // lines of one (parity, block) link slab
+                constexpr int CL = 72 * SB * sizeof(T) / LINE;            // lines of one clover block
+                if (grp == 0 % G) {
+                    const char* l = (const char*)(a.gauge + ((size_t)(a.parity * NB + pb) * 4) * (RECON * SB));
+                    for (int i = lu; i < GL; i += UT) asm volatile("prefetch.global.L2 [%0];" ::"l"(l + (size_t)i * LINE));
+                }
+                if (grp == 1 % G) {
+                    const char* l = (const char*)(a.gauge + ((size_t)((1 - a.parity) * NB + pb) * 4) * (RECON * SB));
+                    for (int i = lu; i < GL; i += UT) asm volatile("prefetch.global.L2 [%0];" ::"l"(l + (size_t)i * LINE));
+                }
+                if (grp == 2 % G && a.clover != nullptr) {
+                    const char* l = (const char*)(a.clover + (size_t)pb * (72 * SB));
+                    for (int i = lu; i < CL; i += UT) asm volatile("prefetch.global.L2 [%0];" ::"l"(l + (size_t)i * LINE));
+                }
+            }
         }
     }
 
@@ -186,28 +209,11 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
     const T c0 = (FORM == FORM_B) ? a.coef : T(1);
     const T cp = (sc.t + 1 == sc.Lt) ? c0 * a.tsign : c0;     // boundary sign on the wrapped t terms
     const T cm = (sc.t == 0) ? c0 * a.tsign : c0;
-    if constexpr (MODE == MODE_PIPE || MODE == MODE_PIPE_L2PF) {
-        NbData<S, RPT> da, db;
-#define LQ_LOAD(D, buf) { const int nb_ = neighbour<D>(sc); hop_load<S, RPT, R, RECON>(LQ_NB_PTR(nb_), LQ_NB_NRM(nb_), LQ_LINK(D, nb_), LQ_LINK_S(D, nb_), buf); }
-#define LQ_COMP(D, buf) hop_compute<S, RPT, RECON, ((D) >> 1), (((D) & 1) == 0)>(buf, (D) == 6 ? cp : ((D) == 7 ? cm : c0), ((D) & 1) ? -a.dsign : a.dsign, acc);
-        LQ_LOAD(0, da)
-        LQ_LOAD(1, db) LQ_COMP(0, da)
-        LQ_LOAD(2, da) LQ_COMP(1, db)
-        LQ_LOAD(3, db) LQ_COMP(2, da)
-        LQ_LOAD(4, da) LQ_COMP(3, db)
-        LQ_LOAD(5, db) LQ_COMP(4, da)
-        LQ_LOAD(6, da) LQ_COMP(5, db)
-        LQ_LOAD(7, db) LQ_COMP(6, da)
-        LQ_COMP(7, db)
-#undef LQ_LOAD
-#undef LQ_COMP
-    } else {
 #define LQ_HOP(D) { const int nb_ = neighbour<D>(sc); \
         hop_dir<S, RPT, R, RECON, ((D) >> 1), (((D) & 1) == 0)>(LQ_NB_PTR(nb_), LQ_NB_NRM(nb_), LQ_LINK(D, nb_), LQ_LINK_S(D, nb_), \
                 (D) == 6 ? cp : ((D) == 7 ? cm : c0), ((D) & 1) ? -a.dsign : a.dsign, acc); }
-        LQ_HOP(0) LQ_HOP(1) LQ_HOP(2) LQ_HOP(3) LQ_HOP(4) LQ_HOP(5) LQ_HOP(6) LQ_HOP(7)
+    LQ_HOP(0) LQ_HOP(1) LQ_HOP(2) LQ_HOP(3) LQ_HOP(4) LQ_HOP(5) LQ_HOP(6) LQ_HOP(7)
 #undef LQ_HOP
-    }
 #undef LQ_NB_PTR
 #undef LQ_NB_NRM
 #undef LQ_LINK

@@ -2,44 +2,40 @@
 #pragma once
 #include "dslash_kernel.cuh"
 
-template <class S, int RPT, int R, int RECON, int FORM, int MINB, int MODE>
+template <class S, int RPT, int R, int RECON, int FORM, int MINB>
 static int launch_one(lq_ctx* c, DslashArgs<S> a) {
     constexpr int BLOCK = 128;
-    a.G = a.N / R;
     const long long threads = (long long)a.g.NB * a.G * SB * (R / RPT);
     const int grid = (int)((threads + BLOCK - 1) / BLOCK);
-    dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, MODE><<<grid, BLOCK, 0, c->stream>>>(a);
+    dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB><<<grid, BLOCK, 0, c->stream>>>(a);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
 
 // Register budget per thread = 65536 / (128 * MINB): MINB 2 -> 255, 3 -> 168, 4 -> 128, 5 -> 96 (rounded by ptxas).
-// `variant` (a tuning knob for profiling runs; fp32, RHS groups of 4 only): bit 0 selects the alternative budget of
-// the base mode; bits 1-2 select the kernel mode (1 = L2 prefetch, 2 = software-pipelined directions, 3 = both).
+// `variant` (tuning knob): 0 = default budget, 1 = alternative budget (fp32 only).
 template <class S, int RPT, int R, int RECON, int FORM>
 static int launch_rpt(lq_ctx* c, DslashArgs<S> a, int variant) {
     constexpr bool F64K = S::prec == LQ_FP64;
     constexpr int DEF = F64K ? (RPT == 2 ? 2 : 3) : (RPT == 4 ? 2 : (RPT == 2 ? 3 : 4));
+    a.G = a.N / R;
+    a.dG = make_fastdiv(a.G);
+    a.pfd = c->dslash_pfd;
     if constexpr (S::prec == LQ_FP32) {
         constexpr int ALT = RPT == 4 ? 3 : (RPT == 2 ? 4 : 5);
-        if constexpr (R == 4) {
-            constexpr int PB = RPT == 1 ? 4 : 2;     // pipelined modes hold two neighbours in registers
-            const int mode = (variant >> 1) & 3;
-            if (mode == MODE_L2PF) return launch_one<S, RPT, R, RECON, FORM, DEF, MODE_L2PF>(c, a);
-            if (mode == MODE_PIPE) return launch_one<S, RPT, R, RECON, FORM, PB, MODE_PIPE>(c, a);
-            if (mode == MODE_PIPE_L2PF) return launch_one<S, RPT, R, RECON, FORM, PB, MODE_PIPE_L2PF>(c, a);
-        }
-        if (variant & 1) return launch_one<S, RPT, R, RECON, FORM, ALT, MODE_BASE>(c, a);
+        if (variant == 1) return launch_one<S, RPT, R, RECON, FORM, ALT>(c, a);
     }
-    return launch_one<S, RPT, R, RECON, FORM, DEF, MODE_BASE>(c, a);
+    return launch_one<S, RPT, R, RECON, FORM, DEF>(c, a);
 }
 
+// rpt = right-hand sides per thread; 0 = default: 2 for groups of 4 (measured best on B200 for fp32 at N = 4, 8, 16:
+// 168 registers, 12 warps per SM), else the group width; fp64 caps at 2.
 template <class S, int RECON, int FORM>
 int launch_dslash(lq_ctx* c, DslashArgs<S> a, int rpt, int variant) {
     constexpr int MAXRPT = (S::prec == LQ_FP64) ? 2 : 4;
     const int R = group_width(a.N);
-    if (rpt <= 0) rpt = R;
+    if (rpt <= 0) rpt = (R == 4) ? 2 : R;
     if (rpt > MAXRPT) rpt = MAXRPT;
     if (rpt > R) rpt = R;
     if (R % rpt != 0) return set_err(c, LQ_EINVAL, "rhs-per-thread must divide the RHS group width");

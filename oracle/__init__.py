@@ -180,3 +180,28 @@ def solve_full(dims, U, A, kappa: float, b, tol: float, maxit: int = 10000, t_bc
     it = lib().orc_solve_full(_dims(dims), ctypes.c_int(t_bc), _c(U), _c(A), ctypes.c_double(kappa), _c(b), _c(x),
                               ctypes.c_double(tol), ctypes.c_int(maxit), ctypes.byref(rel))
     return x, int(it), float(rel.value)
+
+
+def site_eval(dims, kind: int, sites, kappa: float, csw: float, coef: float = 0.0, t_bc: int = -1, rhs: int = 0,
+              U=None, gauge_seed: int = 0, eps: float = 0.0, psi=None, in_seed: int = 0, xin=None, x_seed: int = 0) -> np.ndarray:
+    """Site-local hop (kind 0), kernel A (1) or kernel B (2) at `sites` [n][4] = (x, y, z, t) (step 12(ii)).
+    Links come from the host array U or, if U is None, from the counter-based generator (gauge_seed, eps);
+    the input spinor from psi (one RHS, [V][12]) or the generator (in_seed, rhs); likewise xin / x_seed for
+    kernel B.  Returns out[n][4][3]."""
+    V = _vol(dims)
+    sites = np.ascontiguousarray(sites, dtype=np.int32).reshape(-1, 4)
+    n = sites.shape[0]
+    out = np.empty((n, 4, 3), dtype=np.complex128)
+    Ua = _cc(U, (4, V, 3, 3)) if U is not None else None
+    pa = _cc(psi, (V, 12)) if psi is not None else None
+    xa = _cc(xin, (V, 12)) if xin is not None else None
+    f = lib().orc_site_eval
+    f.restype = ctypes.c_int
+    rc = f(_dims(dims), ctypes.c_int(t_bc), ctypes.c_int(kind), ctypes.c_double(kappa), ctypes.c_double(csw), ctypes.c_double(coef),
+           _c(Ua) if Ua is not None else None, ctypes.c_uint64(gauge_seed), ctypes.c_double(eps),
+           _c(pa) if pa is not None else None, ctypes.c_uint64(in_seed),
+           _c(xa) if xa is not None else None, ctypes.c_uint64(x_seed), ctypes.c_long(rhs),
+           ctypes.c_long(n), sites.ctypes.data_as(ctypes.c_void_p), _c(out))
+    if rc != 0:
+        raise ArithmeticError("singular clover block")
+    return out

@@ -108,48 +108,99 @@ static inline void m3_mul(const cplx *a, const cplx *b, cplx *o) {      /* o = a
 static inline void m3_dag(const cplx *a, cplx *o) {
     for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) o[3 * i + j] = conj(a[3 * j + i]);
 }
-static inline const cplx *link_at(const geom_t *g, const cplx *U, int mu, const int *c) {
-    return U + ((long)mu * g->V + site_index(g, c)) * 9;
+
+/* ---------------------------------------------------------------- input sources */
+/* The operator routines below read links and spinors through these two accessors, so that the same
+ * arithmetic serves host arrays (full-lattice entry points) and inputs regenerated per site from the
+ * counter-based generator (site-local entry points, reading #4).
+ * The generator is the oracle's OWN C statement of the recipe in paper_2510_26313_b200/inputs.py:
+ *   mix(z): z += 0x9E3779B97F4A7C15; z = (z ^ z>>30)*0xBF58476D1CE4E5B9; z = (z ^ z>>27)*0x94D049BB133111EB; z ^ z>>31
+ *   key = mix(mix(seed) + stream); b_w = mix(key + 2*i + w); u1 = ((b_0>>11)+0.5)/2^53; u2 = (b_1>>11)/2^53
+ *   cgauss = sqrt(-ln u1) * exp(2 pi i u2)                          (CN(0,1), reading #2)
+ * streams: 1 gauge (index (site*4+mu)*9 + 3*row+col), 2 spinor (index (k*V+site)*12 + 3*spin+colour). */
+static uint64_t mix64(uint64_t z) {
+    z += 0x9E3779B97F4A7C15ULL;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+static cplx cgauss(uint64_t seed, uint64_t stream, uint64_t idx) {
+    uint64_t key = mix64(mix64(seed) + stream);
+    uint64_t b0 = mix64(key + 2 * idx), b1 = mix64(key + 2 * idx + 1);
+    double u1 = ((double)(b0 >> 11) + 0.5) * (1.0 / 9007199254740992.0);
+    double u2 = (double)(b1 >> 11) * (1.0 / 9007199254740992.0);
+    return sqrt(-log(u1)) * cexp(2.0 * 3.14159265358979323846 * u2 * I);
+}
+typedef struct { const cplx *U; uint64_t seed; double eps; } linksrc_t;       /* U != NULL: host array */
+typedef struct { const cplx *psi; uint64_t seed; long rhs; } spinsrc_t;       /* psi != NULL: host array */
+
+/* step 3: W = 1 + eps G; rows a, b: a <- a/|a|; b <- b - (a^dag b) a; b <- b/|b|; c = conj(a x b) */
+static void generated_link(const geom_t *g, const linksrc_t *src, int mu, const int *c, cplx *u) {
+    uint64_t base = ((uint64_t)site_index(g, c) * 4 + (uint64_t)mu) * 9;
+    cplx w[9];
+    for (int e = 0; e < 9; e++) w[e] = src->eps * cgauss(src->seed, 1, base + e) + ((e % 4 == 0) ? 1.0 : 0.0);
+    double n = 0; for (int k = 0; k < 3; k++) n += creal(w[k] * conj(w[k]));
+    n = sqrt(n); for (int k = 0; k < 3; k++) w[k] /= n;
+    cplx d = 0; for (int k = 0; k < 3; k++) d += conj(w[k]) * w[3 + k];
+    for (int k = 0; k < 3; k++) w[3 + k] -= d * w[k];
+    n = 0; for (int k = 0; k < 3; k++) n += creal(w[3 + k] * conj(w[3 + k]));
+    n = sqrt(n); for (int k = 0; k < 3; k++) w[3 + k] /= n;
+    for (int k = 0; k < 3; k++) { int k1 = (k + 1) % 3, k2 = (k + 2) % 3; w[6 + k] = conj(w[k1] * w[3 + k2] - w[k2] * w[3 + k1]); }
+    memcpy(u, w, sizeof w);
+}
+static inline void get_link(const geom_t *g, const linksrc_t *src, int mu, const int *c, cplx *u) {
+    if (src->U) memcpy(u, src->U + ((long)mu * g->V + site_index(g, c)) * 9, 9 * sizeof(cplx));
+    else generated_link(g, src, mu, c, u);
+}
+static inline void get_spinor(const geom_t *g, const spinsrc_t *src, const int *c, cplx *p) {
+    long i = site_index(g, c);
+    if (src->psi) memcpy(p, src->psi + i * 12, 12 * sizeof(cplx));
+    else for (int e = 0; e < 12; e++) p[e] = cgauss(src->seed, 2, ((uint64_t)src->rhs * (uint64_t)g->V + (uint64_t)i) * 12 + e);
 }
 
 /* ---------------------------------------------------------------- hopping term */
 /* step 4: (D psi)(x) = sum_mu [ (1-g_mu) U_mu(x) psi(x+mu) + (1+g_mu) U_mu(x-mu)^dag psi(x-mu) ],
  * step 1: a hop that wraps around t multiplies the hopped term by t_bc (-1 antiperiodic). */
+static void hop_site(const geom_t *g, int t_bc, const linksrc_t *ls, const spinsrc_t *ss, cplx gam[4][4][4], const int *c, cplx acc[4][3]) {
+    int cn[4];
+    memset(acc, 0, 12 * sizeof(cplx));
+    for (int mu = 0; mu < 4; mu++) {
+        cplx tmp[4][3], u[9], p[12];
+        /* forward */
+        shifted(g, c, mu, +1, cn);
+        get_link(g, ls, mu, c, u);
+        get_spinor(g, ss, cn, p);
+        double sgn = (mu == 3 && c[3] == g->L[3] - 1) ? (double)t_bc : 1.0;
+        for (int s = 0; s < 4; s++) for (int a = 0; a < 3; a++) {
+            cplx z = 0; for (int b = 0; b < 3; b++) z += u[3 * a + b] * p[3 * s + b]; tmp[s][a] = z; }
+        for (int s = 0; s < 4; s++) for (int a = 0; a < 3; a++) {
+            cplx z = 0;
+            for (int sp = 0; sp < 4; sp++) z += ((s == sp ? 1.0 : 0.0) - gam[mu][s][sp]) * tmp[sp][a];
+            acc[s][a] += sgn * z; }
+        /* backward */
+        shifted(g, c, mu, -1, cn);
+        get_link(g, ls, mu, cn, u);
+        get_spinor(g, ss, cn, p);
+        sgn = (mu == 3 && c[3] == 0) ? (double)t_bc : 1.0;
+        for (int s = 0; s < 4; s++) for (int a = 0; a < 3; a++) {
+            cplx z = 0; for (int b = 0; b < 3; b++) z += conj(u[3 * b + a]) * p[3 * s + b]; tmp[s][a] = z; }
+        for (int s = 0; s < 4; s++) for (int a = 0; a < 3; a++) {
+            cplx z = 0;
+            for (int sp = 0; sp < 4; sp++) z += ((s == sp ? 1.0 : 0.0) + gam[mu][s][sp]) * tmp[sp][a];
+            acc[s][a] += sgn * z; }
+    }
+}
 void orc_hop(const int *dims, int t_bc, const cplx *U, const cplx *in, cplx *out) {
     geom_t g = make_geom(dims);
     cplx gam[4][4][4];
     for (int mu = 0; mu < 4; mu++) gamma_matrix(mu, gam[mu]);
+    linksrc_t ls = {U, 0, 0.0}; spinsrc_t ss = {in, 0, 0};
 #pragma omp parallel for schedule(static)
     for (long i = 0; i < g.V; i++) {
-        int c[4], cn[4];
+        int c[4];
         site_coords(&g, i, c);
         cplx acc[4][3];
-        memset(acc, 0, sizeof acc);
-        for (int mu = 0; mu < 4; mu++) {
-            cplx tmp[4][3];
-            /* forward */
-            shifted(&g, c, mu, +1, cn);
-            const cplx *u = link_at(&g, U, mu, c);
-            const cplx *p = in + site_index(&g, cn) * 12;
-            double sgn = (mu == 3 && c[3] == g.L[3] - 1) ? (double)t_bc : 1.0;
-            for (int s = 0; s < 4; s++) for (int a = 0; a < 3; a++) {
-                cplx z = 0; for (int b = 0; b < 3; b++) z += u[3 * a + b] * p[3 * s + b]; tmp[s][a] = z; }
-            for (int s = 0; s < 4; s++) for (int a = 0; a < 3; a++) {
-                cplx z = 0;
-                for (int sp = 0; sp < 4; sp++) z += ((s == sp ? 1.0 : 0.0) - gam[mu][s][sp]) * tmp[sp][a];
-                acc[s][a] += sgn * z; }
-            /* backward */
-            shifted(&g, c, mu, -1, cn);
-            u = link_at(&g, U, mu, cn);
-            p = in + site_index(&g, cn) * 12;
-            sgn = (mu == 3 && c[3] == 0) ? (double)t_bc : 1.0;
-            for (int s = 0; s < 4; s++) for (int a = 0; a < 3; a++) {
-                cplx z = 0; for (int b = 0; b < 3; b++) z += conj(u[3 * b + a]) * p[3 * s + b]; tmp[s][a] = z; }
-            for (int s = 0; s < 4; s++) for (int a = 0; a < 3; a++) {
-                cplx z = 0;
-                for (int sp = 0; sp < 4; sp++) z += ((s == sp ? 1.0 : 0.0) + gam[mu][s][sp]) * tmp[sp][a];
-                acc[s][a] += sgn * z; }
-        }
+        hop_site(&g, t_bc, &ls, &ss, gam, c, acc);
         memcpy(out + i * 12, acc, sizeof acc);
     }
 }
@@ -157,37 +208,41 @@ void orc_hop(const int *dims, int t_bc, const cplx *U, const cplx *in, cplx *out
 /* ---------------------------------------------------------------- field strength */
 /* step 5: Q_{mu nu}(x) = sum of the four plaquette leaves starting and ending at x, all with
  * the same orientation; F = (Q - Q^dag)/(8i).  Periodic wrap, no boundary sign. */
-static void clover_leaf_sum(const geom_t *g, const cplx *U, const int *x, int mu, int nu, cplx *Q) {
+static void clover_leaf_sum(const geom_t *g, const linksrc_t *ls, const int *x, int mu, int nu, cplx *Q) {
     int a[4], b[4], c[4];
-    cplx t1[9], t2[9], d1[9], d2[9];
+    cplx t1[9], t2[9], d1[9], d2[9], u1[9], u2[9], u3[9], u4[9];
     memset(Q, 0, 9 * sizeof(cplx));
     /* leaf 1: U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag */
     shifted(g, x, mu, 1, a); shifted(g, x, nu, 1, b);
-    m3_mul(link_at(g, U, mu, x), link_at(g, U, nu, a), t1);
-    m3_dag(link_at(g, U, mu, b), d1); m3_mul(t1, d1, t2);
-    m3_dag(link_at(g, U, nu, x), d2); m3_mul(t2, d2, t1);
+    get_link(g, ls, mu, x, u1); get_link(g, ls, nu, a, u2); get_link(g, ls, mu, b, u3); get_link(g, ls, nu, x, u4);
+    m3_mul(u1, u2, t1);
+    m3_dag(u3, d1); m3_mul(t1, d1, t2);
+    m3_dag(u4, d2); m3_mul(t2, d2, t1);
     for (int k = 0; k < 9; k++) Q[k] += t1[k];
     /* leaf 2: U_nu(x) U_mu(x-mu+nu)^dag U_nu(x-mu)^dag U_mu(x-mu) */
     shifted(g, x, mu, -1, a); shifted(g, a, nu, 1, b);
-    m3_dag(link_at(g, U, mu, b), d1); m3_mul(link_at(g, U, nu, x), d1, t1);
-    m3_dag(link_at(g, U, nu, a), d2); m3_mul(t1, d2, t2);
-    m3_mul(t2, link_at(g, U, mu, a), t1);
+    get_link(g, ls, nu, x, u1); get_link(g, ls, mu, b, u2); get_link(g, ls, nu, a, u3); get_link(g, ls, mu, a, u4);
+    m3_dag(u2, d1); m3_mul(u1, d1, t1);
+    m3_dag(u3, d2); m3_mul(t1, d2, t2);
+    m3_mul(t2, u4, t1);
     for (int k = 0; k < 9; k++) Q[k] += t1[k];
     /* leaf 3: U_mu(x-mu)^dag U_nu(x-mu-nu)^dag U_mu(x-mu-nu) U_nu(x-nu) */
     shifted(g, x, mu, -1, a); shifted(g, a, nu, -1, b); shifted(g, x, nu, -1, c);
-    m3_dag(link_at(g, U, mu, a), d1); m3_dag(link_at(g, U, nu, b), d2); m3_mul(d1, d2, t1);
-    m3_mul(t1, link_at(g, U, mu, b), t2); m3_mul(t2, link_at(g, U, nu, c), t1);
+    get_link(g, ls, mu, a, u1); get_link(g, ls, nu, b, u2); get_link(g, ls, mu, b, u3); get_link(g, ls, nu, c, u4);
+    m3_dag(u1, d1); m3_dag(u2, d2); m3_mul(d1, d2, t1);
+    m3_mul(t1, u3, t2); m3_mul(t2, u4, t1);
     for (int k = 0; k < 9; k++) Q[k] += t1[k];
     /* leaf 4: U_nu(x-nu)^dag U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^dag */
     shifted(g, x, nu, -1, a); shifted(g, a, mu, 1, b);
-    m3_dag(link_at(g, U, nu, a), d1); m3_mul(d1, link_at(g, U, mu, a), t1);
-    m3_mul(t1, link_at(g, U, nu, b), t2);
-    m3_dag(link_at(g, U, mu, x), d2); m3_mul(t2, d2, t1);
+    get_link(g, ls, nu, a, u1); get_link(g, ls, mu, a, u2); get_link(g, ls, nu, b, u3); get_link(g, ls, mu, x, u4);
+    m3_dag(u1, d1); m3_mul(d1, u2, t1);
+    m3_mul(t1, u3, t2);
+    m3_dag(u4, d2); m3_mul(t2, d2, t1);
     for (int k = 0; k < 9; k++) Q[k] += t1[k];
 }
-static void field_strength_site(const geom_t *g, const cplx *U, const int *x, int mu, int nu, cplx *F) {
+static void field_strength_site(const geom_t *g, const linksrc_t *ls, const int *x, int mu, int nu, cplx *F) {
     cplx Q[9], Qd[9];
-    clover_leaf_sum(g, U, x, mu, nu, Q);
+    clover_leaf_sum(g, ls, x, mu, nu, Q);
     m3_dag(Q, Qd);
     for (int k = 0; k < 9; k++) F[k] = (Q[k] - Qd[k]) / (8.0 * I);
 }
@@ -195,20 +250,21 @@ static void field_strength_site(const geom_t *g, const cplx *U, const int *x, in
 void orc_field_strength(const int *dims, const cplx *U, cplx *F) {
     geom_t g = make_geom(dims);
     static const int PL[6][2] = {{0, 1}, {0, 2}, {0, 3}, {1, 2}, {1, 3}, {2, 3}};
+    linksrc_t ls = {U, 0, 0.0};
 #pragma omp parallel for schedule(static)
     for (long i = 0; i < g.V; i++) {
         int c[4]; site_coords(&g, i, c);
-        for (int p = 0; p < 6; p++) field_strength_site(&g, U, c, PL[p][0], PL[p][1], F + ((long)p * g.V + i) * 9);
+        for (int p = 0; p < 6; p++) field_strength_site(&g, &ls, c, PL[p][0], PL[p][1], F + ((long)p * g.V + i) * 9);
     }
 }
 
 /* ---------------------------------------------------------------- clover term */
 /* step 6: A(x) = 1 - kappa*csw * sum_{mu<nu} sigma_{mu nu} (x) F_{mu nu}(x), dense 12x12. */
-static void clover_site(const geom_t *g, const cplx *U, const int *x, double kappa, double csw, cplx *A) {
+static void clover_site(const geom_t *g, const linksrc_t *ls, const int *x, double kappa, double csw, cplx *A) {
     for (int r = 0; r < 12; r++) for (int c = 0; c < 12; c++) A[12 * r + c] = (r == c) ? 1.0 : 0.0;
     for (int mu = 0; mu < 4; mu++) for (int nu = mu + 1; nu < 4; nu++) {
         cplx F[9], sg[4][4];
-        field_strength_site(g, U, x, mu, nu, F);
+        field_strength_site(g, ls, x, mu, nu, F);
         sigma_matrix(mu, nu, sg);
         for (int s = 0; s < 4; s++) for (int sp = 0; sp < 4; sp++)
             for (int a = 0; a < 3; a++) for (int b = 0; b < 3; b++)
@@ -217,8 +273,9 @@ static void clover_site(const geom_t *g, const cplx *U, const int *x, double kap
 }
 void orc_clover(const int *dims, const cplx *U, double kappa, double csw, cplx *A) {
     geom_t g = make_geom(dims);
+    linksrc_t ls = {U, 0, 0.0};
 #pragma omp parallel for schedule(static)
-    for (long i = 0; i < g.V; i++) { int c[4]; site_coords(&g, i, c); clover_site(&g, U, c, kappa, csw, A + i * 144); }
+    for (long i = 0; i < g.V; i++) { int c[4]; site_coords(&g, i, c); clover_site(&g, &ls, c, kappa, csw, A + i * 144); }
 }
 
 /* general complex n x n inverse, Gauss-Jordan with partial pivoting; returns 0 ok, -1 singular */
@@ -432,4 +489,47 @@ int orc_num_threads(void) {
 #else
     return 1;
 #endif
+}
+
+/* ---------------------------------------------------------------- site-local evaluators */
+/* hop / kernel-A / kernel-B output at single sites, with links and input spinors
+ * either taken from host arrays (U, psi != NULL: used to pin this routine against the full-lattice one) or
+ * regenerated on the fly from the counter-based generator (U == NULL: gauge seed/eps; psi == NULL: spinor seed,
+ * rhs index), building F_{mu nu}, A and A^{-1} for the site from its 4-leaf neighbourhood.  This is what makes
+ * parity checkable at 32^3x64 and 64^3x128 without host copies of the fields.
+ *   kind 0: out = (D in)(x)
+ *   kind 1: out = A(x)^{-1} (D in)(x)                               "kernel A"
+ *   kind 2: out = A(x) xin(x) + coef (D in)(x)                      "kernel B" (row a4; coef = -kappa^2 there)
+ * sites[n][4] = (x, y, z, t); out[n][12].  `in` lives on the parity opposite to the listed sites; the
+ * generated spinor stream gives every site of the lattice a value, only the neighbours are read. */
+int orc_site_eval(const int *dims, int t_bc, int kind, double kappa, double csw, double coef,
+                  const cplx *U, uint64_t gauge_seed, double eps,
+                  const cplx *psi, uint64_t in_seed, const cplx *xin, uint64_t x_seed, long rhs,
+                  long nsites, const int *sites, cplx *out) {
+    geom_t g = make_geom(dims);
+    cplx gam[4][4][4];
+    for (int mu = 0; mu < 4; mu++) gamma_matrix(mu, gam[mu]);
+    linksrc_t ls = {U, gauge_seed, eps};
+    spinsrc_t ss = {psi, in_seed, rhs};
+    spinsrc_t xs = {xin, x_seed, rhs};
+    int bad = 0;
+#pragma omp parallel for schedule(dynamic, 16) reduction(| : bad)
+    for (long n = 0; n < nsites; n++) {
+        const int *c = sites + 4 * n;
+        cplx d[4][3], A[144], Ainv[144], r[12];
+        hop_site(&g, t_bc, &ls, &ss, gam, c, d);
+        const cplx *dv = &d[0][0];
+        if (kind == 0) { memcpy(out + n * 12, dv, 12 * sizeof(cplx)); continue; }
+        clover_site(&g, &ls, c, kappa, csw, A);
+        if (kind == 1) {
+            if (dense_inverse(12, A, Ainv)) { bad |= 1; continue; }
+            for (int i = 0; i < 12; i++) { cplx z = 0; for (int j = 0; j < 12; j++) z += Ainv[12 * i + j] * dv[j]; r[i] = z; }
+        } else {
+            cplx xv[12];
+            get_spinor(&g, &xs, c, xv);
+            for (int i = 0; i < 12; i++) { cplx z = 0; for (int j = 0; j < 12; j++) z += A[12 * i + j] * xv[j]; r[i] = z + coef * dv[i]; }
+        }
+        memcpy(out + n * 12, r, sizeof r);
+    }
+    return bad ? -1 : 0;
 }

@@ -40,6 +40,14 @@ template <class S> struct DslashArgs {
 __device__ __forceinline__ float fm(float a, float b, float c) { return fmaf(a, b, c); }
 __device__ __forceinline__ double fm(double a, double b, double c) { return fma(a, b, c); }
 
+// two int16 packed in a 32-bit word -> two floats
+__device__ __forceinline__ void s16x2_to_f32(unsigned w, float& lo, float& hi) {
+    int a, b;
+    asm("prmt.b32 %0, %1, 0, 0x9910;" : "=r"(a) : "r"(w));   // bytes b0 b1 sign(b1) sign(b1)
+    asm("prmt.b32 %0, %1, 0, 0xBB32;" : "=r"(b) : "r"(w));   // bytes b2 b3 sign(b3) sign(b3)
+    lo = (float)a; hi = (float)b;
+}
+
 // ---- RPT-wide loads / stores of one real of one site ------------------------------------------------
 template <class S, int RPT>
 __device__ __forceinline__ void load_comp(const typename S::store_t* __restrict__ p, typename S::comp_t* o) {
@@ -54,9 +62,11 @@ __device__ __forceinline__ void load_comp(const typename S::store_t* __restrict_
         } else if constexpr (RPT == 2) { double2 v = __ldg((const double2*)p); o[0] = v.x; o[1] = v.y; }
         else { o[0] = __ldg(p); }
     } else {
-        if constexpr (RPT == 4) { short4 v = __ldg((const short4*)p); o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
-        else if constexpr (RPT == 2) { short2 v = __ldg((const short2*)p); o[0] = v.x; o[1] = v.y; }
-        else { o[0] = __ldg(p); }
+        // int16 -> fp32 as byte-permute sign extension + I2FP.F32.S32 (full rate); the direct I2F.S16 form that the
+        // compiler picks for (float)short runs on the 16-lane conversion unit and made this kernel slower than fp32
+        if constexpr (RPT == 4) { uint2 v = __ldg((const uint2*)p); s16x2_to_f32(v.x, o[0], o[1]); s16x2_to_f32(v.y, o[2], o[3]); }
+        else if constexpr (RPT == 2) { unsigned v = __ldg((const unsigned*)p); s16x2_to_f32(v, o[0], o[1]); }
+        else { int v = __ldg(p); int w; asm("mov.b32 %0, %1;" : "=r"(w) : "r"(v)); o[0] = (float)w; }
     }
 }
 template <int RPT> __device__ __forceinline__ void load_norm(const float* __restrict__ p, float* o) {

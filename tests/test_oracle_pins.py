@@ -368,3 +368,51 @@ def test_config0_solve(oracle_lib, rough):
     x2, it2, res2 = oracle_lib.solve_full(DIMS, r["U"], r["A"], r["kappa"], b, 1e-10)
     assert it2 > 0 and rel(x, x2) < 1e-9
     assert it <= it2           # even-odd preconditioning does not make CG slower
+
+
+# ------------------------------------------------------------------ site-local evaluator
+def _all_sites(dims, parity):
+    x, y, z, t = lex_coords(dims)
+    m = ((x + y + z + t) % 2 == parity)
+    return np.stack([x[m], y[m], z[m], t[m]], axis=1).astype(np.int32)
+
+
+def test_site_local_evaluator_matches_full_lattice(oracle_lib):
+    """The per-site routine used for full-size parity (32^3x64, 64^3x128) against the pinned full-lattice
+    operator on host arrays: hop, kernel A = A^-1 D, kernel B = A x - kappa^2 D y, every odd / even site."""
+    import oracle
+    dims, kappa, csw = (4, 6, 4, 8), 0.124, 1.1
+    U = inputs.make_links(dims, 31, 0.3)
+    psi = inputs.gaussian_spinors(dims, 1, 32)[0].reshape(-1, 12)
+    xin = inputs.gaussian_spinors(dims, 1, 33)[0].reshape(-1, 12)
+    A = oracle.clover(dims, U, kappa, csw)
+    Ainv = oracle.clover_inverse(A)
+    Lx, Ly, Lz, Lt = dims
+    full_hop = oracle.hop(dims, U, psi).reshape(Lt, Lz, Ly, Lx, 4, 3)
+    full_A = oracle.apply_site_matrix(Ainv, full_hop.reshape(-1, 12)).reshape(Lt, Lz, Ly, Lx, 4, 3)
+    full_B = (oracle.apply_site_matrix(A, xin) - kappa ** 2 * full_hop.reshape(-1, 12)).reshape(Lt, Lz, Ly, Lx, 4, 3)
+    for parity in (0, 1):
+        s = _all_sites(dims, parity)
+        pick = lambda f: f[s[:, 3], s[:, 2], s[:, 1], s[:, 0]]
+        assert rel(oracle.site_eval(dims, 0, s, kappa, csw, U=U, psi=psi), pick(full_hop)) < 1e-14
+        assert rel(oracle.site_eval(dims, 1, s, kappa, csw, U=U, psi=psi), pick(full_A)) < 1e-13
+        assert rel(oracle.site_eval(dims, 2, s, kappa, csw, coef=-kappa ** 2, U=U, psi=psi, xin=xin), pick(full_B)) < 1e-14
+
+
+def test_site_local_generator_matches_input_recipe(oracle_lib):
+    """The oracle's own C copy of the counter-based generator (links, spinors of any RHS index) against the numpy
+    statement of the recipe in inputs.py: regenerated inputs give the same outputs as host arrays."""
+    import oracle
+    dims, kappa, csw, eps = (4, 4, 6, 4), 0.12, 1.0, 0.3
+    U = inputs.make_links(dims, 1002, eps)
+    psi = inputs.gaussian_spinors(dims, 3, 7001)
+    xin = inputs.gaussian_spinors(dims, 3, 7002)
+    s = _all_sites(dims, 1)
+    for k in (0, 2):
+        want = oracle.site_eval(dims, 2, s, kappa, csw, coef=-0.3, U=U, psi=psi[k].reshape(-1, 12), xin=xin[k].reshape(-1, 12))
+        got = oracle.site_eval(dims, 2, s, kappa, csw, coef=-0.3, rhs=k, gauge_seed=1002, eps=eps, in_seed=7001, x_seed=7002)
+        assert rel(got, want) < 1e-13
+    # periodic time boundary flag is honoured by the site routine too
+    a = oracle.site_eval(dims, 0, s, kappa, csw, t_bc=+1, U=U, psi=psi[0].reshape(-1, 12))
+    b = oracle.hop(dims, U, psi[0].reshape(-1, 12), t_bc=+1).reshape(dims[3], dims[2], dims[1], dims[0], 4, 3)[s[:, 3], s[:, 2], s[:, 1], s[:, 0]]
+    assert rel(a, b) < 1e-14

@@ -134,6 +134,12 @@ int lq_unpack(lq_ctx* ctx, void* canonical_out, const void* native_in, int nrhs,
 /* Bench only: complex-Gaussian spinors written straight into a native device buffer (full lattice if
  * parity_only == 0, else that many sites of parity `parity`), same counter-based generator. */
 int lq_fill_spinor_random(lq_ctx* ctx, void* native_out, int nrhs, int prec, uint64_t seed, int parity_only, int parity);
+/* Read back selected sites of ONE parity block of a native device buffer (what makes parity checkable at
+ * 64^3x128 without a canonical copy of the field, SURVEY 8(d) configs[4]): sites_xyzt is a HOST array of
+ * nsites x 4 ints (x, y, z, t), every site of the parity the block holds; out is a HOST array of
+ * nsites x nrhs x 24 doubles (spin-major, colour, re/im; half storage dequantised).  Synchronises the stream. */
+int lq_gather_sites(lq_ctx* ctx, double* out, const void* native_parity_block, int nrhs, int prec,
+                    long long nsites, const int* sites_xyzt);
 
 /* ---- batched mixed-precision solve (rows a2, a6-a11) ---------------------------------------------- */
 typedef struct {

@@ -25,7 +25,7 @@ PREC = {"fp64": LQ_FP64, "fp32": LQ_FP32, "half": LQ_HALF}
 
 EXPORTS = ["lq_create", "lq_destroy", "lq_last_error", "lq_set_allocator", "lq_load_gauge", "lq_fill_gauge_random",
            "lq_build_clover", "lq_apply", "lq_native_bytes", "lq_pack", "lq_unpack", "lq_fill_spinor_random", "lq_solve",
-           "lq_set_tuning", "lq_kernel_launches"]
+           "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites"]
 
 
 class SolveParam(ctypes.Structure):
@@ -74,6 +74,7 @@ def load_library():
     lib.lq_fill_spinor_random.argtypes = [vp, vp, ci, ci, u64, ci, ci]
     lib.lq_solve.argtypes = [vp, vp, vp, ci, ci, ci, ctypes.POINTER(SolveParam), ctypes.POINTER(SolveInfo)]
     lib.lq_set_tuning.argtypes = [vp, ci, ci, ci]
+    lib.lq_gather_sites.argtypes = [vp, vp, vp, ci, ci, ctypes.c_longlong, vp]
     lib.lq_kernel_launches.argtypes = [vp]; lib.lq_kernel_launches.restype = ctypes.c_longlong
     _lib = lib
     return lib
@@ -196,6 +197,15 @@ class Context:
     def fill_spinor_random(self, native, nrhs: int, prec: int, seed: int, parity_only: bool = False, parity: int = 0):
         self._enter()
         self._check(self.lib.lq_fill_spinor_random(self.h, ctypes.c_void_p(native.data_ptr()), nrhs, prec, seed, int(parity_only), parity))
+
+    def gather_sites(self, native_parity_block, nrhs: int, prec: int, sites) -> np.ndarray:
+        """Values of one parity block of a native device buffer at sites [n][4] = (x, y, z, t): complex128 [n][nrhs][4][3]."""
+        self._enter()
+        sites = np.ascontiguousarray(sites, dtype=np.int32).reshape(-1, 4)
+        out = np.empty((sites.shape[0], nrhs, 24), dtype=np.float64)
+        self._check(self.lib.lq_gather_sites(self.h, ctypes.c_void_p(out.ctypes.data), ctypes.c_void_p(native_parity_block.data_ptr()),
+                                             nrhs, prec, sites.shape[0], ctypes.c_void_p(sites.ctypes.data)))
+        return out.view(np.complex128).reshape(sites.shape[0], nrhs, 4, 3)
 
     # ------------------------------------------------------------------ operator
     def apply_native(self, op: int, out, inp, nrhs: int, prec: int, in2=None):

@@ -181,6 +181,23 @@ int lq_fill_spinor_random(lq_ctx* c, void* native_out, int nrhs, int prec, uint6
     return fill_spinor(c, native_out, nrhs, prec, seed, parity_only, parity);
 }
 
+int lq_gather_sites(lq_ctx* c, double* out, const void* native_parity_block, int nrhs, int prec, long long nsites, const int* sites_xyzt) {
+    if (!c || !out || !native_parity_block || !sites_xyzt || !nrhs_ok(nrhs) || nsites < 1) return set_err(c, LQ_EINVAL, "lq_gather_sites: bad argument");
+    if (prec != LQ_FP64 && prec != LQ_FP32 && prec != LQ_HALF) return set_err(c, LQ_EINVAL, "bad precision");
+    for (long long n = 0; n < nsites; n++)
+        for (int k = 0; k < 4; k++) if (sites_xyzt[4 * n + k] < 0 || sites_xyzt[4 * n + k] >= c->g.L[k]) return set_err(c, LQ_EINVAL, "lq_gather_sites: site out of range");
+    cudaSetDevice(c->device);
+    int* d_sites = (int*)dev_alloc(c, (size_t)nsites * 4 * sizeof(int));
+    double* d_out = (double*)dev_alloc(c, (size_t)nsites * nrhs * 24 * sizeof(double));
+    int rc = (!d_sites || !d_out) ? LQ_ENOMEM : 0;
+    if (rc == 0 && cudaMemcpyAsync(d_sites, sites_xyzt, (size_t)nsites * 4 * sizeof(int), cudaMemcpyHostToDevice, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "H2D copy failed");
+    if (rc == 0) rc = spinor_gather_sites(c, d_out, native_parity_block, nrhs, prec, nsites, d_sites);
+    if (rc == 0 && cudaMemcpyAsync(out, d_out, (size_t)nsites * nrhs * 24 * sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "D2H copy failed");
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess && rc == 0) rc = set_err(c, LQ_ECUDA, "lq_gather_sites failed");
+    if (d_sites) dev_free(c, d_sites);
+    if (d_out) dev_free(c, d_out);
+    return rc;
+}
 // the operator on native buffers
 static int apply_native(lq_ctx* c, int op, void* out, const void* in, const void* in2, int n, int prec) {
     const size_t pb = parity_bytes(c->g, n, prec);

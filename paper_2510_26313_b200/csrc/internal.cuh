@@ -23,6 +23,7 @@ int spinor_pack(lq_ctx* c, void* native_full, const void* dev_canonical, int nrh
 int spinor_unpack(lq_ctx* c, void* dev_canonical, const void* native_full, int nrhs, int prec, int out_prec);
 int spinor_convert(lq_ctx* c, void* dst, int dst_prec, const void* src, int src_prec, int nrhs, const double* d_scale /*per rhs, multiplies*/, int invert_scale);
 int spinor_zero_parity(lq_ctx* c, void* parity_block, int nrhs, int prec);
+int spinor_gather_sites(lq_ctx* c, double* dev_out, const void* parity_block, int nrhs, int prec, long long nsites, const int* dev_sites);
 int canonical_zero_parity(lq_ctx* c, void* dev_canonical, int nrhs, int prec, int parity);
 
 // clover.cu

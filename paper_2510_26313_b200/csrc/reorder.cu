@@ -191,3 +191,29 @@ int canonical_zero_parity(lq_ctx* c, void* dev_canonical, int nrhs, int prec, in
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
+
+// ---- read back selected sites of one parity block ----------------------------------------------------------------
+template <class S>
+__global__ void gather_sites_kernel(Geom g, int N, SView<S> v, long long nsites, const int* __restrict__ sites, double* __restrict__ out) {
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= nsites * N) return;
+    const int k = (int)(tid % N);
+    const long long n = tid / N;
+    int parity, cb;
+    coords_to_cb(g, sites[4 * n], sites[4 * n + 1], sites[4 * n + 2], sites[4 * n + 3], parity, cb);
+    double o[24];
+    load_site<S>(v, N, cb, k, o);
+#pragma unroll
+    for (int j = 0; j < 24; j++) out[(n * N + k) * 24 + j] = o[j];
+}
+int spinor_gather_sites(lq_ctx* c, double* dev_out, const void* parity_block, int nrhs, int prec, long long nsites, const int* dev_sites) {
+    const long long threads = nsites * nrhs;
+    const int block = 128; const int grid = (int)((threads + block - 1) / block);
+    void* pb = const_cast<void*>(parity_block);
+    if (prec == LQ_FP64) gather_sites_kernel<F64><<<grid, block, 0, c->stream>>>(c->g, nrhs, make_view<F64>(c->g, pb, nrhs, 0), nsites, dev_sites, dev_out);
+    else if (prec == LQ_FP32) gather_sites_kernel<F32><<<grid, block, 0, c->stream>>>(c->g, nrhs, make_view<F32>(c->g, pb, nrhs, 0), nsites, dev_sites, dev_out);
+    else gather_sites_kernel<H16><<<grid, block, 0, c->stream>>>(c->g, nrhs, make_view<H16>(c->g, pb, nrhs, 0), nsites, dev_sites, dev_out);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
+}

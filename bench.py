@@ -138,6 +138,17 @@ def time_dslash(ctx, B, kind: str, prec: str, nrhs: int, recon: int, iters: int 
                 gbs=bps * Vh * nrhs / sec * 1e-9, gflops=flop * Vh * nrhs / sec * 1e-9, nsets=nsets)
 
 
+def ncu_traffic(lattice, r):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of this kernel from the committed ncu --set full
+    capture, if one exists for this lattice / kernel / batch (profiles/traffic.json, written by hand from the ncu report)."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        d = json.load(f)
+    return d.get("%s:%s:%s:%d" % (lattice, r["kind"], r["prec"], r["nrhs"]))
+
+
 def roofline_entry(r, peak, peak_src, traffic=None):
     return {"bound": "hbm", "kernel": "dslash_kernel<%s,N=%d,recon=%d,form=%s>" % (r["prec"], r["nrhs"], r["recon"], r["kind"]),
             "achieved": round(r["gbs"], 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s",
@@ -225,6 +236,29 @@ def run_reference(args, rank, world):
     print(json.dumps(line))
 
 
+# ------------------------------------------------------------------------------------------------ multi-rank plumbing
+def max_over_ranks(values, device=None):
+    """Replicas-only scaling: every rank runs the same step on its own RHS batch; the job's time is the
+    slowest rank's.  Works on whatever torch.distributed backend is initialised (nccl on GPUs, gloo in the CPU tests)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    t = torch.tensor(list(values), dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_seconds_per_rhs(seconds_total, steps, nrhs_per_rank, world):
+    """metric value: seconds per RHS of the whole job = max-over-ranks step time / RHS solved by all ranks per step."""
+    return seconds_total / steps / (nrhs_per_rank * world)
+
+
+def rank_gauge_seed(base_seed, rank):
+    """Each replica works on its own gauge configuration (independent tasks)."""
+    return base_seed + rank
+
+
 # ------------------------------------------------------------------------------------------------ single-operator mode
 def run_op(args, B, device):
     f = args.op.split(":")
@@ -243,7 +277,7 @@ def run_op(args, B, device):
     r = time_dslash(ctx, B, kind, prec, n, c["recon"], iters=args.op_iters, warmup=max(args.warmup, 3))
     clocks = sampler.stop()
     ctx.close()
-    e = roofline_entry(r, peak, peak_src)
+    e = roofline_entry(r, peak, peak_src, ncu_traffic("x".join(map(str, c["dims"])), r))
     e.update({"op": args.op, "lattice": "x".join(map(str, c["dims"])), "iters": args.op_iters, "clocks": clocks})
     print(json.dumps(e))
 
@@ -285,9 +319,9 @@ def main():
     peak, peak_src, _ = measured_peaks()
     ctx = B.Context(dims, device=local)
     if wl["cfg"] == 1:
-        ctx.load_gauge(inputs.make_links(dims, c["gauge_seed"] + rank, c["eps"]), recon=c["recon"])
+        ctx.load_gauge(inputs.make_links(dims, rank_gauge_seed(c["gauge_seed"], rank), c["eps"]), recon=c["recon"])
     else:
-        ctx.fill_gauge_random(c["gauge_seed"] + rank, c["eps"], recon=c["recon"])
+        ctx.fill_gauge_random(rank_gauge_seed(c["gauge_seed"], rank), c["eps"], recon=c["recon"])
     ctx.build_clover(c["kappa"], c["csw"])
     b_host = torch.from_numpy(make_sources_host(wl["cfg"])).pin_memory()
     x_host = torch.empty_like(b_host).pin_memory()
@@ -325,10 +359,7 @@ def main():
     torch.cuda.synchronize()
     t_e2e = time.perf_counter() - w0
     clocks = sampler.stop() if sampler else None
-    if world > 1:
-        tt = torch.tensor([t_dev, t_e2e], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_dev, t_e2e = float(tt[0]), float(tt[1])
+    t_dev, t_e2e = max_over_ranks([t_dev, t_e2e], device="cuda")
 
     # ---- dominant kernel alone (roofline), same lattice and batch
     rA = time_dslash(ctx, B, "A", "half" if wl["inner"] == "half" else "fp32", nrhs, c["recon"], iters=50)
@@ -347,7 +378,7 @@ def main():
         extras["cpu_baseline"] = cpu_baseline(wl["cfg"])
     total_rhs = nrhs * world
     line = {
-        "metric": "batched CG sec/RHS", "value": t_dev / args.steps / total_rhs, "unit": "s/RHS", "n_gpus": world, "steps": args.steps,
+        "metric": "batched CG sec/RHS", "value": whole_job_seconds_per_rhs(t_dev, args.steps, nrhs, world), "unit": "s/RHS", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if wl["inner"] == "fp32" else "i16+f32", "data": "synthetic",
         "config": {"workload": wl["desc"], "lattice": "x".join(map(str, dims)), "nrhs_per_gpu": nrhs, "parallelism": "replicas only (RHS-independent)",
@@ -355,11 +386,11 @@ def main():
                    "cuda_graph": not args.no_graph, "kappa": c["kappa"], "csw": c["csw"], "tol": c["tol"]},
         "solver": {"outer_cycles": info["outer_cycles"], "inner_iters": info["inner_iters"], "true_rel_residual_max": max(info["true_rel_residual"]),
                    "dslash_applies_per_step": info["dslash_applies"]},
-        "e2e": {"value": t_e2e / args.steps / total_rhs, "unit": "s/RHS", "h2d_bytes_per_step": b_host.numel() * 16, "d2h_bytes_per_step": x_host.numel() * 16},
+        "e2e": {"value": whole_job_seconds_per_rhs(t_e2e, args.steps, nrhs, world), "unit": "s/RHS", "h2d_bytes_per_step": b_host.numel() * 16, "d2h_bytes_per_step": x_host.numel() * 16},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "roofline": roofline_entry(rA, peak, peak_src),
-        "roofline_kernel_B": roofline_entry(rB, peak, peak_src),
+        "roofline": roofline_entry(rA, peak, peak_src, ncu_traffic("x".join(map(str, dims)), rA)),
+        "roofline_kernel_B": roofline_entry(rB, peak, peak_src, ncu_traffic("x".join(map(str, dims)), rB)),
     }
     line.update(extras)
     print(json.dumps(line))

@@ -27,6 +27,14 @@ void dev_free(lq_ctx* c, void* p) {
     else if (!c->alloc_fn) cudaFree(p);
 }
 
+int ensure_partials(lq_ctx* c, size_t elems) {
+    if (elems <= c->red_partials_elems) return 0;
+    if (c->red_partials) dev_free(c, c->red_partials);
+    c->red_partials_elems = elems * 2;
+    c->red_partials = (double*)dev_alloc(c, c->red_partials_elems * sizeof(double));
+    if (!c->red_partials) { c->red_partials_elems = 0; return LQ_ENOMEM; }
+    return 0;
+}
 static bool nrhs_ok(int n) { return n == 1 || n == 2 || n == 4 || n == 8 || n == 12 || n == 16; }
 
 extern "C" {

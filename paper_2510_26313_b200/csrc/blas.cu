@@ -8,6 +8,7 @@
 // block to finish.  Deterministic; results stay on the device.
 #include "internal.cuh"
 #include "dslash_kernel.cuh"
+#include "reduce.cuh"
 
 template <int VW, int R> struct BlasIdx {
     static constexpr int TPG = R / VW, UT = SB * TPG, US = 24 * SB * R, UN = SB * R, PL = SB * R;
@@ -26,56 +27,6 @@ template <int VW, int R> struct BlasIdx {
         rhs0 = grp * R + hoff;
     }
 };
-
-// part[VW] are this thread's sums for right-hand sides rhs0 + k.  Block size must be a multiple of 32.
-template <int VW, int R>
-__device__ void reduce_per_rhs(double (&part)[VW], int N, int G, double* partials, unsigned int* counter, double* out) {
-    constexpr int TPG = R / VW;
-    extern __shared__ double sm[];       // [max(nwarps * R, blockDim.x)]
-    const int t = threadIdx.x, nt = blockDim.x, lane = t & 31, w = t >> 5, nw = nt >> 5;
-#pragma unroll
-    for (int k = 0; k < VW; k++) {
-#pragma unroll
-        for (int off = 16; off >= TPG; off >>= 1) part[k] += __shfl_xor_sync(0xffffffffu, part[k], off);
-    }
-    if (lane < TPG) {
-#pragma unroll
-        for (int k = 0; k < VW; k++) sm[w * R + lane * VW + k] = part[k];
-    }
-    __syncthreads();
-    if (t < N) {
-        // warps of this block whose unit belongs to group t / R, in warp order
-        const long long gw0 = (long long)blockIdx.x * nw;
-        const int grp = t / R, r = t - grp * R;
-        double s = 0.0;
-        for (int ww = 0; ww < nw; ww++) {
-            const long long u = (gw0 + ww) / TPG;
-            if ((int)(u % G) == grp) s += sm[ww * R + r];
-        }
-        partials[(size_t)blockIdx.x * N + t] = s;
-    }
-    __shared__ bool last;
-    __threadfence();
-    __syncthreads();
-    if (t == 0) last = (atomicInc(counter, gridDim.x - 1) == gridDim.x - 1);
-    __syncthreads();
-    if (!last) return;
-    __threadfence();
-    // final: thread t handles RHS r = t % N, slice q = t / N of the blocks; Q = largest power of two with N*Q <= nt
-    int Q = 1;
-    while (N * Q * 2 <= nt) Q <<= 1;
-    const int r = t % N, q = t / N;
-    double s = 0.0;
-    if (q < Q) for (unsigned b = q; b < gridDim.x; b += Q) s += partials[(size_t)b * N + r];
-    __syncthreads();
-    if (q < Q) sm[t] = s;
-    __syncthreads();
-    for (int stride = Q >> 1; stride >= 1; stride >>= 1) {
-        if (q < stride) sm[t] += sm[t + stride * N];
-        __syncthreads();
-    }
-    if (t < N) out[t] = sm[t];
-}
 
 struct BlasGeom { Geom g; int N, G; };
 
@@ -151,6 +102,36 @@ __global__ void cg_update_p_kernel(BlasGeom bg, SView<S> p, SView<S> r, const do
     store_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, a);
 }
 
+// e += alpha p ; p = z + beta p   (alpha = rr / pAp, beta = rr_new / rr)
+template <class S, int VW, int R>
+__global__ void cg_update_ep_kernel(BlasGeom bg, SView<S> e, SView<S> p, SView<S> z, const double* __restrict__ rr, const double* __restrict__ pAp,
+                                    const double* __restrict__ rr_new) {
+    using T = typename S::comp_t;
+    BlasIdx<VW, R> ix(bg.g, bg.G);
+    if (!ix.valid) return;
+    T alpha[VW], beta[VW];
+#pragma unroll
+    for (int k = 0; k < VW; k++) {
+        const double d = pAp[ix.rhs0 + k], r0 = rr[ix.rhs0 + k];
+        alpha[k] = (T)(d > 0.0 ? r0 / d : 0.0);
+        beta[k] = (T)(r0 > 0.0 ? rr_new[ix.rhs0 + k] / r0 : 0.0);
+    }
+    T a[24][VW], b[24][VW];
+    load_site_regs<S, VW, R>(e.d + ix.own, S::has_norm ? e.n + ix.own_n : nullptr, a);
+    load_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, b);
+#pragma unroll
+    for (int j = 0; j < 24; j++)
+#pragma unroll
+        for (int k = 0; k < VW; k++) a[j][k] += alpha[k] * b[j][k];
+    store_site_regs<S, VW, R>(e.d + ix.own, S::has_norm ? e.n + ix.own_n : nullptr, a);
+    load_site_regs<S, VW, R>(z.d + ix.own, S::has_norm ? z.n + ix.own_n : nullptr, a);
+#pragma unroll
+    for (int j = 0; j < 24; j++)
+#pragma unroll
+        for (int k = 0; k < VW; k++) b[j][k] = a[j][k] + beta[k] * b[j][k];
+    store_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, b);
+}
+
 // y (fp64) += s_k * e
 template <class S, int VW, int R>
 __global__ void axpy_mixed_kernel(BlasGeom bg, double* __restrict__ y, SView<S> ev, const double* __restrict__ scale) {
@@ -196,12 +177,7 @@ static int plan(lq_ctx* c, int nrhs, int maxvw, Launch& L) {
     const long long threads = (long long)c->g.NB * L.bg.G * SB * (R / L.vw);
     L.grid = (int)((threads + L.block - 1) / L.block);
     L.smem = (size_t)L.block * sizeof(double);
-    if ((size_t)L.grid * nrhs > c->red_partials_elems) {
-        if (c->red_partials) dev_free(c, c->red_partials);
-        c->red_partials_elems = (size_t)L.grid * nrhs * 2;
-        c->red_partials = (double*)dev_alloc(c, c->red_partials_elems * sizeof(double));
-        if (!c->red_partials) { c->red_partials_elems = 0; return LQ_ENOMEM; }
-    }
+    LQ_TRY(ensure_partials(c, (size_t)L.grid * nrhs));
     return 0;
 }
 // dispatch on (VW, R): fp32/half (4,4) (2,2) (1,1); fp64 (2,4) (2,2) (1,1)
@@ -254,6 +230,20 @@ int blas_cg_update_p(lq_ctx* c, int prec, int nrhs, void* p, const void* r, cons
     if (prec == LQ_FP64) return p_t<F64>(c, nrhs, p, r, d_rr_new, d_rr);
     if (prec == LQ_FP32) return p_t<F32>(c, nrhs, p, r, d_rr_new, d_rr);
     return p_t<H16>(c, nrhs, p, r, d_rr_new, d_rr);
+}
+
+template <class S> static int ep_t(lq_ctx* c, int nrhs, void* e, void* p, const void* z, const double* rr, const double* pAp, const double* rrn) {
+    Launch L; LQ_TRY(plan(c, nrhs, S::prec == LQ_FP64 ? 2 : 4, L));
+    SView<S> ve = make_view<S>(c->g, e, nrhs, 0), vp = make_view<S>(c->g, p, nrhs, 0), vz = make_view<S>(c->g, const_cast<void*>(z), nrhs, 0);
+    VW_DISPATCH(L, S, cg_update_ep_kernel, 0, L.bg, ve, vp, vz, rr, pAp, rrn);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
+}
+int blas_cg_update_ep(lq_ctx* c, int prec, int nrhs, void* e, void* p, const void* z, const double* d_rr, const double* d_pAp, const double* d_rr_new) {
+    if (prec == LQ_FP64) return ep_t<F64>(c, nrhs, e, p, z, d_rr, d_pAp, d_rr_new);
+    if (prec == LQ_FP32) return ep_t<F32>(c, nrhs, e, p, z, d_rr, d_pAp, d_rr_new);
+    return ep_t<H16>(c, nrhs, e, p, z, d_rr, d_pAp, d_rr_new);
 }
 
 template <class S> static int axpy_t(lq_ctx* c, int nrhs, void* y, const void* e, const double* s) {

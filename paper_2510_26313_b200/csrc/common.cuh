@@ -184,6 +184,7 @@ struct lq_ctx {
 int set_err(lq_ctx* c, int code, const std::string& msg);
 void* dev_alloc(lq_ctx* c, size_t bytes);          // nullptr on failure (error recorded)
 void dev_free(lq_ctx* c, void* p);
+int ensure_partials(lq_ctx* c, size_t elems);      // reduction scratch of at least `elems` doubles
 
 #define LQ_CUDA(ctx, call)                                                                     \
     do {                                                                                       \

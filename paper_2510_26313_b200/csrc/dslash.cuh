@@ -21,6 +21,8 @@
 #include "common.cuh"
 
 enum { FORM_HOP = 0, FORM_A = 1, FORM_B = 2 };
+// fused epilogues of kernel B: per-RHS ||out||^2, or out <- out - (num/den)_k * result with per-RHS ||out||^2
+enum { EPI_NONE = 0, EPI_NORM = 1, EPI_XMAY = 2 };
 
 template <class S> struct DslashArgs {
     using T = typename S::comp_t;
@@ -35,6 +37,10 @@ template <class S> struct DslashArgs {
     T tsign;               // t_bc
     T dsign;               // +1, -1 = dagger
     int pfd;               // L2 prefetch distance in site blocks (0 = off)
+    int epi;               // FORM_B epilogue
+    const double *epi_num, *epi_den;   // EPI_XMAY: alpha_k = num_k / den_k (device, per RHS)
+    double* epi_out;                   // per-RHS sums (device)
+    double* red_partials; unsigned int* red_counter;   // reduction scratch of the context
 };
 
 __device__ __forceinline__ float fm(float a, float b, float c) { return fmaf(a, b, c); }

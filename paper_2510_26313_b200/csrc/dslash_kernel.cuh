@@ -1,6 +1,7 @@
 // dslash_kernel.cuh -- kernel body, clover block multiply, half-storage epilogue and the launcher declaration.
 #pragma once
 #include "dslash.cuh"
+#include "reduce.cuh"
 
 // o = C v for one chirality block: cl = 6 real diagonal entries then 15 complex lower-triangular entries
 // L(i,j), i > j, at index i(i-1)/2 + j (clover as 2 x (6x6 Hermitian), 72 reals per site).
@@ -130,13 +131,17 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
     const int G = a.G;
     const int tid = blockIdx.x * BLOCK + threadIdx.x;
     const int u = tid / UT;                 // unit = blk*G + grp
-    if (u >= a.g.NB * G) return;
     const int lu = tid - u * UT;
     const int blk = a.dG.div(u), grp = u - blk * G;
     const int s = lu / TPG, hoff = (lu - s * TPG) * RPT;
     SiteCtx sc;
     sc.cb = blk * SB + s;
-    if (sc.cb >= a.g.Vh) return;            // padding sites of the last block
+    // threads beyond the last unit and padding sites of the last block do no work (but reach the fused reduction)
+    const bool valid = (u < a.g.NB * G) && (sc.cb < a.g.Vh);
+    double part[RPT];
+#pragma unroll
+    for (int k = 0; k < RPT; k++) part[k] = 0.0;
+    if (valid) {
     cb_coords(a.g, a.parity, sc.cb, sc.xh, sc.y, sc.z, sc.t, sc.odd);
     sc.Lxh = a.g.Lxh; sc.Ly = a.g.L[1]; sc.Lz = a.g.L[2]; sc.Lt = a.g.L[3];
 
@@ -222,8 +227,38 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
     // ---- epilogue (FORM_A): acc <- C acc -----------------------------------------------------------------
     if constexpr (FORM == FORM_A) clover_apply_regs<T, RPT>(a.clover + (size_t)blk * (72 * SB), s, acc);
 
-    // ---- store ----------------------------------------------------------------------------------------------
+    // ---- fused block-BLAS epilogues of kernel B and store ---------------------------------
+    if constexpr (FORM == FORM_B) {
+        if (a.epi == EPI_XMAY) {
+            // out <- out - alpha_k acc  (the CG residual update z -= alpha q without ever storing q), alpha = rr / pAp
+            T zv[24][RPT], al[RPT];
+            load_site_regs<S, RPT, R>(a.out.d + own, S::has_norm ? a.out.n + own_n : nullptr, zv);
+#pragma unroll
+            for (int k = 0; k < RPT; k++) { const double d = a.epi_den[grp * R + hoff + k]; al[k] = (T)(d > 0.0 ? a.epi_num[grp * R + hoff + k] / d : 0.0); }
+#pragma unroll
+            for (int j = 0; j < 24; j++)
+#pragma unroll
+                for (int k = 0; k < RPT; k++) acc[j][k] = zv[j][k] - al[k] * acc[j][k];
+        }
+        if (a.epi != EPI_NONE) {
+            // the 24 squares of one site are summed in the compute type (relative error ~1e-7 in fp32, far below the
+            // solver's use of these norms); sites are summed in fp64 by the reduction
+            T ps[RPT];
+#pragma unroll
+            for (int k = 0; k < RPT; k++) ps[k] = 0;
+#pragma unroll
+            for (int j = 0; j < 24; j++)
+#pragma unroll
+                for (int k = 0; k < RPT; k++) ps[k] = fm(acc[j][k], acc[j][k], ps[k]);
+#pragma unroll
+            for (int k = 0; k < RPT; k++) part[k] = (double)ps[k];
+        }
+    }
     store_site_regs<S, RPT, R>(a.out.d + own, S::has_norm ? a.out.n + own_n : nullptr, acc);
+    }   // valid
+    if constexpr (FORM == FORM_B) {
+        if (a.epi != EPI_NONE) reduce_per_rhs<RPT, R>(part, a.N, G, a.red_partials, a.red_counter, a.epi_out);
+    }
 }
 
 // ---- launcher -----------------------------------------------------------------------------------------------

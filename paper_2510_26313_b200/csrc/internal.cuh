@@ -13,6 +13,10 @@ int op_hop(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void*
 int op_kernel_a(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* in, int dagger);
 // out(parity) = C x + coef D in ; use_clover: 1 -> A(parity), 0 -> identity
 int op_kernel_b(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger);
+// kernel B with a fused block-BLAS epilogue: EPI_NORM: epi_out[k] = ||out_k||^2 ; EPI_XMAY: out_k <- out_k - (num_k/den_k) (C x + coef D in)_k
+// and epi_out[k] = ||out_k||^2 (out is read and written)
+int op_kernel_b_epi(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger,
+                    int epi, const double* num, const double* den, double* epi_out);
 // out(parity) = A x or A^{-1} x (site-local)
 int op_clover(lq_ctx* c, int prec, int nrhs, int parity, void* out, const void* x, int inverse);
 
@@ -37,6 +41,8 @@ int blas_cg_update_xr(lq_ctx* c, int prec, int nrhs, void* x, void* r, const voi
 // CG step 2: beta_k = rr_new_k / rr_k;  p = r + beta p
 int blas_cg_update_p(lq_ctx* c, int prec, int nrhs, void* p, const void* r, const double* d_rr_new, const double* d_rr);
 // y (fp64) += s_k * e (prec)       (defect-correction accumulate)
+// fused CG vector update: alpha_k = rr_k / pAp_k, beta_k = rr_new_k / rr_k;  e += alpha p;  p = z + beta p
+int blas_cg_update_ep(lq_ctx* c, int prec, int nrhs, void* e, void* p, const void* z, const double* d_rr, const double* d_pAp, const double* d_rr_new);
 int blas_axpy_mixed(lq_ctx* c, int prec, int nrhs, void* y64, const void* e, const double* d_scale);
 // r = b - t (fp64), d_out[k] = ||r_k||^2
 int blas_residual(lq_ctx* c, int nrhs, void* r, const void* b, const void* t, double* d_out);

@@ -13,6 +13,7 @@ static DslashArgs<S> base_args(lq_ctx* c, int nrhs, int out_parity, void* out, c
     if constexpr (S::prec == LQ_FP64) a.gauge = c->gauge64; else a.gauge = c->gauge32;
     a.clover = nullptr;
     a.coef = T(1); a.tsign = T(c->t_bc); a.dsign = dagger ? T(-1) : T(1);
+    a.epi = EPI_NONE; a.epi_num = a.epi_den = nullptr; a.epi_out = nullptr; a.red_partials = nullptr; a.red_counter = nullptr;
     return a;
 }
 
@@ -47,16 +48,22 @@ int op_kernel_a(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const 
     return kernel_a_t<H16>(c, nrhs, out_parity, out, in, dagger);
 }
 
-template <class S> static int kernel_b_t(lq_ctx* c, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger) {
+template <class S> static int kernel_b_t(lq_ctx* c, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger,
+                                         int epi, const double* num, const double* den, double* epi_out) {
     auto a = base_args<S>(c, nrhs, out_parity, out, in, x, dagger);
     a.clover = use_clover ? clover_ptr<S>(c, out_parity, 0) : nullptr;
     a.coef = (typename S::comp_t)coef;
+    a.epi = epi; a.epi_num = num; a.epi_den = den; a.epi_out = epi_out;
     return run_form<S, FORM_B>(c, a);
 }
+int op_kernel_b_epi(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger,
+                    int epi, const double* num, const double* den, double* epi_out) {
+    if (prec == LQ_FP64) return kernel_b_t<F64>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, epi, num, den, epi_out);
+    if (prec == LQ_FP32) return kernel_b_t<F32>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, epi, num, den, epi_out);
+    return kernel_b_t<H16>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, epi, num, den, epi_out);
+}
 int op_kernel_b(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger) {
-    if (prec == LQ_FP64) return kernel_b_t<F64>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger);
-    if (prec == LQ_FP32) return kernel_b_t<F32>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger);
-    return kernel_b_t<H16>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger);
+    return op_kernel_b_epi(c, prec, nrhs, out_parity, out, x, in, coef, use_clover, dagger, EPI_NONE, nullptr, nullptr, nullptr);
 }
 
 // ---- site-local clover apply: out = C x --------------------------------------------------------------------

@@ -67,15 +67,17 @@ static int fetch(lq_ctx* c, const double* d, int n, double* h) {
     return 0;
 }
 
-// one inner CG iteration; rr/rrn are swapped by the caller
+// one inner CG iteration (5 launches); rr/rrn are swapped by the caller.  The two block-BLAS reductions and the residual
+// update ride in the kernel-B epilogues: q = Mhat^dag t is never stored.
 static int cg_iteration(lq_ctx* c, Workspace* w, int prec, int n, double* rr, double* pAp, double* rrn) {
-    LQ_TRY(apply_mhat(c, prec, n, w->t, w->p, w->tmp, 0));          // t = Mhat p
-    LQ_TRY(blas_norm2(c, prec, n, w->t, pAp));                        // <p, Mhat^dag Mhat p> = ||t||^2
-    LQ_TRY(apply_mhat(c, prec, n, w->q, w->t, w->tmp, 1));          // q = Mhat^dag t
-    LQ_TRY(blas_cg_update_xr(c, prec, n, w->e, w->z, w->p, w->q, rr, pAp, rrn));
-    return blas_cg_update_p(c, prec, n, w->p, w->z, rrn, rr);
+    const double k2 = -c->kappa * c->kappa;
+    LQ_TRY(op_kernel_a(c, prec, n, 1, w->tmp, w->p, 0));
+    LQ_TRY(op_kernel_b_epi(c, prec, n, 0, w->t, w->p, w->tmp, k2, 1, 0, EPI_NORM, nullptr, nullptr, pAp));   // t = Mhat p, pAp = ||t||^2
+    LQ_TRY(op_kernel_a(c, prec, n, 1, w->tmp, w->t, 1));
+    LQ_TRY(op_kernel_b_epi(c, prec, n, 0, w->z, w->t, w->tmp, k2, 1, 1, EPI_XMAY, rr, pAp, rrn));          // z -= alpha Mhat^dag t, rrn = ||z||^2
+    return blas_cg_update_ep(c, prec, n, w->e, w->p, w->z, rr, pAp, rrn);                                    // e += alpha p ; p = z + beta p
 }
-static const int KERNELS_PER_ITER = 7;
+static const int KERNELS_PER_ITER = 5;
 
 int solve_native(lq_ctx* c, void* x_full, const void* b_full, int n, const lq_solve_param* prm, lq_solve_info* info) {
     if (!c->has_gauge || !c->has_clover) return set_err(c, LQ_ESTATE, "gauge field and clover term must be loaded before lq_solve");

@@ -172,28 +172,31 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
             const int pb = blk + a.pfd;
             if (pb < NB) {
                 constexpr int LINE = 128;
+#define LQ_PF_LINES(base, nlines) { _Pragma("unroll") for (int i0_ = 0; i0_ < (nlines); i0_ += UT) { const int i_ = i0_ + lu; \
+                    if (i_ < (nlines)) asm volatile("prefetch.global.L2 [%0];" ::"l"((base) + (size_t)i_ * LINE)); } }
                 const int st32 = (sc.Lxh * sc.Ly * sc.Lz) / SB;
                 int pbt = pb + st32; if (pbt >= NB) pbt -= NB;
                 const char* q = (const char*)(a.in.d + ((size_t)pbt * G + grp) * US);
-                for (int i = lu; i < (int)(US * sizeof(ST) / LINE); i += UT) asm volatile("prefetch.global.L2 [%0];" ::"l"(q + (size_t)i * LINE));
+                LQ_PF_LINES(q, (int)(US * sizeof(ST) / LINE))
                 if constexpr (FORM == FORM_B) {
                     const char* qx = (const char*)(a.x.d + ((size_t)pb * G + grp) * US);
-                    for (int i = lu; i < (int)(US * sizeof(ST) / LINE); i += UT) asm volatile("prefetch.global.L2 [%0];" ::"l"(qx + (size_t)i * LINE));
+                    LQ_PF_LINES(qx, (int)(US * sizeof(ST) / LINE))
                 }
                 constexpr int GL = 4 * RECON * SB * sizeof(T) / LINE;     // lines of one (parity, block) link slab
                 constexpr int CL = 72 * SB * sizeof(T) / LINE;            // lines of one clover block
                 if (grp == 0 % G) {
                     const char* l = (const char*)(a.gauge + ((size_t)(a.parity * NB + pb) * 4) * (RECON * SB));
-                    for (int i = lu; i < GL; i += UT) asm volatile("prefetch.global.L2 [%0];" ::"l"(l + (size_t)i * LINE));
+                    LQ_PF_LINES(l, GL)
                 }
                 if (grp == 1 % G) {
                     const char* l = (const char*)(a.gauge + ((size_t)((1 - a.parity) * NB + pb) * 4) * (RECON * SB));
-                    for (int i = lu; i < GL; i += UT) asm volatile("prefetch.global.L2 [%0];" ::"l"(l + (size_t)i * LINE));
+                    LQ_PF_LINES(l, GL)
                 }
                 if (grp == 2 % G && a.clover != nullptr) {
                     const char* l = (const char*)(a.clover + (size_t)pb * (72 * SB));
-                    for (int i = lu; i < CL; i += UT) asm volatile("prefetch.global.L2 [%0];" ::"l"(l + (size_t)i * LINE));
+                    LQ_PF_LINES(l, CL)
                 }
+#undef LQ_PF_LINES
             }
         }
     }

@@ -169,7 +169,8 @@ typedef struct {
 int lq_solve(lq_ctx* ctx, void* x, const void* b, int nrhs, int loc, int layout, const lq_solve_param* param, lq_solve_info* info);
 
 /* Launch-parameter knobs of the stencil kernels (the paper's autotuning, reduced to an
- * offline sweep): kernel variant (0 = default register budget, 1 = alternative; see csrc/dslash_launch.cuh),
+ * offline sweep): kernel variant (bits 0-7: 0 = default register budget, 1 = alternative; bits 8-15: z-chunk of the
+ * sweep order, 0 = automatic, 0xFF = memory order; see csrc/dslash_launch.cuh),
  * right-hand sides per thread (0 = auto: 2 for nrhs % 4 == 0, else the RHS group width 2 / 1; fp64 caps at 2;
  * must divide the group width), and
  * the L2 prefetch distance of the stencil kernels in 32-site blocks (0 = off, negative = library default). */

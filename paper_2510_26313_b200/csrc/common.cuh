@@ -173,6 +173,7 @@ struct lq_ctx {
     int dslash_rpt;                 // tuning knob (0 = auto)
     int dslash_variant;             // tuning knob: kernel variant (0 = default)
     int dslash_pfd;                 // tuning knob: L2 prefetch distance in site blocks (0 = off)
+    int dslash_zc;                  // tuning knob: z-chunk of the sweep order (0 = auto, -1 = memory order)
     std::string err;
     // reduction scratch
     double* red_partials; size_t red_partials_elems;

@@ -37,6 +37,9 @@ template <class S> struct DslashArgs {
     T tsign;               // t_bc
     T dsign;               // +1, -1 = dagger
     int pfd;               // L2 prefetch distance in site blocks (0 = off)
+    // sweep order: launch-order block index -> site block, [z chunk][t][z in chunk][y-x blocks], so that the three
+    // time-slices a chunk needs stay in L2 between their uses (zc = 0: memory order)
+    int zc, nby; FastDiv dnby, dzc, dLt;
     int epi;               // FORM_B epilogue
     const double *epi_num, *epi_den;   // EPI_XMAY: alpha_k = num_k / den_k (device, per RHS)
     double* epi_out;                   // per-RHS sums (device)

@@ -120,6 +120,15 @@ template <int D> __device__ __forceinline__ int neighbour(const SiteCtx& c) {
     }
 }
 
+// launch-order block index -> site block (see DslashArgs::zc)
+template <class S> __device__ __forceinline__ int sweep_block(const DslashArgs<S>& a, int b) {
+    if (a.zc == 0) return b;
+    int r = a.dnby.div(b); const int yb = b - r * a.nby;
+    int q = a.dzc.div(r); const int zi = r - q * a.zc;
+    const int zch = a.dLt.div(q); const int t = q - zch * a.g.L[3];
+    return yb + a.nby * ((zch * a.zc + zi) + a.g.L[2] * t);
+}
+
 template <class S, int RPT, int R, int RECON, int FORM, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S> a) {
     using T = typename S::comp_t;
@@ -132,7 +141,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
     const int tid = blockIdx.x * BLOCK + threadIdx.x;
     const int u = tid / UT;                 // unit = blk*G + grp
     const int lu = tid - u * UT;
-    const int blk = a.dG.div(u), grp = u - blk * G;
+    const int lblk = a.dG.div(u), grp = u - lblk * G;      // launch-order block
+    const int blk = sweep_block(a, lblk);
     const int s = lu / TPG, hoff = (lu - s * TPG) * RPT;
     SiteCtx sc;
     sc.cb = blk * SB + s;
@@ -145,8 +155,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
     cb_coords(a.g, a.parity, sc.cb, sc.xh, sc.y, sc.z, sc.t, sc.odd);
     sc.Lxh = a.g.Lxh; sc.Ly = a.g.L[1]; sc.Lz = a.g.L[2]; sc.Lt = a.g.L[3];
 
-    const size_t own = (size_t)u * US + s * R + hoff;
-    const size_t own_n = (size_t)u * UN + s * R + hoff;
+    const size_t own = (size_t)(blk * G + grp) * US + s * R + hoff;
+    const size_t own_n = (size_t)(blk * G + grp) * UN + s * R + hoff;
 
     const int NB = a.g.NB;
     // forward links live on the output site, backward links on the neighbour (other parity)
@@ -169,8 +179,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
     // block.  One 128-byte line per lane per instruction; ~10 instructions per thread.
     {
         if (a.pfd > 0) {
-            const int pb = blk + a.pfd;
-            if (pb < NB) {
+            const int lpb = lblk + a.pfd;
+            if (lpb < NB) {
+                const int pb = sweep_block(a, lpb);
                 constexpr int LINE = 128;
 #define LQ_PF_LINES(base, nlines) { _Pragma("unroll") for (int i0_ = 0; i0_ < (nlines); i0_ += UT) { const int i_ = i0_ + lu; \
                     if (i_ < (nlines)) asm volatile("prefetch.global.L2 [%0];" ::"l"((base) + (size_t)i_ * LINE)); } }

@@ -17,6 +17,27 @@ static int launch_one(lq_ctx* c, DslashArgs<S> a) {
     return 0;
 }
 
+// Sweep order (DslashArgs::zc): chunk the z extent so that one time-slice of a chunk of the input batch is <= ~6.5 MB and the
+// slices t-1, t, t+1 of the chunk plus the streamed links / clover / output stay inside the 126 MB L2 between their uses.
+// Needs whole x-y planes per site block (Lx/2 * Ly % 32 == 0); otherwise memory order.
+template <class S>
+static void plan_sweep(lq_ctx* c, DslashArgs<S>& a) {
+    a.zc = 0; a.nby = 1; a.dnby = a.dzc = a.dLt = make_fastdiv(1);
+    if (c->dslash_zc < 0 || a.g.Vh % SB != 0 || (a.g.Lxh * a.g.L[1]) % SB != 0) return;
+    const int Lz = a.g.L[2];
+    int zc = c->dslash_zc;
+    if (zc == 0) {
+        const double layer = (double)a.g.Lxh * a.g.L[1] * a.N * 24.0 * sizeof(typename S::store_t);
+        const double slice = layer * Lz;
+        if (slice <= 6.6e6) return;                   // measured on B200: chunks of <= ~6.5 MB per time-slice are best
+        zc = 1;
+        for (int d = 1; d <= Lz; d++) if (Lz % d == 0 && d * layer <= 6.6e6) zc = d;
+    }
+    if (zc >= Lz || Lz % zc != 0) return;
+    a.zc = zc; a.nby = a.g.Lxh * a.g.L[1] / SB;
+    a.dnby = make_fastdiv(a.nby); a.dzc = make_fastdiv(zc); a.dLt = make_fastdiv(a.g.L[3]);
+}
+
 // Register budget per thread = 65536 / (128 * MINB): MINB 2 -> 255, 3 -> 168, 4 -> 128, 5 -> 96 (rounded by ptxas).
 // `variant` (tuning knob): 0 = default budget, 1 = alternative budget (fp32 only).
 template <class S, int RPT, int R, int RECON, int FORM>
@@ -26,6 +47,7 @@ static int launch_rpt(lq_ctx* c, DslashArgs<S> a, int variant) {
     a.G = a.N / R;
     a.dG = make_fastdiv(a.G);
     a.pfd = c->dslash_pfd;
+    plan_sweep<S>(c, a);
     if constexpr (S::prec == LQ_FP32) {
         constexpr int ALT = RPT == 4 ? 3 : (RPT == 2 ? 4 : 5);
         if (variant == 1) return launch_one<S, RPT, R, RECON, FORM, ALT>(c, a);

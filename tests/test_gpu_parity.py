@@ -77,6 +77,19 @@ def test_rhs_per_thread_variants(nrhs, rpt, variant):
     ctx.close()
 
 
+@pytest.mark.parametrize("dims", [(8, 8, 4, 6), (16, 4, 8, 4), (32, 2, 6, 2)])
+@pytest.mark.parametrize("zc", [1, 2, 0xFF])
+def test_sweep_order_z_chunks(dims, zc):
+    """The z-chunked sweep order (launch-order block -> site block permutation, used on large lattices so that three
+    time-slices of a chunk stay in L2) together with the distance prefetch: forced chunk sizes on small lattices."""
+    ctx, orc = make_case(dims, 888, 0.3, 0.124, 1.0)
+    for pfd in (0, 3):
+        ctx.set_tuning(dslash_variant=zc << 8, dslash_pfd=pfd)
+        for nrhs, prec in ((8, B.LQ_FP32), (12, B.LQ_HALF), (4, B.LQ_FP64), (1, B.LQ_FP32)):
+            check_ops(ctx, orc, nrhs, prec, ops=[B.LQ_OP_MHAT_DAG, B.LQ_OP_KERNEL_A, B.LQ_OP_KERNEL_B])
+    ctx.close()
+
+
 @pytest.mark.parametrize("nrhs", [1, 4, 12])
 @pytest.mark.parametrize("prec", [B.LQ_FP64, B.LQ_FP32, B.LQ_HALF])
 def test_l2_prefetch_distances(nrhs, prec):

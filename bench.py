@@ -194,6 +194,33 @@ def cpu_baseline(cfg_id: int, budget_s: float = 25.0):
                       "iteration) on %s, tol %g; iterations %s" % (n, "x".join(map(str, dims)), c["tol"], its)}
 
 
+def cpu_dslash_baseline():
+    """The oracle's full operator M and its site-local kernel A on the host cores, ns per site per RHS (SURVEY 8(d) CPU
+    baseline; lattice capped at 16^3x32: per-site cost is volume-independent beyond cache)."""
+    import oracle
+    c = inputs.CONFIGS[1]
+    dims = c["dims"]
+    V = inputs.volume(dims)
+    U = inputs.make_links(dims, c["gauge_seed"], c["eps"])
+    A = oracle.clover(dims, U, c["kappa"], c["csw"])
+    psi = inputs.gaussian_spinors(dims, 1, 4242)[0]
+    oracle.M(dims, U, A, c["kappa"], psi)
+    t0 = time.perf_counter(); n = 0
+    while time.perf_counter() - t0 < 3.0:
+        oracle.M(dims, U, A, c["kappa"], psi); n += 1
+    dt_M = (time.perf_counter() - t0) / n
+    rng = np.random.default_rng(5)
+    sites = np.stack([rng.integers(0, d, 20000) for d in dims], axis=1)
+    sites = sites[(sites.sum(axis=1) % 2) == 1].astype(np.int32)
+    t0 = time.perf_counter()
+    oracle.site_eval(dims, 1, sites, c["kappa"], c["csw"], U=U, psi=psi.reshape(-1, 12))
+    dt_A = time.perf_counter() - t0
+    return {"kind": "oracle", "cores": oracle.num_threads(), "lattice": "x".join(map(str, dims)),
+            "full_M_ns_per_site_rhs": round(dt_M / V * 1e9, 1), "full_M_gflops_1824": round(1824.0 * V / dt_M * 1e-9, 2),
+            "site_local_kernel_A_ns_per_site_rhs": round(dt_A / len(sites) * 1e9, 1),
+            "note": "kernel A by the site-local evaluator rebuilds F_mu_nu, A and A^-1 at every site (that is its definition), so it is not comparable with a stored-clover kernel"}
+
+
 def operator_sweeps(B, device, peak):
     """configs[2]: 32^3x64 fp32 sweep over N_rhs (kernel A, kernel B, bare hop); configs[4]: 64^3x128, N=4, 12-real links."""
     import torch
@@ -431,6 +458,7 @@ def main():
     extras = {}
     if not args.no_extras and world == 1:
         extras["dslash"] = operator_sweeps(B, local, peak)
+        extras["dslash"]["cpu_baseline"] = cpu_dslash_baseline()
         extras["cpu_baseline"] = cpu_baseline(wl["cfg"])
     total_rhs = nrhs * world
     line = {

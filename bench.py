@@ -100,6 +100,9 @@ def time_dslash(ctx, B, kind: str, prec: str, nrhs: int, recon: int, iters: int 
     """Average device time of one single-parity stencil launch (kernel A, kernel B or the bare hop), native layout,
     rotating buffer sets so that no launch starts with its operands in L2.  Returns a dict of seconds / GB/s / GFLOP/s."""
     import torch
+    # fresh device allocations for every measurement: the same kernel on buffers carved out of the torch caching
+    # allocator's older segments measured up to 8 % slower (placement-dependent), which made the sweep order matter
+    torch.cuda.empty_cache()
     P = B.PREC[prec]
     pbytes = ctx.native_bytes(nrhs, P, True)
     per_set = pbytes * (3 if kind == "B" else 2)

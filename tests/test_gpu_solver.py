@@ -105,3 +105,34 @@ def test_not_converged_is_reported():
     assert not info["converged"] and max(info["true_rel_residual"]) > 1e-12
     assert np.all(np.isfinite(x.view(np.float64)))
     ctx.close()
+
+
+@pytest.mark.parametrize("inner", [B.LQ_FP32, B.LQ_HALF])
+def test_solve_is_bitwise_reproducible(inner):
+    """The per-RHS reductions (fused kernel-B epilogues and block-BLAS) are fixed-order: two solves of the same system
+    give bit-identical solutions and iteration counts, with and without CUDA-graph replay."""
+    dims = (8, 8, 8, 8)
+    ctx, orc = setup(dims, 77, 0.25, 0.124, 1.1)
+    b = inputs.laph_sources(dims, 8, 2, 78)
+    runs = []
+    for use_graph in (False, False, True):
+        x, info = ctx.solve(b, tol=1e-8, inner_prec=inner, delta=1e-2, check_every=4, use_graph=use_graph)
+        assert info["converged"]
+        runs.append((x.copy(), info["inner_iters"], info["outer_cycles"]))
+    for x, it, oc in runs[1:]:
+        assert it == runs[0][1] and oc == runs[0][2]
+        assert np.array_equal(x, runs[0][0])
+    assert np.all(true_residuals(orc, runs[0][0], b) <= 1e-8)
+    ctx.close()
+
+
+@pytest.mark.parametrize("nrhs", [1, 2, 12, 16])
+def test_every_batch_width_solves(nrhs):
+    """RHS group widths 1, 2 and 4 and 1, 3 and 4 groups per site block through the fused CG iteration (fp32 inner)."""
+    dims = (6, 6, 4, 8)          # Vh = 432: 13.5 site blocks, the last one half padding
+    ctx, orc = setup(dims, 91, 0.3, 0.123, 1.0)
+    b = inputs.gaussian_spinors(dims, nrhs, 92)
+    x, info = ctx.solve(b, tol=1e-9, inner_prec=B.LQ_FP32, delta=1e-3, check_every=6, use_graph=True)
+    assert info["converged"], info
+    assert np.all(true_residuals(orc, x, b) <= 1e-9)
+    ctx.close()

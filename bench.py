@@ -162,7 +162,7 @@ def roofline_entry(r, peak, peak_src, traffic=None):
 
 # ------------------------------------------------------------------------------------------------ workloads
 SOLVER_WORKLOADS = {
-    "cfg1": dict(cfg=1, inner="fp32", delta=1e-3, desc="configs[1]: 16^3x32, 8 RHS LapH time/spin-diluted, fp32 inner CG + fp64 defect correction, tol 1e-8"),
+    "cfg1": dict(cfg=1, inner="fp32", delta=1e-4, desc="configs[1]: 16^3x32, 8 RHS LapH time/spin-diluted, fp32 inner CG + fp64 defect correction, tol 1e-8"),
     "cfg3": dict(cfg=3, inner="half", delta=1e-2, desc="configs[3]: 48^3x96, 12 RHS LapH-diluted, int16+norm inner CG, fp32 clover, fp64 outer, tol 1e-9"),
 }
 
@@ -277,7 +277,7 @@ def run_big_solve(args, B, device, wl, c, peak, peak_src):
     ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=c["recon"])
     ctx.build_clover(c["kappa"], c["csw"])
     b_host = make_sources_host(wl["cfg"])
-    kw = dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=wl["delta"], check_every=10, use_graph=not args.no_graph, native=True, nrhs=nrhs)
+    kw = dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=args.delta or wl["delta"], check_every=args.check_every, use_graph=not args.no_graph, native=True, nrhs=nrhs)
     sampler = ClockSampler(device)
     w0 = time.perf_counter()
     nb = ctx.pack(b_host, nrhs, B.LQ_FP64)
@@ -374,6 +374,8 @@ def main():
     ap.add_argument("--workload", default="cfg1", choices=sorted(SOLVER_WORKLOADS))
     ap.add_argument("--no-extras", action="store_true", help="skip the configs[2]/[4] operator sweep and the CPU baseline")
     ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--check-every", type=int, default=4, help="inner iterations between convergence polls")
+    ap.add_argument("--delta", type=float, default=0.0, help="inner CG reduction per cycle (0 = the workload default)")
     ap.add_argument("--op", default=None, metavar="CFG:KIND:PREC:N",
                     help="time ONE stencil kernel only, e.g. cfg2:A:fp32:8 (lattice and links of configs[CFG]; KIND A|B|hop; "
                          "PREC fp64|fp32|half); optional :variant:rpt:pfd tuning suffix.  Prints its own JSON line (used for ncu captures)")
@@ -413,7 +415,7 @@ def main():
     x_host = torch.empty_like(b_host).pin_memory()
     b_dev = b_host.cuda()
     x_dev = torch.empty_like(b_dev)
-    kw = dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=wl["delta"], check_every=10, use_graph=not args.no_graph)
+    kw = dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=args.delta or wl["delta"], check_every=args.check_every, use_graph=not args.no_graph)
 
     def barrier():
         if world > 1:

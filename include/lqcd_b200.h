@@ -150,6 +150,9 @@ typedef struct {
     double delta;        /* inner CG stops when ||z_k|| <= delta*||z_k(0)|| for every RHS k           */
     int check_every;     /* inner iterations between convergence polls (host sync of N scalars)       */
     int use_graph;       /* 1: replay the inner iteration body as a CUDA graph                        */
+    int keep_direction;  /* 1: reliable updates (SURVEY 8(c.2) reading #11, 8(f) #3): after each fp64 residual refresh the
+                            CG search direction is kept, p <- z_new + c (p - z_old), instead of restarting at p = z   */
+    int reserved;        /* must be 0                                                                  */
 } lq_solve_param;
 
 typedef struct {

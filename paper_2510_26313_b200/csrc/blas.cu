@@ -132,6 +132,30 @@ __global__ void cg_update_ep_kernel(BlasGeom bg, SView<S> e, SView<S> p, SView<S
     store_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, b);
 }
 
+// p <- z_new + c (p - z_old)
+template <class S, int VW, int R>
+__global__ void keep_direction_kernel(BlasGeom bg, SView<S> p, SView<S> zo, SView<S> zn, const double* __restrict__ cs) {
+    using T = typename S::comp_t;
+    BlasIdx<VW, R> ix(bg.g, bg.G);
+    if (!ix.valid) return;
+    T cf[VW];
+#pragma unroll
+    for (int k = 0; k < VW; k++) cf[k] = (T)cs[ix.rhs0 + k];
+    T a[24][VW], b[24][VW];
+    load_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, a);
+    load_site_regs<S, VW, R>(zo.d + ix.own, S::has_norm ? zo.n + ix.own_n : nullptr, b);
+#pragma unroll
+    for (int j = 0; j < 24; j++)
+#pragma unroll
+        for (int k = 0; k < VW; k++) a[j][k] = cf[k] * (a[j][k] - b[j][k]);
+    load_site_regs<S, VW, R>(zn.d + ix.own, S::has_norm ? zn.n + ix.own_n : nullptr, b);
+#pragma unroll
+    for (int j = 0; j < 24; j++)
+#pragma unroll
+        for (int k = 0; k < VW; k++) a[j][k] += b[j][k];
+    store_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, a);
+}
+
 // y (fp64) += s_k * e
 template <class S, int VW, int R>
 __global__ void axpy_mixed_kernel(BlasGeom bg, double* __restrict__ y, SView<S> ev, const double* __restrict__ scale) {
@@ -244,6 +268,20 @@ int blas_cg_update_ep(lq_ctx* c, int prec, int nrhs, void* e, void* p, const voi
     if (prec == LQ_FP64) return ep_t<F64>(c, nrhs, e, p, z, d_rr, d_pAp, d_rr_new);
     if (prec == LQ_FP32) return ep_t<F32>(c, nrhs, e, p, z, d_rr, d_pAp, d_rr_new);
     return ep_t<H16>(c, nrhs, e, p, z, d_rr, d_pAp, d_rr_new);
+}
+
+template <class S> static int keep_t(lq_ctx* c, int nrhs, void* p, const void* zo, const void* zn, const double* cs) {
+    Launch L; LQ_TRY(plan(c, nrhs, S::prec == LQ_FP64 ? 2 : 4, L));
+    SView<S> vp = make_view<S>(c->g, p, nrhs, 0), vo = make_view<S>(c->g, const_cast<void*>(zo), nrhs, 0), vn = make_view<S>(c->g, const_cast<void*>(zn), nrhs, 0);
+    VW_DISPATCH(L, S, keep_direction_kernel, 0, L.bg, vp, vo, vn, cs);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
+}
+int blas_keep_direction(lq_ctx* c, int prec, int nrhs, void* p, const void* z_old, const void* z_new, const double* d_c) {
+    if (prec == LQ_FP64) return keep_t<F64>(c, nrhs, p, z_old, z_new, d_c);
+    if (prec == LQ_FP32) return keep_t<F32>(c, nrhs, p, z_old, z_new, d_c);
+    return keep_t<H16>(c, nrhs, p, z_old, z_new, d_c);
 }
 
 template <class S> static int axpy_t(lq_ctx* c, int nrhs, void* y, const void* e, const double* s) {

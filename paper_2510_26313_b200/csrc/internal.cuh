@@ -43,6 +43,8 @@ int blas_cg_update_p(lq_ctx* c, int prec, int nrhs, void* p, const void* r, cons
 // y (fp64) += s_k * e (prec)       (defect-correction accumulate)
 // fused CG vector update: alpha_k = rr_k / pAp_k, beta_k = rr_new_k / rr_k;  e += alpha p;  p = z + beta p
 int blas_cg_update_ep(lq_ctx* c, int prec, int nrhs, void* e, void* p, const void* z, const double* d_rr, const double* d_pAp, const double* d_rr_new);
+// reliable update of the search direction: p_k <- z_new_k + c_k (p_k - z_old_k), c per RHS on the device
+int blas_keep_direction(lq_ctx* c, int prec, int nrhs, void* p, const void* z_old, const void* z_new, const double* d_c);
 int blas_axpy_mixed(lq_ctx* c, int prec, int nrhs, void* y64, const void* e, const double* d_scale);
 // r = b - t (fp64), d_out[k] = ||r_k||^2
 int blas_residual(lq_ctx* c, int nrhs, void* r, const void* b, const void* t, double* d_out);

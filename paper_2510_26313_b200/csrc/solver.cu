@@ -90,7 +90,7 @@ int solve_native(lq_ctx* c, void* x_full, const void* b_full, int n, const lq_so
     char* x_e = (char*)x_full; char* x_o = x_e + pb64;
     double* S = w->d_scal;
     double *d_rr = S, *d_rrn = S + LQ_MAX_RHS, *d_pAp = S + 2 * LQ_MAX_RHS, *d_rn = S + 3 * LQ_MAX_RHS, *d_bn = S + 4 * LQ_MAX_RHS,
-           *d_scale = S + 6 * LQ_MAX_RHS;
+           *d_scale = S + 6 * LQ_MAX_RHS, *d_cs = S + 7 * LQ_MAX_RHS;
     const double kappa = c->kappa;
     int check_every = prm->check_every > 0 ? prm->check_every : 10;
     if (prm->use_graph && (check_every & 1)) check_every++;           // graph body must leave rr/rrn un-swapped
@@ -121,6 +121,8 @@ int solve_native(lq_ctx* c, void* x_full, const void* b_full, int n, const lq_so
     int status = LQ_ENOTCONVERGED;
     cudaGraphExec_t gexec = nullptr;
     int total_inner = 0, cycle = 0;
+    double prev_rnorm[LQ_MAX_RHS];
+    for (int k = 0; k < n; k++) prev_rnorm[k] = 0.0;
     for (;; cycle++) {
         double rn2[LQ_MAX_RHS], rnorm[LQ_MAX_RHS];
         LQ_TRY(fetch(c, d_rn, n, rn2));
@@ -137,9 +139,21 @@ int solve_native(lq_ctx* c, void* x_full, const void* b_full, int n, const lq_so
         // rt = lowprec(r / ||r_k||): per-RHS scaling keeps fp32 / half in range
         LQ_CUDA(c, cudaMemcpyAsync(d_scale, rnorm, n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
         LQ_TRY(spinor_convert(c, w->rt, prec, w->r, LQ_FP64, n, d_scale, 1));
-        // z = Mhat^dag rt ; p = z ; e = 0
-        LQ_TRY(apply_mhat(c, prec, n, w->z, w->rt, w->tmp, 1));
-        LQ_TRY(blas_copy(c, prec, n, w->p, w->z));
+        // z = Mhat^dag rt ; e = 0 ; p = z (restart) or, with reliable updates, p <- z + c (p - z_old): the old direction
+        // survives the residual refresh, rescaled by c_k = ||r_k||_old / ||r_k||_new because the inner system is
+        // normalised by ||r_k|| (in exact arithmetic z = c z_old, so the correction only carries the rounding difference)
+        if (prm->keep_direction && cycle > 0) {
+            double cs[LQ_MAX_RHS];
+            for (int k = 0; k < n; k++) cs[k] = (rnorm[k] > 0 && prev_rnorm[k] > 0) ? prev_rnorm[k] / rnorm[k] : 0.0;
+            LQ_CUDA(c, cudaMemcpyAsync(d_cs, cs, n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+            LQ_TRY(apply_mhat(c, prec, n, w->q, w->rt, w->tmp, 1));
+            LQ_TRY(blas_keep_direction(c, prec, n, w->p, w->z, w->q, d_cs));
+            void* sw = w->z; w->z = w->q; w->q = sw;
+        } else {
+            LQ_TRY(apply_mhat(c, prec, n, w->z, w->rt, w->tmp, 1));
+            LQ_TRY(blas_copy(c, prec, n, w->p, w->z));
+        }
+        for (int k = 0; k < n; k++) prev_rnorm[k] = rnorm[k];
         LQ_TRY(spinor_zero_parity(c, w->e, n, prec));
         LQ_TRY(blas_norm2(c, prec, n, w->z, d_rr));
         double rr0[LQ_MAX_RHS], thresh[LQ_MAX_RHS];

@@ -26,8 +26,8 @@ def test_library_builds_and_exports_every_declared_symbol():
 
 
 def test_struct_layouts_match_header():
-    # lq_solve_param: double,int,int,int,(pad),double,int,int ; lq_solve_info as declared
-    assert ctypes.sizeof(binding.SolveParam) == 40
+    # lq_solve_param: double,int,int,int,(pad),double,int,int,int,int ; lq_solve_info as declared
+    assert ctypes.sizeof(binding.SolveParam) == 48
     assert ctypes.sizeof(binding.SolveInfo) == 4 * 3 + 4 * 16 + 4 + 8 * 16 + 8 + 8
     assert binding.LQ_MAX_RHS == 16
 

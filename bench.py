@@ -163,7 +163,7 @@ def roofline_entry(r, peak, peak_src, traffic=None):
 # ------------------------------------------------------------------------------------------------ workloads
 SOLVER_WORKLOADS = {
     "cfg1": dict(cfg=1, inner="fp32", delta=1e-4, desc="configs[1]: 16^3x32, 8 RHS LapH time/spin-diluted, fp32 inner CG + fp64 defect correction, tol 1e-8"),
-    "cfg3": dict(cfg=3, inner="half", delta=1e-2, desc="configs[3]: 48^3x96, 12 RHS LapH-diluted, int16+norm inner CG, fp32 clover, fp64 outer, tol 1e-9"),
+    "cfg3": dict(cfg=3, inner="half", delta=1e-3, desc="configs[3]: 48^3x96, 12 RHS LapH-diluted, int16+norm inner CG, fp32 clover, fp64 outer, tol 1e-9"),
 }
 
 

@@ -205,3 +205,14 @@ def site_eval(dims, kind: int, sites, kappa: float, csw: float, coef: float = 0.
     if rc != 0:
         raise ArithmeticError("singular clover block")
     return out
+
+
+def laplacian(dims, U, v) -> np.ndarray:
+    """3-d gauge-covariant Laplacian on every time-slice (SURVEY 8(f) #2): v[vec][t][z][y][x][3] -> same shape."""
+    V = _vol(dims)
+    U = _cc(U, (4, V, 3, 3))
+    v = np.ascontiguousarray(v, dtype=np.complex128)
+    nvec = v.size // (3 * V)
+    out = np.empty_like(v)
+    lib().orc_laplacian(_dims(dims), _c(U), ctypes.c_long(nvec), _c(v), _c(out))
+    return out

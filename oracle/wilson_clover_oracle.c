@@ -533,3 +533,34 @@ int orc_site_eval(const int *dims, int t_bc, int kind, double kappa, double csw,
     }
     return bad ? -1 : 0;
 }
+
+/* ---------------------------------------------------------------- 3-d gauge-covariant Laplacian */
+/* The LapH smearing operator of PAPER.md L98, L106: on every time-slice t independently (L127: "the temporal
+ * extent ... is an independent batching dimension") and for each colour-vector field v,
+ *   (Lap v)(x) = sum_{i = x,y,z} [ U_i(x) v(x + i) + U_i(x - i)^dag v(x - i) - 2 v(x) ],
+ * periodic in space, no boundary sign (colour vectors carry no spin), the time links are not used.
+ * Layouts: U[mu][t][z][y][x][3][3] (as everywhere), v[vec][t][z][y][x][3]. */
+void orc_laplacian(const int *dims, const cplx *U, long nvec, const cplx *v, cplx *out) {
+    geom_t g = make_geom(dims);
+    linksrc_t ls = {U, 0, 0.0};
+#pragma omp parallel for schedule(static) collapse(2)
+    for (long k = 0; k < nvec; k++)
+        for (long i = 0; i < g.V; i++) {
+            int c[4], cn[4];
+            site_coords(&g, i, c);
+            const cplx *vk = v + k * g.V * 3;
+            cplx acc[3] = {0, 0, 0}, u[9];
+            for (int mu = 0; mu < 3; mu++) {
+                shifted(&g, c, mu, +1, cn);
+                get_link(&g, &ls, mu, c, u);
+                const cplx *p = vk + site_index(&g, cn) * 3;
+                for (int a = 0; a < 3; a++) for (int b = 0; b < 3; b++) acc[a] += u[3 * a + b] * p[b];
+                shifted(&g, c, mu, -1, cn);
+                get_link(&g, &ls, mu, cn, u);
+                p = vk + site_index(&g, cn) * 3;
+                for (int a = 0; a < 3; a++) for (int b = 0; b < 3; b++) acc[a] += conj(u[3 * b + a]) * p[b];
+                for (int a = 0; a < 3; a++) acc[a] -= 2.0 * vk[i * 3 + a];
+            }
+            memcpy(out + (k * g.V + i) * 3, acc, sizeof acc);
+        }
+}

@@ -416,3 +416,70 @@ def test_site_local_generator_matches_input_recipe(oracle_lib):
     a = oracle.site_eval(dims, 0, s, kappa, csw, t_bc=+1, U=U, psi=psi[0].reshape(-1, 12))
     b = oracle.hop(dims, U, psi[0].reshape(-1, 12), t_bc=+1).reshape(dims[3], dims[2], dims[1], dims[0], 4, 3)[s[:, 3], s[:, 2], s[:, 1], s[:, 0]]
     assert rel(a, b) < 1e-14
+
+
+# ------------------------------------------------------------------ 3-d covariant Laplacian
+def _colour_fields(dims, nvec, seed):
+    Lx, Ly, Lz, Lt = dims
+    idx = np.arange(nvec * Lt * Lz * Ly * Lx * 3, dtype=np.int64)
+    return inputs.cgauss(seed, inputs.STREAM_COLORVEC, idx).reshape(nvec, Lt, Lz, Ly, Lx, 3)
+
+
+def test_laplacian_free_field_closed_form(oracle_lib):
+    """U = 1: plane waves exp(i p.x) f(t) chi are eigenvectors with eigenvalue -sum_i 4 sin^2(p_i/2), for ANY time profile
+    f(t) (time-slices are independent) and any colour vector chi."""
+    import oracle
+    dims = (4, 6, 4, 4)
+    U = inputs.unit_links(dims)
+    x, y, z, t = lex_coords(dims)
+    for n in [(1, 2, 3), (0, 0, 0), (3, 5, 1)]:
+        p = [2 * np.pi * n[i] / dims[i] for i in range(3)]
+        lam = -sum(4 * np.sin(pi / 2) ** 2 for pi in p)
+        f = np.exp(1.3j * t) * (1 + t)                      # arbitrary time dependence
+        chi = np.array([0.3 - 1j, 2.0, -0.5j])
+        v = (np.exp(1j * (p[0] * x + p[1] * y + p[2] * z)) * f)[..., None] * chi
+        out = oracle.laplacian(dims, U, v[None])[0]
+        assert np.abs(out - lam * v).max() < 1e-12
+
+
+def test_laplacian_twisted_links_place_U_and_Udag(oracle_lib):
+    """Constant diagonal links U_i = diag(exp(i theta_i^c)): colour c sees p_i -> p_i + theta_i^c.  A swapped U / U^dag or a
+    transposed colour index changes the eigenvalue."""
+    import oracle
+    dims = (4, 4, 6, 2)
+    rng = np.random.default_rng(3)
+    theta = rng.uniform(-1, 1, (3, 3)); theta[:, 2] = -theta[:, 0] - theta[:, 1]
+    U = inputs.unit_links(dims).copy()
+    for mu in range(3):
+        U[mu] = np.diag(np.exp(1j * theta[mu]))
+    x, y, z, t = lex_coords(dims)
+    n = (1, 3, 2)
+    p = [2 * np.pi * n[i] / dims[i] for i in range(3)]
+    for c in range(3):
+        chi = np.zeros(3, complex); chi[c] = 1.0
+        v = np.exp(1j * (p[0] * x + p[1] * y + p[2] * z))[..., None] * chi
+        lam = -sum(4 * np.sin((p[i] + theta[i, c]) / 2) ** 2 for i in range(3))
+        out = oracle.laplacian(dims, U, v[None])[0]
+        assert np.abs(out - lam * v).max() < 1e-12
+
+
+def test_laplacian_hermitian_negative_covariant_and_time_local(oracle_lib, rough):
+    import oracle
+    dims, U = DIMS, rough["U"]
+    u, v = _colour_fields(dims, 2, 41)
+    Lu, Lv = oracle.laplacian(dims, U, np.stack([u, v]))
+    assert abs(vdot(u, Lv) - vdot(Lu, v)) < 1e-10 * abs(vdot(u, Lv))          # Hermitian
+    assert vdot(v, Lv).real < 0 and abs(vdot(v, Lv).imag) < 1e-10             # negative (semi-)definite
+    g = inputs.random_gauge_transform(dims, 42)                                # g[t][z][y][x][3][3]
+    Ug = np.empty_like(U)
+    for mu in range(4):
+        gs = np.roll(g, -1, axis=3 - mu)                                       # g(x + mu)
+        Ug[mu] = g @ U[mu] @ np.conj(np.swapaxes(gs, -1, -2))
+    gv = np.einsum("...ab,...b->...a", g, v)
+    lhs = oracle.laplacian(dims, Ug, gv[None])[0]
+    assert rel(lhs, np.einsum("...ab,...b->...a", g, Lv)) < 1e-13              # Lap[U^g](g v) = g Lap[U] v
+    # time-slices do not talk to each other, and the time links are never read
+    w = v.copy(); w[1:] = 0
+    U2 = U.copy(); U2[3] = inputs.make_links(dims, 99, 0.3)[3]
+    assert np.abs(oracle.laplacian(dims, U2, w[None])[0][1:]).max() == 0
+    assert np.array_equal(oracle.laplacian(dims, U2, w[None])[0][0], Lv[0])

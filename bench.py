@@ -152,6 +152,36 @@ def ncu_traffic(lattice, r):
     return d.get("%s:%s:%s:%d" % (lattice, r["kind"], r["prec"], r["nrhs"]))
 
 
+def time_laplacian(ctx, B, nvec, prec="fp32", iters=20, warmup=3):
+    """Batched 3-d covariant Laplacian on native colour-vector fields, rotating buffer sets.
+    Algorithmic bytes per site per vector: 6 reals in + 6 reals out + 3 links of 18 reals shared by the batch."""
+    import torch
+    torch.cuda.empty_cache()
+    P = B.PREC[prec]
+    s = 8.0 if prec == "fp64" else 4.0
+    nb = int(ctx.lib.lq_cv_native_bytes(ctx.h, nvec, P))
+    nsets = min(64, max(3, int(np.ceil(2.5 * L2_BYTES / (2 * nb))) + 1))
+    sets = []
+    for i in range(nsets):
+        a, b = ctx.cv_native_empty(nvec, P), ctx.cv_native_empty(nvec, P)
+        ctx.cv_fill_random(b, nvec, P, 9000 + i)
+        sets.append((a, b))
+    for i in range(warmup):
+        ctx.laplacian_native(sets[i % nsets][0], sets[i % nsets][1], nvec, P)
+    ctx.stream.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(ctx.stream)
+    for i in range(iters):
+        ctx.laplacian_native(sets[(warmup + i) % nsets][0], sets[(warmup + i) % nsets][1], nvec, P)
+    e1.record(ctx.stream)
+    e1.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3 / iters
+    bps = 12 * s + 3 * 18 * s / nvec
+    del sets
+    return {"nvec": nvec, "prec": prec, "us": round(sec * 1e6, 1), "bytes_per_site_vec": bps, "gbs": round(bps * ctx.V * nvec / sec * 1e-9, 1),
+            "gflops": round(6 * 72.0 * ctx.V * nvec / sec * 1e-9, 1)}
+
+
 def roofline_entry(r, peak, peak_src, traffic=None):
     return {"bound": "hbm", "kernel": "dslash_kernel<%s,N=%d,recon=%d,form=%s>" % (r["prec"], r["nrhs"], r["recon"], r["kind"]),
             "achieved": round(r["gbs"], 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s",
@@ -239,6 +269,12 @@ def operator_sweeps(B, device, peak):
                 r = time_dslash(ctx, B, kind, "fp32", n, c["recon"], iters=20)
                 out[key].append({"kernel": kind, "nrhs": n, "us": round(r["seconds"] * 1e6, 1), "gbs": round(r["gbs"], 1), "gflops": round(r["gflops"], 1),
                                  "frac_measured_hbm": round(r["gbs"] / peak, 4), "frac_8TBs": round(r["gbs"] / 8000.0, 4)})
+        if cfg_id == 2:
+            out["laplacian_32x32x32x64_fp32"] = []
+            for n in (1, 4, 8, 16):
+                r = time_laplacian(ctx, B, n)
+                r["frac_measured_hbm"] = round(r["gbs"] / peak, 4)
+                out["laplacian_32x32x32x64_fp32"].append(r)
         ctx.close()
         torch.cuda.empty_cache()
     return out

@@ -171,6 +171,18 @@ typedef struct {
  * (SURVEY 8(c.1) step 11).  Returns LQ_ENOTCONVERGED (x, info still valid) if any RHS misses tol. */
 int lq_solve(lq_ctx* ctx, void* x, const void* b, int nrhs, int loc, int layout, const lq_solve_param* param, lq_solve_info* info);
 
+/* ---- 3-d gauge-covariant Laplacian ------------------------
+ * (Lap v)(x) = sum_{i=x,y,z} [ U_i(x) v(x+i) + U_i(x-i)^dag v(x-i) ] - 6 v(x) on every time-slice independently,
+ * periodic in space, for nvec colour-vector fields at once (nvec in {1,2,4,8,12,16}); uses the loaded gauge field
+ * (fp64 links for LQ_FP64, the fp32 18- or 12-real links for LQ_FP32; LQ_HALF is not supported).
+ * lq_laplacian: in/out canonical [vec][t][z][y][x][colour] complex double at `loc`; out must not alias in.
+ * lq_laplacian_native: device buffers of lq_cv_native_bytes() bytes in the library's blocked even/odd layout
+ * (for timing); lq_cv_fill_random writes bench-only pseudo-random values into such a buffer. */
+int lq_laplacian(lq_ctx* ctx, void* out, const void* in, int nvec, int prec, int loc);
+int lq_laplacian_native(lq_ctx* ctx, void* out, const void* in, int nvec, int prec);
+size_t lq_cv_native_bytes(const lq_ctx* ctx, int nvec, int prec);
+int lq_cv_fill_random(lq_ctx* ctx, void* native_out, int nvec, int prec, uint64_t seed);
+
 /* Launch-parameter knobs of the stencil kernels (the paper's autotuning, reduced to an
  * offline sweep): kernel variant (bits 0-7: 0 = default register budget, 1 = alternative; bits 8-15: z-chunk of the
  * sweep order, 0 = automatic, 0xFF = memory order; see csrc/dslash_launch.cuh),

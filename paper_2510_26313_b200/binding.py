@@ -25,7 +25,8 @@ PREC = {"fp64": LQ_FP64, "fp32": LQ_FP32, "half": LQ_HALF}
 
 EXPORTS = ["lq_create", "lq_destroy", "lq_last_error", "lq_set_allocator", "lq_load_gauge", "lq_fill_gauge_random",
            "lq_build_clover", "lq_apply", "lq_native_bytes", "lq_pack", "lq_unpack", "lq_fill_spinor_random", "lq_solve",
-           "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites"]
+           "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites",
+           "lq_laplacian", "lq_laplacian_native", "lq_cv_native_bytes", "lq_cv_fill_random"]
 
 
 class SolveParam(ctypes.Structure):
@@ -76,6 +77,11 @@ def load_library():
     lib.lq_solve.argtypes = [vp, vp, vp, ci, ci, ci, ctypes.POINTER(SolveParam), ctypes.POINTER(SolveInfo)]
     lib.lq_set_tuning.argtypes = [vp, ci, ci, ci]
     lib.lq_gather_sites.argtypes = [vp, vp, vp, ci, ci, ctypes.c_longlong, vp]
+    lib.lq_laplacian.argtypes = [vp, vp, vp, ci, ci, ci]
+    lib.lq_laplacian_native.argtypes = [vp, vp, vp, ci, ci]
+    lib.lq_cv_native_bytes.argtypes = [vp, ci, ci]
+    lib.lq_cv_native_bytes.restype = ctypes.c_size_t
+    lib.lq_cv_fill_random.argtypes = [vp, vp, ci, ci, u64]
     lib.lq_kernel_launches.argtypes = [vp]; lib.lq_kernel_launches.restype = ctypes.c_longlong
     _lib = lib
     return lib
@@ -207,6 +213,26 @@ class Context:
         self._check(self.lib.lq_gather_sites(self.h, ctypes.c_void_p(out.ctypes.data), ctypes.c_void_p(native_parity_block.data_ptr()),
                                              nrhs, prec, sites.shape[0], ctypes.c_void_p(sites.ctypes.data)))
         return out.view(np.complex128).reshape(sites.shape[0], nrhs, 4, 3)
+
+    # ------------------------------------------------------------------ 3-d covariant Laplacian
+    def laplacian(self, v: np.ndarray, prec: int = LQ_FP64) -> np.ndarray:
+        """v[vec][t][z][y][x][3] complex128 (host) -> Lap v, same shape."""
+        self._enter()
+        v = np.ascontiguousarray(v, dtype=np.complex128)
+        out = np.empty_like(v)
+        self._check(self.lib.lq_laplacian(self.h, ctypes.c_void_p(out.ctypes.data), ctypes.c_void_p(v.ctypes.data), v.shape[0], prec, LQ_HOST))
+        return out
+
+    def cv_native_empty(self, nvec: int, prec: int):
+        return self.torch.empty(int(self.lib.lq_cv_native_bytes(self.h, nvec, prec)), dtype=self.torch.uint8, device="cuda:%d" % self.device)
+
+    def cv_fill_random(self, native, nvec: int, prec: int, seed: int):
+        self._enter()
+        self._check(self.lib.lq_cv_fill_random(self.h, ctypes.c_void_p(native.data_ptr()), nvec, prec, seed))
+
+    def laplacian_native(self, out, inp, nvec: int, prec: int):
+        self._enter()
+        self._check(self.lib.lq_laplacian_native(self.h, ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(inp.data_ptr()), nvec, prec))
 
     # ------------------------------------------------------------------ operator
     def apply_native(self, op: int, out, inp, nrhs: int, prec: int, in2=None):

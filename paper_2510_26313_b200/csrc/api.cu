@@ -208,6 +208,45 @@ int lq_gather_sites(lq_ctx* c, double* out, const void* native_parity_block, int
     if (d_out) dev_free(c, d_out);
     return rc;
 }
+int lq_laplacian_native(lq_ctx* c, void* out, const void* in, int nvec, int prec) {
+    if (!c || !out || !in || out == in || !nrhs_ok(nvec)) return set_err(c, LQ_EINVAL, "lq_laplacian_native: bad argument");
+    if (prec != LQ_FP64 && prec != LQ_FP32) return set_err(c, LQ_EINVAL, "Laplacian precision must be fp64 or fp32");
+    if (!c->has_gauge) return set_err(c, LQ_ESTATE, "gauge field not loaded");
+    cudaSetDevice(c->device);
+    return laplacian_native(c, out, in, nvec, prec);
+}
+size_t lq_cv_native_bytes(const lq_ctx* c, int nvec, int prec) {
+    if (!c || nvec < 1 || (prec != LQ_FP64 && prec != LQ_FP32)) return 0;
+    return cv_native_bytes(c, nvec, prec);
+}
+int lq_cv_fill_random(lq_ctx* c, void* native_out, int nvec, int prec, uint64_t seed) {
+    if (!c || !native_out || !nrhs_ok(nvec) || (prec != LQ_FP64 && prec != LQ_FP32)) return set_err(c, LQ_EINVAL, "lq_cv_fill_random: bad argument");
+    cudaSetDevice(c->device);
+    return cv_fill(c, native_out, nvec, prec, seed);
+}
+int lq_laplacian(lq_ctx* c, void* out, const void* in, int nvec, int prec, int loc) {
+    if (!c || !out || !in || out == in || !nrhs_ok(nvec)) return set_err(c, LQ_EINVAL, "lq_laplacian: bad argument");
+    if (prec != LQ_FP64 && prec != LQ_FP32) return set_err(c, LQ_EINVAL, "Laplacian precision must be fp64 or fp32");
+    if (!c->has_gauge) return set_err(c, LQ_ESTATE, "gauge field not loaded");
+    cudaSetDevice(c->device);
+    const size_t cbytes = (size_t)nvec * c->g.V * 6 * sizeof(double), nbytes = cv_native_bytes(c, nvec, prec);
+    void *st_in = nullptr, *st_out = nullptr;
+    void *n_in = dev_alloc(c, nbytes), *n_out = dev_alloc(c, nbytes);
+    int rc = (!n_in || !n_out) ? LQ_ENOMEM : 0;
+    const void* d_in = nullptr;
+    if (rc == 0) { d_in = stage_in(c, in, cbytes, loc, &st_in); if (!d_in) rc = LQ_ENOMEM; }
+    if (rc == 0 && cudaMemsetAsync(n_in, 0, nbytes, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "memset failed");
+    if (rc == 0) rc = cv_pack(c, n_in, (const double*)d_in, nvec, prec);
+    if (rc == 0) rc = laplacian_native(c, n_out, n_in, nvec, prec);
+    void* d_out = out;
+    if (rc == 0 && loc == LQ_HOST) { st_out = dev_alloc(c, cbytes); if (!st_out) rc = LQ_ENOMEM; d_out = st_out; }
+    if (rc == 0) rc = cv_unpack(c, (double*)d_out, n_out, nvec, prec);
+    if (rc == 0 && st_out && cudaMemcpyAsync(out, st_out, cbytes, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "D2H copy failed");
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess && rc == 0) rc = set_err(c, LQ_ECUDA, std::string("lq_laplacian: ") + cudaGetErrorString(cudaGetLastError()));
+    void* tofree[] = {st_in, st_out, n_in, n_out};
+    for (void* p : tofree) if (p) dev_free(c, p);
+    return rc;
+}
 // the operator on native buffers
 static int apply_native(lq_ctx* c, int op, void* out, const void* in, const void* in2, int n, int prec) {
     const size_t pb = parity_bytes(c->g, n, prec);

@@ -56,3 +56,10 @@ int fill_spinor(lq_ctx* c, void* native, int nrhs, int prec, uint64_t seed, int 
 
 // solver.cu
 int solve_native(lq_ctx* c, void* x_full64, const void* b_full64, int nrhs, const lq_solve_param* p, lq_solve_info* info);
+
+// laplace.cu : batched 3-d gauge-covariant Laplacian on native colour-vector fields
+int laplacian_native(lq_ctx* c, void* out, const void* in, int nvec, int prec);
+size_t cv_native_bytes(const lq_ctx* c, int nvec, int prec);
+int cv_pack(lq_ctx* c, void* native, const double* dev_canon, int nvec, int prec);
+int cv_unpack(lq_ctx* c, double* dev_canon, const void* native, int nvec, int prec);
+int cv_fill(lq_ctx* c, void* native, int nvec, int prec, unsigned long long seed);

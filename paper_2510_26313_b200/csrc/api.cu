@@ -55,7 +55,7 @@ int lq_create(lq_ctx** out, const int dims[4], int device, void* cuda_stream) {
     c->clov64 = c->clovinv64 = nullptr; c->clov32 = c->clovinv32 = nullptr;
     c->kappa = c->csw = 0; c->has_gauge = c->has_clover = false;
     c->alloc_fn = nullptr; c->free_fn = nullptr; c->alloc_user = nullptr;
-    c->launches = 0; c->dslash_block = 0; c->dslash_rpt = 0; c->dslash_variant = 0; c->dslash_pfd = LQ_DEFAULT_PFD; c->dslash_zc = 0;
+    c->launches = 0; c->dslash_rpt = 0; c->dslash_variant = 0; c->dslash_pfd = LQ_DEFAULT_PFD; c->dslash_zc = 0;
     c->red_partials = nullptr; c->red_partials_elems = 0; c->red_counter = nullptr; c->h_scalars = nullptr; c->d_flag = nullptr;
     if (cudaMalloc(&c->red_counter, 256) != cudaSuccess || cudaMemset(c->red_counter, 0, 256) != cudaSuccess ||
         cudaMallocHost(&c->h_scalars, 8 * LQ_MAX_RHS * sizeof(double)) != cudaSuccess) { cudaGetLastError(); delete c; return LQ_ECUDA; }

@@ -48,60 +48,6 @@ __global__ void norm2_kernel(BlasGeom bg, SView<S> x, double* partials, unsigned
     reduce_per_rhs<VW, R>(part, bg.N, bg.G, partials, counter, out);
 }
 
-template <class S, int VW, int R>
-__global__ void cg_update_xr_kernel(BlasGeom bg, SView<S> x, SView<S> r, SView<S> p, SView<S> q, const double* __restrict__ rr,
-                                    const double* __restrict__ pAp, double* partials, unsigned int* counter, double* rr_new) {
-    using T = typename S::comp_t;
-    BlasIdx<VW, R> ix(bg.g, bg.G);
-    double part[VW];
-#pragma unroll
-    for (int k = 0; k < VW; k++) part[k] = 0.0;
-    if (ix.valid) {
-        T alpha[VW];
-#pragma unroll
-        for (int k = 0; k < VW; k++) { const double d = pAp[ix.rhs0 + k]; alpha[k] = (T)(d > 0.0 ? rr[ix.rhs0 + k] / d : 0.0); }
-        {
-            T a[24][VW], b[24][VW];
-            load_site_regs<S, VW, R>(x.d + ix.own, S::has_norm ? x.n + ix.own_n : nullptr, a);
-            load_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, b);
-#pragma unroll
-            for (int j = 0; j < 24; j++)
-#pragma unroll
-                for (int k = 0; k < VW; k++) a[j][k] += alpha[k] * b[j][k];
-            store_site_regs<S, VW, R>(x.d + ix.own, S::has_norm ? x.n + ix.own_n : nullptr, a);
-        }
-        {
-            T a[24][VW], b[24][VW];
-            load_site_regs<S, VW, R>(r.d + ix.own, S::has_norm ? r.n + ix.own_n : nullptr, a);
-            load_site_regs<S, VW, R>(q.d + ix.own, S::has_norm ? q.n + ix.own_n : nullptr, b);
-#pragma unroll
-            for (int j = 0; j < 24; j++)
-#pragma unroll
-                for (int k = 0; k < VW; k++) { a[j][k] -= alpha[k] * b[j][k]; part[k] += (double)a[j][k] * (double)a[j][k]; }
-            store_site_regs<S, VW, R>(r.d + ix.own, S::has_norm ? r.n + ix.own_n : nullptr, a);
-        }
-    }
-    reduce_per_rhs<VW, R>(part, bg.N, bg.G, partials, counter, rr_new);
-}
-
-template <class S, int VW, int R>
-__global__ void cg_update_p_kernel(BlasGeom bg, SView<S> p, SView<S> r, const double* __restrict__ rr_new, const double* __restrict__ rr) {
-    using T = typename S::comp_t;
-    BlasIdx<VW, R> ix(bg.g, bg.G);
-    if (!ix.valid) return;
-    T beta[VW];
-#pragma unroll
-    for (int k = 0; k < VW; k++) { const double d = rr[ix.rhs0 + k]; beta[k] = (T)(d > 0.0 ? rr_new[ix.rhs0 + k] / d : 0.0); }
-    T a[24][VW], b[24][VW];
-    load_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, a);
-    load_site_regs<S, VW, R>(r.d + ix.own, S::has_norm ? r.n + ix.own_n : nullptr, b);
-#pragma unroll
-    for (int j = 0; j < 24; j++)
-#pragma unroll
-        for (int k = 0; k < VW; k++) a[j][k] = b[j][k] + beta[k] * a[j][k];
-    store_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, a);
-}
-
 // e += alpha p ; p = z + beta p   (alpha = rr / pAp, beta = rr_new / rr)
 template <class S, int VW, int R>
 __global__ void cg_update_ep_kernel(BlasGeom bg, SView<S> e, SView<S> p, SView<S> z, const double* __restrict__ rr, const double* __restrict__ pAp,
@@ -225,35 +171,6 @@ int blas_norm2(lq_ctx* c, int prec, int nrhs, const void* x, double* d_out) {
     if (prec == LQ_FP64) return norm2_t<F64>(c, nrhs, x, d_out);
     if (prec == LQ_FP32) return norm2_t<F32>(c, nrhs, x, d_out);
     return norm2_t<H16>(c, nrhs, x, d_out);
-}
-
-template <class S> static int xr_t(lq_ctx* c, int nrhs, void* x, void* r, const void* p, const void* q, const double* rr, const double* pAp, double* rrn) {
-    Launch L; LQ_TRY(plan(c, nrhs, S::prec == LQ_FP64 ? 2 : 4, L));
-    SView<S> vx = make_view<S>(c->g, x, nrhs, 0), vr = make_view<S>(c->g, r, nrhs, 0);
-    SView<S> vp = make_view<S>(c->g, const_cast<void*>(p), nrhs, 0), vq = make_view<S>(c->g, const_cast<void*>(q), nrhs, 0);
-    VW_DISPATCH(L, S, cg_update_xr_kernel, L.smem, L.bg, vx, vr, vp, vq, rr, pAp, c->red_partials, c->red_counter, rrn);
-    LQ_LAUNCHED(c);
-    LQ_CUDA(c, cudaGetLastError());
-    return 0;
-}
-int blas_cg_update_xr(lq_ctx* c, int prec, int nrhs, void* x, void* r, const void* p, const void* q, const double* d_rr, const double* d_pAp, double* d_rr_new) {
-    if (prec == LQ_FP64) return xr_t<F64>(c, nrhs, x, r, p, q, d_rr, d_pAp, d_rr_new);
-    if (prec == LQ_FP32) return xr_t<F32>(c, nrhs, x, r, p, q, d_rr, d_pAp, d_rr_new);
-    return xr_t<H16>(c, nrhs, x, r, p, q, d_rr, d_pAp, d_rr_new);
-}
-
-template <class S> static int p_t(lq_ctx* c, int nrhs, void* p, const void* r, const double* rrn, const double* rr) {
-    Launch L; LQ_TRY(plan(c, nrhs, S::prec == LQ_FP64 ? 2 : 4, L));
-    SView<S> vp = make_view<S>(c->g, p, nrhs, 0), vr = make_view<S>(c->g, const_cast<void*>(r), nrhs, 0);
-    VW_DISPATCH(L, S, cg_update_p_kernel, 0, L.bg, vp, vr, rrn, rr);
-    LQ_LAUNCHED(c);
-    LQ_CUDA(c, cudaGetLastError());
-    return 0;
-}
-int blas_cg_update_p(lq_ctx* c, int prec, int nrhs, void* p, const void* r, const double* d_rr_new, const double* d_rr) {
-    if (prec == LQ_FP64) return p_t<F64>(c, nrhs, p, r, d_rr_new, d_rr);
-    if (prec == LQ_FP32) return p_t<F32>(c, nrhs, p, r, d_rr_new, d_rr);
-    return p_t<H16>(c, nrhs, p, r, d_rr_new, d_rr);
 }
 
 template <class S> static int ep_t(lq_ctx* c, int nrhs, void* e, void* p, const void* z, const double* rr, const double* pAp, const double* rrn) {

@@ -169,7 +169,6 @@ struct lq_ctx {
     lq_alloc_fn alloc_fn; lq_free_fn free_fn; void* alloc_user;
     std::vector<void*> owned;       // everything from dev_alloc still alive
     long long launches;
-    int dslash_block;               // tuning knob (0 = default)
     int dslash_rpt;                 // tuning knob (0 = auto)
     int dslash_variant;             // tuning knob: kernel variant (0 = default)
     int dslash_pfd;                 // tuning knob: L2 prefetch distance in site blocks (0 = off)

@@ -35,11 +35,6 @@ int clover_build(lq_ctx* c, double kappa, double csw);
 
 // blas.cu : per-RHS block BLAS on one parity block; results stay on the device
 int blas_norm2(lq_ctx* c, int prec, int nrhs, const void* x, double* d_out);                       // d_out[k] = ||x_k||^2
-// CG step 1: alpha_k = rr_k / pAp_k;  x += alpha p;  r -= alpha q;  rr_new_k = ||r_k||^2
-int blas_cg_update_xr(lq_ctx* c, int prec, int nrhs, void* x, void* r, const void* p, const void* q,
-                      const double* d_rr, const double* d_pAp, double* d_rr_new);
-// CG step 2: beta_k = rr_new_k / rr_k;  p = r + beta p
-int blas_cg_update_p(lq_ctx* c, int prec, int nrhs, void* p, const void* r, const double* d_rr_new, const double* d_rr);
 // y (fp64) += s_k * e (prec)       (defect-correction accumulate)
 // fused CG vector update: alpha_k = rr_k / pAp_k, beta_k = rr_new_k / rr_k;  e += alpha p;  p = z + beta p
 int blas_cg_update_ep(lq_ctx* c, int prec, int nrhs, void* e, void* p, const void* z, const double* d_rr, const double* d_pAp, const double* d_rr_new);

@@ -14,7 +14,6 @@ struct Workspace {
     void *e = nullptr, *z = nullptr, *p = nullptr, *t = nullptr, *q = nullptr, *tmp = nullptr, *rt = nullptr;  // inner precision
     double* d_scal = nullptr;                                                       // 8 x LQ_MAX_RHS doubles
 };
-static Workspace g_ws_dummy;
 
 struct WsHolder { lq_ctx* c; Workspace ws; };
 static std::vector<WsHolder> g_ws;      // one cached workspace per context

@@ -185,6 +185,61 @@ __device__ __forceinline__ void hop_mulacc(const T (&h)[2][3][2][RPT], const T (
         }
 }
 
+// ---- packed-FP32 variant of hop_mulacc for 2 right-hand sides per thread (sm_100 FFMA2: one instruction = the same FMA
+// on both right-hand sides; the link element is duplicated into a register pair).  Same arithmetic, same rounding.
+#ifdef LQ_USE_FFMA2
+template <int RPT, int MU, bool FWD>
+__device__ __forceinline__ void hop_mulacc_f2(const float (&h)[2][3][2][RPT], const float (&u)[18], const float (&cuk)[RPT], const float (&clk)[RPT],
+                                              float (&acc)[24][RPT]) {
+#pragma unroll
+  for (int k0 = 0; k0 < RPT; k0 += 2) {
+    const float2 cu2 = make_float2(cuk[k0], cuk[k0 + 1]), cl2 = make_float2(clk[k0], clk[k0 + 1]), ncl2 = make_float2(-clk[k0], -clk[k0 + 1]);
+#define A2(j) make_float2(acc[j][k0], acc[j][k0 + 1])
+#define SETA(j, v) { const float2 t_ = (v); acc[j][k0] = t_.x; acc[j][k0 + 1] = t_.y; }
+#pragma unroll
+    for (int r = 0; r < 3; r++) {
+        float2 wr[2], wi[2];
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const float ur = FWD ? u[2 * (3 * r + c)] : u[2 * (3 * c + r)];
+            const float ui = FWD ? u[2 * (3 * r + c) + 1] : -u[2 * (3 * c + r) + 1];
+            const float2 ur2 = make_float2(ur, ur), ui2 = make_float2(ui, ui), nui2 = make_float2(-ui, -ui);
+#pragma unroll
+            for (int s = 0; s < 2; s++) {
+                const float2 hr = make_float2(h[s][c][0][k0], h[s][c][0][k0 + 1]), hi = make_float2(h[s][c][1][k0], h[s][c][1][k0 + 1]);
+                if (c == 0) { wr[s] = __fmul2_rn(ur2, hr); wi[s] = __fmul2_rn(ur2, hi); }
+                else { wr[s] = __ffma2_rn(ur2, hr, wr[s]); wi[s] = __ffma2_rn(ur2, hi, wi[s]); }
+                wr[s] = __ffma2_rn(nui2, hi, wr[s]);
+                wi[s] = __ffma2_rn(ui2, hr, wi[s]);
+            }
+        }
+#pragma unroll
+        for (int s = 0; s < 2; s++) {
+            const int ju = 2 * (3 * s + r);
+            SETA(ju, __ffma2_rn(cu2, wr[s], A2(ju))) SETA(ju + 1, __ffma2_rn(cu2, wi[s], A2(ju + 1)))
+            if constexpr (MU == 0) {
+                const int jl = 2 * (3 * (3 - s) + r);
+                SETA(jl, __ffma2_rn(ncl2, wi[s], A2(jl))) SETA(jl + 1, __ffma2_rn(cl2, wr[s], A2(jl + 1)))
+            } else if constexpr (MU == 1) {
+                const int jl = 2 * (3 * (3 - s) + r);
+                if (s == 0) { SETA(jl, __ffma2_rn(cl2, wr[s], A2(jl))) SETA(jl + 1, __ffma2_rn(cl2, wi[s], A2(jl + 1))) }
+                else { SETA(jl, __ffma2_rn(ncl2, wr[s], A2(jl))) SETA(jl + 1, __ffma2_rn(ncl2, wi[s], A2(jl + 1))) }
+            } else if constexpr (MU == 2) {
+                const int jl = 2 * (3 * (2 + s) + r);
+                if (s == 0) { SETA(jl, __ffma2_rn(ncl2, wi[s], A2(jl))) SETA(jl + 1, __ffma2_rn(cl2, wr[s], A2(jl + 1))) }
+                else { SETA(jl, __ffma2_rn(cl2, wi[s], A2(jl))) SETA(jl + 1, __ffma2_rn(ncl2, wr[s], A2(jl + 1))) }
+            } else {
+                const int jl = 2 * (3 * (2 + s) + r);
+                SETA(jl, __ffma2_rn(ncl2, wr[s], A2(jl))) SETA(jl + 1, __ffma2_rn(ncl2, wi[s], A2(jl + 1)))
+            }
+        }
+    }
+#undef A2
+#undef SETA
+  }
+}
+#endif
+
 // ---- one of the eight hopping terms -------------------------------------------------------------------
 // acc[j][k] += cu * (1 - sigma*gamma_MU) W psi(nb),  W = U (FWD) or U^dag (backward), sigma = +-1.
 // `nb` points at real 0 of the neighbour's RPT right-hand sides; real j is at nb + j*SB*R.
@@ -219,6 +274,32 @@ __device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ 
         for (int s = 0; s < 4; s++)
 #pragma unroll
             for (int ri = 0; ri < 2; ri++) load_comp<S, RPT>(nb + (2 * (3 * s + c) + ri) * PL, p[s][ri]);
+#ifdef LQ_USE_FFMA2
+        if constexpr (sizeof(T) == 4 && RPT % 2 == 0) {
+#pragma unroll
+            for (int k = 0; k < RPT; k += 2) {
+                const float2 sg = make_float2(sigma, sigma), ns = make_float2(-sigma, -sigma);
+#define P2(s_, ri_) make_float2(p[s_][ri_][k], p[s_][ri_][k + 1])
+#define SETH(s_, ri_, v) { const float2 t_ = (v); h[s_][c][ri_][k] = t_.x; h[s_][c][ri_][k + 1] = t_.y; }
+                if constexpr (MU == 0) {
+                    SETH(0, 0, __ffma2_rn(sg, P2(3, 1), P2(0, 0))) SETH(0, 1, __ffma2_rn(ns, P2(3, 0), P2(0, 1)))
+                    SETH(1, 0, __ffma2_rn(sg, P2(2, 1), P2(1, 0))) SETH(1, 1, __ffma2_rn(ns, P2(2, 0), P2(1, 1)))
+                } else if constexpr (MU == 1) {
+                    SETH(0, 0, __ffma2_rn(sg, P2(3, 0), P2(0, 0))) SETH(0, 1, __ffma2_rn(sg, P2(3, 1), P2(0, 1)))
+                    SETH(1, 0, __ffma2_rn(ns, P2(2, 0), P2(1, 0))) SETH(1, 1, __ffma2_rn(ns, P2(2, 1), P2(1, 1)))
+                } else if constexpr (MU == 2) {
+                    SETH(0, 0, __ffma2_rn(sg, P2(2, 1), P2(0, 0))) SETH(0, 1, __ffma2_rn(ns, P2(2, 0), P2(0, 1)))
+                    SETH(1, 0, __ffma2_rn(ns, P2(3, 1), P2(1, 0))) SETH(1, 1, __ffma2_rn(sg, P2(3, 0), P2(1, 1)))
+                } else {
+                    SETH(0, 0, __ffma2_rn(ns, P2(2, 0), P2(0, 0))) SETH(0, 1, __ffma2_rn(ns, P2(2, 1), P2(0, 1)))
+                    SETH(1, 0, __ffma2_rn(ns, P2(3, 0), P2(1, 0))) SETH(1, 1, __ffma2_rn(ns, P2(3, 1), P2(1, 1)))
+                }
+#undef P2
+#undef SETH
+            }
+        } else
+#endif
+        {
 #pragma unroll
         for (int k = 0; k < RPT; k++) {
             if constexpr (MU == 0) {        // h0 = p0 - s i p3, h1 = p1 - s i p2
@@ -235,6 +316,10 @@ __device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ 
                 h[1][c][0][k] = fm(-sigma, p[3][0][k], p[1][0][k]); h[1][c][1][k] = fm(-sigma, p[3][1][k], p[1][1][k]);
             }
         }
+        }
     }
+#ifdef LQ_USE_FFMA2
+    if constexpr (sizeof(T) == 4 && RPT % 2 == 0) { hop_mulacc_f2<RPT, MU, FWD>(h, u, cuk, clk, acc); return; }
+#endif
     hop_mulacc<T, RPT, MU, FWD>(h, u, cuk, clk, acc);
 }

@@ -8,6 +8,32 @@
 // 22 FP instructions per output row and RHS: 2 multiplies by the real diagonal + 5 complex fused multiply-adds.
 template <typename T, int RPT>
 __device__ __forceinline__ void clover_block_mul(const T* cl, const T (&v)[6][2][RPT], T (&o)[6][2][RPT]) {
+#ifdef LQ_USE_FFMA2
+    if constexpr (sizeof(T) == 4 && RPT % 2 == 0) {      // packed FP32: one FFMA2 per pair of right-hand sides
+#pragma unroll
+        for (int k = 0; k < RPT; k += 2) {
+#define V2(j_, ri_) make_float2(v[j_][ri_][k], v[j_][ri_][k + 1])
+#pragma unroll
+            for (int i = 0; i < 6; i++) {
+                const float2 d2 = make_float2(cl[i], cl[i]);
+                float2 orr = __fmul2_rn(d2, V2(i, 0)), oi = __fmul2_rn(d2, V2(i, 1));
+#pragma unroll
+                for (int j = 0; j < 6; j++) {
+                    if (j == i) continue;
+                    const int idx = (i > j) ? (i * (i - 1) / 2 + j) : (j * (j - 1) / 2 + i);
+                    const float lr = cl[6 + 2 * idx];
+                    const float li = (i > j) ? cl[7 + 2 * idx] : -cl[7 + 2 * idx];
+                    const float2 lr2 = make_float2(lr, lr), li2 = make_float2(li, li), nli2 = make_float2(-li, -li);
+                    orr = __ffma2_rn(lr2, V2(j, 0), orr); orr = __ffma2_rn(nli2, V2(j, 1), orr);
+                    oi = __ffma2_rn(lr2, V2(j, 1), oi); oi = __ffma2_rn(li2, V2(j, 0), oi);
+                }
+                o[i][0][k] = orr.x; o[i][0][k + 1] = orr.y; o[i][1][k] = oi.x; o[i][1][k + 1] = oi.y;
+            }
+#undef V2
+        }
+        return;
+    }
+#endif
 #pragma unroll
     for (int i = 0; i < 6; i++) {
 #pragma unroll

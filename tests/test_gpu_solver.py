@@ -136,3 +136,24 @@ def test_every_batch_width_solves(nrhs):
     assert info["converged"], info
     assert np.all(true_residuals(orc, x, b) <= 1e-9)
     ctx.close()
+
+
+@pytest.mark.parametrize("keep_direction", [False, True])
+def test_restart_and_reliable_update_variants(keep_direction):
+    """Both outer-loop variants (SURVEY 8(c.2) reading #11): restart defect correction (p = z after every fp64 residual
+    refresh) and reliable updates (the direction survives the refresh).  Both must reach the tolerance; keeping the
+    direction must not cost iterations."""
+    dims = (8, 8, 8, 16)
+    ctx, orc = setup(dims, 55, 0.25, 0.124, 1.15)
+    b = inputs.laph_sources(dims, 8, 2, 56)
+    x, info = ctx.solve(b, tol=1e-9, inner_prec=B.LQ_FP32, delta=1e-2, check_every=2, use_graph=True, keep_direction=keep_direction)
+    assert info["converged"], info
+    assert np.all(true_residuals(orc, x, b) <= 1e-9)
+    test_restart_and_reliable_update_variants.iters[keep_direction] = info["inner_iters"]
+    if len(test_restart_and_reliable_update_variants.iters) == 2:
+        it = test_restart_and_reliable_update_variants.iters
+        assert it[True] <= it[False]
+    ctx.close()
+
+
+test_restart_and_reliable_update_variants.iters = {}

@@ -216,3 +216,23 @@ def laplacian(dims, U, v) -> np.ndarray:
     out = np.empty_like(v)
     lib().orc_laplacian(_dims(dims), _c(U), ctypes.c_long(nvec), _c(v), _c(out))
     return out
+
+
+def laph_eigen(dims, U, n_ev: int):
+    """Lowest n_ev eigenpairs of -Laplacian on every time-slice by the plain definition: the dense
+    3*Ls^3 x 3*Ls^3 matrix of each slice is assembled by applying `laplacian` to unit vectors and handed to
+    numpy.linalg.eigh.  Small lattices only.  Returns (evals[Lt][n_ev] ascending, evecs[Lt][n_ev][z][y][x][3])."""
+    Lx, Ly, Lz, Lt = dims
+    K = 3 * Lx * Ly * Lz
+    basis = np.zeros((K, Lt, Lz, Ly, Lx, 3), dtype=np.complex128)
+    flat = basis.reshape(K, Lt, K)
+    for k in range(K):
+        flat[k, :, k] = 1.0                       # the same unit vector on every slice: slices do not couple
+    cols = laplacian(dims, U, basis).reshape(K, Lt, K)
+    evals = np.empty((Lt, n_ev)); evecs = np.empty((Lt, n_ev, Lz, Ly, Lx, 3), dtype=np.complex128)
+    for t in range(Lt):
+        A = -cols[:, t, :].T                      # A[:, k] = -Lap e_k
+        w, v = np.linalg.eigh(0.5 * (A + A.conj().T))
+        evals[t] = w[:n_ev]
+        evecs[t] = v[:, :n_ev].T.reshape(n_ev, Lz, Ly, Lx, 3)
+    return evals, evecs

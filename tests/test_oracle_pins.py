@@ -483,3 +483,26 @@ def test_laplacian_hermitian_negative_covariant_and_time_local(oracle_lib, rough
     U2 = U.copy(); U2[3] = inputs.make_links(dims, 99, 0.3)[3]
     assert np.abs(oracle.laplacian(dims, U2, w[None])[0][1:]).max() == 0
     assert np.array_equal(oracle.laplacian(dims, U2, w[None])[0][0], Lv[0])
+
+
+def test_laph_eigen_free_field_and_gauge_invariance(oracle_lib):
+    """Dense eigen-decomposition of -Laplacian per time-slice: free-field spectrum = the multiset {sum_i 4 sin^2(p_i/2)} x 3
+    colours; the spectrum on rough links is invariant under a gauge transformation; A v = lambda v holds for what comes back."""
+    import oracle
+    dims = (4, 4, 2, 2)
+    ev, vec = oracle.laph_eigen(dims, inputs.unit_links(dims), 12)
+    ps = sorted(sum(4 * np.sin(np.pi * n[i] / dims[i]) ** 2 for i in range(3)) for n in np.ndindex(4, 4, 2) for _ in range(3))
+    assert np.allclose(ev[0], ps[:12], atol=1e-12) and np.allclose(ev[1], ps[:12], atol=1e-12)
+    U = inputs.make_links(dims, 17, 0.3)
+    ev, vec = oracle.laph_eigen(dims, U, 10)
+    g = inputs.random_gauge_transform(dims, 18)
+    Ug = np.empty_like(U)
+    for mu in range(4):
+        Ug[mu] = g @ U[mu] @ np.conj(np.swapaxes(np.roll(g, -1, axis=3 - mu), -1, -2))
+    ev_g, _ = oracle.laph_eigen(dims, Ug, 10)
+    assert np.allclose(ev, ev_g, atol=1e-12)
+    assert np.all(ev > -1e-12) and np.all(np.diff(ev, axis=1) >= -1e-12)
+    v = np.zeros((10, 2, 2, 4, 4, 3), dtype=complex)
+    v[:, 1] = vec[1]                                   # the slice-1 eigenvectors, zero elsewhere
+    Lv = oracle.laplacian(dims, U, v)
+    assert np.abs(-Lv[:, 1] - ev[1][:, None, None, None, None] * v[:, 1]).max() < 1e-12

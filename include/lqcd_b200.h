@@ -183,6 +183,32 @@ int lq_laplacian_native(lq_ctx* ctx, void* out, const void* in, int nvec, int pr
 size_t lq_cv_native_bytes(const lq_ctx* ctx, int nvec, int prec);
 int lq_cv_fill_random(lq_ctx* ctx, void* native_out, int nvec, int prec, uint64_t seed);
 
+/* ---- time-batched Lanczos for the LapH eigenvectors -------------------
+ * Lowest n_ev eigenpairs of A = -Laplacian on EVERY time-slice (the Lt slices are independent eigenproblems that advance
+ * in lockstep): thick-restart Lanczos with full reorthogonalisation on the Chebyshev polynomial
+ * T_degree((2A - (cheb_a + cheb_b)) / (cheb_b - cheb_a)); cheb_a = cut just above the wanted eigenvalues, cheb_b >= the
+ * largest eigenvalue of A (12 is a bound).  fp64 throughout. */
+typedef struct {
+    int n_ev;            /* eigenpairs wanted per time-slice                                          */
+    int m;               /* Krylov space size, n_ev + 2 <= m <= 64                                     */
+    int cheb_degree;     /* degree of the Chebyshev filter (>= 1)                                      */
+    int max_restarts;
+    double cheb_a, cheb_b;
+    double tol;          /* Ritz residual |beta_m q_mi| <= tol * |theta_max| for all wanted pairs, all slices */
+    unsigned long long seed;   /* start vector                                                          */
+} lq_eig_param;
+typedef struct {
+    int restarts, converged;
+    double lap_applies;        /* Laplacian applications (each on one field = all time-slices)          */
+    double max_ritz_residual;  /* the convergence measure above, worst pair and slice                   */
+    double max_true_residual;  /* max over pairs and slices of ||A v - lambda v||_2 of the returned vectors (||v|| = 1) */
+    double seconds;
+} lq_eig_info;
+/* evals: HOST array [Lt][n_ev] (ascending per slice); evecs: canonical [n_ev][t][z][y][x][colour] complex double at
+ * `loc`, or NULL.  Each returned vector has unit norm on every time-slice.  Returns LQ_ENOTCONVERGED (outputs still
+ * filled) if max_restarts is reached. */
+int lq_laph_eigensolve(lq_ctx* ctx, double* evals, void* evecs, int loc, const lq_eig_param* param, lq_eig_info* info);
+
 /* Launch-parameter knobs of the stencil kernels (the paper's autotuning, reduced to an
  * offline sweep): kernel variant (bits 0-7: 0 = default register budget, 1 = alternative; bits 8-15: z-chunk of the
  * sweep order, 0 = automatic, 0xFF = memory order; see csrc/dslash_launch.cuh),

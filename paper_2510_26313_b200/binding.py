@@ -26,13 +26,23 @@ PREC = {"fp64": LQ_FP64, "fp32": LQ_FP32, "half": LQ_HALF}
 EXPORTS = ["lq_create", "lq_destroy", "lq_last_error", "lq_set_allocator", "lq_load_gauge", "lq_fill_gauge_random",
            "lq_build_clover", "lq_apply", "lq_native_bytes", "lq_pack", "lq_unpack", "lq_fill_spinor_random", "lq_solve",
            "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites",
-           "lq_laplacian", "lq_laplacian_native", "lq_cv_native_bytes", "lq_cv_fill_random"]
+           "lq_laplacian", "lq_laplacian_native", "lq_cv_native_bytes", "lq_cv_fill_random", "lq_laph_eigensolve"]
 
 
 class SolveParam(ctypes.Structure):
     _fields_ = [("tol", ctypes.c_double), ("max_outer", ctypes.c_int), ("max_inner", ctypes.c_int), ("inner_prec", ctypes.c_int),
                 ("delta", ctypes.c_double), ("check_every", ctypes.c_int), ("use_graph", ctypes.c_int),
                 ("keep_direction", ctypes.c_int), ("reserved", ctypes.c_int)]
+
+
+class EigParam(ctypes.Structure):
+    _fields_ = [("n_ev", ctypes.c_int), ("m", ctypes.c_int), ("cheb_degree", ctypes.c_int), ("max_restarts", ctypes.c_int),
+                ("cheb_a", ctypes.c_double), ("cheb_b", ctypes.c_double), ("tol", ctypes.c_double), ("seed", ctypes.c_ulonglong)]
+
+
+class EigInfo(ctypes.Structure):
+    _fields_ = [("restarts", ctypes.c_int), ("converged", ctypes.c_int), ("lap_applies", ctypes.c_double),
+                ("max_ritz_residual", ctypes.c_double), ("max_true_residual", ctypes.c_double), ("seconds", ctypes.c_double)]
 
 
 class SolveInfo(ctypes.Structure):
@@ -82,6 +92,7 @@ def load_library():
     lib.lq_cv_native_bytes.argtypes = [vp, ci, ci]
     lib.lq_cv_native_bytes.restype = ctypes.c_size_t
     lib.lq_cv_fill_random.argtypes = [vp, vp, ci, ci, u64]
+    lib.lq_laph_eigensolve.argtypes = [vp, vp, vp, ci, ctypes.POINTER(EigParam), ctypes.POINTER(EigInfo)]
     lib.lq_kernel_launches.argtypes = [vp]; lib.lq_kernel_launches.restype = ctypes.c_longlong
     _lib = lib
     return lib
@@ -222,6 +233,22 @@ class Context:
         out = np.empty_like(v)
         self._check(self.lib.lq_laplacian(self.h, ctypes.c_void_p(out.ctypes.data), ctypes.c_void_p(v.ctypes.data), v.shape[0], prec, LQ_HOST))
         return out
+
+    def laph_eigensolve(self, n_ev: int, m: int, cheb_degree: int, cheb_a: float, cheb_b: float = 12.5, tol: float = 1e-10,
+                        max_restarts: int = 100, seed: int = 1, want_vectors: bool = True):
+        """Lowest n_ev eigenpairs of -Laplacian on every time-slice.  Returns (evals[Lt][n_ev], evecs[n_ev][t][z][y][x][3] or None, info)."""
+        self._enter()
+        Lx, Ly, Lz, Lt = self.dims
+        prm = EigParam(n_ev, m, cheb_degree, max_restarts, cheb_a, cheb_b, tol, seed)
+        info = EigInfo()
+        evals = np.empty((Lt, n_ev), dtype=np.float64)
+        evecs = np.empty((n_ev, Lt, Lz, Ly, Lx, 3), dtype=np.complex128) if want_vectors else None
+        rc = self.lib.lq_laph_eigensolve(self.h, ctypes.c_void_p(evals.ctypes.data), ctypes.c_void_p(evecs.ctypes.data) if want_vectors else None,
+                                         LQ_HOST, ctypes.byref(prm), ctypes.byref(info))
+        self._check(rc, allow=(LQ_ENOTCONVERGED,))
+        d = dict(converged=bool(info.converged), restarts=info.restarts, lap_applies=info.lap_applies, max_ritz_residual=info.max_ritz_residual,
+                 max_true_residual=info.max_true_residual, seconds=info.seconds)
+        return evals, evecs, d
 
     def cv_native_empty(self, nvec: int, prec: int):
         return self.torch.empty(int(self.lib.lq_cv_native_bytes(self.h, nvec, prec)), dtype=self.torch.uint8, device="cuda:%d" % self.device)

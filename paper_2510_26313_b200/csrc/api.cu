@@ -247,6 +247,22 @@ int lq_laplacian(lq_ctx* c, void* out, const void* in, int nvec, int prec, int l
     for (void* p : tofree) if (p) dev_free(c, p);
     return rc;
 }
+int lq_laph_eigensolve(lq_ctx* c, double* evals, void* evecs, int loc, const lq_eig_param* param, lq_eig_info* info) {
+    if (!c || !evals || !param || !info) return set_err(c, LQ_EINVAL, "lq_laph_eigensolve: null argument");
+    if (!c->has_gauge) return set_err(c, LQ_ESTATE, "gauge field not loaded");
+    cudaSetDevice(c->device);
+    memset(info, 0, sizeof(*info));
+    const size_t cbytes = (size_t)(param->n_ev > 0 ? param->n_ev : 0) * c->g.V * 6 * sizeof(double);
+    void* st = nullptr; double* d_ev = (double*)evecs;
+    if (evecs && loc == LQ_HOST) { st = dev_alloc(c, cbytes); if (!st) return LQ_ENOMEM; d_ev = (double*)st; }
+    int rc = laph_eigensolve(c, evals, d_ev, param, info);
+    if ((rc == 0 || rc == LQ_ENOTCONVERGED) && st) {
+        if (cudaMemcpyAsync(evecs, st, cbytes, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess || cudaStreamSynchronize(c->stream) != cudaSuccess)
+            rc = set_err(c, LQ_ECUDA, "D2H copy failed");
+    }
+    if (st) dev_free(c, st);
+    return rc;
+}
 // the operator on native buffers
 static int apply_native(lq_ctx* c, int op, void* out, const void* in, const void* in2, int n, int prec) {
     const size_t pb = parity_bytes(c->g, n, prec);

@@ -1,0 +1,252 @@
+// eigen.cu -- time-batched thick-restart Lanczos for the lowest eigenpairs of -Laplacian on every time-slice
+// ("a highly-scalable batched Lanczos eigensolver", the time extent is the batch).
+//
+// All Lt slices advance in lockstep through the same kernels; every scalar of the iteration (Gram-Schmidt coefficients,
+// norms, projected matrices, Ritz rotations) exists once per slice.  The operator handed to Lanczos is the Chebyshev
+// polynomial B = T_d((2A - (a+b)) / (b-a)) of A = -Laplacian: eigenvalues of A below the cut `a` are mapped to the
+// largest |eigenvalues| of B, which Lanczos finds first.  The Krylov basis is kept fully orthogonal (two classical
+// Gram-Schmidt passes per step), so the projected matrix T = V^dag B V is real symmetric and is simply re-diagonalised
+// (cyclic Jacobi, host, m x m per slice) at every restart; the k best Ritz vectors and the residual vector seed the
+// next sweep (thick restart).  Eigenvalues of A are returned as Rayleigh quotients <v, A v> of the final Ritz vectors.
+#include <math.h>
+#include <algorithm>
+#include <vector>
+#include "internal.cuh"
+#include "eigen_kernels.cuh"
+
+namespace {
+
+struct Eig {
+    lq_ctx* c; SliceGeom sg; int Lt, nchunk; size_t fbytes;
+    double2 *d_partial, *d_H;     // dot partials; coefficient rows [m+2][Lt]
+    double* d_scale;              // [Lt]
+    std::vector<double2> h_H;
+    long long lap_applies = 0;
+};
+
+int grid_sites(const Eig& e) { return (int)((2LL * e.sg.Vh + 127) / 128); }
+
+int dot(Eig& e, const double* a, const double* b, double2* d_out) {
+    slice_dot_kernel<<<e.Lt * e.nchunk, 256, 0, e.c->stream>>>(e.sg, e.nchunk, a, b, e.d_partial);
+    slice_dot_final_kernel<<<(e.Lt + 63) / 64, 64, 0, e.c->stream>>>(e.Lt, e.nchunk, e.d_partial, d_out);
+    e.c->launches += 2;
+    LQ_CUDA(e.c, cudaGetLastError());
+    return 0;
+}
+__global__ void negate_kernel(int n, double2* h) { const int i = blockIdx.x * blockDim.x + threadIdx.x; if (i < n) { h[i].x = -h[i].x; h[i].y = -h[i].y; } }
+__global__ void inv_norm_kernel(int Lt, const double2* nn, double* inv, double* beta) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= Lt) return;
+    const double b = sqrt(fmax(nn[t].x, 0.0));
+    beta[t] = b; inv[t] = b > 0.0 ? 1.0 / b : 0.0;
+}
+
+// w <- B w0 = T_d(L) w0, L = (2A - (a+b))/(b-a), A = -Laplacian; y0, y1, tmp are scratch fields
+int chebyshev(Eig& e, double* out, const double* v, int degree, double a, double b, double* y0, double* y1, double* tmp) {
+    const double c1 = -2.0 / (b - a), c0 = -(b + a) / (b - a);
+    const int grid = grid_sites(e);
+    LQ_TRY(laplacian_native(e.c, tmp, v, 1, LQ_FP64)); e.lap_applies++;
+    // y1 = L v
+    cv_axpbypcz_kernel<<<grid, 128, 0, e.c->stream>>>(e.sg, y1, c1, tmp, c0, v, 0.0); e.c->launches++;
+    if (degree == 1) { LQ_CUDA(e.c, cudaMemcpyAsync(out, y1, e.fbytes, cudaMemcpyDeviceToDevice, e.c->stream)); return 0; }
+    LQ_CUDA(e.c, cudaMemcpyAsync(y0, v, e.fbytes, cudaMemcpyDeviceToDevice, e.c->stream));
+    double *prev = y0, *cur = y1;
+    for (int n = 1; n < degree; n++) {
+        LQ_TRY(laplacian_native(e.c, tmp, cur, 1, LQ_FP64)); e.lap_applies++;
+        // prev <- 2 L cur - prev
+        cv_axpbypcz_kernel<<<grid, 128, 0, e.c->stream>>>(e.sg, prev, 2.0 * c1, tmp, 2.0 * c0, cur, -1.0); e.c->launches++;
+        std::swap(prev, cur);
+    }
+    LQ_CUDA(e.c, cudaMemcpyAsync(out, cur, e.fbytes, cudaMemcpyDeviceToDevice, e.c->stream));
+    LQ_CUDA(e.c, cudaGetLastError());
+    return 0;
+}
+
+// cyclic Jacobi for a real symmetric n x n matrix (row-major a, destroyed); eigenvalues d, eigenvectors columns of q
+void jacobi(int n, std::vector<double>& a, std::vector<double>& d, std::vector<double>& q) {
+    q.assign((size_t)n * n, 0.0);
+    for (int i = 0; i < n; i++) q[(size_t)i * n + i] = 1.0;
+    for (int sweep = 0; sweep < 60; sweep++) {
+        double offd = 0.0;
+        for (int i = 0; i < n; i++) for (int j = i + 1; j < n; j++) offd += a[(size_t)i * n + j] * a[(size_t)i * n + j];
+        if (offd < 1e-300) break;
+        for (int p = 0; p < n; p++)
+            for (int r = p + 1; r < n; r++) {
+                const double apr = a[(size_t)p * n + r];
+                if (fabs(apr) < 1e-300) continue;
+                const double theta = (a[(size_t)r * n + r] - a[(size_t)p * n + p]) / (2.0 * apr);
+                const double tt = (theta >= 0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
+                const double cs = 1.0 / sqrt(tt * tt + 1.0), sn = tt * cs;
+                for (int k = 0; k < n; k++) {
+                    const double akp = a[(size_t)k * n + p], akr = a[(size_t)k * n + r];
+                    a[(size_t)k * n + p] = cs * akp - sn * akr; a[(size_t)k * n + r] = sn * akp + cs * akr;
+                }
+                for (int k = 0; k < n; k++) {
+                    const double apk = a[(size_t)p * n + k], ark = a[(size_t)r * n + k];
+                    a[(size_t)p * n + k] = cs * apk - sn * ark; a[(size_t)r * n + k] = sn * apk + cs * ark;
+                }
+                for (int k = 0; k < n; k++) {
+                    const double qkp = q[(size_t)k * n + p], qkr = q[(size_t)k * n + r];
+                    q[(size_t)k * n + p] = cs * qkp - sn * qkr; q[(size_t)k * n + r] = sn * qkp + cs * qkr;
+                }
+            }
+    }
+    d.resize(n);
+    for (int i = 0; i < n; i++) d[i] = a[(size_t)i * n + i];
+}
+
+}  // namespace
+
+int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const lq_eig_param* p, lq_eig_info* info) {
+    const int Lt = c->g.L[3], n_ev = p->n_ev, m = p->m;
+    constexpr int MMAX = 64;
+    if (n_ev < 1 || m < n_ev + 2 || m > MMAX || p->cheb_degree < 1 || !(p->cheb_b > p->cheb_a) || !(p->tol > 0) || p->max_restarts < 1)
+        return set_err(c, LQ_EINVAL, "lq_laph_eigensolve: bad parameters (need n_ev + 2 <= m <= 64, degree >= 1, cheb_a < cheb_b)");
+    const int S3h = c->g.Lxh * c->g.L[1] * c->g.L[2];
+    if (n_ev > 6 * S3h - 1) return set_err(c, LQ_EINVAL, "lq_laph_eigensolve: more eigenpairs than the slice dimension");
+    Eig e; e.c = c; e.Lt = Lt;
+    e.sg.Vh = c->g.Vh; e.sg.S3h = S3h; e.sg.Lt = Lt; e.sg.dS3h = make_fastdiv(S3h);
+    e.fbytes = cv_native_bytes(c, 1, LQ_FP64); e.sg.pbe = e.fbytes / 2 / sizeof(double);
+    e.nchunk = std::max(1, std::min(64, (2 * S3h + 2047) / 2048));
+    const int keep = std::min(m - 2, n_ev + std::max(2, n_ev / 4));      // Ritz vectors kept at a restart
+
+    std::vector<void*> allocs;
+    auto alloc = [&](size_t bytes) { void* q = dev_alloc(c, bytes); if (q) allocs.push_back(q); return q; };
+    auto cleanup = [&]() { for (void* q : allocs) dev_free(c, q); };
+    std::vector<double*> V(m + 1), W(m);
+    bool ok = true;
+    for (int i = 0; i <= m; i++) { V[i] = (double*)alloc(e.fbytes); ok = ok && V[i]; }
+    for (int i = 0; i < keep; i++) { W[i] = (double*)alloc(e.fbytes); ok = ok && W[i]; }
+    double* w = (double*)alloc(e.fbytes); double* y0 = (double*)alloc(e.fbytes); double* y1 = (double*)alloc(e.fbytes); double* tmp = (double*)alloc(e.fbytes);
+    e.d_partial = (double2*)alloc(sizeof(double2) * Lt * e.nchunk);
+    e.d_H = (double2*)alloc(sizeof(double2) * (size_t)(2 * m + 4) * Lt);
+    e.d_scale = (double*)alloc(sizeof(double) * 2 * Lt);
+    double* d_Q = (double*)alloc(sizeof(double) * (size_t)Lt * m * m);
+    double** d_ptr = (double**)alloc(sizeof(double*) * (size_t)(2 * m + 2));
+    ok = ok && w && y0 && y1 && tmp && e.d_partial && e.d_H && e.d_scale && d_Q && d_ptr;
+    if (!ok) { cleanup(); return LQ_ENOMEM; }
+    const int grid = grid_sites(e);
+    cudaEvent_t ev0, ev1;
+    cudaEventCreate(&ev0); cudaEventCreate(&ev1);
+    cudaEventRecord(ev0, c->stream);
+
+    int rc = 0;
+#define EIG_TRY(x) do { rc = (x); if (rc) goto done; } while (0)
+#define EIG_CUDA(x) do { if ((x) != cudaSuccess) { rc = set_err(c, LQ_ECUDA, #x); goto done; } } while (0)
+    {
+    std::vector<double> T((size_t)Lt * m * m, 0.0), beta_m(Lt, 0.0), hbuf;
+    std::vector<double2> hH((size_t)(2 * m + 4) * Lt);
+    std::vector<double> hQ((size_t)Lt * m * m), theta((size_t)Lt * m);
+    int k = 0, restarts = 0; bool converged = false; double worst = 0.0;
+    // v_0: pseudo-random, normalised on every slice; zero the padding first
+    EIG_CUDA(cudaMemsetAsync(V[0], 0, e.fbytes, c->stream));
+    for (int i = 1; i <= m; i++) EIG_CUDA(cudaMemsetAsync(V[i], 0, e.fbytes, c->stream));
+    EIG_CUDA(cudaMemsetAsync(w, 0, e.fbytes, c->stream)); EIG_CUDA(cudaMemsetAsync(y0, 0, e.fbytes, c->stream));
+    EIG_CUDA(cudaMemsetAsync(y1, 0, e.fbytes, c->stream)); EIG_CUDA(cudaMemsetAsync(tmp, 0, e.fbytes, c->stream));
+    for (int i = 0; i < keep; i++) EIG_CUDA(cudaMemsetAsync(W[i], 0, e.fbytes, c->stream));
+    EIG_TRY(cv_fill(c, tmp, 1, LQ_FP64, 0x5EEDull + p->seed));
+    {   // copy only real sites (padding stays zero): scale by 1 through the slice kernel
+        std::vector<double> ones(Lt, 1.0);
+        EIG_CUDA(cudaMemcpyAsync(e.d_scale, ones.data(), sizeof(double) * Lt, cudaMemcpyHostToDevice, c->stream));
+        slice_scale_kernel<<<grid, 128, 0, c->stream>>>(e.sg, V[0], tmp, e.d_scale); c->launches++;
+        EIG_CUDA(cudaStreamSynchronize(c->stream));
+    }
+    EIG_TRY(dot(e, V[0], V[0], e.d_H));
+    inv_norm_kernel<<<(Lt + 63) / 64, 64, 0, c->stream>>>(Lt, e.d_H, e.d_scale, e.d_scale + Lt);
+    slice_scale_kernel<<<grid, 128, 0, c->stream>>>(e.sg, V[0], V[0], e.d_scale); c->launches += 2;
+
+    for (restarts = 0; restarts < p->max_restarts; restarts++) {
+        for (int j = k; j < m; j++) {
+            EIG_TRY(chebyshev(e, w, V[j], p->cheb_degree, p->cheb_a, p->cheb_b, y0, y1, tmp));
+            // two classical Gram-Schmidt passes against v_0 .. v_j; the coefficients are the column j of T
+            for (int pass = 0; pass < 2; pass++) {
+                double2* H = e.d_H + (size_t)pass * (m + 1) * Lt;
+                for (int i = 0; i <= j; i++) EIG_TRY(dot(e, V[i], w, H + (size_t)i * Lt));
+                EIG_CUDA(cudaMemcpyAsync(hH.data() + (size_t)pass * (m + 1) * Lt, H, sizeof(double2) * (size_t)(j + 1) * Lt, cudaMemcpyDeviceToHost, c->stream));
+                negate_kernel<<<((j + 1) * Lt + 127) / 128, 128, 0, c->stream>>>((j + 1) * Lt, H); c->launches++;
+                for (int i = 0; i <= j; i++) { slice_axpy_kernel<<<grid, 128, 0, c->stream>>>(e.sg, w, V[i], H + (size_t)i * Lt); c->launches++; }
+            }
+            EIG_TRY(dot(e, w, w, e.d_H + (size_t)(2 * m + 2) * Lt));
+            inv_norm_kernel<<<(Lt + 63) / 64, 64, 0, c->stream>>>(Lt, e.d_H + (size_t)(2 * m + 2) * Lt, e.d_scale, e.d_scale + Lt);
+            slice_scale_kernel<<<grid, 128, 0, c->stream>>>(e.sg, V[j + 1], w, e.d_scale); c->launches += 2;
+            hbuf.resize(Lt);
+            EIG_CUDA(cudaMemcpyAsync(hbuf.data(), e.d_scale + Lt, sizeof(double) * Lt, cudaMemcpyDeviceToHost, c->stream));
+            EIG_CUDA(cudaStreamSynchronize(c->stream));
+            for (int t = 0; t < Lt; t++) {
+                double* Tt = T.data() + (size_t)t * m * m;
+                for (int i = 0; i <= j; i++) {
+                    const double h = hH[(size_t)i * Lt + t].x + hH[(size_t)(m + 1 + i) * Lt + t].x;
+                    if (i >= k || j == k || i == j) { Tt[(size_t)i * m + j] = h; Tt[(size_t)j * m + i] = h; }
+                }
+                if (j + 1 < m) { Tt[(size_t)(j + 1) * m + j] = hbuf[t]; Tt[(size_t)j * m + j + 1] = hbuf[t]; }
+                else beta_m[t] = hbuf[t];
+            }
+        }
+        // Ritz pairs of every slice
+        worst = 0.0; converged = true;
+        for (int t = 0; t < Lt; t++) {
+            std::vector<double> a(T.begin() + (size_t)t * m * m, T.begin() + (size_t)(t + 1) * m * m), d, q;
+            jacobi(m, a, d, q);
+            std::vector<int> ord(m);
+            for (int i = 0; i < m; i++) ord[i] = i;
+            std::sort(ord.begin(), ord.end(), [&](int x, int y) { return fabs(d[x]) > fabs(d[y]); });   // T_d(x < -1) is negative for odd d
+            for (int cidx = 0; cidx < m; cidx++) theta[(size_t)t * m + cidx] = d[ord[cidx]];
+            for (int cidx = 0; cidx < keep; cidx++)
+                for (int i = 0; i < m; i++) hQ[((size_t)t * m + i) * keep + cidx] = q[(size_t)i * m + ord[cidx]];
+            for (int cidx = 0; cidx < n_ev; cidx++) {
+                const double res = fabs(beta_m[t] * q[(size_t)(m - 1) * m + ord[cidx]]);
+                const double rel = res / fmax(fabs(d[ord[0]]), 1e-300);
+                worst = fmax(worst, rel);
+                if (!(rel <= p->tol)) converged = false;
+            }
+        }
+        // thick restart: V[0..keep) <- V Q[:, 0..keep), V[keep] <- v_m, T <- diag(theta) (the arrow is rebuilt by the sweep)
+        EIG_CUDA(cudaMemcpyAsync(d_Q, hQ.data(), sizeof(double) * (size_t)Lt * m * keep, cudaMemcpyHostToDevice, c->stream));
+        {
+            std::vector<double*> ptrs(2 * m + 2);
+            for (int i = 0; i < m; i++) ptrs[i] = V[i];
+            for (int i = 0; i < keep; i++) ptrs[m + i] = W[i];
+            EIG_CUDA(cudaMemcpyAsync(d_ptr, ptrs.data(), sizeof(double*) * (size_t)(2 * m + 2), cudaMemcpyHostToDevice, c->stream));
+            slice_rotate_kernel<MMAX><<<grid, 128, 0, c->stream>>>(e.sg, m, keep, d_ptr, d_ptr + m, d_Q); c->launches++;
+            EIG_CUDA(cudaStreamSynchronize(c->stream));
+            for (int i = 0; i < keep; i++) std::swap(V[i], W[i]);
+            std::swap(V[keep], V[m]);
+        }
+        std::fill(T.begin(), T.end(), 0.0);
+        for (int t = 0; t < Lt; t++) for (int i = 0; i < keep; i++) T[(size_t)t * m * m + (size_t)i * m + i] = theta[(size_t)t * m + i];
+        k = keep;
+        if (converged) { restarts++; break; }
+    }
+    // eigenvalues of A = -Laplacian as Rayleigh quotients, true residuals, canonical eigenvectors
+    double maxres = 0.0;
+    for (int i = 0; i < n_ev; i++) {
+        EIG_TRY(laplacian_native(c, tmp, V[i], 1, LQ_FP64)); e.lap_applies++;
+        EIG_TRY(dot(e, V[i], tmp, e.d_H));
+        EIG_CUDA(cudaMemcpyAsync(hH.data(), e.d_H, sizeof(double2) * Lt, cudaMemcpyDeviceToHost, c->stream));
+        EIG_CUDA(cudaStreamSynchronize(c->stream));
+        std::vector<double2> lam(Lt);
+        for (int t = 0; t < Lt; t++) { h_evals[(size_t)t * n_ev + i] = -hH[t].x; lam[t] = make_double2(-hH[t].x, 0.0); }
+        // r = A v - lambda v = -(tmp) - lambda v  ->  tmp += lambda v ; ||tmp||
+        EIG_CUDA(cudaMemcpyAsync(e.d_H, lam.data(), sizeof(double2) * Lt, cudaMemcpyHostToDevice, c->stream));
+        slice_axpy_kernel<<<grid, 128, 0, c->stream>>>(e.sg, tmp, V[i], e.d_H); c->launches++;
+        EIG_TRY(dot(e, tmp, tmp, e.d_H + Lt));
+        EIG_CUDA(cudaMemcpyAsync(hH.data(), e.d_H + Lt, sizeof(double2) * Lt, cudaMemcpyDeviceToHost, c->stream));
+        EIG_CUDA(cudaStreamSynchronize(c->stream));
+        for (int t = 0; t < Lt; t++) maxres = fmax(maxres, sqrt(fmax(hH[t].x, 0.0)));
+        if (dev_canon_evecs) EIG_TRY(cv_unpack(c, dev_canon_evecs + (size_t)i * c->g.V * 6, V[i], 1, LQ_FP64));
+    }
+    cudaEventRecord(ev1, c->stream);
+    EIG_CUDA(cudaEventSynchronize(ev1));
+    float ms = 0; cudaEventElapsedTime(&ms, ev0, ev1);
+    info->restarts = restarts; info->converged = converged ? 1 : 0; info->lap_applies = (double)e.lap_applies;
+    info->max_ritz_residual = worst; info->max_true_residual = maxres; info->seconds = ms * 1e-3;
+    if (!converged) rc = LQ_ENOTCONVERGED;
+    }
+done:
+    cudaStreamSynchronize(c->stream);
+    cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+    cleanup();
+    return rc;
+#undef EIG_TRY
+#undef EIG_CUDA
+}

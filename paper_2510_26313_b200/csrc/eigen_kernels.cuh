@@ -1,0 +1,102 @@
+// eigen_kernels.cuh -- per-time-slice vector kernels of the batched Lanczos eigensolver (
+// "batched Lanczos", the time extent is the batch).  One colour-vector field = native cv layout
+// with N = 1 (common layout of laplace.cu): element (parity, cb, j) at parity*pbe + ((cb/32)*6 + j)*32 + cb%32, fp64.
+// Every kernel takes per-slice coefficients: the Lt time-slices are independent eigenproblems advancing in lockstep.
+#pragma once
+#include "common.cuh"
+
+struct SliceGeom { int Vh, S3h, Lt; size_t pbe; FastDiv dS3h; };   // S3h = sites of one time-slice per parity
+
+// thread i < 2*Vh -> (parity, cb); returns the element offset of real 0 and the slice
+__device__ __forceinline__ bool slice_site(const SliceGeom& g, long long i, size_t& off, int& t) {
+    if (i >= 2LL * g.Vh) return false;
+    const int parity = i >= g.Vh ? 1 : 0;
+    const int cb = (int)(i - (long long)parity * g.Vh);
+    t = g.dS3h.div(cb);
+    off = (size_t)parity * g.pbe + (size_t)(cb / SB) * (6 * SB) + (cb % SB);
+    return true;
+}
+
+// partial[t][chunk] = sum over the sites of the chunk of conj(a) b  (complex); chunks never straddle slices:
+// grid = Lt * nchunk blocks of 256 threads, each thread strides over the slice's 2*S3h sites.
+__global__ void slice_dot_kernel(SliceGeom g, int nchunk, const double* __restrict__ a, const double* __restrict__ b, double2* __restrict__ partial) {
+    const int t = blockIdx.x / nchunk, ch = blockIdx.x - t * nchunk;
+    double sr = 0.0, si = 0.0;
+    const int per_slice = 2 * g.S3h;
+    for (int i = ch * blockDim.x + threadIdx.x; i < per_slice; i += nchunk * blockDim.x) {
+        const int parity = i >= g.S3h ? 1 : 0;
+        const int cb = t * g.S3h + (i - parity * g.S3h);
+        const size_t off = (size_t)parity * g.pbe + (size_t)(cb / SB) * (6 * SB) + (cb % SB);
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const double ar = a[off + (2 * c) * SB], ai = a[off + (2 * c + 1) * SB];
+            const double br = b[off + (2 * c) * SB], bi = b[off + (2 * c + 1) * SB];
+            sr += ar * br + ai * bi; si += ar * bi - ai * br;
+        }
+    }
+    __shared__ double shr[256], shi[256];
+    shr[threadIdx.x] = sr; shi[threadIdx.x] = si;
+    __syncthreads();
+    for (int s = blockDim.x >> 1; s > 0; s >>= 1) {
+        if (threadIdx.x < s) { shr[threadIdx.x] += shr[threadIdx.x + s]; shi[threadIdx.x] += shi[threadIdx.x + s]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = make_double2(shr[0], shi[0]);
+}
+// out[t] = sum over chunks in fixed order
+__global__ void slice_dot_final_kernel(int Lt, int nchunk, const double2* __restrict__ partial, double2* __restrict__ out) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= Lt) return;
+    double sr = 0.0, si = 0.0;
+    for (int c = 0; c < nchunk; c++) { sr += partial[t * nchunk + c].x; si += partial[t * nchunk + c].y; }
+    out[t] = make_double2(sr, si);
+}
+
+// y += coef[t] * x   (complex coefficient per slice)
+__global__ void slice_axpy_kernel(SliceGeom g, double* __restrict__ y, const double* __restrict__ x, const double2* __restrict__ coef) {
+    size_t off; int t;
+    if (!slice_site(g, (long long)blockIdx.x * blockDim.x + threadIdx.x, off, t)) return;
+    const double cr = coef[t].x, ci = coef[t].y;
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const double xr = x[off + (2 * c) * SB], xi = x[off + (2 * c + 1) * SB];
+        y[off + (2 * c) * SB] += cr * xr - ci * xi;
+        y[off + (2 * c + 1) * SB] += cr * xi + ci * xr;
+    }
+}
+// y = s[t] * x   (real scale per slice; y may alias x)
+__global__ void slice_scale_kernel(SliceGeom g, double* __restrict__ y, const double* __restrict__ x, const double* __restrict__ s) {
+    size_t off; int t;
+    if (!slice_site(g, (long long)blockIdx.x * blockDim.x + threadIdx.x, off, t)) return;
+    const double f = s[t];
+#pragma unroll
+    for (int j = 0; j < 6; j++) y[off + j * SB] = f * x[off + j * SB];
+}
+// z = alpha x + beta y + gamma z   (global real scalars: the Chebyshev three-term recurrence)
+__global__ void cv_axpbypcz_kernel(SliceGeom g, double* __restrict__ z, double alpha, const double* __restrict__ x, double beta, const double* __restrict__ y, double gamma) {
+    size_t off; int t;
+    if (!slice_site(g, (long long)blockIdx.x * blockDim.x + threadIdx.x, off, t)) return;
+#pragma unroll
+    for (int j = 0; j < 6; j++) {
+        const size_t e = off + j * SB;
+        z[e] = alpha * x[e] + beta * y[e] + (gamma != 0.0 ? gamma * z[e] : 0.0);
+    }
+}
+// basis rotation: out[c] = sum_i Q[t][i][c] * V[i]  for c < k (real Q from the projected eigenproblem of slice t)
+template <int MMAX>
+__global__ void slice_rotate_kernel(SliceGeom g, int m, int k, const double* const* __restrict__ V, double* const* __restrict__ out, const double* __restrict__ Q) {
+    size_t off; int t;
+    if (!slice_site(g, (long long)blockIdx.x * blockDim.x + threadIdx.x, off, t)) return;
+    const double* q = Q + (size_t)t * m * k;
+    for (int j = 0; j < 6; j++) {
+        double in[MMAX];
+#pragma unroll
+        for (int i = 0; i < MMAX; i++) in[i] = i < m ? V[i][off + j * SB] : 0.0;
+        for (int c = 0; c < k; c++) {
+            double acc = 0.0;
+#pragma unroll
+            for (int i = 0; i < MMAX; i++) if (i < m) acc += q[i * k + c] * in[i];
+            out[c][off + j * SB] = acc;
+        }
+    }
+}

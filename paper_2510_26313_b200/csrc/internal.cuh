@@ -58,3 +58,6 @@ size_t cv_native_bytes(const lq_ctx* c, int nvec, int prec);
 int cv_pack(lq_ctx* c, void* native, const double* dev_canon, int nvec, int prec);
 int cv_unpack(lq_ctx* c, double* dev_canon, const void* native, int nvec, int prec);
 int cv_fill(lq_ctx* c, void* native, int nvec, int prec, unsigned long long seed);
+
+// eigen.cu : time-batched thick-restart Lanczos on the Chebyshev-filtered -Laplacian
+int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const lq_eig_param* p, lq_eig_info* info);

@@ -254,6 +254,20 @@ def cpu_dslash_baseline():
             "note": "kernel A by the site-local evaluator rebuilds F_mu_nu, A and A^-1 at every site (that is its definition), so it is not comparable with a stored-clover kernel"}
 
 
+def time_eigensolve(B, device):
+    """Time-batched Lanczos (SURVEY 8(f) #2) on the configs[1] lattice: lowest 16 eigenpairs of -Laplacian on each of the 32 slices."""
+    c = inputs.CONFIGS[1]
+    ctx = B.Context(c["dims"], device=device)
+    ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=18)
+    kw = dict(n_ev=16, m=48, cheb_degree=24, cheb_a=0.5, cheb_b=12.5, tol=1e-9, max_restarts=50, want_vectors=False)
+    ctx.laph_eigensolve(**kw)
+    ev, _, info = ctx.laph_eigensolve(**kw)
+    ctx.close()
+    return {"lattice": "x".join(map(str, c["dims"])), "n_ev": 16, "krylov": 48, "cheb_degree": 24, "seconds": round(info["seconds"], 4),
+            "restarts": info["restarts"], "laplacian_applies": info["lap_applies"], "converged": info["converged"],
+            "max_true_residual": info["max_true_residual"], "eigenvalue_range": [float(ev.min()), float(ev.max())]}
+
+
 def operator_sweeps(B, device, peak):
     """configs[2]: 32^3x64 fp32 sweep over N_rhs (kernel A, kernel B, bare hop); configs[4]: 64^3x128, N=4, 12-real links."""
     import torch
@@ -500,6 +514,7 @@ def main():
     if not args.no_extras and world == 1:
         extras["dslash"] = operator_sweeps(B, local, peak)
         extras["dslash"]["cpu_baseline"] = cpu_dslash_baseline()
+        extras["laph_eigensolve"] = time_eigensolve(B, local)
         extras["cpu_baseline"] = cpu_baseline(wl["cfg"])
     total_rhs = nrhs * world
     line = {

@@ -123,7 +123,8 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
     e.d_scale = (double*)alloc(sizeof(double) * 2 * Lt);
     double* d_Q = (double*)alloc(sizeof(double) * (size_t)Lt * m * m);
     double** d_ptr = (double**)alloc(sizeof(double*) * (size_t)(2 * m + 2));
-    ok = ok && w && y0 && y1 && tmp && e.d_partial && e.d_H && e.d_scale && d_Q && d_ptr;
+    double2* d_mpart = (double2*)alloc(sizeof(double2) * (size_t)Lt * e.nchunk * (m + 1));
+    ok = ok && w && y0 && y1 && tmp && e.d_partial && e.d_H && e.d_scale && d_Q && d_ptr && d_mpart;
     if (!ok) { cleanup(); return LQ_ENOMEM; }
     const int grid = grid_sites(e);
     cudaEvent_t ev0, ev1;
@@ -156,15 +157,22 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
     slice_scale_kernel<<<grid, 128, 0, c->stream>>>(e.sg, V[0], V[0], e.d_scale); c->launches += 2;
 
     for (restarts = 0; restarts < p->max_restarts; restarts++) {
+        {   // device table of the basis vectors (changes at every restart)
+            std::vector<double*> ptrs(V.begin(), V.end());
+            EIG_CUDA(cudaMemcpyAsync(d_ptr, ptrs.data(), sizeof(double*) * (size_t)(m + 1), cudaMemcpyHostToDevice, c->stream));
+            EIG_CUDA(cudaStreamSynchronize(c->stream));
+        }
         for (int j = k; j < m; j++) {
             EIG_TRY(chebyshev(e, w, V[j], p->cheb_degree, p->cheb_a, p->cheb_b, y0, y1, tmp));
             // two classical Gram-Schmidt passes against v_0 .. v_j; the coefficients are the column j of T
             for (int pass = 0; pass < 2; pass++) {
                 double2* H = e.d_H + (size_t)pass * (m + 1) * Lt;
-                for (int i = 0; i <= j; i++) EIG_TRY(dot(e, V[i], w, H + (size_t)i * Lt));
-                EIG_CUDA(cudaMemcpyAsync(hH.data() + (size_t)pass * (m + 1) * Lt, H, sizeof(double2) * (size_t)(j + 1) * Lt, cudaMemcpyDeviceToHost, c->stream));
-                negate_kernel<<<((j + 1) * Lt + 127) / 128, 128, 0, c->stream>>>((j + 1) * Lt, H); c->launches++;
-                for (int i = 0; i <= j; i++) { slice_axpy_kernel<<<grid, 128, 0, c->stream>>>(e.sg, w, V[i], H + (size_t)i * Lt); c->launches++; }
+                const int nv = j + 1;
+                slice_multidot_kernel<<<dim3(Lt * e.nchunk, (nv + 7) / 8), 256, 0, c->stream>>>(e.sg, e.nchunk, nv, d_ptr, w, d_mpart);
+                slice_multidot_final_kernel<<<(Lt * nv + 127) / 128, 128, 0, c->stream>>>(Lt, e.nchunk, nv, d_mpart, H);
+                EIG_CUDA(cudaMemcpyAsync(hH.data() + (size_t)pass * (m + 1) * Lt, H, sizeof(double2) * (size_t)nv * Lt, cudaMemcpyDeviceToHost, c->stream));
+                slice_multiaxpy_kernel<<<grid, 128, 0, c->stream>>>(e.sg, nv, w, d_ptr, H);
+                c->launches += 3;
             }
             EIG_TRY(dot(e, w, w, e.d_H + (size_t)(2 * m + 2) * Lt));
             inv_norm_kernel<<<(Lt + 63) / 64, 64, 0, c->stream>>>(Lt, e.d_H + (size_t)(2 * m + 2) * Lt, e.d_scale, e.d_scale + Lt);

@@ -100,3 +100,78 @@ __global__ void slice_rotate_kernel(SliceGeom g, int m, int k, const double* con
         }
     }
 }
+
+// Gram-Schmidt as two batched kernels (the tall-skinny GEMV pair of the Lanczos step):
+// multidot:  partial[t][chunk][i] = sum over the chunk of conj(V[i0+i]) w  for up to 8 vectors per block (blockIdx.y = tile)
+__global__ void slice_multidot_kernel(SliceGeom g, int nchunk, int nv, const double* const* __restrict__ V, const double* __restrict__ w,
+                                      double2* __restrict__ partial /*[Lt*nchunk][nv]*/) {
+    constexpr int TV = 8;
+    const int t = blockIdx.x / nchunk, ch = blockIdx.x - t * nchunk, i0 = blockIdx.y * TV;
+    const int nt = min(TV, nv - i0);
+    double sr[TV], si[TV];
+#pragma unroll
+    for (int i = 0; i < TV; i++) { sr[i] = 0.0; si[i] = 0.0; }
+    const int per_slice = 2 * g.S3h;
+    for (int s = ch * blockDim.x + threadIdx.x; s < per_slice; s += nchunk * blockDim.x) {
+        const int parity = s >= g.S3h ? 1 : 0;
+        const int cb = t * g.S3h + (s - parity * g.S3h);
+        const size_t off = (size_t)parity * g.pbe + (size_t)(cb / SB) * (6 * SB) + (cb % SB);
+        double wv[6];
+#pragma unroll
+        for (int j = 0; j < 6; j++) wv[j] = w[off + j * SB];
+#pragma unroll
+        for (int i = 0; i < TV; i++) {
+            if (i < nt) {
+                const double* v = V[i0 + i];
+#pragma unroll
+                for (int c = 0; c < 3; c++) {
+                    const double ar = v[off + (2 * c) * SB], ai = v[off + (2 * c + 1) * SB];
+                    sr[i] += ar * wv[2 * c] + ai * wv[2 * c + 1]; si[i] += ar * wv[2 * c + 1] - ai * wv[2 * c];
+                }
+            }
+        }
+    }
+    __shared__ double sh[8][2 * TV];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int i = 0; i < TV; i++) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) { sr[i] += __shfl_xor_sync(0xffffffffu, sr[i], o); si[i] += __shfl_xor_sync(0xffffffffu, si[i], o); }
+        if (lane == 0) { sh[wid][2 * i] = sr[i]; sh[wid][2 * i + 1] = si[i]; }
+    }
+    __syncthreads();
+    if (threadIdx.x < nt) {
+        double a = 0.0, b = 0.0;
+        for (int q = 0; q < (int)(blockDim.x >> 5); q++) { a += sh[q][2 * threadIdx.x]; b += sh[q][2 * threadIdx.x + 1]; }
+        partial[(size_t)blockIdx.x * nv + i0 + threadIdx.x] = make_double2(a, b);
+    }
+}
+// out[i][t] = sum over chunks (fixed order)
+__global__ void slice_multidot_final_kernel(int Lt, int nchunk, int nv, const double2* __restrict__ partial, double2* __restrict__ out) {
+    const int id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= Lt * nv) return;
+    const int i = id / Lt, t = id - i * Lt;
+    double sr = 0.0, si = 0.0;
+    for (int c = 0; c < nchunk; c++) { const double2 p = partial[(size_t)(t * nchunk + c) * nv + i]; sr += p.x; si += p.y; }
+    out[(size_t)i * Lt + t] = make_double2(sr, si);
+}
+// w -= sum_i H[i][t] V[i]
+__global__ void slice_multiaxpy_kernel(SliceGeom g, int nv, double* __restrict__ w, const double* const* __restrict__ V, const double2* __restrict__ H) {
+    size_t off; int t;
+    if (!slice_site(g, (long long)blockIdx.x * blockDim.x + threadIdx.x, off, t)) return;
+    double acc[6];
+#pragma unroll
+    for (int j = 0; j < 6; j++) acc[j] = w[off + j * SB];
+    for (int i = 0; i < nv; i++) {
+        const double cr = H[(size_t)i * g.Lt + t].x, ci = H[(size_t)i * g.Lt + t].y;
+        const double* v = V[i];
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const double xr = v[off + (2 * c) * SB], xi = v[off + (2 * c + 1) * SB];
+            acc[2 * c] -= cr * xr - ci * xi;
+            acc[2 * c + 1] -= cr * xi + ci * xr;
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 6; j++) w[off + j * SB] = acc[j];
+}

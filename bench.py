@@ -406,6 +406,13 @@ def run_op(args, B, device):
     if variant or rpt or pfd >= 0:
         ctx.set_tuning(variant, rpt, pfd)
     sampler = ClockSampler(device)
+    if kind == "lap":      # batched 3-d covariant Laplacian
+        r = time_laplacian(ctx, B, n, prec, iters=args.op_iters, warmup=max(args.warmup, 3))
+        clocks = sampler.stop()
+        ctx.close()
+        r.update({"op": args.op, "lattice": "x".join(map(str, c["dims"])), "frac_measured_hbm": round(r["gbs"] / peak, 4), "clocks": clocks})
+        print(json.dumps(r))
+        return
     r = time_dslash(ctx, B, kind, prec, n, c["recon"], iters=args.op_iters, warmup=max(args.warmup, 3))
     clocks = sampler.stop()
     ctx.close()
@@ -427,7 +434,7 @@ def main():
     ap.add_argument("--check-every", type=int, default=4, help="inner iterations between convergence polls")
     ap.add_argument("--delta", type=float, default=0.0, help="inner CG reduction per cycle (0 = the workload default)")
     ap.add_argument("--op", default=None, metavar="CFG:KIND:PREC:N",
-                    help="time ONE stencil kernel only, e.g. cfg2:A:fp32:8 (lattice and links of configs[CFG]; KIND A|B|hop; "
+                    help="time ONE stencil kernel only, e.g. cfg2:A:fp32:8 (lattice and links of configs[CFG]; KIND A|B|hop|lap; "
                          "PREC fp64|fp32|half); optional :variant:rpt:pfd tuning suffix.  Prints its own JSON line (used for ncu captures)")
     ap.add_argument("--op-iters", type=int, default=20)
     args = ap.parse_args()

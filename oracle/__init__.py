@@ -236,3 +236,10 @@ def laph_eigen(dims, U, n_ev: int):
         evals[t] = w[:n_ev]
         evecs[t] = v[:, :n_ev].T.reshape(n_ev, Lz, Ly, Lx, 3)
     return evals, evecs
+
+
+def project(v, psi) -> np.ndarray:
+    """Eigenvector projection: P[t][alpha][j][k] = sum_{x,c} conj(v_j(x,t,c)) psi_k(x,t,alpha,c),
+    v[j][t][z][y][x][3], psi[k][t][z][y][x][4][3]; the plain definition as one einsum."""
+    v = np.asarray(v, dtype=np.complex128); psi = np.asarray(psi, dtype=np.complex128)
+    return np.einsum("jtzyxc,ktzyxac->tajk", v.conj(), psi)

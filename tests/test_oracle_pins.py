@@ -506,3 +506,39 @@ def test_laph_eigen_free_field_and_gauge_invariance(oracle_lib):
     v[:, 1] = vec[1]                                   # the slice-1 eigenvectors, zero elsewhere
     Lv = oracle.laplacian(dims, U, v)
     assert np.abs(-Lv[:, 1] - ev[1][:, None, None, None, None] * v[:, 1]).max() < 1e-12
+
+
+def test_projection_definition_and_invariants(oracle_lib):
+    """P[t][a][j][k] = <v_j(t), psi_k(t, a)>: explicit loops on a tiny case, recovery of expansion coefficients in an
+    orthonormal basis, gauge invariance."""
+    import oracle
+    dims = (2, 2, 2, 3)
+    Lx, Ly, Lz, Lt = dims
+    rng = np.random.default_rng(8)
+    v = rng.normal(size=(3, Lt, Lz, Ly, Lx, 3)) + 1j * rng.normal(size=(3, Lt, Lz, Ly, Lx, 3))
+    psi = rng.normal(size=(2, Lt, Lz, Ly, Lx, 4, 3)) + 1j * rng.normal(size=(2, Lt, Lz, Ly, Lx, 4, 3))
+    P = oracle.project(v, psi)
+    for t in range(Lt):
+        for a in range(4):
+            for j in range(3):
+                for k in range(2):
+                    s = 0
+                    for z in range(Lz):
+                        for y in range(Ly):
+                            for x in range(Lx):
+                                for c in range(3):
+                                    s += np.conj(v[j, t, z, y, x, c]) * psi[k, t, z, y, x, a, c]
+                    assert abs(P[t, a, j, k] - s) < 1e-12
+    # orthonormal basis per slice (QR) and a field inside its span: the projection returns the coefficients
+    q = np.empty_like(v)
+    for t in range(Lt):
+        Q, _ = np.linalg.qr(v[:, t].reshape(3, -1).T)
+        q[:, t] = Q.T.reshape(3, Lz, Ly, Lx, 3)
+    coef = rng.normal(size=(Lt, 4, 3, 2)) + 1j * rng.normal(size=(Lt, 4, 3, 2))
+    field = np.einsum("tajk,jtzyxc->ktzyxac", coef, q)
+    assert np.abs(oracle.project(q, field) - coef).max() < 1e-12
+    # gauge invariance
+    g = inputs.random_gauge_transform(dims, 9)
+    gv = np.einsum("tzyxab,jtzyxb->jtzyxa", g, v)
+    gpsi = np.einsum("tzyxab,ktzyxsb->ktzyxsa", g, psi)
+    assert np.abs(oracle.project(gv, gpsi) - P).max() < 1e-11

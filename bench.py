@@ -268,6 +268,33 @@ def time_eigensolve(B, device):
             "max_true_residual": info["max_true_residual"], "eigenvalue_range": [float(ev.min()), float(ev.max())]}
 
 
+def time_projection(B, device, peak):
+    """Eigenvector projection (SURVEY 8(f) #1) on the configs[1] lattice: 32 eigenvector fields x 8 solutions, device arrays."""
+    import torch
+    c = inputs.CONFIGS[1]
+    Lx, Ly, Lz, Lt = c["dims"]
+    ctx = B.Context(c["dims"], device=device)
+    n_ev, n_sol = 32, 8
+    g = torch.Generator(device="cuda").manual_seed(7)
+    v = torch.randn((n_ev, Lt, Lz, Ly, Lx, 3, 2), generator=g, device="cuda", dtype=torch.float64)
+    x = torch.randn((n_sol, Lt, Lz, Ly, Lx, 4, 3, 2), generator=g, device="cuda", dtype=torch.float64)
+    vc, xc = torch.view_as_complex(v), torch.view_as_complex(x)
+    for _ in range(3):
+        ctx.project(vc, xc)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(10):
+        ctx.project(vc, xc)
+    torch.cuda.synchronize()
+    sec = (time.perf_counter() - t0) / 10
+    ctx.close()
+    nbytes = v.numel() * 8 + x.numel() * 8
+    flops = 8.0 * n_ev * 4 * n_sol * 3 * Lx * Ly * Lz * Lt
+    return {"lattice": "x".join(map(str, c["dims"])), "n_ev": n_ev, "n_sol": n_sol, "dtype": "f64 (no tensor cores yet)", "us": round(sec * 1e6, 1),
+            "compulsory_gbs": round(nbytes / sec * 1e-9, 1), "frac_measured_hbm": round(nbytes / sec * 1e-9 / peak, 4), "gflops": round(flops / sec * 1e-9, 1),
+            "note": "wall clock around the synchronous C-ABI call (device arrays), inputs 151 MB: L2-resident between calls"}
+
+
 def operator_sweeps(B, device, peak):
     """configs[2]: 32^3x64 fp32 sweep over N_rhs (kernel A, kernel B, bare hop); configs[4]: 64^3x128, N=4, 12-real links."""
     import torch
@@ -522,6 +549,7 @@ def main():
         extras["dslash"] = operator_sweeps(B, local, peak)
         extras["dslash"]["cpu_baseline"] = cpu_dslash_baseline()
         extras["laph_eigensolve"] = time_eigensolve(B, local)
+        extras["projection"] = time_projection(B, local, peak)
         extras["cpu_baseline"] = cpu_baseline(wl["cfg"])
     total_rhs = nrhs * world
     line = {

@@ -26,7 +26,7 @@ PREC = {"fp64": LQ_FP64, "fp32": LQ_FP32, "half": LQ_HALF}
 EXPORTS = ["lq_create", "lq_destroy", "lq_last_error", "lq_set_allocator", "lq_load_gauge", "lq_fill_gauge_random",
            "lq_build_clover", "lq_apply", "lq_native_bytes", "lq_pack", "lq_unpack", "lq_fill_spinor_random", "lq_solve",
            "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites",
-           "lq_laplacian", "lq_laplacian_native", "lq_cv_native_bytes", "lq_cv_fill_random", "lq_laph_eigensolve"]
+           "lq_laplacian", "lq_laplacian_native", "lq_cv_native_bytes", "lq_cv_fill_random", "lq_laph_eigensolve", "lq_project"]
 
 
 class SolveParam(ctypes.Structure):
@@ -92,6 +92,7 @@ def load_library():
     lib.lq_cv_native_bytes.argtypes = [vp, ci, ci]
     lib.lq_cv_native_bytes.restype = ctypes.c_size_t
     lib.lq_cv_fill_random.argtypes = [vp, vp, ci, ci, u64]
+    lib.lq_project.argtypes = [vp, vp, vp, ci, vp, ci, ci]
     lib.lq_laph_eigensolve.argtypes = [vp, vp, vp, ci, ctypes.POINTER(EigParam), ctypes.POINTER(EigInfo)]
     lib.lq_kernel_launches.argtypes = [vp]; lib.lq_kernel_launches.restype = ctypes.c_longlong
     _lib = lib
@@ -249,6 +250,21 @@ class Context:
         d = dict(converged=bool(info.converged), restarts=info.restarts, lap_applies=info.lap_applies, max_ritz_residual=info.max_ritz_residual,
                  max_true_residual=info.max_true_residual, seconds=info.seconds)
         return evals, evecs, d
+
+    def project(self, evecs, sols):
+        """P[t][alpha][j][k] = <v_j(t), psi_k(t, alpha)>; evecs [j][t][z][y][x][3], sols [k][t][z][y][x][4][3]: complex128 numpy (host) or
+        torch (device) arrays.  Returns the same kind of array, shape [Lt][4][n_ev][n_sol]."""
+        self._enter()
+        Lt = self.dims[3]
+        n_ev, n_sol = evecs.shape[0], sols.shape[0]
+        if isinstance(evecs, np.ndarray):
+            evecs = np.ascontiguousarray(evecs, dtype=np.complex128); sols = np.ascontiguousarray(sols, dtype=np.complex128)
+            out = np.empty((Lt, 4, n_ev, n_sol), dtype=np.complex128)
+        else:
+            out = self.torch.empty((Lt, 4, n_ev, n_sol), dtype=self.torch.complex128, device=evecs.device)
+        pv, loc = _ptr(evecs); px, _ = _ptr(sols); po, _ = _ptr(out)
+        self._check(self.lib.lq_project(self.h, po, pv, n_ev, px, n_sol, loc))
+        return out
 
     def cv_native_empty(self, nvec: int, prec: int):
         return self.torch.empty(int(self.lib.lq_cv_native_bytes(self.h, nvec, prec)), dtype=self.torch.uint8, device="cuda:%d" % self.device)

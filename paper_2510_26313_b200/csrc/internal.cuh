@@ -61,3 +61,6 @@ int cv_fill(lq_ctx* c, void* native, int nvec, int prec, unsigned long long seed
 
 // eigen.cu : time-batched thick-restart Lanczos on the Chebyshev-filtered -Laplacian
 int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const lq_eig_param* p, lq_eig_info* info);
+
+// project.cu : projection of solutions onto LapH eigenvectors
+int project_device(lq_ctx* c, double* dev_P, const double* dev_V, int n_ev, const double* dev_X, int n_sol);

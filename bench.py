@@ -279,20 +279,23 @@ def time_projection(B, device, peak):
     v = torch.randn((n_ev, Lt, Lz, Ly, Lx, 3, 2), generator=g, device="cuda", dtype=torch.float64)
     x = torch.randn((n_sol, Lt, Lz, Ly, Lx, 4, 3, 2), generator=g, device="cuda", dtype=torch.float64)
     vc, xc = torch.view_as_complex(v), torch.view_as_complex(x)
-    for _ in range(3):
-        ctx.project(vc, xc)
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    for _ in range(10):
-        ctx.project(vc, xc)
-    torch.cuda.synchronize()
-    sec = (time.perf_counter() - t0) / 10
-    ctx.close()
     nbytes = v.numel() * 8 + x.numel() * 8
     flops = 8.0 * n_ev * 4 * n_sol * 3 * Lx * Ly * Lz * Lt
-    return {"lattice": "x".join(map(str, c["dims"])), "n_ev": n_ev, "n_sol": n_sol, "dtype": "f64 (no tensor cores yet)", "us": round(sec * 1e6, 1),
-            "compulsory_gbs": round(nbytes / sec * 1e-9, 1), "frac_measured_hbm": round(nbytes / sec * 1e-9 / peak, 4), "gflops": round(flops / sec * 1e-9, 1),
-            "note": "wall clock around the synchronous C-ABI call (device arrays), inputs 151 MB: L2-resident between calls"}
+    out = {"lattice": "x".join(map(str, c["dims"])), "n_ev": n_ev, "n_sol": n_sol,
+           "note": "wall clock around the synchronous C-ABI call (device arrays), inputs 151 MB: L2-resident between calls"}
+    for name, prec in (("f64_fma", B.LQ_FP64), ("tcgen05_3xtf32", B.LQ_FP32)):
+        for _ in range(3):
+            ctx.project(vc, xc, prec)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(10):
+            ctx.project(vc, xc, prec)
+        torch.cuda.synchronize()
+        sec = (time.perf_counter() - t0) / 10
+        out[name] = {"us": round(sec * 1e6, 1), "compulsory_gbs": round(nbytes / sec * 1e-9, 1), "frac_measured_hbm": round(nbytes / sec * 1e-9 / peak, 4),
+                     "gflops": round(flops / sec * 1e-9, 1)}
+    ctx.close()
+    return out
 
 
 def operator_sweeps(B, device, peak):

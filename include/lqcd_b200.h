@@ -212,8 +212,10 @@ int lq_laph_eigensolve(lq_ctx* ctx, double* evals, void* evecs, int loc, const l
 /* ---- eigenvector projection ----------------------------------------
  * P[t][alpha][j][k] = sum_{x, c} conj(v_j(x, t, c)) psi_k(x, t, alpha, c)  for n_ev eigenvector fields v
  * (canonical [j][t][z][y][x][colour]) and n_sol solution fields psi (canonical [k][t][z][y][x][spin][colour]), all
- * complex double at `loc`; P: [Lt][4][n_ev][n_sol] complex double at `loc`.  1 <= n_ev <= 1024, 1 <= n_sol <= 64. */
-int lq_project(lq_ctx* ctx, void* P, const void* evecs, int n_ev, const void* sols, int n_sol, int loc);
+ * complex double at `loc`; P: [Lt][4][n_ev][n_sol] complex double at `loc`.  1 <= n_ev <= 1024, 1 <= n_sol <= 64.
+ * prec = LQ_FP64: fp64 FMAs (exact to rounding); prec = LQ_FP32: tcgen05 tensor cores, every operand split into two TF32
+ * numbers (3xTF32), fp32 accumulation over 256 sites, fp64 sum over the rest: relative error ~1e-6 of max |P|. */
+int lq_project(lq_ctx* ctx, void* P, const void* evecs, int n_ev, const void* sols, int n_sol, int loc, int prec);
 
 /* Launch-parameter knobs of the stencil kernels (the paper's autotuning, reduced to an
  * offline sweep): kernel variant (bits 0-7: 0 = default register budget, 1 = alternative; bits 8-15: z-chunk of the

@@ -92,7 +92,7 @@ def load_library():
     lib.lq_cv_native_bytes.argtypes = [vp, ci, ci]
     lib.lq_cv_native_bytes.restype = ctypes.c_size_t
     lib.lq_cv_fill_random.argtypes = [vp, vp, ci, ci, u64]
-    lib.lq_project.argtypes = [vp, vp, vp, ci, vp, ci, ci]
+    lib.lq_project.argtypes = [vp, vp, vp, ci, vp, ci, ci, ci]
     lib.lq_laph_eigensolve.argtypes = [vp, vp, vp, ci, ctypes.POINTER(EigParam), ctypes.POINTER(EigInfo)]
     lib.lq_kernel_launches.argtypes = [vp]; lib.lq_kernel_launches.restype = ctypes.c_longlong
     _lib = lib
@@ -251,7 +251,7 @@ class Context:
                  max_true_residual=info.max_true_residual, seconds=info.seconds)
         return evals, evecs, d
 
-    def project(self, evecs, sols):
+    def project(self, evecs, sols, prec: int = LQ_FP64):
         """P[t][alpha][j][k] = <v_j(t), psi_k(t, alpha)>; evecs [j][t][z][y][x][3], sols [k][t][z][y][x][4][3]: complex128 numpy (host) or
         torch (device) arrays.  Returns the same kind of array, shape [Lt][4][n_ev][n_sol]."""
         self._enter()
@@ -263,7 +263,7 @@ class Context:
         else:
             out = self.torch.empty((Lt, 4, n_ev, n_sol), dtype=self.torch.complex128, device=evecs.device)
         pv, loc = _ptr(evecs); px, _ = _ptr(sols); po, _ = _ptr(out)
-        self._check(self.lib.lq_project(self.h, po, pv, n_ev, px, n_sol, loc))
+        self._check(self.lib.lq_project(self.h, po, pv, n_ev, px, n_sol, loc, prec))
         return out
 
     def cv_native_empty(self, nvec: int, prec: int):

@@ -263,8 +263,9 @@ int lq_laph_eigensolve(lq_ctx* c, double* evals, void* evecs, int loc, const lq_
     if (st) dev_free(c, st);
     return rc;
 }
-int lq_project(lq_ctx* c, void* P, const void* evecs, int n_ev, const void* sols, int n_sol, int loc) {
+int lq_project(lq_ctx* c, void* P, const void* evecs, int n_ev, const void* sols, int n_sol, int loc, int prec) {
     if (!c || !P || !evecs || !sols || n_ev < 1 || n_ev > 1024 || n_sol < 1 || n_sol > 64) return set_err(c, LQ_EINVAL, "lq_project: bad argument");
+    if (prec != LQ_FP64 && prec != LQ_FP32) return set_err(c, LQ_EINVAL, "lq_project: precision must be fp64 or fp32");
     cudaSetDevice(c->device);
     const size_t vb = (size_t)n_ev * c->g.V * 6 * sizeof(double), xb = (size_t)n_sol * c->g.V * 24 * sizeof(double);
     const size_t pb = (size_t)c->g.L[3] * 4 * n_ev * n_sol * 2 * sizeof(double);
@@ -274,7 +275,8 @@ int lq_project(lq_ctx* c, void* P, const void* evecs, int n_ev, const void* sols
     int rc = (!d_v || !d_x) ? LQ_ENOMEM : 0;
     void* d_p = P;
     if (rc == 0 && loc == LQ_HOST) { st_p = dev_alloc(c, pb); if (!st_p) rc = LQ_ENOMEM; d_p = st_p; }
-    if (rc == 0) rc = project_device(c, (double*)d_p, (const double*)d_v, n_ev, (const double*)d_x, n_sol);
+    if (rc == 0) rc = prec == LQ_FP64 ? project_device(c, (double*)d_p, (const double*)d_v, n_ev, (const double*)d_x, n_sol)
+                                      : project_device_tc(c, (double*)d_p, (const double*)d_v, n_ev, (const double*)d_x, n_sol);
     if (rc == 0 && st_p) {
         if (cudaMemcpyAsync(P, st_p, pb, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess || cudaStreamSynchronize(c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "D2H copy failed");
     }

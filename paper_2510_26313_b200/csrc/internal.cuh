@@ -64,3 +64,5 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
 
 // project.cu : projection of solutions onto LapH eigenvectors
 int project_device(lq_ctx* c, double* dev_P, const double* dev_V, int n_ev, const double* dev_X, int n_sol);
+// project_tc.cu : the same contraction on tcgen05 tensor cores (3xTF32, fp32 TMEM accumulator, fp64 split-K sum)
+int project_device_tc(lq_ctx* c, double* dev_P, const double* dev_V, int n_ev, const double* dev_X, int n_sol);

@@ -18,8 +18,25 @@ def test_projection_matches_einsum(dims, n_ev, n_sol):
     want = oracle.project(v, psi)
     ctx = B.Context(dims)
     got = ctx.project(v, psi)
+    got_tc = ctx.project(v, psi, B.LQ_FP32)          # tcgen05 tensor cores, 3xTF32
     ctx.close()
     assert np.abs(got - want).max() <= 1e-12 * np.abs(want).max() * np.sqrt(3 * Lx * Ly * Lz)
+    assert np.abs(got_tc - want).max() <= 3e-6 * np.abs(want).max()
+
+
+def test_tensor_core_projection_tiles_and_padding():
+    """More eigenvectors than one 128-row tile, more solutions than one 8-solution tile, a slice that is not a multiple of the
+    256-site K chunk or the 16-site block."""
+    dims, n_ev, n_sol = (6, 6, 10, 2), 150, 11
+    Lx, Ly, Lz, Lt = dims
+    rng = np.random.default_rng(6)
+    v = rng.normal(size=(n_ev, Lt, Lz, Ly, Lx, 3)) + 1j * rng.normal(size=(n_ev, Lt, Lz, Ly, Lx, 3))
+    psi = inputs.gaussian_spinors(dims, n_sol, 82)
+    want = oracle.project(v, psi)
+    ctx = B.Context(dims)
+    got_tc = ctx.project(v, psi, B.LQ_FP32)
+    ctx.close()
+    assert np.abs(got_tc - want).max() <= 3e-6 * np.abs(want).max()
 
 
 def test_laph_chain_eigensolve_solve_project():

@@ -24,7 +24,9 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo, uint3
     return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)((lbo >> 4) & 0x3FFF) << 16) | ((uint64_t)((sbo >> 4) & 0x3FFF) << 32) | ((uint64_t)1 << 46);
 }
 __device__ __forceinline__ void split_tf32(float x, float& hi, float& lo) {
-    hi = __uint_as_float(__float_as_uint(x) & 0xFFFFE000u);
+    // round to nearest, ties away (cvt.rna.tf32.f32 written as two full-rate integer instructions): the error of the low
+    // part, which the tensor core truncates, then has no preferred sign
+    hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u);
     lo = x - hi;
 }
 __device__ __forceinline__ void split4(float4 x, float4& h, float4& l) {
@@ -36,28 +38,50 @@ __device__ __forceinline__ void mma_tf32(uint32_t tmem, uint64_t da, uint64_t db
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}\n" ::"r"(tmem), "l"(da), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
 }
 
-// TN = accumulator columns (8 per solution), SPB = sites per shared-memory stage (K = 6 SPB real terms)
-template <int TN, int SPB>
+// TN = accumulator columns (8 per solution), SPB = sites per stage (K = 6 SPB real terms), RING = raw stages in flight.
+// Pipeline per stage i: cp.async brings the fp64 fields of stage i+RING into a raw shared-memory ring (no registers held in
+// flight); all threads convert raw stage i into the operand tiles once the MMAs of stage i-1 have released them; thread 0
+// issues the MMAs of stage i into TMEM bank i%2; the accumulator of stage i-1 (other bank) is then added into registers
+// while the tensor core works.  The tensor core adds into its fp32 accumulator with truncation, so its chains are kept to
+// one stage and the running sum is carried in registers (round to nearest).
+template <int TN, int SPB, int RING>
+struct TcShape {
+    static constexpr int KB = SPB * 6, NCH = KB / 4;                       // real K terms / 16-byte operand chunks per stage
+    static constexpr int A_STRIDE = SPB * 48 + 16;                         // raw bytes per eigenvector row (+16: bank-conflict-free reads)
+    // raw solutions in pairs, the odd one 64 bytes further than its size: two solutions per quarter-warp read without conflicts
+    static constexpr int B_PAIR = 2 * SPB * 192 + 64;
+    __host__ __device__ static constexpr int b_offset(int kl) { return (kl >> 1) * B_PAIR + (kl & 1) * (SPB * 192 + 64); }
+    static constexpr int A_RAW = TM * A_STRIDE, B_RAW = (TN / 16) * B_PAIR, RAW = A_RAW + B_RAW;
+    static constexpr int OPER = (2 * TM + 2 * TN) * KB * 4;
+    static constexpr size_t SMEM = (size_t)OPER + (size_t)RING * RAW + 64;
+};
+
+__device__ __forceinline__ void cp_async16(void* dst, const void* src, bool valid) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s32(dst)), "l"(src), "r"(valid ? 16 : 0) : "memory");
+}
+
+template <int TN, int SPB, int RING>
 __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchunk, int n_ev, int n_sol, int j0, int k0,
                                                         const double2* __restrict__ V, const double2* __restrict__ X, float* __restrict__ partial, int* __restrict__ err) {
-    constexpr int KB = SPB * 6, NCH = KB / 4;                 // real K terms and 16-byte chunks per stage
-    constexpr int A_UNITS = (TM / 8) * (NCH / 4) / (NT / 32);  // (8 rows x 4 chunks) units per warp
-    constexpr int B_TASKS = (TN / 8) * 4 * NCH;                // (solution, spin, chunk) tasks per stage
-    constexpr int B_PER_THREAD = (B_TASKS + NT - 1) / NT;
+    using Sh = TcShape<TN, SPB, RING>;
+    constexpr int KB = Sh::KB, NCH = Sh::NCH;
+    constexpr int A_PIECES = TM * SPB * 3, B_PIECES = (TN / 8) * SPB * 12;   // 16-byte pieces per raw stage
+    constexpr int A_TASKS = TM * NCH, B_TASKS = (TN / 8) * 4 * NCH;          // float4 conversion tasks per stage
     constexpr int COLS = TN / 4;                               // accumulator columns per warp (4 column groups x 4 lane quadrants)
-    static_assert((TM / 8) * (NCH / 4) % (NT / 32) == 0 && NCH % 4 == 0, "stage shape");
+    static_assert(NCH % 2 == 0 && 2 * TN <= 512, "stage shape");
     extern __shared__ __align__(1024) unsigned char smem[];
     float4* sAh = (float4*)smem;               // [NCH][TM/8][8] x 16 bytes
     float4* sAl = sAh + TM * NCH;
     float4* sBh = sAl + TM * NCH;              // [NCH][TN/8][8] x 16 bytes
     float4* sBl = sBh + TN * NCH;
-    uint64_t* bar = (uint64_t*)(sBl + TN * NCH);
+    unsigned char* raw = smem + Sh::OPER;      // RING x { A rows [TM][A_STRIDE], B [TN/8][SPB][12] double2 }
+    uint64_t* bar = (uint64_t*)(raw + (size_t)RING * Sh::RAW);
     uint32_t* tptr = (uint32_t*)(bar + 1);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int t = blockIdx.x / nchunk, ch = blockIdx.x - t * nchunk;
     if (tid == 0) { asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(s32(bar))); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(s32(tptr)), "n"(TN));
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(s32(tptr)), "n"(2 * TN));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
@@ -66,97 +90,72 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
     const uint32_t tmem = *tptr;
     const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TN >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);   // F32 acc, TF32 x TF32, K-major
     const int s_begin = ch * SITES_PER_CTA, s_end = min(S3, s_begin + SITES_PER_CTA);
+    const int nst = (s_end - s_begin + SPB - 1) / SPB;
     const int nj = min(TM, n_ev - j0), nk = min(TN / 8, n_sol - k0);
-    uint32_t phase = 0;
-    bool ok = true;
-    float acc[COLS];                           // TMEM lanes 32 (warp % 4) + lane, columns COLS (warp / 4) ..., summed over the stages
+    const double2* Vt = V + ((size_t)j0 * Lt + t) * S3 * 3;    // row r: + r * Lt * S3 * 3
+    const double2* Xt = X + ((size_t)k0 * Lt + t) * S3 * 12;   // solution kl: + kl * Lt * S3 * 12
+    const size_t vrow = (size_t)Lt * S3 * 3, xrow = (size_t)Lt * S3 * 12;
+
+    // Per-thread copy pieces and conversion tasks are the same in every stage (the slice size is a multiple of 8 sites, so a
+    // stage is never ragged): precompute their addresses once, the stage loop only adds the stage offset.
+    constexpr int NPA = (A_PIECES + NT - 1) / NT, NPB = (B_PIECES + NT - 1) / NT;
+    const double2* srcA[NPA]; uint32_t dstA[NPA];              // source of stage 0, byte offset in the raw slot; dst = ~0: no piece
+    const double2* srcB[NPB]; uint32_t dstB[NPB];
 #pragma unroll
-    for (int i = 0; i < COLS; i++) acc[i] = 0.f;
-    // global loads of one stage into registers; issued for stage i+1 right after the MMAs of stage i, so that their latency
-    // overlaps the tensor-core work and the accumulator read-out
-    double2 va[A_UNITS][2], xb[B_PER_THREAD][2];
-    auto load_stage = [&](int sb) {
-        const int e_end = (s_end - sb) * 3;    // complex elements of V left in this CTA's range (<= 0: nothing)
-        // ---- A': rows = eigenvectors j0 .. j0+127; lane = (row % 8, chunk % 4): a quarter-warp stores one 128-byte row group
+    for (int k = 0; k < NPA; k++) {
+        const int p = tid + k * NT, r = p / (SPB * 3), e = p - r * (SPB * 3);
+        const bool have = p < A_PIECES;
+        dstA[k] = have ? (uint32_t)(r * Sh::A_STRIDE + e * 16) : 0xFFFFFFFFu;
+        srcA[k] = (have && r < nj) ? Vt + r * vrow + (size_t)s_begin * 3 + e : nullptr;
+    }
 #pragma unroll
-        for (int u = 0; u < A_UNITS; u++) {
-            const int unit = warp * A_UNITS + u, r = (unit / (NCH / 4)) * 8 + (lane & 7), chunk = (unit % (NCH / 4)) * 4 + (lane >> 3);
-            const double2* src = V + (((size_t)(j0 + r) * Lt + t) * S3 + sb) * 3 + 2 * chunk;
-            const bool row = r < nj;
-            va[u][0] = (row && 2 * chunk < e_end) ? src[0] : make_double2(0.0, 0.0);
-            va[u][1] = (row && 2 * chunk + 1 < e_end) ? src[1] : make_double2(0.0, 0.0);
+    for (int k = 0; k < NPB; k++) {
+        const int p = tid + k * NT, kl = p / (SPB * 12), w = p - kl * (SPB * 12);
+        const bool have = p < B_PIECES;
+        dstB[k] = have ? (uint32_t)(Sh::A_RAW + Sh::b_offset(kl) + w * 16) : 0xFFFFFFFFu;
+        srcB[k] = (have && kl < nk) ? Xt + kl * xrow + (size_t)s_begin * 12 + w : nullptr;
+    }
+    // raw stage `st` -> ring slot st % RING; rows / solutions beyond the problem are zero-filled
+    auto fetch_stage = [&](int st) {
+        if (st < nst) {
+            unsigned char* slot = raw + (size_t)(st % RING) * Sh::RAW;
+#pragma unroll
+            for (int k = 0; k < NPA; k++)
+                if (dstA[k] != 0xFFFFFFFFu) cp_async16(slot + dstA[k], srcA[k] ? srcA[k] + (size_t)st * (SPB * 3) : V, srcA[k] != nullptr);
+#pragma unroll
+            for (int k = 0; k < NPB; k++)
+                if (dstB[k] != 0xFFFFFFFFu) cp_async16(slot + dstB[k], srcB[k] ? srcB[k] + (size_t)st * (SPB * 12) : X, srcB[k] != nullptr);
         }
-        // ---- B': rows 2n, 2n+1 with n = (solution, spin); task = (solution, chunk, spin), spin fastest across lanes
-#pragma unroll
-        for (int u = 0; u < B_PER_THREAD; u++) {
-            const int q = tid + u * NT, a = q & 3, chunk = (q >> 2) % NCH, kl = (q >> 2) / NCH;
-            xb[u][0] = xb[u][1] = make_double2(0.0, 0.0);
-            if (q < B_TASKS && kl < nk) {
-                const double2* base = X + ((size_t)(k0 + kl) * Lt + t) * S3 * 12 + 3 * a;
-                const int e0 = 2 * chunk, e1 = e0 + 1;
-                if (e0 < e_end) xb[u][0] = base[(size_t)(sb + e0 / 3) * 12 + e0 % 3];
-                if (e1 < e_end) xb[u][1] = base[(size_t)(sb + e1 / 3) * 12 + e1 % 3];
-            }
-        }
+        asm volatile("cp.async.commit_group;" ::: "memory");    // one group per call, also when empty: uniform counting
     };
-    load_stage(s_begin);
-    for (int sb = s_begin; sb < s_end; sb += SPB) {
+    // conversion tasks: raw byte offset(s) in the slot and float4 index in the operand tile (~0: no task)
+    constexpr int NTA = (A_TASKS + NT - 1) / NT, NTB = (B_TASKS + NT - 1) / NT;
+    uint32_t rawA[NTA], opA[NTA], rawB0[NTB], rawB1[NTB], opB[NTB];
 #pragma unroll
-        for (int u = 0; u < A_UNITS; u++) {
-            const int unit = warp * A_UNITS + u, r = (unit / (NCH / 4)) * 8 + (lane & 7), chunk = (unit % (NCH / 4)) * 4 + (lane >> 3);
-            float4 h, l;
-            split4(make_float4((float)va[u][0].x, (float)va[u][0].y, (float)va[u][1].x, (float)va[u][1].y), h, l);
-            sAh[chunk_index<TM>(r, chunk)] = h; sAl[chunk_index<TM>(r, chunk)] = l;
-        }
+    for (int k = 0; k < NTA; k++) {
+        // unit = 16 rows x 2 chunks; lane = (row % 8, chunk % 2, (row / 8) % 2): a quarter-warp reads 8 raw rows without bank
+        // conflicts and stores one 128-byte core-matrix row group
+        const int q = tid + k * NT, unit = q >> 5, r = ((unit / (NCH / 2)) * 2 + (lane >> 4)) * 8 + (lane & 7), chunk = (unit % (NCH / 2)) * 2 + ((lane >> 3) & 1);
+        rawA[k] = (uint32_t)(r * Sh::A_STRIDE + chunk * 32);
+        opA[k] = q < A_TASKS ? (uint32_t)chunk_index<TM>(r, chunk) : 0xFFFFFFFFu;
+    }
 #pragma unroll
-        for (int u = 0; u < B_PER_THREAD; u++) {
-            const int q = tid + u * NT, a = q & 3, chunk = (q >> 2) % NCH, kl = (q >> 2) / NCH;
-            if (q < B_TASKS) {
-                float4 h, l;
-                split4(make_float4((float)xb[u][0].x, (float)xb[u][0].y, (float)xb[u][1].x, (float)xb[u][1].y), h, l);
-                const float4 h1 = make_float4(h.y, -h.x, h.w, -h.z), l1 = make_float4(l.y, -l.x, l.w, -l.z);
-                const int r0 = 2 * (kl * 4 + a);
-                // odd chunks store the odd row first: the 8 lanes of a quarter-warp then cover the 8 rows of one core matrix
-                if (chunk & 1) {
-                    sBh[chunk_index<TN>(r0 + 1, chunk)] = h1; sBh[chunk_index<TN>(r0, chunk)] = h;
-                    sBl[chunk_index<TN>(r0 + 1, chunk)] = l1; sBl[chunk_index<TN>(r0, chunk)] = l;
-                } else {
-                    sBh[chunk_index<TN>(r0, chunk)] = h; sBh[chunk_index<TN>(r0 + 1, chunk)] = h1;
-                    sBl[chunk_index<TN>(r0, chunk)] = l; sBl[chunk_index<TN>(r0 + 1, chunk)] = l1;
-                }
-            }
-        }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        __syncthreads();
-        asm volatile("tcgen05.fence::after_thread_sync;");
-        if (tid == 0) {
-#pragma unroll 1
-            for (int s = 0; s < KB / 8; s++) {
-                const uint64_t ah = smem_desc(s32(sAh) + (2 * s) * (TM * 16), TM * 16, 128), al = smem_desc(s32(sAl) + (2 * s) * (TM * 16), TM * 16, 128);
-                const uint64_t bh = smem_desc(s32(sBh) + (2 * s) * (TN * 16), TN * 16, 128), bl = smem_desc(s32(sBl) + (2 * s) * (TN * 16), TN * 16, 128);
-                mma_tf32(tmem, al, bh, idesc, s == 0 ? 0u : 1u);
-                mma_tf32(tmem, ah, bl, idesc, 1u);
-                mma_tf32(tmem, ah, bh, idesc, 1u);
-            }
-            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(s32(bar)) : "memory");
-        }
-        load_stage(sb + SPB);
-        // every thread waits for the MMAs of this stage (bounded spin: a fault must not hang the GPU)
-        bool done = false;
-        for (int spin = 0; spin < 20000000 && !done; spin++) {
-            uint32_t r;
-            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(r) : "r"(s32(bar)), "r"(phase) : "memory");
-            done = r != 0;
-        }
-        if (!done) { ok = false; break; }
-        phase ^= 1;
-        asm volatile("tcgen05.fence::after_thread_sync;");
-        // the tensor core adds into its fp32 accumulator with truncation: keep its chains short (one stage) and carry the
-        // running sum in registers (round to nearest)
+    for (int k = 0; k < NTB; k++) {
+        // rows 2n, 2n+1 with n = (solution, spin); lane = (spin, solution % 2, chunk % 4): a quarter-warp reads two solutions x four
+        // spins of one chunk (conflict-free with the padded solution stride) and, odd solutions storing the odd row first, covers
+        // the 8 rows of a core matrix in each store
+        const int q = tid + k * NT, a = q & 3, chunk = (q >> 3) % NCH, kl = 2 * ((q >> 3) / NCH) + ((q >> 2) & 1);
+        const int e0 = 2 * chunk, e1 = e0 + 1;
+        const uint32_t base = (uint32_t)(Sh::A_RAW + Sh::b_offset(kl) + a * 48);
+        rawB0[k] = base + ((e0 / 3) * 12 + e0 % 3) * 16;
+        rawB1[k] = base + ((e1 / 3) * 12 + e1 % 3) * 16;
+        opB[k] = q < B_TASKS ? (uint32_t)chunk_index<TN>(2 * (kl * 4 + a), chunk) : 0xFFFFFFFFu;
+    }
+    auto flush_bank = [&](int bank, float* acc) {
 #pragma unroll
         for (int c0 = 0; c0 < COLS; c0 += 8) {
             uint32_t v[8];
-            const uint32_t taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (warp >> 2) * COLS + c0;
+            const uint32_t taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + bank * TN + (warp >> 2) * COLS + c0;
             asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                          : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]) : "r"(taddr));
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
@@ -164,6 +163,76 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
             for (int i = 0; i < 8; i++) acc[c0 + i] += __uint_as_float(v[i]);
         }
         asm volatile("tcgen05.fence::before_thread_sync;");
+    };
+    // every thread waits for the MMAs of one stage (bounded spin: a fault must not hang the GPU)
+    auto wait_mma = [&](uint32_t parity) {
+        bool done = false;
+        for (int spin = 0; spin < 20000000 && !done; spin++) {
+            uint32_t r;
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(r) : "r"(s32(bar)), "r"(parity) : "memory");
+            done = r != 0;
+        }
+        asm volatile("tcgen05.fence::after_thread_sync;");
+        return done;
+    };
+
+    float acc[COLS];                           // TMEM lanes 32 (warp % 4) + lane, columns COLS (warp / 4) ..., summed over the stages
+#pragma unroll
+    for (int i = 0; i < COLS; i++) acc[i] = 0.f;
+    bool ok = true;
+#pragma unroll
+    for (int st = 0; st < RING; st++) fetch_stage(st);
+    for (int i = 0; i < nst; i++) {
+        asm volatile("cp.async.wait_group %0;" ::"n"(RING - 1) : "memory");
+        __syncthreads();                                         // raw stage i is complete for every thread
+        if (i > 0 && !wait_mma((uint32_t)((i - 1) & 1))) { ok = false; break; }   // operand tiles released by the MMAs of stage i-1
+        const unsigned char* slot = raw + (size_t)(i % RING) * Sh::RAW;
+#pragma unroll
+        for (int k = 0; k < NTA; k++) {
+            if (opA[k] == 0xFFFFFFFFu) continue;
+            const double2* src = (const double2*)(slot + rawA[k]);
+            const double2 v0 = src[0], v1 = src[1];
+            float4 h, l;
+            split4(make_float4((float)v0.x, (float)v0.y, (float)v1.x, (float)v1.y), h, l);
+            sAh[opA[k]] = h; sAl[opA[k]] = l;
+        }
+#pragma unroll
+        for (int k = 0; k < NTB; k++) {
+            if (opB[k] == 0xFFFFFFFFu) continue;
+            const double2 x0 = *(const double2*)(slot + rawB0[k]), x1 = *(const double2*)(slot + rawB1[k]);
+            float4 h, l;
+            split4(make_float4((float)x0.x, (float)x0.y, (float)x1.x, (float)x1.y), h, l);
+            const float4 h1 = make_float4(h.y, -h.x, h.w, -h.z), l1 = make_float4(l.y, -l.x, l.w, -l.z);
+            // odd solutions store the odd row first (selects, not branches: one store instruction must cover all 8 rows)
+            const bool odd = (lane >> 2) & 1;
+            const uint32_t i0 = opB[k] + (odd ? 1u : 0u), i1 = opB[k] + (odd ? 0u : 1u);
+            const float4 ha = odd ? h1 : h, hb = odd ? h : h1, la = odd ? l1 : l, lb = odd ? l : l1;
+            sBh[i0] = ha; sBl[i0] = la;
+            sBh[i1] = hb; sBl[i1] = lb;
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("tcgen05.fence::before_thread_sync;");
+        __syncthreads();                                         // operands visible; raw slot i % RING is free again
+        asm volatile("tcgen05.fence::after_thread_sync;");
+        if (tid == 0) {
+            const uint32_t d = tmem + (i & 1) * TN;
+#pragma unroll 1
+            for (int s = 0; s < KB / 8; s++) {
+                const uint64_t ah = smem_desc(s32(sAh) + (2 * s) * (TM * 16), TM * 16, 128), al = smem_desc(s32(sAl) + (2 * s) * (TM * 16), TM * 16, 128);
+                const uint64_t bh = smem_desc(s32(sBh) + (2 * s) * (TN * 16), TN * 16, 128), bl = smem_desc(s32(sBl) + (2 * s) * (TN * 16), TN * 16, 128);
+                mma_tf32(d, al, bh, idesc, s == 0 ? 0u : 1u);
+                mma_tf32(d, ah, bl, idesc, 1u);
+                mma_tf32(d, ah, bh, idesc, 1u);
+            }
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(s32(bar)) : "memory");
+        }
+        fetch_stage(i + RING);
+        if (i > 0) flush_bank((i - 1) & 1, acc);                 // overlaps the MMAs of stage i (other bank)
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (ok && nst > 0) {
+        ok = wait_mma((uint32_t)((nst - 1) & 1));
+        if (ok) flush_bank((nst - 1) & 1, acc);
     }
     if (!ok && lane == 0) atomicAdd(err, 1);
     // accumulator row r = TMEM lane r, column n'; partial[t][chunk][r][n']
@@ -175,7 +244,7 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TN));
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(2 * TN));
 }
 
 // out[t][alpha][j0+r][k0+kl] = fixed-order fp64 sum over chunks of partial[t][chunk][r][2*(kl*4+alpha) + (re|im)]
@@ -195,12 +264,13 @@ __global__ void project_tc_final_kernel(int Lt, int nchunk, int n_ev, int n_sol,
     out[(((size_t)t * 4 + a) * n_ev + (j0 + r)) * n_sol + (k0 + kl)] = make_double2(re, im);
 }
 
-template <int TN, int SPB>
+template <int TN, int SPB, int RING>
 int project_tc_run(lq_ctx* c, int Lt, int S3, int n_ev, int n_sol, const double* dev_V, const double* dev_X, double* dev_P) {
     const int nchunk = (S3 + SITES_PER_CTA - 1) / SITES_PER_CTA;
-    const size_t smem = (size_t)(2 * TM + 2 * TN) * SPB * 6 * sizeof(float) + 64;
+    const size_t smem = TcShape<TN, SPB, RING>::SMEM;
+    static_assert(TcShape<TN, SPB, RING>::SMEM <= 232448, "shared memory per CTA");
     static bool configured = false;
-    if (!configured) { LQ_CUDA(c, cudaFuncSetAttribute(project_tc_kernel<TN, SPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); configured = true; }
+    if (!configured) { LQ_CUDA(c, cudaFuncSetAttribute(project_tc_kernel<TN, SPB, RING>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); configured = true; }
     float* partial = (float*)dev_alloc(c, sizeof(float) * (size_t)Lt * nchunk * TM * TN);
     int* d_err = (int*)dev_alloc(c, sizeof(int));
     if (!partial || !d_err) { if (partial) dev_free(c, partial); if (d_err) dev_free(c, d_err); return LQ_ENOMEM; }
@@ -208,7 +278,7 @@ int project_tc_run(lq_ctx* c, int Lt, int S3, int n_ev, int n_sol, const double*
     int rc = 0;
     for (int j0 = 0; j0 < n_ev && rc == 0; j0 += TM)
         for (int k0 = 0; k0 < n_sol && rc == 0; k0 += TN / 8) {
-            project_tc_kernel<TN, SPB><<<Lt * nchunk, NT, smem, c->stream>>>(Lt, S3, nchunk, n_ev, n_sol, j0, k0, (const double2*)dev_V, (const double2*)dev_X, partial, d_err);
+            project_tc_kernel<TN, SPB, RING><<<Lt * nchunk, NT, smem, c->stream>>>(Lt, S3, nchunk, n_ev, n_sol, j0, k0, (const double2*)dev_V, (const double2*)dev_X, partial, d_err);
             const int nj = std::min(TM, n_ev - j0), nk = std::min(TN / 8, n_sol - k0);
             project_tc_final_kernel<<<(Lt * nj * nk * 4 + 127) / 128, 128, 0, c->stream>>>(Lt, nchunk, n_ev, n_sol, j0, k0, TN, partial, (double2*)dev_P);
             c->launches += 2;
@@ -226,8 +296,8 @@ int project_tc_run(lq_ctx* c, int Lt, int S3, int n_ev, int n_sol, const double*
 int project_device_tc(lq_ctx* c, double* dev_P, const double* dev_V, int n_ev, const double* dev_X, int n_sol) {
     const int Lt = c->g.L[3];
     const long long S3l = (long long)c->g.L[0] * c->g.L[1] * c->g.L[2];
-    if (S3l > (1LL << 30)) return set_err(c, LQ_EINVAL, "lq_project: slice too large");
-    // 8 solutions per pass (N = 64, 16-site stages) or 32 (N = 256, 8-site stages): the eigenvectors are read once per pass
-    if (n_sol <= 8) return project_tc_run<64, 16>(c, Lt, (int)S3l, n_ev, n_sol, dev_V, dev_X, dev_P);
-    return project_tc_run<256, 8>(c, Lt, (int)S3l, n_ev, n_sol, dev_V, dev_X, dev_P);
+    if (S3l > (1LL << 30) || S3l % 8 != 0) return set_err(c, LQ_EINVAL, "lq_project: bad slice size");   // even extents: 8 | S3
+    // 8 solutions per pass (N = 64, 8-site stages) or 32 (N = 256, 4-site stages): the eigenvectors are read once per pass
+    if (n_sol <= 8) return project_tc_run<64, 8, 2>(c, Lt, (int)S3l, n_ev, n_sol, dev_V, dev_X, dev_P);
+    return project_tc_run<256, 4, 3>(c, Lt, (int)S3l, n_ev, n_sol, dev_V, dev_X, dev_P);
 }

@@ -308,6 +308,130 @@ def time_projection(B, device, peak, shapes=((32, 8), (128, 32)), precs=("f64_fm
     return out
 
 
+def operator_sweeps(B, device, peak):
+    """configs[2]: 32^3x64 fp32 sweep over N_rhs (kernel A, kernel B, bare hop); configs[4]: 64^3x128, N=4, 12-real links."""
+    import torch
+    out = {"unit": "GB/s (algorithmic bytes / CUDA-event time)", "peak_gbs": peak, "cfg2_32x32x32x64_fp32_recon18": [], "cfg4_64x64x64x128_fp32_recon12": []}
+    for cfg_id, key in ((2, "cfg2_32x32x32x64_fp32_recon18"), (4, "cfg4_64x64x64x128_fp32_recon12")):
+        c = inputs.CONFIGS[cfg_id]
+        ctx = B.Context(c["dims"], device=device)
+        ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=c["recon"])
+        ctx.build_clover(c["kappa"], c["csw"])
+        ns = c["nrhs"] if isinstance(c["nrhs"], tuple) else (c["nrhs"],)
+        for n in ns:
+            for kind in ("A", "B", "hop"):
+                r = time_dslash(ctx, B, kind, "fp32", n, c["recon"], iters=20)
+                out[key].append({"kernel": kind, "nrhs": n, "us": round(r["seconds"] * 1e6, 1), "gbs": round(r["gbs"], 1), "gflops": round(r["gflops"], 1),
+                                 "frac_measured_hbm": round(r["gbs"] / peak, 4), "frac_8TBs": round(r["gbs"] / 8000.0, 4)})
+        if cfg_id == 2:
+            out["laplacian_32x32x32x64_fp32"] = []
+            for n in (1, 4, 8, 16):
+                r = time_laplacian(ctx, B, n)
+                r["frac_measured_hbm"] = round(r["gbs"] / peak, 4)
+                out["laplacian_32x32x32x64_fp32"].append(r)
+        ctx.close()
+        torch.cuda.empty_cache()
+    return out
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+def run_reference(args, rank, world):
+    """`--impl reference`: this tier has no reference implementation to install; the arm times the CPU oracle as it stands
+    on the host cores (rank 0 only), on the same config / metric / unit."""
+    if rank != 0:
+        return
+    wl = SOLVER_WORKLOADS[args.workload]
+    c = inputs.CONFIGS[wl["cfg"]]
+    vals = []
+    cb = None
+    for _ in range(max(1, min(args.steps, 2))):
+        cb = cpu_baseline(wl["cfg"], budget_s=20.0)
+        vals.append(cb["value"])
+    v = float(np.mean(vals))
+    line = {"impl": "reference", "metric": "batched CG sec/RHS", "value": v, "unit": "s/RHS", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": v * c["nrhs"] * 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": wl["desc"], "note": "CPU oracle, bounded sample per step"},
+            "cpu_baseline": dict(cb, value=v), "e2e": {"value": v, "unit": "s/RHS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------ large-lattice solve (configs[3])
+def run_big_solve(args, B, device, wl, c, peak, peak_src):
+    """configs[3] (48^3x96, 12 RHS, int16+norm inner CG): too large to keep canonical AND native copies of b and x on the
+    device next to the solver workspace, so the step is: host canonical b -> lq_pack (H2D + reorder) -> native solve ->
+    lq_unpack (reorder + D2H).  `value` = the native device-resident solve; `e2e` = the whole host-to-host step."""
+    import torch
+    dims, nrhs = c["dims"], c["nrhs"]
+    ctx = B.Context(dims, device=device)
+    ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=c["recon"])
+    ctx.build_clover(c["kappa"], c["csw"])
+    b_host = make_sources_host(wl["cfg"])
+    kw = dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=args.delta or wl["delta"], check_every=args.check_every, use_graph=not args.no_graph, native=True, nrhs=nrhs)
+    sampler = ClockSampler(device)
+    w0 = time.perf_counter()
+    nb = ctx.pack(b_host, nrhs, B.LQ_FP64)
+    torch.cuda.synchronize()
+    t_pack = time.perf_counter() - w0
+    nx = ctx.native_empty(nrhs, B.LQ_FP64)
+    info = None
+    steps = max(1, min(args.steps, 2))
+    _, info = ctx.solve(nb, x_out=nx, **kw)                       # one warm-up solve (workspace allocation, graph build)
+    l0 = ctx.launches
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(ctx.stream)
+    for _ in range(steps):
+        _, info = ctx.solve(nb, x_out=nx, **kw)
+    e1.record(ctx.stream)
+    e1.synchronize()
+    t_dev = e0.elapsed_time(e1) * 1e-3 / steps
+    launches = (ctx.launches - l0) // steps
+    w0 = time.perf_counter()
+    x_host = ctx.unpack(nx, nrhs, B.LQ_FP64)
+    t_unpack = time.perf_counter() - w0
+    clocks = sampler.stop()
+    del nb, nx
+    rA = time_dslash(ctx, B, "A", wl["inner"], nrhs, c["recon"], iters=10)
+    rB = time_dslash(ctx, B, "B", wl["inner"], nrhs, c["recon"], iters=10)
+    ctx.close()
+    line = {"metric": "batched CG sec/RHS", "value": t_dev / nrhs, "unit": "s/RHS", "n_gpus": 1, "steps": steps, "warmup": 1,
+            "ms_per_step": t_dev * 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "i16+f32", "data": "synthetic",
+            "config": {"workload": wl["desc"], "lattice": "x".join(map(str, dims)), "nrhs_per_gpu": nrhs, "parallelism": "replicas only (RHS-independent)",
+                       "l2": "every vector of the iteration (3.3 GB) exceeds the 126 MB L2", "cuda_graph": not args.no_graph,
+                       "kappa": c["kappa"], "csw": c["csw"], "tol": c["tol"]},
+            "solver": {"converged": info["converged"], "outer_cycles": info["outer_cycles"], "inner_iters": info["inner_iters"],
+                       "true_rel_residual_max": max(info["true_rel_residual"]), "dslash_applies_per_step": info["dslash_applies"]},
+            "e2e": {"value": (t_pack + t_dev + t_unpack) / nrhs, "unit": "s/RHS", "h2d_bytes_per_step": int(b_host.nbytes), "d2h_bytes_per_step": int(x_host.nbytes),
+                    "note": "pageable host arrays; pack %.2f s + solve %.2f s + unpack %.2f s" % (t_pack, t_dev, t_unpack)},
+            "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": roofline_entry(rA, peak, peak_src), "roofline_kernel_B": roofline_entry(rB, peak, peak_src)}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------ multi-rank plumbing
+def max_over_ranks(values, device=None):
+    """Replicas-only scaling: every rank runs the same step on its own RHS batch; the job's time is the
+    slowest rank's.  Works on whatever torch.distributed backend is initialised (nccl on GPUs, gloo in the CPU tests)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    t = torch.tensor(list(values), dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_seconds_per_rhs(seconds_total, steps, nrhs_per_rank, world):
+    """metric value: seconds per RHS of the whole job = max-over-ranks step time / RHS solved by all ranks per step."""
+    return seconds_total / steps / (nrhs_per_rank * world)
+
+
+def rank_gauge_seed(base_seed, rank):
+    """Each replica works on its own gauge configuration (independent tasks)."""
+    return base_seed + rank
+
+
+# ------------------------------------------------------------------------------------------------ single-operator mode
 def run_op(args, B, device):
     f = args.op.split(":")
     cfg_id, kind, prec, n = int(f[0].replace("cfg", "")), f[1], f[2], int(f[3])

@@ -28,9 +28,9 @@ void dev_free(lq_ctx* c, void* p) {
 }
 
 int ensure_partials(lq_ctx* c, size_t elems) {
-    if (elems <= c->red_partials_elems) return 0;
+    if (elems + elems / 16 + 64 * LQ_MAX_RHS <= c->red_partials_elems) return 0;
     if (c->red_partials) dev_free(c, c->red_partials);
-    c->red_partials_elems = elems * 2;
+    c->red_partials_elems = elems * 2 + elems / 8 + 64 * LQ_MAX_RHS;   // rows of every level of the reduction tree (reduce.cuh)
     c->red_partials = (double*)dev_alloc(c, c->red_partials_elems * sizeof(double));
     if (!c->red_partials) { c->red_partials_elems = 0; return LQ_ENOMEM; }
     return 0;
@@ -57,7 +57,7 @@ int lq_create(lq_ctx** out, const int dims[4], int device, void* cuda_stream) {
     c->alloc_fn = nullptr; c->free_fn = nullptr; c->alloc_user = nullptr;
     c->launches = 0; c->dslash_rpt = 0; c->dslash_variant = 0; c->dslash_pfd = LQ_DEFAULT_PFD; c->dslash_zc = 0;
     c->red_partials = nullptr; c->red_partials_elems = 0; c->red_counter = nullptr; c->h_scalars = nullptr; c->d_flag = nullptr;
-    if (cudaMalloc(&c->red_counter, 256) != cudaSuccess || cudaMemset(c->red_counter, 0, 256) != cudaSuccess ||
+    if (cudaMalloc(&c->red_counter, RED_COUNTER_BYTES) != cudaSuccess || cudaMemset(c->red_counter, 0, RED_COUNTER_BYTES) != cudaSuccess ||
         cudaMallocHost(&c->h_scalars, 8 * LQ_MAX_RHS * sizeof(double)) != cudaSuccess) { cudaGetLastError(); delete c; return LQ_ECUDA; }
     c->d_flag = (int*)(c->red_counter + 16);
     *out = c;

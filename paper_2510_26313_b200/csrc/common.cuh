@@ -184,6 +184,12 @@ struct lq_ctx {
 int set_err(lq_ctx* c, int code, const std::string& msg);
 void* dev_alloc(lq_ctx* c, size_t bytes);          // nullptr on failure (error recorded)
 void dev_free(lq_ctx* c, void* p);
+// deterministic reduction tree (reduce.cuh): fan-in, where its counters start in lq_ctx::red_counter (the first 64 words are
+// flags) and how many there are (enough for 4M blocks)
+constexpr int RED_FAN = 32;
+constexpr int RED_COUNTER_BASE = 64;
+constexpr int RED_COUNTERS = 1 << 17;
+constexpr size_t RED_COUNTER_BYTES = (size_t)(RED_COUNTER_BASE + RED_COUNTERS) * sizeof(unsigned int);
 int ensure_partials(lq_ctx* c, size_t elems);      // reduction scratch of at least `elems` doubles
 
 #define LQ_CUDA(ctx, call)                                                                     \

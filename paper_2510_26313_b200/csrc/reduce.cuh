@@ -31,38 +31,39 @@ __device__ void reduce_per_rhs(double (&part)[VW], int N, int G, double* partial
         }
         partials[(size_t)blockIdx.x * N + t] = s;
     }
+    // Fan-in tree over the blocks (RED_FAN per node, fixed grouping and order: bitwise reproducible).  The last block to
+    // finish in a group of RED_FAN adds the group's rows and becomes the group's representative one level up; the tail that
+    // runs after all other blocks have retired is then a few short rounds instead of one block reading every partial.
+    // Level l rows live behind those of level l-1 in `partials`, its self-resetting counters behind those of level l-1.
     __shared__ bool last;
-    __threadfence();
-    __syncthreads();
-    if (t == 0) last = (atomicInc(counter, gridDim.x - 1) == gridDim.x - 1);
-    __syncthreads();
-    if (!last) return;
-    __threadfence();
-    // final: thread t handles RHS r = t % N, slice q = t / N of the blocks; Q = largest power of two with N*Q <= nt
-    int Q = 1;
+    int Q = 1;                             // thread t handles RHS t % N, row slice t / N; Q = largest power of two with N*Q <= nt
     while (N * Q * 2 <= nt) Q <<= 1;
     const int r = t % N, q = t / N;
-    double s = 0.0;
-    if (q < Q) {
-        // same fixed summation order as a plain loop, but eight loads in flight: this tail runs in ONE block after
-        // all others have retired, so its latency is pure serial time of the launch
-        unsigned b = q;
-        for (; b + 7u * Q < gridDim.x; b += 8u * Q) {
-            double v[8];
-#pragma unroll
-            for (int i = 0; i < 8; i++) v[i] = __ldcg(partials + (size_t)(b + (unsigned)i * Q) * N + r);
-#pragma unroll
-            for (int i = 0; i < 8; i++) s += v[i];
-        }
-        for (; b < gridDim.x; b += Q) s += __ldcg(partials + (size_t)b * N + r);
-    }
-    __syncthreads();
-    if (q < Q) sm[t] = s;
-    __syncthreads();
-    for (int stride = Q >> 1; stride >= 1; stride >>= 1) {
-        if (q < stride) sm[t] += sm[t + stride * N];
+    unsigned idx = blockIdx.x, n = gridDim.x;
+    double* src = partials;
+    unsigned int* cnt = counter + RED_COUNTER_BASE;
+    for (;;) {
+        const unsigned grp = idx / RED_FAN, ngrp = (n + RED_FAN - 1) / RED_FAN;
+        const unsigned gsize = min((unsigned)RED_FAN, n - grp * RED_FAN);
+        __threadfence();
         __syncthreads();
+        if (t == 0) last = (atomicInc(cnt + grp, gsize - 1) == gsize - 1);
+        __syncthreads();
+        if (!last) return;
+        __threadfence();
+        const double* rows = src + (size_t)grp * RED_FAN * N;
+        double s = 0.0;
+        if (q < Q) for (unsigned b = q; b < gsize; b += Q) s += __ldcg(rows + (size_t)b * N + r);
+        __syncthreads();
+        if (q < Q) sm[t] = s;
+        __syncthreads();
+        for (int stride = Q >> 1; stride >= 1; stride >>= 1) {
+            if (q < stride) sm[t] += sm[t + stride * N];
+            __syncthreads();
+        }
+        if (ngrp == 1) { if (t < N) out[t] = sm[t]; return; }
+        double* dst = src + (size_t)n * N;
+        if (t < N) dst[(size_t)grp * N + t] = sm[t];
+        src = dst; cnt += ngrp; idx = grp; n = ngrp;
     }
-    if (t < N) out[t] = sm[t];
 }
-

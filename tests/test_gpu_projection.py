@@ -39,6 +39,31 @@ def test_tensor_core_projection_tiles_and_padding():
     assert np.abs(got_tc - want).max() <= 3e-6 * np.abs(want).max()
 
 
+def test_projection_bench_size_sampled():
+    """The shape bench.py times (16^3x32, 128 eigenvectors x 32 solutions, device arrays): sampled outputs against the oracle's
+    einsum on the matching slices, and the tensor-core kernel against the fp64 kernel on every output."""
+    import torch
+    dims, n_ev, n_sol = inputs.CONFIGS[1]["dims"], 128, 32
+    Lx, Ly, Lz, Lt = dims
+    g = torch.Generator(device="cuda").manual_seed(7)
+    v = torch.view_as_complex(torch.randn((n_ev, Lt, Lz, Ly, Lx, 3, 2), generator=g, device="cuda", dtype=torch.float64))
+    x = torch.view_as_complex(torch.randn((n_sol, Lt, Lz, Ly, Lx, 4, 3, 2), generator=g, device="cuda", dtype=torch.float64))
+    ctx = B.Context(dims)
+    p64 = ctx.project(v, x)
+    ptc = ctx.project(v, x, B.LQ_FP32)
+    ctx.close()
+    scale = p64.abs().max().item()
+    assert (ptc - p64).abs().max().item() <= 3e-6 * scale
+    rng = np.random.default_rng(11)
+    for _ in range(24):
+        t, j, k = int(rng.integers(Lt)), int(rng.integers(n_ev)), int(rng.integers(n_sol))
+        want = oracle.project(v[j:j + 1, t:t + 1].cpu().numpy(), x[k:k + 1, t:t + 1].cpu().numpy())     # [1][4][1][1]
+        got64 = p64[t, :, j, k].cpu().numpy()
+        gottc = ptc[t, :, j, k].cpu().numpy()
+        assert np.abs(got64 - want[0, :, 0, 0]).max() <= 1e-12 * scale
+        assert np.abs(gottc - want[0, :, 0, 0]).max() <= 3e-6 * scale
+
+
 def test_laph_chain_eigensolve_solve_project():
     """Sources built from GPU eigenvectors of one time-slice, propagated by lq_solve, projected back: compared with the same
     chain done by the oracle (dense eigenvectors fix the phases, so the GPU vectors are used for both projections)."""

@@ -404,7 +404,7 @@ def run_big_solve(args, B, device, wl, c, peak, peak_src):
             "e2e": {"value": (t_pack + t_dev + t_unpack) / nrhs, "unit": "s/RHS", "h2d_bytes_per_step": int(b_host.nbytes), "d2h_bytes_per_step": int(x_host.nbytes),
                     "note": "pageable host arrays; pack %.2f s + solve %.2f s + unpack %.2f s" % (t_pack, t_dev, t_unpack)},
             "gpu_launches": int(launches), "clocks": clocks,
-            "roofline": roofline_entry(rA, peak, peak_src), "roofline_kernel_B": roofline_entry(rB, peak, peak_src)}
+            "roofline": roofline_entry(rB, peak, peak_src), "roofline_kernel_A": roofline_entry(rA, peak, peak_src)}
     print(json.dumps(line))
 
 
@@ -583,8 +583,9 @@ def main():
         "e2e": {"value": whole_job_seconds_per_rhs(t_e2e, args.steps, nrhs, world), "unit": "s/RHS", "h2d_bytes_per_step": b_host.numel() * 16, "d2h_bytes_per_step": x_host.numel() * 16},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "roofline": roofline_entry(rA, peak, peak_src, ncu_traffic("x".join(map(str, dims)), rA)),
-        "roofline_kernel_B": roofline_entry(rB, peak, peak_src, ncu_traffic("x".join(map(str, dims)), rB)),
+        # the dominant kernel of the step by device-time share (profiles/r01e_launches_cfg1.md): kernel B 50 %, kernel A 31 %
+        "roofline": roofline_entry(rB, peak, peak_src, ncu_traffic("x".join(map(str, dims)), rB)),
+        "roofline_kernel_A": roofline_entry(rA, peak, peak_src, ncu_traffic("x".join(map(str, dims)), rA)),
     }
     line.update(extras)
     print(json.dumps(line))

@@ -255,17 +255,21 @@ def cpu_dslash_baseline():
 
 
 def time_eigensolve(B, device):
-    """Time-batched Lanczos (SURVEY 8(f) #2) on the configs[1] lattice: lowest 16 eigenpairs of -Laplacian on each of the 32 slices."""
+    """Time-batched Lanczos on the configs[1] lattice: lowest 16 / 64 / 128 eigenpairs of -Laplacian on each of
+    the 32 slices (Chebyshev cut just above the wanted part of the spectrum)."""
     c = inputs.CONFIGS[1]
     ctx = B.Context(c["dims"], device=device)
     ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=18)
-    kw = dict(n_ev=16, m=48, cheb_degree=24, cheb_a=0.5, cheb_b=12.5, tol=1e-9, max_restarts=50, want_vectors=False)
-    ctx.laph_eigensolve(**kw)
-    ev, _, info = ctx.laph_eigensolve(**kw)
+    out = {"lattice": "x".join(map(str, c["dims"])), "cases": []}
+    for n_ev, m, cut in ((16, 48, 0.5), (64, 144, 1.0), (128, 288, 1.6)):
+        kw = dict(n_ev=n_ev, m=m, cheb_degree=24, cheb_a=cut, cheb_b=12.5, tol=1e-9, max_restarts=50, want_vectors=False)
+        ctx.laph_eigensolve(**kw)
+        ev, _, info = ctx.laph_eigensolve(**kw)
+        out["cases"].append({"n_ev": n_ev, "krylov": m, "cheb_degree": 24, "seconds": round(info["seconds"], 4), "restarts": info["restarts"],
+                             "laplacian_applies": info["lap_applies"], "converged": info["converged"],
+                             "max_true_residual": info["max_true_residual"], "eigenvalue_range": [float(ev.min()), float(ev.max())]})
     ctx.close()
-    return {"lattice": "x".join(map(str, c["dims"])), "n_ev": 16, "krylov": 48, "cheb_degree": 24, "seconds": round(info["seconds"], 4),
-            "restarts": info["restarts"], "laplacian_applies": info["lap_applies"], "converged": info["converged"],
-            "max_true_residual": info["max_true_residual"], "eigenvalue_range": [float(ev.min()), float(ev.max())]}
+    return out
 
 
 def time_projection(B, device, peak, shapes=((32, 8), (128, 32)), precs=("f64_fma", "tcgen05_3xtf32"), iters=10):

@@ -190,7 +190,7 @@ int lq_cv_fill_random(lq_ctx* ctx, void* native_out, int nvec, int prec, uint64_
  * largest eigenvalue of A (12 is a bound).  fp64 throughout. */
 typedef struct {
     int n_ev;            /* eigenpairs wanted per time-slice                                          */
-    int m;               /* Krylov space size, n_ev + 2 <= m <= 64                                     */
+    int m;               /* Krylov space size, n_ev + 2 <= m <= 512                                    */
     int cheb_degree;     /* degree of the Chebyshev filter (>= 1)                                      */
     int max_restarts;
     double cheb_a, cheb_b;

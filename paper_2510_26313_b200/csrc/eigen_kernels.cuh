@@ -82,21 +82,27 @@ __global__ void cv_axpbypcz_kernel(SliceGeom g, double* __restrict__ z, double a
         z[e] = alpha * x[e] + beta * y[e] + (gamma != 0.0 ? gamma * z[e] : 0.0);
     }
 }
-// basis rotation: out[c] = sum_i Q[t][i][c] * V[i]  for c < k (real Q from the projected eigenproblem of slice t)
-template <int MMAX>
+// basis rotation: out[c] = sum_i Q[t][i][c] * V[i]  for c < k (real Q from the projected eigenproblem of slice t): a tall-skinny
+// GEMM per slice; one thread = one real element row, 16 output columns per pass (the basis is re-read from L1/L2 once per pass)
 __global__ void slice_rotate_kernel(SliceGeom g, int m, int k, const double* const* __restrict__ V, double* const* __restrict__ out, const double* __restrict__ Q) {
+    constexpr int TC = 16;
     size_t off; int t;
     if (!slice_site(g, (long long)blockIdx.x * blockDim.x + threadIdx.x, off, t)) return;
     const double* q = Q + (size_t)t * m * k;
     for (int j = 0; j < 6; j++) {
-        double in[MMAX];
+        for (int c0 = 0; c0 < k; c0 += TC) {
+            const int nc = min(TC, k - c0);
+            double acc[TC];
 #pragma unroll
-        for (int i = 0; i < MMAX; i++) in[i] = i < m ? V[i][off + j * SB] : 0.0;
-        for (int c = 0; c < k; c++) {
-            double acc = 0.0;
+            for (int cc = 0; cc < TC; cc++) acc[cc] = 0.0;
+            for (int i = 0; i < m; i++) {
+                const double v = V[i][off + j * SB];
+                const double* qi = q + (size_t)i * k + c0;
 #pragma unroll
-            for (int i = 0; i < MMAX; i++) if (i < m) acc += q[i * k + c] * in[i];
-            out[c][off + j * SB] = acc;
+                for (int cc = 0; cc < TC; cc++) if (cc < nc) acc[cc] += qi[cc] * v;
+            }
+#pragma unroll
+            for (int cc = 0; cc < TC; cc++) if (cc < nc) out[c0 + cc][off + j * SB] = acc[cc];
         }
     }
 }

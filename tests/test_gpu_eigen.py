@@ -9,7 +9,8 @@ import oracle  # noqa: E402
 from paper_2510_26313_b200 import binding as B, inputs  # noqa: E402
 
 
-@pytest.mark.parametrize("dims,n_ev,m,deg", [((4, 4, 4, 4), 8, 24, 6), ((6, 4, 4, 2), 5, 16, 8), ((4, 4, 2, 6), 12, 30, 5)])
+@pytest.mark.parametrize("dims,n_ev,m,deg", [((4, 4, 4, 4), 8, 24, 6), ((6, 4, 4, 2), 5, 16, 8), ((4, 4, 2, 6), 12, 30, 5),
+                                              ((4, 4, 4, 2), 70, 110, 6)])          # Krylov space beyond 64: tiled rotation, threaded Ritz step
 def test_lanczos_matches_dense_eigh(dims, n_ev, m, deg):
     U = inputs.make_links(dims, 71, 0.3)
     Lx, Ly, Lz, Lt = dims

@@ -39,6 +39,22 @@ def test_tensor_core_projection_tiles_and_padding():
     assert np.abs(got_tc - want).max() <= 3e-6 * np.abs(want).max()
 
 
+def test_projection_is_bitwise_reproducible():
+    """Both kernels sum in a fixed order (no atomics): two calls on the same inputs return identical bits."""
+    import torch
+    dims, n_ev, n_sol = (8, 8, 8, 4), 40, 12
+    Lx, Ly, Lz, Lt = dims
+    g = torch.Generator(device="cuda").manual_seed(3)
+    v = torch.view_as_complex(torch.randn((n_ev, Lt, Lz, Ly, Lx, 3, 2), generator=g, device="cuda", dtype=torch.float64))
+    x = torch.view_as_complex(torch.randn((n_sol, Lt, Lz, Ly, Lx, 4, 3, 2), generator=g, device="cuda", dtype=torch.float64))
+    ctx = B.Context(dims)
+    for prec in (B.LQ_FP64, B.LQ_FP32):
+        a = ctx.project(v, x, prec)
+        b = ctx.project(v, x, prec)
+        assert torch.equal(torch.view_as_real(a), torch.view_as_real(b))
+    ctx.close()
+
+
 def test_projection_bench_size_sampled():
     """The shape bench.py times (16^3x32, 128 eigenvectors x 32 solutions, device arrays): sampled outputs against the oracle's
     einsum on the matching slices, and the tensor-core kernel against the fp64 kernel on every output."""

@@ -214,7 +214,7 @@ int lq_laph_eigensolve(lq_ctx* ctx, double* evals, void* evecs, int loc, const l
  * (canonical [j][t][z][y][x][colour]) and n_sol solution fields psi (canonical [k][t][z][y][x][spin][colour]), all
  * complex double at `loc`; P: [Lt][4][n_ev][n_sol] complex double at `loc`.  1 <= n_ev <= 1024, 1 <= n_sol <= 64.
  * prec = LQ_FP64: fp64 FMAs (exact to rounding); prec = LQ_FP32: tcgen05 tensor cores, every operand split into two TF32
- * numbers (3xTF32), fp32 accumulation (tensor core over 4 or 8 sites, registers over 256), fp64 sum over the rest:
+ * numbers (3xTF32), fp32 accumulation (tensor core over 4 or 8 sites, registers over the 64..1024 sites of one CTA), fp64 sum over the rest:
  * measured error <= 4e-7 of max |P|; deterministic.  Errors: LQ_EINVAL (bad sizes / precision), LQ_ENOMEM (scratch), LQ_ECUDA (incl. a
  * tensor-core completion barrier that timed out: the kernel never hangs). */
 int lq_project(lq_ctx* ctx, void* P, const void* evecs, int n_ev, const void* sols, int n_sol, int loc, int prec);

@@ -5,7 +5,7 @@
 //   kk = ((site, colour), re|im),  A'[j][kk] = (Re v, Im v),  B'[2n][kk] = (Re psi, Im psi),  B'[2n+1][kk] = (Im psi, -Re psi),
 // so that C'[j][2n] = Re P, C'[j][2n+1] = Im P.  Precision: every fp32 operand is split into two TF32 numbers,
 // x = hi + lo, and three MMAs (lo*hi, hi*lo, hi*hi) are accumulated in the fp32 TMEM accumulator ("3xTF32", ~2^-21 per
-// product) over 16 sites at a time; the 16-site sums are carried in fp64 registers, K is split over CTAs (256 sites each)
+// product) over 16 sites at a time; the 16-site sums are carried in fp64 registers, K is split over CTAs (64 .. 1024 sites each)
 // and the partial sums are added in fp64 in a fixed order.
 // One CTA = 512 threads: all threads load fp64, convert and lay out the operands in shared memory (canonical no-swizzle
 // K-major UMMA layout: 8-row x 16-byte core matrices; lanes are mapped so that a quarter-warp stores one 128-byte core
@@ -15,7 +15,7 @@
 #include "internal.cuh"
 
 namespace {
-constexpr int TM = 128, SITES_PER_CTA = 256, NT = 512;
+constexpr int TM = 128, NT = 512;
 
 __device__ __forceinline__ uint32_t s32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 // shared-memory matrix descriptor (cute::UMMA::SmemDescriptor bit layout): start >> 4, leading byte offset >> 4 at bit 16,
@@ -61,7 +61,7 @@ __device__ __forceinline__ void cp_async16(void* dst, const void* src, bool vali
 }
 
 template <int TN, int SPB, int RING>
-__global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchunk, int n_ev, int n_sol, int j0, int k0,
+__global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchunk, int spc, int n_ev, int n_sol, int j0, int k0,
                                                         const double2* __restrict__ V, const double2* __restrict__ X, float* __restrict__ partial, int* __restrict__ err) {
     using Sh = TcShape<TN, SPB, RING>;
     constexpr int KB = Sh::KB, NCH = Sh::NCH;
@@ -89,7 +89,7 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
     asm volatile("tcgen05.fence::after_thread_sync;");
     const uint32_t tmem = *tptr;
     const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TN >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);   // F32 acc, TF32 x TF32, K-major
-    const int s_begin = ch * SITES_PER_CTA, s_end = min(S3, s_begin + SITES_PER_CTA);
+    const int s_begin = ch * spc, s_end = min(S3, s_begin + spc);          // spc = sites per CTA (a multiple of 8)
     const int nst = (s_end - s_begin + SPB - 1) / SPB;
     const int nj = min(TM, n_ev - j0), nk = min(TN / 8, n_sol - k0);
     const double2* Vt = V + ((size_t)j0 * Lt + t) * S3 * 3;    // row r: + r * Lt * S3 * 3
@@ -266,7 +266,21 @@ __global__ void project_tc_final_kernel(int Lt, int nchunk, int n_ev, int n_sol,
 
 template <int TN, int SPB, int RING>
 int project_tc_run(lq_ctx* c, int Lt, int S3, int n_ev, int n_sol, const double* dev_V, const double* dev_X, double* dev_P) {
-    const int nchunk = (S3 + SITES_PER_CTA - 1) / SITES_PER_CTA;
+    // K split: spc sites per CTA (multiple of 8), chosen among 64 .. 1024 to minimise (waves of CTAs over the SMs) x (stages per
+    // CTA): with one CTA per SM the last wave otherwise idles up to half of the machine (16^3x32: 512 CTAs of 256 sites = 3.5
+    // waves on 148 SMs -> 288 CTAs of 456 sites = 1.95 waves)
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    int spc = std::min(256, S3);
+    {
+        long long best = -1;
+        for (int cand = 64; cand <= 1024 && cand <= S3; cand += 8) {
+            const long long nch = (S3 + cand - 1) / cand, waves = ((long long)Lt * nch + sms - 1) / sms;
+            const long long cost = waves * ((cand + SPB - 1) / SPB + 3);       // + a few stage-times of prologue / epilogue per CTA
+            if (best < 0 || cost < best) { best = cost; spc = cand; }
+        }
+    }
+    const int nchunk = (S3 + spc - 1) / spc;
     const size_t smem = TcShape<TN, SPB, RING>::SMEM;
     static_assert(TcShape<TN, SPB, RING>::SMEM <= 232448, "shared memory per CTA");
     static bool configured = false;
@@ -278,7 +292,7 @@ int project_tc_run(lq_ctx* c, int Lt, int S3, int n_ev, int n_sol, const double*
     int rc = 0;
     for (int j0 = 0; j0 < n_ev && rc == 0; j0 += TM)
         for (int k0 = 0; k0 < n_sol && rc == 0; k0 += TN / 8) {
-            project_tc_kernel<TN, SPB, RING><<<Lt * nchunk, NT, smem, c->stream>>>(Lt, S3, nchunk, n_ev, n_sol, j0, k0, (const double2*)dev_V, (const double2*)dev_X, partial, d_err);
+            project_tc_kernel<TN, SPB, RING><<<Lt * nchunk, NT, smem, c->stream>>>(Lt, S3, nchunk, spc, n_ev, n_sol, j0, k0, (const double2*)dev_V, (const double2*)dev_X, partial, d_err);
             const int nj = std::min(TM, n_ev - j0), nk = std::min(TN / 8, n_sol - k0);
             project_tc_final_kernel<<<(Lt * nj * nk * 4 + 127) / 128, 128, 0, c->stream>>>(Lt, nchunk, n_ev, n_sol, j0, k0, TN, partial, (double2*)dev_P);
             c->launches += 2;

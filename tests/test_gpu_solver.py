@@ -157,3 +157,22 @@ def test_restart_and_reliable_update_variants(keep_direction):
 
 
 test_restart_and_reliable_update_variants.iters = {}
+
+
+def test_config1_full_size_bench_configuration():
+    """configs[1] itself (16^3x32, 8 LapH-diluted RHS) in the launch configuration bench.py times (fp32 inner CG, delta 1e-4, poll every
+    4 iterations, CUDA-graph replay, reliable updates): the oracle recomputes the true residual of every RHS with its full M, and
+    one solution is compared with the oracle's own fp64 CG."""
+    cfg = inputs.CONFIGS[1]
+    dims, nrhs = cfg["dims"], cfg["nrhs"]
+    ctx, orc = setup(dims, cfg["gauge_seed"], cfg["eps"], cfg["kappa"], cfg["csw"])
+    b = inputs.laph_sources(dims, nrhs, cfg["n_t"], cfg["source_seed"])
+    x, info = ctx.solve(b, tol=cfg["tol"], inner_prec=B.LQ_FP32, delta=1e-4, check_every=4, use_graph=True, keep_direction=True)
+    ctx.close()
+    assert info["converged"], info
+    res = true_residuals(orc, x, b)
+    assert np.all(res <= cfg["tol"]), res
+    assert np.allclose(res, info["true_rel_residual"], rtol=1e-3, atol=cfg["tol"] * 1e-3)
+    k = 5
+    xo, _, _ = oracle.solve_eo(dims, orc.U, orc.A, orc.Ainv, cfg["kappa"], b[k], cfg["tol"] * 1e-2)
+    assert rel_err(x[k], xo.reshape(x[k].shape)) <= 50 * cfg["tol"]

@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
     constexpr int A_PIECES = TM * SPB * 3, B_PIECES = (TN / 8) * SPB * 12;   // 16-byte pieces per raw stage
     constexpr int A_TASKS = TM * NCH, B_TASKS = (TN / 8) * 4 * NCH;          // float4 conversion tasks per stage
     constexpr int COLS = TN / 4;                               // accumulator columns per warp (4 column groups x 4 lane quadrants)
-    static_assert(NCH % 2 == 0 && 2 * TN <= 512, "stage shape");
+    static_assert(NCH % 2 == 0 && 2 * TN <= 512 && A_TASKS % 32 == 0, "stage shape");
     extern __shared__ __align__(1024) unsigned char smem[];
     float4* sAh = (float4*)smem;               // [NCH][TM/8][8] x 16 bytes
     float4* sAl = sAh + TM * NCH;
@@ -128,28 +128,32 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
         }
         asm volatile("cp.async.commit_group;" ::: "memory");    // one group per call, also when empty: uniform counting
     };
-    // conversion tasks: raw byte offset(s) in the slot and float4 index in the operand tile (~0: no task)
-    constexpr int NTA = (A_TASKS + NT - 1) / NT, NTB = (B_TASKS + NT - 1) / NT;
-    uint32_t rawA[NTA], opA[NTA], rawB0[NTB], rawB1[NTB], opB[NTB];
+    // conversion tasks: the A' tasks followed by the B' tasks form one list dealt round-robin to the threads (every thread gets
+    // the same number, +-1); per task: the byte offsets of its two raw complex numbers in the slot, the float4 index in the
+    // operand tile, and its kind (0 none, 1 A', 2 B'; uniform inside a warp because A_TASKS is a multiple of 32)
+    constexpr int NTK = (A_TASKS + B_TASKS + NT - 1) / NT;
+    uint32_t raw0[NTK], raw1[NTK], op[NTK];
+    int kind[NTK];
 #pragma unroll
-    for (int k = 0; k < NTA; k++) {
-        // unit = 16 rows x 2 chunks; lane = (row % 8, chunk % 2, (row / 8) % 2): a quarter-warp reads 8 raw rows without bank
-        // conflicts and stores one 128-byte core-matrix row group
-        const int q = tid + k * NT, unit = q >> 5, r = ((unit / (NCH / 2)) * 2 + (lane >> 4)) * 8 + (lane & 7), chunk = (unit % (NCH / 2)) * 2 + ((lane >> 3) & 1);
-        rawA[k] = (uint32_t)(r * Sh::A_STRIDE + chunk * 32);
-        opA[k] = q < A_TASKS ? (uint32_t)chunk_index<TM>(r, chunk) : 0xFFFFFFFFu;
-    }
-#pragma unroll
-    for (int k = 0; k < NTB; k++) {
-        // rows 2n, 2n+1 with n = (solution, spin); lane = (spin, solution % 2, chunk % 4): a quarter-warp reads two solutions x four
-        // spins of one chunk (conflict-free with the padded solution stride) and, odd solutions storing the odd row first, covers
-        // the 8 rows of a core matrix in each store
-        const int q = tid + k * NT, a = q & 3, chunk = (q >> 3) % NCH, kl = 2 * ((q >> 3) / NCH) + ((q >> 2) & 1);
-        const int e0 = 2 * chunk, e1 = e0 + 1;
-        const uint32_t base = (uint32_t)(Sh::A_RAW + Sh::b_offset(kl) + a * 48);
-        rawB0[k] = base + ((e0 / 3) * 12 + e0 % 3) * 16;
-        rawB1[k] = base + ((e1 / 3) * 12 + e1 % 3) * 16;
-        opB[k] = q < B_TASKS ? (uint32_t)chunk_index<TN>(2 * (kl * 4 + a), chunk) : 0xFFFFFFFFu;
+    for (int k = 0; k < NTK; k++) {
+        const int g = tid + k * NT;
+        if (g < A_TASKS) {
+            // unit = 16 rows x 2 chunks; lane = (row % 8, chunk % 2, (row / 8) % 2): a quarter-warp reads 8 raw rows without bank
+            // conflicts and stores one 128-byte core-matrix row group
+            const int unit = g >> 5, r = ((unit / (NCH / 2)) * 2 + (lane >> 4)) * 8 + (lane & 7), chunk = (unit % (NCH / 2)) * 2 + ((lane >> 3) & 1);
+            raw0[k] = (uint32_t)(r * Sh::A_STRIDE + chunk * 32); raw1[k] = raw0[k] + 16;
+            op[k] = (uint32_t)chunk_index<TM>(r, chunk); kind[k] = 1;
+        } else if (g < A_TASKS + B_TASKS) {
+            // rows 2n, 2n+1 with n = (solution, spin); lane = (spin, solution % 2, chunk % 4): a quarter-warp reads two solutions x
+            // four spins of one chunk (conflict-free with the pair layout) and, odd solutions storing the odd row first, covers
+            // the 8 rows of a core matrix in each store
+            const int q = g - A_TASKS, a = q & 3, chunk = (q >> 3) % NCH, kl = 2 * ((q >> 3) / NCH) + ((q >> 2) & 1);
+            const int e0 = 2 * chunk, e1 = e0 + 1;
+            const uint32_t base = (uint32_t)(Sh::A_RAW + Sh::b_offset(kl) + a * 48);
+            raw0[k] = base + ((e0 / 3) * 12 + e0 % 3) * 16;
+            raw1[k] = base + ((e1 / 3) * 12 + e1 % 3) * 16;
+            op[k] = (uint32_t)chunk_index<TN>(2 * (kl * 4 + a), chunk); kind[k] = 2;
+        } else { raw0[k] = raw1[k] = op[k] = 0; kind[k] = 0; }
     }
     auto flush_bank = [&](int bank, float* acc) {
 #pragma unroll
@@ -188,33 +192,28 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
         if (i > 0 && !wait_mma((uint32_t)((i - 1) & 1))) { ok = false; break; }   // operand tiles released by the MMAs of stage i-1
         const unsigned char* slot = raw + (size_t)(i % RING) * Sh::RAW;
 #pragma unroll
-        for (int k = 0; k < NTA; k++) {
-            if (opA[k] == 0xFFFFFFFFu) continue;
-            const double2* src = (const double2*)(slot + rawA[k]);
-            const double2 v0 = src[0], v1 = src[1];
-            float4 h, l;
-            split4(make_float4((float)v0.x, (float)v0.y, (float)v1.x, (float)v1.y), h, l);
-            sAh[opA[k]] = h; sAl[opA[k]] = l;
-        }
-#pragma unroll
-        for (int k = 0; k < NTB; k++) {
-            if (opB[k] == 0xFFFFFFFFu) continue;
-            const double2 x0 = *(const double2*)(slot + rawB0[k]), x1 = *(const double2*)(slot + rawB1[k]);
+        for (int k = 0; k < NTK; k++) {
+            if (kind[k] == 0) continue;
+            const double2 x0 = *(const double2*)(slot + raw0[k]), x1 = *(const double2*)(slot + raw1[k]);
             float4 h, l;
             split4(make_float4((float)x0.x, (float)x0.y, (float)x1.x, (float)x1.y), h, l);
-            const float4 h1 = make_float4(h.y, -h.x, h.w, -h.z), l1 = make_float4(l.y, -l.x, l.w, -l.z);
-            // odd solutions store the odd row first (selects, not branches: one store instruction must cover all 8 rows)
-            const bool odd = (lane >> 2) & 1;
-            const uint32_t i0 = opB[k] + (odd ? 1u : 0u), i1 = opB[k] + (odd ? 0u : 1u);
-            const float4 ha = odd ? h1 : h, hb = odd ? h : h1, la = odd ? l1 : l, lb = odd ? l : l1;
-            sBh[i0] = ha; sBl[i0] = la;
-            sBh[i1] = hb; sBl[i1] = lb;
+            if (kind[k] == 1) {
+                sAh[op[k]] = h; sAl[op[k]] = l;
+            } else {
+                const float4 h1 = make_float4(h.y, -h.x, h.w, -h.z), l1 = make_float4(l.y, -l.x, l.w, -l.z);
+                // odd solutions store the odd row first (selects, not branches: one store instruction must cover all 8 rows)
+                const bool odd = (lane >> 2) & 1;
+                const uint32_t i0 = op[k] + (odd ? 1u : 0u), i1 = op[k] + (odd ? 0u : 1u);
+                const float4 ha = odd ? h1 : h, hb = odd ? h : h1, la = odd ? l1 : l, lb = odd ? l : l1;
+                sBh[i0] = ha; sBl[i0] = la;
+                sBh[i1] = hb; sBl[i1] = lb;
+            }
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;");
         __syncthreads();                                         // operands visible; raw slot i % RING is free again
         asm volatile("tcgen05.fence::after_thread_sync;");
-        if (tid == 0) {
+        if (tid == NT - 32) {
             const uint32_t d = tmem + (i & 1) * TN;
 #pragma unroll 1
             for (int s = 0; s < KB / 8; s++) {

@@ -40,8 +40,9 @@ __device__ __forceinline__ void mma_tf32(uint32_t tmem, uint64_t da, uint64_t db
 
 // TN = accumulator columns (8 per solution), SPB = sites per stage (K = 6 SPB real terms), RING = raw stages in flight.
 // Pipeline per stage i: cp.async brings the fp64 fields of stage i+RING into a raw shared-memory ring (no registers held in
-// flight); all threads convert raw stage i into the operand tiles once the MMAs of stage i-1 have released them; thread 0
-// issues the MMAs of stage i into TMEM bank i%2; the accumulator of stage i-1 (other bank) is then added into registers
+// flight; each thread's copies arrive on the slot's mbarrier, cp.async.mbarrier.arrive.noinc); all threads convert raw stage i
+// into the operand tiles once the MMAs of stage i-1 have released them; one CTA barrier; one thread of the last warp issues
+// the MMAs of stage i into TMEM bank i%2; the accumulator of stage i-1 (other bank) is then added into registers
 // while the tensor core works.  The tensor core adds into its fp32 accumulator with truncation, so its chains are kept to
 // one stage and the running sum is carried in registers (round to nearest).
 template <int TN, int SPB, int RING>
@@ -76,10 +77,15 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
     float4* sBl = sBh + TN * NCH;
     unsigned char* raw = smem + Sh::OPER;      // RING x { A rows [TM][A_STRIDE], B [TN/8][SPB][12] double2 }
     uint64_t* bar = (uint64_t*)(raw + (size_t)RING * Sh::RAW);
-    uint32_t* tptr = (uint32_t*)(bar + 1);
+    uint64_t* full = bar + 1;                  // full[slot]: every thread's copies of the raw stage in this slot have landed
+    uint32_t* tptr = (uint32_t*)(full + RING);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int t = blockIdx.x / nchunk, ch = blockIdx.x - t * nchunk;
-    if (tid == 0) { asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(s32(bar))); asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(s32(bar)));
+        for (int k = 0; k < RING; k++) asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(s32(full + k)), "r"(NT));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(s32(tptr)), "n"(2 * TN));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
@@ -126,7 +132,9 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
             for (int k = 0; k < NPB; k++)
                 if (dstB[k] != 0xFFFFFFFFu) cp_async16(slot + dstB[k], srcB[k] ? srcB[k] + (size_t)st * (SPB * 12) : X, srcB[k] != nullptr);
         }
-        asm volatile("cp.async.commit_group;" ::: "memory");    // one group per call, also when empty: uniform counting
+        // the copies of this thread arrive on the slot's mbarrier when they complete (count = all NT threads): the consumers wait
+        // on the barrier, no wait_group + CTA barrier
+        if (st < nst) asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(s32(full + st % RING)) : "memory");
     };
     // conversion tasks: the A' tasks followed by the B' tasks form one list dealt round-robin to the threads (every thread gets
     // the same number, +-1); per task: the byte offsets of its two raw complex numbers in the slot, the float4 index in the
@@ -169,13 +177,17 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
         asm volatile("tcgen05.fence::before_thread_sync;");
     };
     // every thread waits for the MMAs of one stage (bounded spin: a fault must not hang the GPU)
-    auto wait_mma = [&](uint32_t parity) {
+    auto wait_bar = [&](uint64_t* b, uint32_t parity) {
         bool done = false;
         for (int spin = 0; spin < 20000000 && !done; spin++) {
             uint32_t r;
-            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(r) : "r"(s32(bar)), "r"(parity) : "memory");
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }" : "=r"(r) : "r"(s32(b)), "r"(parity) : "memory");
             done = r != 0;
         }
+        return done;
+    };
+    auto wait_mma = [&](uint32_t parity) {
+        const bool done = wait_bar(bar, parity);
         asm volatile("tcgen05.fence::after_thread_sync;");
         return done;
     };
@@ -187,8 +199,7 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
 #pragma unroll
     for (int st = 0; st < RING; st++) fetch_stage(st);
     for (int i = 0; i < nst; i++) {
-        asm volatile("cp.async.wait_group %0;" ::"n"(RING - 1) : "memory");
-        __syncthreads();                                         // raw stage i is complete for every thread
+        if (!wait_bar(full + i % RING, (uint32_t)((i / RING) & 1))) { ok = false; break; }       // raw stage i has landed (all threads' copies)
         if (i > 0 && !wait_mma((uint32_t)((i - 1) & 1))) { ok = false; break; }   // operand tiles released by the MMAs of stage i-1
         const unsigned char* slot = raw + (size_t)(i % RING) * Sh::RAW;
 #pragma unroll
@@ -228,7 +239,7 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
         fetch_stage(i + RING);
         if (i > 0) flush_bank((i - 1) & 1, acc);                 // overlaps the MMAs of stage i (other bank)
     }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    asm volatile("cp.async.wait_all;" ::: "memory");
     if (ok && nst > 0) {
         ok = wait_mma((uint32_t)((nst - 1) & 1));
         if (ok) flush_bank((nst - 1) & 1, acc);

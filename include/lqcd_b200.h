@@ -142,6 +142,8 @@ int lq_gather_sites(lq_ctx* ctx, double* out, const void* native_parity_block, i
                     long long nsites, const int* sites_xyzt);
 
 /* ---- batched mixed-precision solve (rows a2, a6-a11) ---------------------------------------------- */
+enum { LQ_ALG_CGNR = 0, LQ_ALG_BICGSTAB = 1 };
+
 typedef struct {
     double tol;          /* target ||b - M x|| / ||b|| per RHS (full system, fp64)                   */
     int max_outer;       /* cap on fp64 defect-correction cycles                                      */
@@ -152,7 +154,9 @@ typedef struct {
     int use_graph;       /* 1: replay the inner iteration body as a CUDA graph                        */
     int keep_direction;  /* 1: reliable updates (SURVEY 8(c.2) reading #11, 8(f) #3): after each fp64 residual refresh the
                             CG search direction is kept, p <- z_new + c (p - z_old), instead of restarting at p = z   */
-    int reserved;        /* must be 0                                                                  */
+    int algorithm;       /* inner solver: LQ_ALG_CGNR (0, default) or LQ_ALG_BICGSTAB (1): batched BiCGStab on Mhat
+                            itself with complex per-RHS scalars, 2 Mhat applications per iteration; no CUDA graph,
+                            keep_direction ignored                                                       */
 } lq_solve_param;
 
 typedef struct {
@@ -167,8 +171,8 @@ typedef struct {
 
 /* Solves M x = b for nrhs independent right-hand sides (no block-Krylov coupling).  b, x: full-lattice
  * complex double, CANONICAL at `loc`, or NATIVE LQ_FP64 device buffers.  x is output only (zero start).
- * Even-odd preconditioned CGNR in inner_prec inside an fp64 restart defect correction
- * (SURVEY 8(c.1) step 11).  Returns LQ_ENOTCONVERGED (x, info still valid) if any RHS misses tol. */
+ * Even-odd preconditioned CGNR (or, param->algorithm = LQ_ALG_BICGSTAB, batched BiCGStab on Mhat) in inner_prec inside an
+ * fp64 defect correction.  Returns LQ_ENOTCONVERGED (x, info still valid) if any RHS misses tol. */
 int lq_solve(lq_ctx* ctx, void* x, const void* b, int nrhs, int loc, int layout, const lq_solve_param* param, lq_solve_info* info);
 
 /* ---- 3-d gauge-covariant Laplacian ------------------------

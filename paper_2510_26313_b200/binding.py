@@ -14,6 +14,7 @@ import numpy as np
 HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.path.join(HERE, "liblqcd_b200.so")
 
+LQ_ALG_CGNR, LQ_ALG_BICGSTAB = 0, 1
 LQ_FP64, LQ_FP32, LQ_HALF = 0, 1, 2
 LQ_HOST, LQ_DEVICE = 0, 1
 LQ_CANONICAL, LQ_NATIVE = 0, 1
@@ -32,7 +33,7 @@ EXPORTS = ["lq_create", "lq_destroy", "lq_last_error", "lq_set_allocator", "lq_l
 class SolveParam(ctypes.Structure):
     _fields_ = [("tol", ctypes.c_double), ("max_outer", ctypes.c_int), ("max_inner", ctypes.c_int), ("inner_prec", ctypes.c_int),
                 ("delta", ctypes.c_double), ("check_every", ctypes.c_int), ("use_graph", ctypes.c_int),
-                ("keep_direction", ctypes.c_int), ("reserved", ctypes.c_int)]
+                ("keep_direction", ctypes.c_int), ("algorithm", ctypes.c_int)]
 
 
 class EigParam(ctypes.Structure):
@@ -300,11 +301,11 @@ class Context:
     # ------------------------------------------------------------------ solve
     def solve(self, b, tol: float, inner_prec: int = LQ_FP32, delta: float = 1e-3, max_outer: int = 50, max_inner: int = 2000,
               check_every: int = 10, use_graph: bool = False, x_out=None, native: bool = False, nrhs: int | None = None,
-              keep_direction: bool = True):
+              keep_direction: bool = True, algorithm: int = 0):
         """Solves M x = b.  b: canonical complex128 numpy / torch array (host or device), or a native fp64 device
         buffer when native=True (then nrhs is required).  Returns (x, info dict)."""
         self._enter()
-        prm = SolveParam(tol, max_outer, max_inner, inner_prec, delta, check_every, int(use_graph), int(keep_direction), 0)
+        prm = SolveParam(tol, max_outer, max_inner, inner_prec, delta, check_every, int(use_graph), int(keep_direction), int(algorithm))
         info = SolveInfo()
         if native:
             x = x_out if x_out is not None else self.native_empty(nrhs, LQ_FP64)

@@ -230,3 +230,208 @@ int blas_copy(lq_ctx* c, int prec, int nrhs, void* dst, const void* src) {
     LQ_CUDA(c, cudaMemcpyAsync(dst, src, parity_bytes(c->g, nrhs, prec), cudaMemcpyDeviceToDevice, c->stream));
     return 0;
 }
+
+// ---- batched BiCGStab block-BLAS (solver variant): per-RHS COMPLEX Krylov scalars ------------------------
+// Component j of a site is (re, im) = (2c, 2c+1), c = 3 spin + colour.  Device scalars are kept as raw sums,
+//   rho[2][LQ_MAX_RHS] = <rhat0, r>,  c1[3][..] = (<rhat0, v>, ||rhat0||^2),  d2[3][..] = (<t, s>, ||t||^2),
+// and every kernel derives alpha = rho / c1, omega = <t, s> / ||t||^2, beta = (rho' / rho)(alpha / omega) from them (zero when a
+// denominator is zero: converged or zero right-hand sides stay put).  Two right-hand sides per thread (registers).
+namespace {
+struct Cplx { double re, im; };
+__device__ __forceinline__ Cplx cdiv(double ar, double ai, double br, double bi) {
+    const double d = br * br + bi * bi;
+    if (!(d > 0.0)) return Cplx{0.0, 0.0};
+    return Cplx{(ar * br + ai * bi) / d, (ai * br - ar * bi) / d};
+}
+__device__ __forceinline__ Cplx cmul(Cplx a, Cplx b) { return Cplx{a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+__device__ __forceinline__ Cplx bicg_alpha(const double* rho, const double* c1, int k) { return cdiv(rho[k], rho[LQ_MAX_RHS + k], c1[k], c1[LQ_MAX_RHS + k]); }
+__device__ __forceinline__ Cplx bicg_omega(const double* d2, int k) {
+    const double tt = d2[2 * LQ_MAX_RHS + k];
+    return tt > 0.0 ? Cplx{d2[k] / tt, d2[LQ_MAX_RHS + k] / tt} : Cplx{0.0, 0.0};
+}
+// y[c] (+)= s * x[c] for the 12 complex components of VW right-hand sides
+template <class T, int VW, bool ACCUM>
+__device__ __forceinline__ void caxpy_regs(const T (&sr)[VW], const T (&si)[VW], const T (&x)[24][VW], T (&y)[24][VW]) {
+#pragma unroll
+    for (int cc = 0; cc < 12; cc++)
+#pragma unroll
+        for (int k = 0; k < VW; k++) {
+            const T xr = x[2 * cc][k], xi = x[2 * cc + 1][k];
+            const T pr = sr[k] * xr - si[k] * xi, pi = sr[k] * xi + si[k] * xr;
+            if (ACCUM) { y[2 * cc][k] += pr; y[2 * cc + 1][k] += pi; } else { y[2 * cc][k] = pr; y[2 * cc + 1][k] = pi; }
+        }
+}
+}  // namespace
+
+// out = (Re <a, b>, Im <a, b>, ||a||^2) per RHS, <a, b> = sum conj(a) b
+template <class S, int VW, int R>
+__global__ void cdot3_kernel(BlasGeom bg, SView<S> a, SView<S> b, double* partials, unsigned int* counter, double* out) {
+    using T = typename S::comp_t;
+    BlasIdx<VW, R> ix(bg.g, bg.G);
+    double part[3][VW];
+#pragma unroll
+    for (int q = 0; q < 3; q++)
+#pragma unroll
+        for (int k = 0; k < VW; k++) part[q][k] = 0.0;
+    if (ix.valid) {
+        T x[24][VW], y[24][VW];
+        load_site_regs<S, VW, R>(a.d + ix.own, S::has_norm ? a.n + ix.own_n : nullptr, x);
+        load_site_regs<S, VW, R>(b.d + ix.own, S::has_norm ? b.n + ix.own_n : nullptr, y);
+#pragma unroll
+        for (int cc = 0; cc < 12; cc++)
+#pragma unroll
+            for (int k = 0; k < VW; k++) {
+                const double ar = x[2 * cc][k], ai = x[2 * cc + 1][k], br = y[2 * cc][k], bi = y[2 * cc + 1][k];
+                part[0][k] += ar * br + ai * bi; part[1][k] += ar * bi - ai * br; part[2][k] += ar * ar + ai * ai;
+            }
+    }
+    reduce_multi<3, VW, R>(part, bg.N, bg.G, partials, counter, out);
+}
+
+// s = r - alpha v
+template <class S, int VW, int R>
+__global__ void bicg_s_kernel(BlasGeom bg, SView<S> s, SView<S> r, SView<S> v, const double* __restrict__ rho, const double* __restrict__ c1) {
+    using T = typename S::comp_t;
+    BlasIdx<VW, R> ix(bg.g, bg.G);
+    if (!ix.valid) return;
+    T ar[VW], ai[VW];
+#pragma unroll
+    for (int k = 0; k < VW; k++) { const Cplx a = bicg_alpha(rho, c1, ix.rhs0 + k); ar[k] = (T)(-a.re); ai[k] = (T)(-a.im); }
+    T x[24][VW], y[24][VW];
+    load_site_regs<S, VW, R>(r.d + ix.own, S::has_norm ? r.n + ix.own_n : nullptr, y);
+    load_site_regs<S, VW, R>(v.d + ix.own, S::has_norm ? v.n + ix.own_n : nullptr, x);
+    caxpy_regs<T, VW, true>(ar, ai, x, y);
+    store_site_regs<S, VW, R>(s.d + ix.own, S::has_norm ? s.n + ix.own_n : nullptr, y);
+}
+
+// e += alpha p + omega s ; r = s - omega t ; out = (<rhat0, r>, ||rhat0||^2 (unused), ...) -> (Re, Im <rhat0, r>, ||r||^2)
+template <class S, int VW, int R>
+__global__ void bicg_xr_kernel(BlasGeom bg, SView<S> e, SView<S> r, SView<S> p, SView<S> s, SView<S> tv, SView<S> rhat,
+                               const double* __restrict__ rho, const double* __restrict__ c1, const double* __restrict__ d2,
+                               double* partials, unsigned int* counter, double* out) {
+    using T = typename S::comp_t;
+    BlasIdx<VW, R> ix(bg.g, bg.G);
+    double part[3][VW];
+#pragma unroll
+    for (int q = 0; q < 3; q++)
+#pragma unroll
+        for (int k = 0; k < VW; k++) part[q][k] = 0.0;
+    if (ix.valid) {
+        T ar[VW], ai[VW], wr[VW], wi[VW], mwr[VW], mwi[VW];
+#pragma unroll
+        for (int k = 0; k < VW; k++) {
+            const Cplx a = bicg_alpha(rho, c1, ix.rhs0 + k), w = bicg_omega(d2, ix.rhs0 + k);
+            ar[k] = (T)a.re; ai[k] = (T)a.im; wr[k] = (T)w.re; wi[k] = (T)w.im; mwr[k] = (T)(-w.re); mwi[k] = (T)(-w.im);
+        }
+        T x[24][VW], y[24][VW], z[24][VW];
+        load_site_regs<S, VW, R>(s.d + ix.own, S::has_norm ? s.n + ix.own_n : nullptr, x);       // x = s
+        load_site_regs<S, VW, R>(e.d + ix.own, S::has_norm ? e.n + ix.own_n : nullptr, y);       // y = e
+        caxpy_regs<T, VW, true>(wr, wi, x, y);                                                    // e += omega s
+        load_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, z);       // z = p
+        caxpy_regs<T, VW, true>(ar, ai, z, y);                                                    // e += alpha p
+        store_site_regs<S, VW, R>(e.d + ix.own, S::has_norm ? e.n + ix.own_n : nullptr, y);
+        load_site_regs<S, VW, R>(tv.d + ix.own, S::has_norm ? tv.n + ix.own_n : nullptr, z);     // z = t
+        caxpy_regs<T, VW, true>(mwr, mwi, z, x);                                                  // x = s - omega t = r
+        store_site_regs<S, VW, R>(r.d + ix.own, S::has_norm ? r.n + ix.own_n : nullptr, x);
+        load_site_regs<S, VW, R>(rhat.d + ix.own, S::has_norm ? rhat.n + ix.own_n : nullptr, z); // z = rhat0
+#pragma unroll
+        for (int cc = 0; cc < 12; cc++)
+#pragma unroll
+            for (int k = 0; k < VW; k++) {
+                const double hr = z[2 * cc][k], hi = z[2 * cc + 1][k], rr = x[2 * cc][k], ri = x[2 * cc + 1][k];
+                part[0][k] += hr * rr + hi * ri; part[1][k] += hr * ri - hi * rr; part[2][k] += rr * rr + ri * ri;
+            }
+    }
+    reduce_multi<3, VW, R>(part, bg.N, bg.G, partials, counter, out);
+}
+
+// p = r + beta (p - omega v), beta = (rho_new / rho)(alpha / omega)
+template <class S, int VW, int R>
+__global__ void bicg_p_kernel(BlasGeom bg, SView<S> p, SView<S> r, SView<S> v, const double* __restrict__ rho, const double* __restrict__ rho_new,
+                              const double* __restrict__ c1, const double* __restrict__ d2) {
+    using T = typename S::comp_t;
+    BlasIdx<VW, R> ix(bg.g, bg.G);
+    if (!ix.valid) return;
+    T br[VW], bi[VW], mwr[VW], mwi[VW];
+#pragma unroll
+    for (int k = 0; k < VW; k++) {
+        const int rh = ix.rhs0 + k;
+        const Cplx a = bicg_alpha(rho, c1, rh), w = bicg_omega(d2, rh);
+        const Cplx q1 = cdiv(rho_new[rh], rho_new[LQ_MAX_RHS + rh], rho[rh], rho[LQ_MAX_RHS + rh]), q2 = cdiv(a.re, a.im, w.re, w.im);
+        const Cplx b = cmul(q1, q2);
+        br[k] = (T)b.re; bi[k] = (T)b.im; mwr[k] = (T)(-w.re); mwi[k] = (T)(-w.im);
+    }
+    T x[24][VW], y[24][VW], z[24][VW];
+    load_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, y);       // y = p
+    load_site_regs<S, VW, R>(v.d + ix.own, S::has_norm ? v.n + ix.own_n : nullptr, x);       // x = v
+    caxpy_regs<T, VW, true>(mwr, mwi, x, y);                                                  // y = p - omega v
+    load_site_regs<S, VW, R>(r.d + ix.own, S::has_norm ? r.n + ix.own_n : nullptr, z);       // z = r
+    caxpy_regs<T, VW, true>(br, bi, y, z);                                                    // z = r + beta y
+    store_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, z);
+}
+
+// two right-hand sides per thread for every precision: (2,4) (2,2) (1,1)
+#define VW2_DISPATCH(L, S, KERNEL, SMEM, ...)                                                  \
+    do {                                                                                       \
+        if (L.R == 4) KERNEL<S, 2, 4><<<L.grid, L.block, SMEM, c->stream>>>(__VA_ARGS__);      \
+        else if (L.R == 2) KERNEL<S, 2, 2><<<L.grid, L.block, SMEM, c->stream>>>(__VA_ARGS__); \
+        else KERNEL<S, 1, 1><<<L.grid, L.block, SMEM, c->stream>>>(__VA_ARGS__);               \
+    } while (0)
+#define PREC_SWITCH(FN, ...)                                   \
+    do {                                                       \
+        if (prec == LQ_FP64) return FN<F64>(c, __VA_ARGS__);   \
+        if (prec == LQ_FP32) return FN<F32>(c, __VA_ARGS__);   \
+        return FN<H16>(c, __VA_ARGS__);                        \
+    } while (0)
+
+template <class S> static int cdot3_t(lq_ctx* c, int nrhs, const void* a, const void* b, double* d_out) {
+    Launch L; LQ_TRY(plan(c, nrhs, 2, L));
+    LQ_TRY(ensure_partials(c, (size_t)L.grid * nrhs * 3));
+    SView<S> va = make_view<S>(c->g, const_cast<void*>(a), nrhs, 0), vb = make_view<S>(c->g, const_cast<void*>(b), nrhs, 0);
+    VW2_DISPATCH(L, S, cdot3_kernel, L.smem, L.bg, va, vb, c->red_partials, c->red_counter, d_out);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
+}
+int blas_cdot3(lq_ctx* c, int prec, int nrhs, const void* a, const void* b, double* d_out) { PREC_SWITCH(cdot3_t, nrhs, a, b, d_out); }
+
+template <class S> static int bicg_s_t(lq_ctx* c, int nrhs, void* s, const void* r, const void* v, const double* rho, const double* c1) {
+    Launch L; LQ_TRY(plan(c, nrhs, 2, L));
+    SView<S> vs = make_view<S>(c->g, s, nrhs, 0), vr = make_view<S>(c->g, const_cast<void*>(r), nrhs, 0), vv = make_view<S>(c->g, const_cast<void*>(v), nrhs, 0);
+    VW2_DISPATCH(L, S, bicg_s_kernel, 0, L.bg, vs, vr, vv, rho, c1);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
+}
+int blas_bicg_s(lq_ctx* c, int prec, int nrhs, void* s, const void* r, const void* v, const double* d_rho, const double* d_c1) { PREC_SWITCH(bicg_s_t, nrhs, s, r, v, d_rho, d_c1); }
+
+template <class S> static int bicg_xr_t(lq_ctx* c, int nrhs, void* e, void* r, const void* p, const void* s, const void* t, const void* rhat,
+                                        const double* rho, const double* c1, const double* d2, double* d_out) {
+    Launch L; LQ_TRY(plan(c, nrhs, 2, L));
+    LQ_TRY(ensure_partials(c, (size_t)L.grid * nrhs * 3));
+    SView<S> ve = make_view<S>(c->g, e, nrhs, 0), vr = make_view<S>(c->g, r, nrhs, 0), vp = make_view<S>(c->g, const_cast<void*>(p), nrhs, 0),
+             vs = make_view<S>(c->g, const_cast<void*>(s), nrhs, 0), vt = make_view<S>(c->g, const_cast<void*>(t), nrhs, 0),
+             vh = make_view<S>(c->g, const_cast<void*>(rhat), nrhs, 0);
+    VW2_DISPATCH(L, S, bicg_xr_kernel, L.smem, L.bg, ve, vr, vp, vs, vt, vh, rho, c1, d2, c->red_partials, c->red_counter, d_out);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
+}
+int blas_bicg_xr(lq_ctx* c, int prec, int nrhs, void* e, void* r, const void* p, const void* s, const void* t, const void* rhat,
+                 const double* d_rho, const double* d_c1, const double* d_d2, double* d_out) {
+    PREC_SWITCH(bicg_xr_t, nrhs, e, r, p, s, t, rhat, d_rho, d_c1, d_d2, d_out);
+}
+
+template <class S> static int bicg_p_t(lq_ctx* c, int nrhs, void* p, const void* r, const void* v, const double* rho, const double* rho_new,
+                                       const double* c1, const double* d2) {
+    Launch L; LQ_TRY(plan(c, nrhs, 2, L));
+    SView<S> vp = make_view<S>(c->g, p, nrhs, 0), vr = make_view<S>(c->g, const_cast<void*>(r), nrhs, 0), vv = make_view<S>(c->g, const_cast<void*>(v), nrhs, 0);
+    VW2_DISPATCH(L, S, bicg_p_kernel, 0, L.bg, vp, vr, vv, rho, rho_new, c1, d2);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
+}
+int blas_bicg_p(lq_ctx* c, int prec, int nrhs, void* p, const void* r, const void* v, const double* d_rho, const double* d_rho_new,
+                const double* d_c1, const double* d_d2) {
+    PREC_SWITCH(bicg_p_t, nrhs, p, r, v, d_rho, d_rho_new, d_c1, d_d2);
+}

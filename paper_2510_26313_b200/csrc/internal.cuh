@@ -44,6 +44,13 @@ int blas_axpy_mixed(lq_ctx* c, int prec, int nrhs, void* y64, const void* e, con
 // r = b - t (fp64), d_out[k] = ||r_k||^2
 int blas_residual(lq_ctx* c, int nrhs, void* r, const void* b, const void* t, double* d_out);
 int blas_copy(lq_ctx* c, int prec, int nrhs, void* dst, const void* src);
+// batched BiCGStab (complex per-RHS scalars kept as raw sums on the device; d_out = 3 x LQ_MAX_RHS doubles)
+int blas_cdot3(lq_ctx* c, int prec, int nrhs, const void* a, const void* b, double* d_out);        // Re <a,b>, Im <a,b>, ||a||^2
+int blas_bicg_s(lq_ctx* c, int prec, int nrhs, void* s, const void* r, const void* v, const double* d_rho, const double* d_c1);
+int blas_bicg_xr(lq_ctx* c, int prec, int nrhs, void* e, void* r, const void* p, const void* s, const void* t, const void* rhat,
+                 const double* d_rho, const double* d_c1, const double* d_d2, double* d_out);       // -> Re, Im <rhat,r>, ||r||^2
+int blas_bicg_p(lq_ctx* c, int prec, int nrhs, void* p, const void* r, const void* v, const double* d_rho, const double* d_rho_new,
+                const double* d_c1, const double* d_d2);
 
 // fill.cu
 int fill_gauge(lq_ctx* c, uint64_t seed, double eps);

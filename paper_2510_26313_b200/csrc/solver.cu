@@ -11,8 +11,9 @@
 struct Workspace {
     int nrhs = 0, prec = -1;
     void *bhat = nullptr, *r = nullptr, *t64 = nullptr, *tmp64 = nullptr;          // fp64, one parity each
-    void *e = nullptr, *z = nullptr, *p = nullptr, *t = nullptr, *q = nullptr, *tmp = nullptr, *rt = nullptr;  // inner precision
+    void *e = nullptr, *z = nullptr, *p = nullptr, *t = nullptr, *q = nullptr, *tmp = nullptr, *rt = nullptr, *s = nullptr;  // inner precision
     double* d_scal = nullptr;                                                       // 8 x LQ_MAX_RHS doubles
+    double* d_bicg = nullptr;                                                       // 12 x LQ_MAX_RHS doubles (BiCGStab sums)
 };
 
 struct WsHolder { lq_ctx* c; Workspace ws; };
@@ -27,7 +28,7 @@ void solver_forget(lq_ctx* c) {
     for (size_t i = 0; i < g_ws.size(); i++) if (g_ws[i].c == c) { g_ws.erase(g_ws.begin() + i); return; }
 }
 static void ws_release(lq_ctx* c, Workspace* w) {
-    void** all[] = {&w->bhat, &w->r, &w->t64, &w->tmp64, &w->e, &w->z, &w->p, &w->t, &w->q, &w->tmp, &w->rt, (void**)&w->d_scal};
+    void** all[] = {&w->bhat, &w->r, &w->t64, &w->tmp64, &w->e, &w->z, &w->p, &w->t, &w->q, &w->tmp, &w->rt, &w->s, (void**)&w->d_scal, (void**)&w->d_bicg};
     for (void** p : all) if (*p) { dev_free(c, *p); *p = nullptr; }
     w->nrhs = 0; w->prec = -1;
 }
@@ -37,10 +38,11 @@ static int ws_prepare(lq_ctx* c, Workspace* w, int nrhs, int prec) {
     const size_t b64 = parity_bytes(c->g, nrhs, LQ_FP64), bin = parity_bytes(c->g, nrhs, prec);
     void** p64[] = {&w->bhat, &w->r, &w->t64, &w->tmp64};
     for (void** p : p64) { *p = dev_alloc(c, b64); if (!*p) return LQ_ENOMEM; }
-    void** pin[] = {&w->e, &w->z, &w->p, &w->t, &w->q, &w->tmp, &w->rt};
+    void** pin[] = {&w->e, &w->z, &w->p, &w->t, &w->q, &w->tmp, &w->rt, &w->s};
     for (void** p : pin) { *p = dev_alloc(c, bin); if (!*p) return LQ_ENOMEM; }
     w->d_scal = (double*)dev_alloc(c, 8 * LQ_MAX_RHS * sizeof(double));
-    if (!w->d_scal) return LQ_ENOMEM;
+    w->d_bicg = (double*)dev_alloc(c, 12 * LQ_MAX_RHS * sizeof(double));
+    if (!w->d_scal || !w->d_bicg) return LQ_ENOMEM;
     w->nrhs = nrhs; w->prec = prec;
     return 0;
 }
@@ -82,6 +84,7 @@ int solve_native(lq_ctx* c, void* x_full, const void* b_full, int n, const lq_so
     if (!c->has_gauge || !c->has_clover) return set_err(c, LQ_ESTATE, "gauge field and clover term must be loaded before lq_solve");
     const int prec = prm->inner_prec;
     if (prec != LQ_FP64 && prec != LQ_FP32 && prec != LQ_HALF) return set_err(c, LQ_EINVAL, "bad inner precision");
+    if (prm->algorithm != LQ_ALG_CGNR && prm->algorithm != LQ_ALG_BICGSTAB) return set_err(c, LQ_EINVAL, "bad solver algorithm");
     Workspace* w = ws_for(c);
     LQ_TRY(ws_prepare(c, w, n, prec));
     const size_t pb64 = parity_bytes(c->g, n, LQ_FP64);
@@ -138,67 +141,109 @@ int solve_native(lq_ctx* c, void* x_full, const void* b_full, int n, const lq_so
         // rt = lowprec(r / ||r_k||): per-RHS scaling keeps fp32 / half in range
         LQ_CUDA(c, cudaMemcpyAsync(d_scale, rnorm, n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
         LQ_TRY(spinor_convert(c, w->rt, prec, w->r, LQ_FP64, n, d_scale, 1));
-        // z = Mhat^dag rt ; e = 0 ; p = z (restart) or, with reliable updates, p <- z + c (p - z_old): the old direction
-        // survives the residual refresh, rescaled by c_k = ||r_k||_old / ||r_k||_new because the inner system is
-        // normalised by ||r_k|| (in exact arithmetic z = c z_old, so the correction only carries the rounding difference)
-        if (prm->keep_direction && cycle > 0) {
-            double cs[LQ_MAX_RHS];
-            for (int k = 0; k < n; k++) cs[k] = (rnorm[k] > 0 && prev_rnorm[k] > 0) ? prev_rnorm[k] / rnorm[k] : 0.0;
-            LQ_CUDA(c, cudaMemcpyAsync(d_cs, cs, n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
-            LQ_TRY(apply_mhat(c, prec, n, w->q, w->rt, w->tmp, 1));
-            LQ_TRY(blas_keep_direction(c, prec, n, w->p, w->z, w->q, d_cs));
-            void* sw = w->z; w->z = w->q; w->q = sw;
-        } else {
-            LQ_TRY(apply_mhat(c, prec, n, w->z, w->rt, w->tmp, 1));
-            LQ_TRY(blas_copy(c, prec, n, w->p, w->z));
-        }
-        for (int k = 0; k < n; k++) prev_rnorm[k] = rnorm[k];
-        LQ_TRY(spinor_zero_parity(c, w->e, n, prec));
-        LQ_TRY(blas_norm2(c, prec, n, w->z, d_rr));
-        double rr0[LQ_MAX_RHS], thresh[LQ_MAX_RHS];
-        LQ_TRY(fetch(c, d_rr, n, rr0));
-        int met[LQ_MAX_RHS];
-        for (int k = 0; k < n; k++) {
-            double want = (rnorm[k] > 0) ? 0.25 * prm->tol * bnorm[k] / rnorm[k] : 1.0;   // reduction still needed
-            double f = prm->delta > want ? prm->delta : want;
-            if (f > 0.5) f = 0.5;
-            thresh[k] = f * f * rr0[k];
-            met[k] = -1;
-        }
-        double *rr = d_rr, *rrn = d_rrn;
         int it = 0;
-        bool graph_ready = false;
-        while (it < prm->max_inner) {
-            if (prm->use_graph && it >= check_every) {
-                if (!graph_ready) {
-                    if (gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }
-                    cudaGraph_t graph;
-                    LQ_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
-                    const long long l0 = c->launches;
-                    int rc = 0;
-                    for (int j = 0; j < check_every && rc == 0; j++) { rc = cg_iteration(c, w, prec, n, rr, d_pAp, rrn); double* s = rr; rr = rrn; rrn = s; }
-                    c->launches = l0;
-                    cudaError_t ce = cudaStreamEndCapture(c->stream, &graph);   // always close the capture, even on failure
-                    if (rc) { if (ce == cudaSuccess && graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
-                    LQ_CUDA(c, ce);
-                    LQ_CUDA(c, cudaGraphInstantiate(&gexec, graph, 0));
-                    cudaGraphDestroy(graph);
-                    graph_ready = true;
-                }
-                LQ_CUDA(c, cudaGraphLaunch(gexec, c->stream));
-                c->launches += (long long)KERNELS_PER_ITER * check_every;
-            } else {
-                for (int j = 0; j < check_every; j++) { LQ_TRY(cg_iteration(c, w, prec, n, rr, d_pAp, rrn)); double* s = rr; rr = rrn; rrn = s; }
-            }
-            it += check_every;
-            double cur[LQ_MAX_RHS];
-            LQ_TRY(fetch(c, rr, n, cur));
-            bool conv = true;
+        int met[LQ_MAX_RHS];
+        double thresh[LQ_MAX_RHS];
+        if (prm->algorithm == LQ_ALG_BICGSTAB) {
+            // ---- batched BiCGStab on Mhat e = rt: rhat0 = rt, r = z, v = q; complex per-RHS scalars on the device
+            double* rho = w->d_bicg; double* rho_new = rho + 3 * LQ_MAX_RHS; double* c1 = rho + 6 * LQ_MAX_RHS; double* d2 = rho + 9 * LQ_MAX_RHS;
+            LQ_TRY(blas_copy(c, prec, n, w->z, w->rt));
+            LQ_TRY(blas_copy(c, prec, n, w->p, w->rt));
+            LQ_TRY(spinor_zero_parity(c, w->e, n, prec));
+            LQ_TRY(blas_cdot3(c, prec, n, w->rt, w->rt, rho));                       // rho = <rhat0, r> = ||rt||^2
+            double rr0[LQ_MAX_RHS];
+            LQ_TRY(fetch(c, rho + 2 * LQ_MAX_RHS, n, rr0));
             for (int k = 0; k < n; k++) {
-                if (cur[k] <= thresh[k] || !(cur[k] == cur[k])) { if (met[k] < 0) met[k] = it; }
-                else { met[k] = -1; conv = false; }
+                double want = (rnorm[k] > 0) ? 0.25 * prm->tol * bnorm[k] / rnorm[k] : 1.0;   // reduction still needed
+                double f = prm->delta > want ? prm->delta : want;
+                if (f > 0.5) f = 0.5;
+                thresh[k] = f * f * rr0[k];
+                met[k] = -1;
             }
-            if (conv) break;
+            while (it < prm->max_inner) {
+                for (int j = 0; j < check_every; j++) {
+                    LQ_TRY(apply_mhat(c, prec, n, w->q, w->p, w->tmp, 0));           // v = Mhat p
+                    LQ_TRY(blas_cdot3(c, prec, n, w->rt, w->q, c1));                 // <rhat0, v>
+                    LQ_TRY(blas_bicg_s(c, prec, n, w->s, w->z, w->q, rho, c1));      // s = r - alpha v
+                    LQ_TRY(apply_mhat(c, prec, n, w->t, w->s, w->tmp, 0));           // t = Mhat s
+                    LQ_TRY(blas_cdot3(c, prec, n, w->t, w->s, d2));                  // <t, s>, ||t||^2
+                    LQ_TRY(blas_bicg_xr(c, prec, n, w->e, w->z, w->p, w->s, w->t, w->rt, rho, c1, d2, rho_new));   // e, r, rho', ||r||^2
+                    LQ_TRY(blas_bicg_p(c, prec, n, w->p, w->z, w->q, rho, rho_new, c1, d2));                      // p
+                    double* sw = rho; rho = rho_new; rho_new = sw;
+                }
+                it += check_every;
+                double cur[LQ_MAX_RHS];
+                LQ_TRY(fetch(c, rho + 2 * LQ_MAX_RHS, n, cur));
+                bool conv = true;
+                for (int k = 0; k < n; k++) {
+                    if (cur[k] <= thresh[k] || !(cur[k] == cur[k])) { if (met[k] < 0) met[k] = it; }
+                    else { met[k] = -1; conv = false; }
+                }
+                if (conv) break;
+            }
+            for (int k = 0; k < n; k++) prev_rnorm[k] = 0.0;                         // no CG direction to carry over
+        } else {
+            // z = Mhat^dag rt ; e = 0 ; p = z (restart) or, with reliable updates, p <- z + c (p - z_old): the old direction
+            // survives the residual refresh, rescaled by c_k = ||r_k||_old / ||r_k||_new because the inner system is
+            // normalised by ||r_k|| (in exact arithmetic z = c z_old, so the correction only carries the rounding difference)
+            if (prm->keep_direction && cycle > 0) {
+                double cs[LQ_MAX_RHS];
+                for (int k = 0; k < n; k++) cs[k] = (rnorm[k] > 0 && prev_rnorm[k] > 0) ? prev_rnorm[k] / rnorm[k] : 0.0;
+                LQ_CUDA(c, cudaMemcpyAsync(d_cs, cs, n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+                LQ_TRY(apply_mhat(c, prec, n, w->q, w->rt, w->tmp, 1));
+                LQ_TRY(blas_keep_direction(c, prec, n, w->p, w->z, w->q, d_cs));
+                void* sw = w->z; w->z = w->q; w->q = sw;
+            } else {
+                LQ_TRY(apply_mhat(c, prec, n, w->z, w->rt, w->tmp, 1));
+                LQ_TRY(blas_copy(c, prec, n, w->p, w->z));
+            }
+            for (int k = 0; k < n; k++) prev_rnorm[k] = rnorm[k];
+            LQ_TRY(spinor_zero_parity(c, w->e, n, prec));
+            LQ_TRY(blas_norm2(c, prec, n, w->z, d_rr));
+            double rr0[LQ_MAX_RHS];
+            LQ_TRY(fetch(c, d_rr, n, rr0));
+            for (int k = 0; k < n; k++) {
+                double want = (rnorm[k] > 0) ? 0.25 * prm->tol * bnorm[k] / rnorm[k] : 1.0;   // reduction still needed
+                double f = prm->delta > want ? prm->delta : want;
+                if (f > 0.5) f = 0.5;
+                thresh[k] = f * f * rr0[k];
+                met[k] = -1;
+            }
+            double *rr = d_rr, *rrn = d_rrn;
+            it = 0;
+            bool graph_ready = false;
+            while (it < prm->max_inner) {
+                if (prm->use_graph && it >= check_every) {
+                    if (!graph_ready) {
+                        if (gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }
+                        cudaGraph_t graph;
+                        LQ_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+                        const long long l0 = c->launches;
+                        int rc = 0;
+                        for (int j = 0; j < check_every && rc == 0; j++) { rc = cg_iteration(c, w, prec, n, rr, d_pAp, rrn); double* s = rr; rr = rrn; rrn = s; }
+                        c->launches = l0;
+                        cudaError_t ce = cudaStreamEndCapture(c->stream, &graph);   // always close the capture, even on failure
+                        if (rc) { if (ce == cudaSuccess && graph) cudaGraphDestroy(graph); cudaGetLastError(); return rc; }
+                        LQ_CUDA(c, ce);
+                        LQ_CUDA(c, cudaGraphInstantiate(&gexec, graph, 0));
+                        cudaGraphDestroy(graph);
+                        graph_ready = true;
+                    }
+                    LQ_CUDA(c, cudaGraphLaunch(gexec, c->stream));
+                    c->launches += (long long)KERNELS_PER_ITER * check_every;
+                } else {
+                    for (int j = 0; j < check_every; j++) { LQ_TRY(cg_iteration(c, w, prec, n, rr, d_pAp, rrn)); double* s = rr; rr = rrn; rrn = s; }
+                }
+                it += check_every;
+                double cur[LQ_MAX_RHS];
+                LQ_TRY(fetch(c, rr, n, cur));
+                bool conv = true;
+                for (int k = 0; k < n; k++) {
+                    if (cur[k] <= thresh[k] || !(cur[k] == cur[k])) { if (met[k] < 0) met[k] = it; }
+                    else { met[k] = -1; conv = false; }
+                }
+                if (conv) break;
+            }
         }
         total_inner += it;
         for (int k = 0; k < n; k++) if (!done[k]) info->iters[k] = total_inner - it + (met[k] > 0 ? met[k] : it);

@@ -371,7 +371,8 @@ def run_big_solve(args, B, device, wl, c, peak, peak_src):
     ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=c["recon"])
     ctx.build_clover(c["kappa"], c["csw"])
     b_host = make_sources_host(wl["cfg"])
-    kw = dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=args.delta or wl["delta"], check_every=args.check_every, use_graph=not args.no_graph, native=True, nrhs=nrhs)
+    kw = dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=args.delta or wl["delta"], check_every=args.check_every, use_graph=not args.no_graph, native=True, nrhs=nrhs,
+              algorithm=1 if args.algorithm == "bicgstab" else 0)
     sampler = ClockSampler(device)
     w0 = time.perf_counter()
     nb = ctx.pack(b_host, nrhs, B.LQ_FP64)
@@ -483,6 +484,7 @@ def main():
     ap.add_argument("--no-graph", action="store_true")
     ap.add_argument("--check-every", type=int, default=4, help="inner iterations between convergence polls")
     ap.add_argument("--delta", type=float, default=0.0, help="inner CG reduction per cycle (0 = the workload default)")
+    ap.add_argument("--algorithm", choices=("cg", "bicgstab"), default="cg", help="inner solver of the timed step (default cg = the metric of BASELINE.json; bicgstab = the solver variant)")
     ap.add_argument("--op", default=None, metavar="CFG:KIND:PREC:N",
                     help="time ONE stencil kernel only, e.g. cfg2:A:fp32:8 (lattice and links of configs[CFG]; KIND A|B|hop|lap|proj; "
                          "PREC fp64|fp32|half); optional :variant:rpt:pfd tuning suffix.  Prints its own JSON line (used for ncu captures)")
@@ -522,7 +524,8 @@ def main():
     x_host = torch.empty_like(b_host).pin_memory()
     b_dev = b_host.cuda()
     x_dev = torch.empty_like(b_dev)
-    kw = dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=args.delta or wl["delta"], check_every=args.check_every, use_graph=not args.no_graph)
+    kw = dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=args.delta or wl["delta"], check_every=args.check_every, use_graph=not args.no_graph,
+              algorithm=1 if args.algorithm == "bicgstab" else 0)
 
     def barrier():
         if world > 1:
@@ -591,7 +594,7 @@ def main():
         "dtype": "f32" if wl["inner"] == "fp32" else "i16+f32", "data": "synthetic",
         "config": {"workload": wl["desc"], "lattice": "x".join(map(str, dims)), "nrhs_per_gpu": nrhs, "parallelism": "replicas only (RHS-independent)",
                    "l2": "working set of one inner iteration (7 inner vectors + fp32 gauge + clover, %.0f MB) exceeds the 126 MB L2; kernel timing rotates buffer sets" % ws_mb,
-                   "cuda_graph": not args.no_graph, "kappa": c["kappa"], "csw": c["csw"], "tol": c["tol"]},
+                   "cuda_graph": not args.no_graph, "algorithm": args.algorithm, "kappa": c["kappa"], "csw": c["csw"], "tol": c["tol"]},
         "solver": {"outer_cycles": info["outer_cycles"], "inner_iters": info["inner_iters"], "true_rel_residual_max": max(info["true_rel_residual"]),
                    "dslash_applies_per_step": info["dslash_applies"]},
         "e2e": {"value": whole_job_seconds_per_rhs(t_e2e, args.steps, nrhs, world), "unit": "s/RHS", "h2d_bytes_per_step": b_host.numel() * 16, "d2h_bytes_per_step": x_host.numel() * 16},

@@ -22,7 +22,8 @@
 
 enum { FORM_HOP = 0, FORM_A = 1, FORM_B = 2 };
 // fused epilogues of kernel B: per-RHS ||out||^2, or out <- out - (num/den)_k * result with per-RHS ||out||^2
-enum { EPI_NONE = 0, EPI_NORM = 1, EPI_XMAY = 2 };
+// or (EPI_CDOT, BiCGStab) the complex inner product of a vector h with the result: (Re, Im <h, out>, ||out||^2), Im negated if epi_conj
+enum { EPI_NONE = 0, EPI_NORM = 1, EPI_XMAY = 2, EPI_CDOT = 3 };
 
 template <class S> struct DslashArgs {
     using T = typename S::comp_t;
@@ -42,7 +43,8 @@ template <class S> struct DslashArgs {
     int zc, nby; FastDiv dnby, dzc, dLt;
     int epi;               // FORM_B epilogue
     const double *epi_num, *epi_den;   // EPI_XMAY: alpha_k = num_k / den_k (device, per RHS)
-    double* epi_out;                   // per-RHS sums (device)
+    double* epi_out;                   // per-RHS sums (device); EPI_CDOT: 3 x LQ_MAX_RHS
+    SView<S> epi_v; int epi_conj;      // EPI_CDOT: h (on `parity`), conjugate the inner product
     double* red_partials; unsigned int* red_counter;   // reduction scratch of the context
 };
 

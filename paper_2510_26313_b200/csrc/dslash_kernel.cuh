@@ -174,9 +174,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
     sc.cb = blk * SB + s;
     // threads beyond the last unit and padding sites of the last block do no work (but reach the fused reduction)
     const bool valid = (u < a.g.NB * G) && (sc.cb < a.g.Vh);
-    double part[RPT];
+    double part[RPT], part_c[2][RPT];       // part_c: EPI_CDOT only
 #pragma unroll
-    for (int k = 0; k < RPT; k++) part[k] = 0.0;
+    for (int k = 0; k < RPT; k++) { part[k] = 0.0; part_c[0][k] = 0.0; part_c[1][k] = 0.0; }
     if (valid) {
     cb_coords(a.g, a.parity, sc.cb, sc.xh, sc.y, sc.z, sc.t, sc.odd);
     sc.Lxh = a.g.Lxh; sc.Ly = a.g.L[1]; sc.Lz = a.g.L[2]; sc.Lt = a.g.L[3];
@@ -280,6 +280,22 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
 #pragma unroll
                 for (int k = 0; k < RPT; k++) acc[j][k] = zv[j][k] - al[k] * acc[j][k];
         }
+        if (a.epi == EPI_CDOT) {
+            // <h, out> for the 12 complex components, summed in the compute type per site like the norms below
+            T hv[24][RPT], pr[RPT], pi[RPT];
+            load_site_regs<S, RPT, R>(a.epi_v.d + own, S::has_norm ? a.epi_v.n + own_n : nullptr, hv);
+#pragma unroll
+            for (int k = 0; k < RPT; k++) { pr[k] = 0; pi[k] = 0; }
+#pragma unroll
+            for (int cc = 0; cc < 12; cc++)
+#pragma unroll
+                for (int k = 0; k < RPT; k++) {
+                    pr[k] = fm(hv[2 * cc][k], acc[2 * cc][k], fm(hv[2 * cc + 1][k], acc[2 * cc + 1][k], pr[k]));
+                    pi[k] = fm(hv[2 * cc][k], acc[2 * cc + 1][k], fm(-hv[2 * cc + 1][k], acc[2 * cc][k], pi[k]));
+                }
+#pragma unroll
+            for (int k = 0; k < RPT; k++) { part_c[0][k] = (double)pr[k]; part_c[1][k] = a.epi_conj ? -(double)pi[k] : (double)pi[k]; }
+        }
         if (a.epi != EPI_NONE) {
             // the 24 squares of one site are summed in the compute type (relative error ~1e-7 in fp32, far below the
             // solver's use of these norms); sites are summed in fp64 by the reduction
@@ -297,7 +313,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
     store_site_regs<S, RPT, R>(a.out.d + own, S::has_norm ? a.out.n + own_n : nullptr, acc);
     }   // valid
     if constexpr (FORM == FORM_B) {
-        if (a.epi != EPI_NONE) reduce_per_rhs<RPT, R>(part, a.N, G, a.red_partials, a.red_counter, a.epi_out);
+        if (a.epi == EPI_CDOT) {
+            double p3[3][RPT];
+#pragma unroll
+            for (int k = 0; k < RPT; k++) { p3[0][k] = part_c[0][k]; p3[1][k] = part_c[1][k]; p3[2][k] = part[k]; }
+            reduce_multi<3, RPT, R>(p3, a.N, G, a.red_partials, a.red_counter, a.epi_out);
+        } else if (a.epi != EPI_NONE) reduce_per_rhs<RPT, R>(part, a.N, G, a.red_partials, a.red_counter, a.epi_out);
     }
 }
 

@@ -8,7 +8,7 @@ static int launch_one(lq_ctx* c, DslashArgs<S> a) {
     const long long threads = (long long)a.g.NB * a.G * SB * (R / RPT);
     const int grid = (int)((threads + BLOCK - 1) / BLOCK);
     if (FORM == FORM_B && a.epi != EPI_NONE) {
-        LQ_TRY(ensure_partials(c, (size_t)grid * a.N));
+        LQ_TRY(ensure_partials(c, (size_t)grid * a.N * (a.epi == EPI_CDOT ? 3 : 1)));
         a.red_partials = c->red_partials; a.red_counter = c->red_counter;
     }
     dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB><<<grid, BLOCK, FORM == FORM_B ? BLOCK * sizeof(double) : 0, c->stream>>>(a);

@@ -17,6 +17,8 @@ int op_kernel_b(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const 
 // and epi_out[k] = ||out_k||^2 (out is read and written)
 int op_kernel_b_epi(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger,
                     int epi, const double* num, const double* den, double* epi_out);
+int op_kernel_b_cdot(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger,
+                     const void* h, int conj, double* epi_out);
 // out(parity) = A x or A^{-1} x (site-local)
 int op_clover(lq_ctx* c, int prec, int nrhs, int parity, void* out, const void* x, int inverse);
 

@@ -14,6 +14,7 @@ static DslashArgs<S> base_args(lq_ctx* c, int nrhs, int out_parity, void* out, c
     a.clover = nullptr;
     a.coef = T(1); a.tsign = T(c->t_bc); a.dsign = dagger ? T(-1) : T(1);
     a.epi = EPI_NONE; a.epi_num = a.epi_den = nullptr; a.epi_out = nullptr; a.red_partials = nullptr; a.red_counter = nullptr;
+    a.epi_v = a.out; a.epi_conj = 0;
     return a;
 }
 
@@ -61,6 +62,22 @@ int op_kernel_b_epi(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, co
     if (prec == LQ_FP64) return kernel_b_t<F64>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, epi, num, den, epi_out);
     if (prec == LQ_FP32) return kernel_b_t<F32>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, epi, num, den, epi_out);
     return kernel_b_t<H16>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, epi, num, den, epi_out);
+}
+// kernel B with the fused complex inner product <h, out> (conj: <out, h>) and ||out||^2: epi_out = 3 x LQ_MAX_RHS doubles
+template <class S> static int kernel_b_cdot_t(lq_ctx* c, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger,
+                                              const void* h, int conj, double* epi_out) {
+    auto a = base_args<S>(c, nrhs, out_parity, out, in, x, dagger);
+    a.clover = use_clover ? clover_ptr<S>(c, out_parity, 0) : nullptr;
+    a.coef = (typename S::comp_t)coef;
+    a.epi = EPI_CDOT; a.epi_num = a.epi_den = nullptr; a.epi_out = epi_out;
+    a.epi_v = make_view<S>(c->g, const_cast<void*>(h), nrhs, 0); a.epi_conj = conj;
+    return run_form<S, FORM_B>(c, a);
+}
+int op_kernel_b_cdot(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger,
+                     const void* h, int conj, double* epi_out) {
+    if (prec == LQ_FP64) return kernel_b_cdot_t<F64>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, h, conj, epi_out);
+    if (prec == LQ_FP32) return kernel_b_cdot_t<F32>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, h, conj, epi_out);
+    return kernel_b_cdot_t<H16>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, h, conj, epi_out);
 }
 int op_kernel_b(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger) {
     return op_kernel_b_epi(c, prec, nrhs, out_parity, out, x, in, coef, use_clover, dagger, EPI_NONE, nullptr, nullptr, nullptr);

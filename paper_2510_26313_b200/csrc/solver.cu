@@ -146,6 +146,7 @@ int solve_native(lq_ctx* c, void* x_full, const void* b_full, int n, const lq_so
         double thresh[LQ_MAX_RHS];
         if (prm->algorithm == LQ_ALG_BICGSTAB) {
             // ---- batched BiCGStab on Mhat e = rt: rhat0 = rt, r = z, v = q; complex per-RHS scalars on the device
+            const double k2b = -c->kappa * c->kappa;
             double* rho = w->d_bicg; double* rho_new = rho + 3 * LQ_MAX_RHS; double* c1 = rho + 6 * LQ_MAX_RHS; double* d2 = rho + 9 * LQ_MAX_RHS;
             LQ_TRY(blas_copy(c, prec, n, w->z, w->rt));
             LQ_TRY(blas_copy(c, prec, n, w->p, w->rt));
@@ -162,11 +163,11 @@ int solve_native(lq_ctx* c, void* x_full, const void* b_full, int n, const lq_so
             }
             while (it < prm->max_inner) {
                 for (int j = 0; j < check_every; j++) {
-                    LQ_TRY(apply_mhat(c, prec, n, w->q, w->p, w->tmp, 0));           // v = Mhat p
-                    LQ_TRY(blas_cdot3(c, prec, n, w->rt, w->q, c1));                 // <rhat0, v>
+                    LQ_TRY(op_kernel_a(c, prec, n, 1, w->tmp, w->p, 0));             // v = Mhat p with <rhat0, v> in the epilogue
+                    LQ_TRY(op_kernel_b_cdot(c, prec, n, 0, w->q, w->p, w->tmp, k2b, 1, 0, w->rt, 0, c1));
                     LQ_TRY(blas_bicg_s(c, prec, n, w->s, w->z, w->q, rho, c1));      // s = r - alpha v
-                    LQ_TRY(apply_mhat(c, prec, n, w->t, w->s, w->tmp, 0));           // t = Mhat s
-                    LQ_TRY(blas_cdot3(c, prec, n, w->t, w->s, d2));                  // <t, s>, ||t||^2
+                    LQ_TRY(op_kernel_a(c, prec, n, 1, w->tmp, w->s, 0));             // t = Mhat s with <t, s> = conj <s, t> and ||t||^2
+                    LQ_TRY(op_kernel_b_cdot(c, prec, n, 0, w->t, w->s, w->tmp, k2b, 1, 0, w->s, 1, d2));
                     LQ_TRY(blas_bicg_xr(c, prec, n, w->e, w->z, w->p, w->s, w->t, w->rt, rho, c1, d2, rho_new));   // e, r, rho', ||r||^2
                     LQ_TRY(blas_bicg_p(c, prec, n, w->p, w->z, w->q, rho, rho_new, c1, d2));                      // p
                     double* sw = rho; rho = rho_new; rho_new = sw;

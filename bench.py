@@ -1,15 +1,21 @@
 #!/usr/bin/env python
 """bench.py -- measures BASELINE.json's metric ("multi-RHS clover Dslash HBM GB/s & % of peak; batched CG sec/RHS").
 
-One "step" is one pass of the whole hot path over one batch of synthetic sources:
-a batched mixed-precision even-odd CG solve M x = b for N_rhs LapH-diluted sources on the workload's lattice
-(default: BASELINE.json configs[1], 16^3 x 32, 8 RHS, fp32 inner CG, fp64 defect correction, tol 1e-8).
-`value` is seconds per RHS with the sources resident in HBM; `e2e` is the same through the C ABI with HOST buffers.
-`roofline` is the dominant kernel (fused kernel A = A^-1 D, fp32) timed alone on the same lattice and batch with
-rotating buffer sets larger than L2.  `dslash` adds the configs[2] sweep (32^3 x 64, N = 1..16) and configs[4]
-(64^3 x 128, N = 4, 12-real links) operator throughput; `cpu_baseline` times the fp64 oracle on the host cores.
+One "step" is one pass of the whole hot path over one batch of synthetic sources: a batched
+mixed-precision even-odd CG solve M x = b for N_rhs LapH-diluted sources.  Default workload: BASELINE.json configs[3]
+(48^3 x 96, 12 RHS, int16+norm inner CG with fp32 clover, fp64 defect correction to 1e-9), the largest solver configuration
+that fits one GPU; `--workload cfg1` is configs[1] (16^3 x 32, 8 RHS, fp32 inner CG).  `--steps K --warmup W` are honoured
+exactly (W >= 3).
+  value    = seconds per RHS, sources resident in HBM in the native layout (K timed solves between CUDA events)
+  e2e      = the same through the C ABI with HOST buffers (pinned canonical arrays in and out: H2D, reorder, solve, reorder, D2H)
+  roofline = the Dslash half of the metric: fused kernel A (A^-1 D, fp32, 18-real links) at N_rhs = 8 on configs[2] (32^3 x 64),
+             timed alone with rotating buffer sets larger than L2, as algorithmic GB/s against the measured HBM peak, with the
+             ALU fraction against an FP32 FMA peak measured in the same run ("report both fractions")
+  rooflines = the same for N = 12 and 16, kernel B, configs[4] (64^3 x 128, N = 4, 12-real links) and the int16 kernels of configs[3]
+  dslash_sweep = the configs[2] sweep over N_rhs in {1, 2, 4, 8, 16} (the paper's batching claim)
+  cpu_baseline = the fp64 oracle on the host cores, bounded sample.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg1|cfg3] [--no-extras]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg3|cfg1] [--no-extras]
 """
 from __future__ import annotations
 
@@ -182,12 +188,37 @@ def time_laplacian(ctx, B, nvec, prec="fp32", iters=20, warmup=3):
             "gflops": round(6 * 72.0 * ctx.V * nvec / sec * 1e-9, 1)}
 
 
-def roofline_entry(r, peak, peak_src, traffic=None):
-    return {"bound": "hbm", "kernel": "dslash_kernel<%s,N=%d,recon=%d,form=%s>" % (r["prec"], r["nrhs"], r["recon"], r["kind"]),
-            "achieved": round(r["gbs"], 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s",
-            "frac": round(r["gbs"] / peak, 4), "frac_of_8TBs": round(r["gbs"] / 8000.0, 4), "traffic": traffic,
-            "us_per_launch": round(r["seconds"] * 1e6, 2), "gflops": round(r["gflops"], 1),
-            "algorithmic_bytes_per_site_rhs": r["bytes_per_site_rhs"]}
+# FP32 instruction slots (one FMA, multiply or add each) per output site per RHS when every complex product is written as fused
+# multiply-adds: hop 8 x (12 project + 72 SU(3) + 24 accumulate) = 864, clover 2 x 6 x 22 = 264
+FP_SLOTS = {"A": 1128.0, "B": 1128.0, "hop": 864.0}
+
+
+def roofline_entry(r, peak, peak_src, traffic=None, fma=None, lattice=None):
+    """HBM fraction (algorithmic bytes / CUDA-event time / measured copy bandwidth) and, when the FP32 FMA peak was measured in
+    this run, the ALU fractions: `alu_frac` = counted flops (1320 + 504 per site per RHS) / peak, `alu_issue_frac` = FP32
+    instruction slots x 2 / peak (what the FMA pipes must issue: adds and multiplies occupy a slot like an FMA)."""
+    e = {"bound": "hbm", "kernel": "dslash_kernel<%s,N=%d,recon=%d,form=%s>" % (r["prec"], r["nrhs"], r["recon"], r["kind"]),
+         "achieved": round(r["gbs"], 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+         "frac": round(r["gbs"] / peak, 4), "frac_of_8TBs": round(r["gbs"] / 8000.0, 4), "traffic": traffic,
+         "us_per_launch": round(r["seconds"] * 1e6, 2), "gflops": round(r["gflops"], 1),
+         "algorithmic_bytes_per_site_rhs": r["bytes_per_site_rhs"]}
+    if lattice:
+        e["lattice"] = lattice
+    if fma:
+        flop = {"A": FLOP_A, "B": FLOP_B, "hop": FLOP_HOP}[r["kind"]]
+        e["alu_peak_tflops"] = fma["scalar_ffma"]
+        e["alu_frac"] = round(r["gflops"] * 1e-3 / fma["scalar_ffma"], 4)
+        e["alu_issue_frac"] = round(r["gflops"] * 1e-3 * (2.0 * FP_SLOTS[r["kind"]] / flop) / fma["scalar_ffma"], 4)
+        e["alu_issue_frac_of_ffma2_shared"] = round(r["gflops"] * 1e-3 * (2.0 * FP_SLOTS[r["kind"]] / flop) / fma["ffma2_shared_operand"], 4)
+    return e
+
+
+def measure_fma_peak(ctx):
+    """FP32 FMA peak through the C ABI (lq_fma_peak): scalar FFMA, packed FFMA2 with three distinct operands, packed FFMA2 with
+    one operand shared by 4 consecutive instructions (the stencil's pattern).  TFLOP/s, 2 flops per FMA lane."""
+    return {"scalar_ffma": round(ctx.fma_peak(0, 150.0), 2), "ffma2_distinct_operands": round(ctx.fma_peak(1, 150.0), 2),
+            "ffma2_shared_operand": round(ctx.fma_peak(2, 150.0), 2), "unit": "TFLOP/s", "nominal_1965MHz": 74.4,
+            "how": "register-only FMA loops, 16 chains per thread, 8 CTAs x 256 threads per SM, ~150 ms each (csrc/fmapeak.cu)"}
 
 
 # ------------------------------------------------------------------------------------------------ workloads
@@ -197,34 +228,62 @@ SOLVER_WORKLOADS = {
 }
 
 
-def make_sources_host(cfg):
+def solve_kwargs(B, wl, c, algorithm="cg", check_every=4, delta=0.0, use_graph=True):
+    """The launch configuration of the timed step (tests/test_gpu_fullsize.py checks the configs[3] solve with exactly these)."""
+    return dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=delta or wl["delta"], check_every=2 if algorithm == "bicgstab" else check_every,
+                use_graph=use_graph, algorithm=1 if algorithm == "bicgstab" else 0)
+
+
+def make_sources_host(cfg, out=None):
     c = inputs.CONFIGS[cfg]
-    return inputs.laph_sources(c["dims"], c["nrhs"], c["n_t"], c["source_seed"])
+    return inputs.laph_sources(c["dims"], c["nrhs"], c["n_t"], c["source_seed"], out=out)
+
+
+ORACLE_SAMPLE_DIMS = (16, 16, 16, 32)
+
+
+def oracle_sample_solve(cfg_id: int, k: int = 0):
+    """One bounded sample of the workload for the CPU oracle: RHS k solved by oracle.solve_eo (fp64 CGNR, true residual
+    recomputed every iteration) on the workload's lattice if that is 16^3 x 32 or smaller, else on a 16^3 x 32 lattice of the
+    same recipe (links, kappa, c_sw, source structure, tolerance): a full 48^3 x 96 oracle solve takes hours.  Returns
+    (seconds, iterations, lattice, volume ratio workload / sample)."""
+    import oracle
+    c = inputs.CONFIGS[cfg_id]
+    dims = c["dims"] if inputs.volume(c["dims"]) <= inputs.volume(ORACLE_SAMPLE_DIMS) else ORACLE_SAMPLE_DIMS
+    key = (cfg_id, dims)
+    if oracle_sample_solve.cache.get("key") != key:
+        U = inputs.make_links(dims, c["gauge_seed"], c["eps"])
+        A = oracle.clover(dims, U, c["kappa"], c["csw"])
+        oracle_sample_solve.cache = {"key": key, "U": U, "A": A, "Ainv": oracle.clover_inverse(A),
+                                     "b": inputs.laph_sources(dims, 4, c["n_t"], c["source_seed"])}
+    q = oracle_sample_solve.cache
+    t0 = time.perf_counter()
+    _, it, _ = oracle.solve_eo(dims, q["U"], q["A"], q["Ainv"], c["kappa"], q["b"][k % 4], c["tol"])
+    return time.perf_counter() - t0, it, dims, inputs.volume(c["dims"]) / inputs.volume(dims)
+
+
+oracle_sample_solve.cache = {}
 
 
 def cpu_baseline(cfg_id: int, budget_s: float = 25.0):
-    """The oracle as it stands on the host cores: full even-odd CG solves of single RHS of the workload, as many as fit
-    the time budget (at least one)."""
+    """The oracle as it stands on the host cores: single-RHS even-odd CG solves (bounded sample, see oracle_sample_solve), as
+    many as fit the time budget (at least one).  `value` is seconds per RHS of the workload: the sample time scaled by the
+    volume ratio when the sample lattice is smaller than the workload's (CG cost per iteration is linear in the volume; the
+    iteration count of these well-conditioned random links does not grow with it)."""
     import oracle
-    c = inputs.CONFIGS[cfg_id]
-    dims = c["dims"]
-    if cfg_id == 3:   # a full 48^3x96 oracle solve takes hours: bounded sample on a 16^3x32 sub-volume of the same recipe
-        dims = (16, 16, 16, 32)
-    U = inputs.make_links(dims, c["gauge_seed"], c["eps"])
-    A = oracle.clover(dims, U, c["kappa"], c["csw"])
-    Ainv = oracle.clover_inverse(A)
-    b = inputs.laph_sources(dims, 4, c["n_t"], c["source_seed"])
     t0 = time.perf_counter()
-    n, its = 0, []
-    while n < 4:
-        x, it, res = oracle.solve_eo(dims, U, A, Ainv, c["kappa"], b[n], c["tol"])
-        its.append(it); n += 1
+    secs, its = [], []
+    dims, ratio = None, 1.0
+    while len(secs) < 4:
+        dt, it, dims, ratio = oracle_sample_solve(cfg_id, len(secs))
+        secs.append(dt); its.append(it)
         if time.perf_counter() - t0 > budget_s * 0.5:
             break
-    dt = time.perf_counter() - t0
-    return {"value": dt / n, "unit": "s/RHS", "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": "%d of the workload's RHS solved one at a time by oracle.solve_eo (fp64 CGNR, true residual recomputed every "
-                      "iteration) on %s, tol %g; iterations %s" % (n, "x".join(map(str, dims)), c["tol"], its)}
+    return {"value": float(np.mean(secs)) * ratio, "unit": "s/RHS", "cores": oracle.num_threads(), "kind": "oracle",
+            "measured_seconds_per_sample_solve": float(np.mean(secs)), "volume_scale": ratio,
+            "sample": "%d single-RHS oracle.solve_eo solves (fp64 CGNR, true residual recomputed every iteration) on %s, tol %g, iterations %s%s"
+                      % (len(secs), "x".join(map(str, dims)), inputs.CONFIGS[cfg_id]["tol"], its,
+                         "" if ratio == 1.0 else "; value = measured seconds x %.0f (volume of the workload / volume of the sample lattice)" % ratio)}
 
 
 def cpu_dslash_baseline():
@@ -312,104 +371,76 @@ def time_projection(B, device, peak, shapes=((32, 8), (128, 32)), precs=("f64_fm
     return out
 
 
-def operator_sweeps(B, device, peak):
-    """configs[2]: 32^3x64 fp32 sweep over N_rhs (kernel A, kernel B, bare hop); configs[4]: 64^3x128, N=4, 12-real links."""
+def dslash_report(B, device, peak, peak_src, quick=False):
+    """The Dslash half of the metric.  configs[2] (32^3 x 64, fp32, 18-real links): kernel A / kernel B / bare hop over
+    N_rhs in {1, 2, 4, 8, 12, 16}; configs[4] (64^3 x 128, N = 4, 12-real links); the int16+norm kernels of configs[3] come from
+    the solver context (caller).  Returns (headline roofline entry, list of further roofline entries, sweep table, fma peaks)."""
     import torch
-    out = {"unit": "GB/s (algorithmic bytes / CUDA-event time)", "peak_gbs": peak, "cfg2_32x32x32x64_fp32_recon18": [], "cfg4_64x64x64x128_fp32_recon12": []}
-    for cfg_id, key in ((2, "cfg2_32x32x32x64_fp32_recon18"), (4, "cfg4_64x64x64x128_fp32_recon12")):
+    rooflines, sweep, head, fma = [], [], None, None
+    for cfg_id in (2, 4):
         c = inputs.CONFIGS[cfg_id]
+        lat = "x".join(map(str, c["dims"]))
         ctx = B.Context(c["dims"], device=device)
+        if fma is None:
+            fma = measure_fma_peak(ctx)
         ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=c["recon"])
         ctx.build_clover(c["kappa"], c["csw"])
-        ns = c["nrhs"] if isinstance(c["nrhs"], tuple) else (c["nrhs"],)
+        ns = (1, 2, 4, 8, 12, 16) if cfg_id == 2 else (c["nrhs"],)
         for n in ns:
             for kind in ("A", "B", "hop"):
+                if quick and (kind == "hop" or n in (1, 2)):
+                    continue
                 r = time_dslash(ctx, B, kind, "fp32", n, c["recon"], iters=20)
-                out[key].append({"kernel": kind, "nrhs": n, "us": round(r["seconds"] * 1e6, 1), "gbs": round(r["gbs"], 1), "gflops": round(r["gflops"], 1),
-                                 "frac_measured_hbm": round(r["gbs"] / peak, 4), "frac_8TBs": round(r["gbs"] / 8000.0, 4)})
-        if cfg_id == 2:
-            out["laplacian_32x32x32x64_fp32"] = []
+                e = roofline_entry(r, peak, peak_src, ncu_traffic(lat, r), fma, lat)
+                sweep.append({"lattice": lat, "kernel": kind, "nrhs": n, "recon": c["recon"], "us": e["us_per_launch"], "gbs": e["achieved"], "gflops": e["gflops"],
+                              "frac_measured_hbm": e["frac"], "frac_8TBs": e["frac_of_8TBs"], "alu_frac": e["alu_frac"], "alu_issue_frac": e["alu_issue_frac"]})
+                if cfg_id == 2 and kind == "A" and n == 8:
+                    head = e
+                elif kind != "hop" and (n >= 8 or cfg_id == 4):
+                    rooflines.append(e)
+        if cfg_id == 2 and not quick:
+            lap = []
             for n in (1, 4, 8, 16):
                 r = time_laplacian(ctx, B, n)
                 r["frac_measured_hbm"] = round(r["gbs"] / peak, 4)
-                out["laplacian_32x32x32x64_fp32"].append(r)
+                lap.append(r)
+            sweep.append({"laplacian_32x32x32x64_fp32": lap})
         ctx.close()
         torch.cuda.empty_cache()
-    return out
+    return head, rooflines, sweep, fma
 
 
 # ------------------------------------------------------------------------------------------------ reference arm
 def run_reference(args, rank, world):
     """`--impl reference`: this tier has no reference implementation to install; the arm times the CPU oracle as it stands
-    on the host cores (rank 0 only), on the same config / metric / unit."""
+    on the host cores (rank 0 only).  Each step is ONE bounded sample of the workload (oracle_sample_solve: a single-RHS
+    oracle CG solve, on a 16^3 x 32 lattice of the same recipe when the workload's lattice is larger); `ms_per_step` is the
+    measured wall time of such a step, so steps x ms_per_step is what this process really spent; `value` (seconds per RHS of
+    the workload) is that time scaled by the volume ratio and is named as an extrapolation when the ratio is not 1."""
     if rank != 0:
         return
+    import oracle
     wl = SOLVER_WORKLOADS[args.workload]
     c = inputs.CONFIGS[wl["cfg"]]
-    vals = []
-    cb = None
-    for _ in range(max(1, min(args.steps, 2))):
-        cb = cpu_baseline(wl["cfg"], budget_s=20.0)
-        vals.append(cb["value"])
-    v = float(np.mean(vals))
+    for i in range(args.warmup):
+        oracle_sample_solve(wl["cfg"], i)
+    secs, its, dims, ratio = [], [], None, 1.0
+    for i in range(max(1, args.steps)):
+        dt, it, dims, ratio = oracle_sample_solve(wl["cfg"], i)
+        secs.append(dt); its.append(it)
+    per = float(np.mean(secs))
+    v = per * ratio
+    sample = ("each step = 1 single-RHS oracle.solve_eo solve (fp64 CGNR) on %s, tol %g; iterations %s" % ("x".join(map(str, dims)), c["tol"], its))
     line = {"impl": "reference", "metric": "batched CG sec/RHS", "value": v, "unit": "s/RHS", "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": v * c["nrhs"] * 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": {"workload": wl["desc"], "note": "CPU oracle, bounded sample per step"},
-            "cpu_baseline": dict(cb, value=v), "e2e": {"value": v, "unit": "s/RHS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "warmup": args.warmup, "ms_per_step": per * 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl["desc"], "note": "CPU oracle; a step is a bounded sample of the workload: " + sample},
+            "value_is_extrapolated": ratio != 1.0,
+            "extrapolation": None if ratio == 1.0 else {"measured_seconds_per_step": per, "rhs_per_step": 1, "sample_lattice": "x".join(map(str, dims)),
+                                                        "volume_scale": ratio, "rule": "value = measured seconds per step x volume_scale (cost per CG iteration is linear in the volume)"},
+            "cpu_baseline": {"value": v, "unit": "s/RHS", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": "s/RHS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
-    print(json.dumps(line))
-
-
-# ------------------------------------------------------------------------------------------------ large-lattice solve (configs[3])
-def run_big_solve(args, B, device, wl, c, peak, peak_src):
-    """configs[3] (48^3x96, 12 RHS, int16+norm inner CG): too large to keep canonical AND native copies of b and x on the
-    device next to the solver workspace, so the step is: host canonical b -> lq_pack (H2D + reorder) -> native solve ->
-    lq_unpack (reorder + D2H).  `value` = the native device-resident solve; `e2e` = the whole host-to-host step."""
-    import torch
-    dims, nrhs = c["dims"], c["nrhs"]
-    ctx = B.Context(dims, device=device)
-    ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=c["recon"])
-    ctx.build_clover(c["kappa"], c["csw"])
-    b_host = make_sources_host(wl["cfg"])
-    kw = dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=args.delta or wl["delta"], check_every=args.check_every, use_graph=not args.no_graph, native=True, nrhs=nrhs,
-              algorithm=1 if args.algorithm == "bicgstab" else 0)
-    sampler = ClockSampler(device)
-    w0 = time.perf_counter()
-    nb = ctx.pack(b_host, nrhs, B.LQ_FP64)
-    torch.cuda.synchronize()
-    t_pack = time.perf_counter() - w0
-    nx = ctx.native_empty(nrhs, B.LQ_FP64)
-    info = None
-    steps = max(1, min(args.steps, 2))
-    _, info = ctx.solve(nb, x_out=nx, **kw)                       # one warm-up solve (workspace allocation, graph build)
-    l0 = ctx.launches
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(ctx.stream)
-    for _ in range(steps):
-        _, info = ctx.solve(nb, x_out=nx, **kw)
-    e1.record(ctx.stream)
-    e1.synchronize()
-    t_dev = e0.elapsed_time(e1) * 1e-3 / steps
-    launches = (ctx.launches - l0) // steps
-    w0 = time.perf_counter()
-    x_host = ctx.unpack(nx, nrhs, B.LQ_FP64)
-    t_unpack = time.perf_counter() - w0
-    clocks = sampler.stop()
-    del nb, nx
-    rA = time_dslash(ctx, B, "A", wl["inner"], nrhs, c["recon"], iters=10)
-    rB = time_dslash(ctx, B, "B", wl["inner"], nrhs, c["recon"], iters=10)
-    ctx.close()
-    line = {"metric": "batched CG sec/RHS", "value": t_dev / nrhs, "unit": "s/RHS", "n_gpus": 1, "steps": steps, "warmup": 1,
-            "ms_per_step": t_dev * 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "i16+f32", "data": "synthetic",
-            "config": {"workload": wl["desc"], "lattice": "x".join(map(str, dims)), "nrhs_per_gpu": nrhs, "parallelism": "replicas only (RHS-independent)",
-                       "l2": "every vector of the iteration (3.3 GB) exceeds the 126 MB L2", "cuda_graph": not args.no_graph,
-                       "kappa": c["kappa"], "csw": c["csw"], "tol": c["tol"]},
-            "solver": {"converged": info["converged"], "outer_cycles": info["outer_cycles"], "inner_iters": info["inner_iters"],
-                       "true_rel_residual_max": max(info["true_rel_residual"]), "dslash_applies_per_step": info["dslash_applies"]},
-            "e2e": {"value": (t_pack + t_dev + t_unpack) / nrhs, "unit": "s/RHS", "h2d_bytes_per_step": int(b_host.nbytes), "d2h_bytes_per_step": int(x_host.nbytes),
-                    "note": "pageable host arrays; pack %.2f s + solve %.2f s + unpack %.2f s" % (t_pack, t_dev, t_unpack)},
-            "gpu_launches": int(launches), "clocks": clocks,
-            "roofline": roofline_entry(rB, peak, peak_src), "roofline_kernel_A": roofline_entry(rA, peak, peak_src)}
     print(json.dumps(line))
 
 
@@ -473,16 +504,29 @@ def run_op(args, B, device):
 
 
 # ------------------------------------------------------------------------------------------------ main
+def pinned_complex(shape):
+    """Pinned host array (torch owns the memory; numpy view for filling)."""
+    import torch
+    try:
+        t = torch.empty(tuple(shape), dtype=torch.complex128, pin_memory=True)
+        pinned = True
+    except Exception:
+        t = torch.empty(tuple(shape), dtype=torch.complex128)
+        pinned = False
+    return t, pinned
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg1", choices=sorted(SOLVER_WORKLOADS))
-    ap.add_argument("--no-extras", action="store_true", help="skip the configs[2]/[4] operator sweep and the CPU baseline")
+    ap.add_argument("--workload", default="cfg3", choices=sorted(SOLVER_WORKLOADS))
+    ap.add_argument("--no-extras", action="store_true", help="skip the extras (configs[1] solve, BiCGStab variant, Lanczos, projection, CPU Dslash baseline)")
+    ap.add_argument("--no-dslash", action="store_true", help="skip the Dslash report (roofline of the configs[2]/[4] kernels) as well")
     ap.add_argument("--no-graph", action="store_true")
-    ap.add_argument("--check-every", type=int, default=4, help="inner iterations between convergence polls")
+    ap.add_argument("--check-every", type=int, default=4, help="inner iterations between convergence tests")
     ap.add_argument("--delta", type=float, default=0.0, help="inner CG reduction per cycle (0 = the workload default)")
     ap.add_argument("--algorithm", choices=("cg", "bicgstab"), default="cg", help="inner solver of the timed step (default cg = the metric of BASELINE.json; bicgstab = the solver variant)")
     ap.add_argument("--op", default=None, metavar="CFG:KIND:PREC:N",
@@ -509,33 +553,27 @@ def main():
     wl = SOLVER_WORKLOADS[args.workload]
     c = inputs.CONFIGS[wl["cfg"]]
     dims, nrhs = c["dims"], c["nrhs"]
+    Lx, Ly, Lz, Lt = dims
     peak, peak_src, _ = measured_peaks()
-    if wl["cfg"] == 3:
-        if world > 1:
-            raise SystemExit("--workload cfg3 is a single-GPU extra")
-        return run_big_solve(args, B, local, wl, c, peak, peak_src)
     ctx = B.Context(dims, device=local)
-    if wl["cfg"] == 1:
-        ctx.load_gauge(inputs.make_links(dims, rank_gauge_seed(c["gauge_seed"], rank), c["eps"]), recon=c["recon"])
-    else:
-        ctx.fill_gauge_random(rank_gauge_seed(c["gauge_seed"], rank), c["eps"], recon=c["recon"])
+    ctx.fill_gauge_random(rank_gauge_seed(c["gauge_seed"], rank), c["eps"], recon=c["recon"])
     ctx.build_clover(c["kappa"], c["csw"])
-    b_host = torch.from_numpy(make_sources_host(wl["cfg"])).pin_memory()
-    x_host = torch.empty_like(b_host).pin_memory()
-    b_dev = b_host.cuda()
-    x_dev = torch.empty_like(b_dev)
-    kw = dict(tol=c["tol"], inner_prec=B.PREC[wl["inner"]], delta=args.delta or wl["delta"], check_every=args.check_every, use_graph=not args.no_graph,
-              algorithm=1 if args.algorithm == "bicgstab" else 0)
+    b_host, pinned = pinned_complex((nrhs, Lt, Lz, Ly, Lx, 4, 3))
+    x_host, _ = pinned_complex((nrhs, Lt, Lz, Ly, Lx, 4, 3))
+    make_sources_host(wl["cfg"], out=b_host.numpy())
+    kw = solve_kwargs(B, wl, c, args.algorithm, args.check_every, args.delta, not args.no_graph)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident steps
+    # ---- device-resident steps: the sources sit in HBM in the native layout before the timed region starts
+    nb = ctx.pack(b_host, nrhs, B.LQ_FP64)
+    nx = ctx.native_empty(nrhs, B.LQ_FP64)
     info = None
     for _ in range(args.warmup):
-        _, info = ctx.solve(b_dev, x_out=x_dev, **kw)
+        _, info = ctx.solve(nb, x_out=nx, native=True, nrhs=nrhs, **kw)
     assert info["converged"], info
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
@@ -543,12 +581,14 @@ def main():
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(ctx.stream)
     for _ in range(args.steps):
-        _, info = ctx.solve(b_dev, x_out=x_dev, **kw)
+        _, info = ctx.solve(nb, x_out=nx, native=True, nrhs=nrhs, **kw)
     e1.record(ctx.stream)
     barrier()
     launches = ctx.launches - l0
     t_dev = e0.elapsed_time(e1) * 1e-3
-    # ---- end to end: host buffers in, host buffers out, through the C ABI
+    del nb, nx
+    torch.cuda.empty_cache()
+    # ---- end to end: host buffers in, host buffers out, through the C ABI (lq_solve stages them a few RHS at a time)
     ctx.solve(b_host, x_out=x_host, **kw)
     barrier()
     w0 = time.perf_counter()
@@ -558,51 +598,72 @@ def main():
     t_e2e = time.perf_counter() - w0
     clocks = sampler.stop() if sampler else None
     t_dev, t_e2e = max_over_ranks([t_dev, t_e2e], device="cuda")
-
-    # ---- solver variant, same sources, device resident: batched BiCGStab instead of CGNR (not the headline metric)
+    h2d, d2h = b_host.numel() * 16, x_host.numel() * 16
+    del x_host
     variant = None
-    if not args.no_extras and world == 1:
-        kb = dict(kw, algorithm=B.LQ_ALG_BICGSTAB, check_every=2)
-        ctx.solve(b_dev, x_out=x_dev, **kb)
-        _, ib = ctx.solve(b_dev, x_out=x_dev, **kb)
+    if not args.no_extras and world == 1 and args.algorithm == "cg":
+        # solver variant, same sources, device resident: batched BiCGStab instead of CGNR (not the headline metric)
+        kb = solve_kwargs(B, wl, c, "bicgstab", use_graph=not args.no_graph)
+        nb = ctx.pack(b_host, nrhs, B.LQ_FP64)
+        nx = ctx.native_empty(nrhs, B.LQ_FP64)
+        ctx.solve(nb, x_out=nx, native=True, nrhs=nrhs, **kb)
+        _, ib = ctx.solve(nb, x_out=nx, native=True, nrhs=nrhs, **kb)
         variant = {"algorithm": "batched BiCGStab on Mhat, complex per-RHS scalars, same defect correction", "seconds_per_rhs": ib["seconds"] / nrhs,
                    "ms_per_step": ib["seconds"] * 1e3, "inner_iters": ib["inner_iters"], "outer_cycles": ib["outer_cycles"],
                    "dslash_applies_per_step": ib["dslash_applies"], "true_rel_residual_max": max(ib["true_rel_residual"]), "converged": ib["converged"]}
-    # ---- dominant kernel alone (roofline), same lattice and batch
-    rA = time_dslash(ctx, B, "A", "half" if wl["inner"] == "half" else "fp32", nrhs, c["recon"], iters=50)
-    rB = time_dslash(ctx, B, "B", "half" if wl["inner"] == "half" else "fp32", nrhs, c["recon"], iters=50)
-    ws_mb = (7 * ctx.native_bytes(nrhs, B.PREC[wl["inner"]], True) + ctx.V * (4 * c["recon"] + 144) * 4) / 1e6
+        del nb, nx
+    del b_host
+    torch.cuda.empty_cache()
+
+    # ---- the kernels of this step alone, same lattice and batch (rotating buffers)
+    inner = wl["inner"]
+    fma0 = measure_fma_peak(ctx) if rank == 0 else None
+    rA = time_dslash(ctx, B, "A", inner, nrhs, c["recon"], iters=20)
+    rB = time_dslash(ctx, B, "B", inner, nrhs, c["recon"], iters=20)
+    lat = "x".join(map(str, dims))
+    step_kernels = [roofline_entry(rA, peak, peak_src, ncu_traffic(lat, rA), fma0, lat), roofline_entry(rB, peak, peak_src, ncu_traffic(lat, rB), fma0, lat)]
     ctx.close()
-    del b_dev, x_dev
     torch.cuda.empty_cache()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
+    # ---- the Dslash half of the metric (configs[2], configs[4]); the oracle on the host cores
+    head, rooflines, sweep, fma = (None, [], [], fma0)
+    if not args.no_dslash and world == 1:
+        head, rooflines, sweep, fma = dslash_report(B, local, peak, peak_src, quick=args.no_extras)
     extras = {}
     if not args.no_extras and world == 1:
-        extras["dslash"] = operator_sweeps(B, local, peak)
-        extras["dslash"]["cpu_baseline"] = cpu_dslash_baseline()
-        extras["solver_variant_bicgstab"] = variant
+        extras["cpu_dslash_baseline"] = cpu_dslash_baseline()
+        if variant is not None:
+            extras["solver_variant_bicgstab"] = variant
         extras["laph_eigensolve"] = time_eigensolve(B, local)
         extras["projection"] = time_projection(B, local, peak)
-        extras["cpu_baseline"] = cpu_baseline(wl["cfg"])
-    total_rhs = nrhs * world
+    t_step = t_dev / args.steps
     line = {
         "metric": "batched CG sec/RHS", "value": whole_job_seconds_per_rhs(t_dev, args.steps, nrhs, world), "unit": "s/RHS", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32" if wl["inner"] == "fp32" else "i16+f32", "data": "synthetic",
-        "config": {"workload": wl["desc"], "lattice": "x".join(map(str, dims)), "nrhs_per_gpu": nrhs, "parallelism": "replicas only (RHS-independent)",
-                   "l2": "working set of one inner iteration (7 inner vectors + fp32 gauge + clover, %.0f MB) exceeds the 126 MB L2; kernel timing rotates buffer sets" % ws_mb,
-                   "cuda_graph": not args.no_graph, "algorithm": args.algorithm, "kappa": c["kappa"], "csw": c["csw"], "tol": c["tol"]},
-        "solver": {"outer_cycles": info["outer_cycles"], "inner_iters": info["inner_iters"], "true_rel_residual_max": max(info["true_rel_residual"]),
-                   "dslash_applies_per_step": info["dslash_applies"]},
-        "e2e": {"value": whole_job_seconds_per_rhs(t_e2e, args.steps, nrhs, world), "unit": "s/RHS", "h2d_bytes_per_step": b_host.numel() * 16, "d2h_bytes_per_step": x_host.numel() * 16},
+        "warmup": args.warmup, "ms_per_step": t_step * 1e3, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if inner == "fp32" else ("i16+f32" if inner == "half" else "f64"), "data": "synthetic",
+        "config": {"workload": wl["desc"], "lattice": lat, "nrhs_per_gpu": nrhs, "parallelism": "replicas only (RHS-independent)",
+                   "l2": "every vector of the iteration (%.0f MB) %s the 126 MB L2; the kernel timings rotate buffer sets larger than L2"
+                         % (ctx.V // 2 * nrhs * (52 if inner == "half" else 96) / 1e6, "exceeds" if ctx.V // 2 * nrhs * 52 > 126e6 else "is comparable to"),
+                   "cuda_graph": not args.no_graph, "algorithm": args.algorithm, "check_every": kw["check_every"], "delta": kw["delta"],
+                   "kappa": c["kappa"], "csw": c["csw"], "tol": c["tol"], "links": "SU(3) projection of 1 + %.1f G, seed %d (device generator)" % (c["eps"], c["gauge_seed"])},
+        "solver": {"converged": info["converged"], "outer_cycles": info["outer_cycles"], "inner_iters": info["inner_iters"],
+                   "true_rel_residual_max": max(info["true_rel_residual"]), "dslash_applies_per_step": info["dslash_applies"],
+                   "model_bytes_per_step": info["model_bytes"], "model_flops_per_step": info["model_flops"],
+                   "model_gbs": round(info["model_bytes"] / t_step * 1e-9, 1), "model_frac_measured_hbm": round(info["model_bytes"] / t_step * 1e-9 / peak, 4),
+                   "model_tflops": round(info["model_flops"] / t_step * 1e-12, 2)},
+        "e2e": {"value": whole_job_seconds_per_rhs(t_e2e, args.steps, nrhs, world), "unit": "s/RHS", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "host_memory": "pinned" if pinned else "pageable"},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        # the dominant kernel of the step by device-time share (profiles/r01e_launches_cfg1.md): kernel B 50 %, kernel A 31 %
-        "roofline": roofline_entry(rB, peak, peak_src, ncu_traffic("x".join(map(str, dims)), rB)),
-        "roofline_kernel_A": roofline_entry(rA, peak, peak_src, ncu_traffic("x".join(map(str, dims)), rA)),
+        # the Dslash half of the metric: fused kernel A, fp32, N_rhs = 8 on configs[2]; without the Dslash report the dominant kernel of the step
+        "roofline": head if head is not None else step_kernels[1],
+        "rooflines": step_kernels + rooflines,
+        "fma_peak": fma,
+        "dslash_sweep": sweep,
+        "cpu_baseline": cpu_baseline(wl["cfg"]),
     }
     line.update(extras)
     print(json.dumps(line))

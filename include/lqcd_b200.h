@@ -23,14 +23,19 @@
  * CANONICAL layouts (row-major, complex = (re, im) pairs of the stated precision):
  *   gauge   U[mu][t][z][y][x][row][col]
  *   spinor  psi[rhs][t][z][y][x][spin][colour]
- * NATIVE spinor layout (what the kernels stream; for timing without reorders):
- *   one parity:  payload[j = 0..23][cb = 0..Vh-1][rhs = 0..N-1]  with j = 2*(3*spin+colour) + (0 re | 1 im),
- *                cb = (site index within the parity) = i_lex / 2 restricted to that parity,
- *                element = double (LQ_FP64), float (LQ_FP32) or int16 (LQ_HALF);
- *   LQ_HALF appends, after the payload rounded up to 256 bytes, fp32 norms[cb][rhs]:
- *                value = q * norm / 32767, norm = max-abs over the 24 reals of that (site, rhs).
- *   full lattice: the even-parity block followed by the odd-parity block (each lq_native_bytes(.., 1)).
- *   The RHS index is innermost so that one SU(3) link / clover block load serves the whole batch.
+ * NATIVE spinor layout (what the kernels stream; for timing without reorders).  One parity of a batch of N right-hand
+ * sides is cut into G = N / R groups of R consecutive right-hand sides (R = 4 if N % 4 == 0, else 2 if N is even, else 1)
+ * and into NB = ceil(Vh / 32) blocks of 32 consecutive checkerboard sites, Vh = V / 2,
+ *                cb = x/2 + (Lx/2) * (y + Ly * (z + Lz * t))   (sites of that parity only; blk = cb / 32, s = cb % 32):
+ *   payload[blk][g][j = 0..23][s = 0..31][r = 0..R-1]   with j = 2*(3*spin + colour) + (0 re | 1 im), rhs = g*R + r,
+ *                i.e. element offset ((blk*G + g)*24 + j)*32*R + s*R + r; elements are double (LQ_FP64), float (LQ_FP32)
+ *                or int16 (LQ_HALF); the payload of one parity is 24*NB*32*N elements rounded up to 256 bytes;
+ *   LQ_HALF appends fp32 norms[blk][g][s][r] (offset (blk*G + g)*32*R + s*R + r; NB*32*N floats rounded up to 256
+ *                bytes): value = q * norm / 32767, norm = max-abs over the 24 reals of that (site, rhs), q = rint(32767 v / norm).
+ *   Sites cb >= Vh of the last block are padding: never read into a result, content unspecified after a call.
+ *   Full lattice: the even-parity block followed by the odd-parity block, each lq_native_bytes(.., parity_only = 1) bytes.
+ *   lq_native_index() returns these offsets, so a caller never has to retype the formula.
+ *   The RHS index is innermost so that one SU(3) link / clover block load serves the whole group.
  *
  * Ownership: the caller owns every buffer it passes; the library copies what it keeps (links)
  * and owns its native copies and scratch.  Device scratch comes from cudaMalloc unless an
@@ -128,6 +133,13 @@ int lq_apply(lq_ctx* ctx, int op, void* out, const void* in, const void* in2, in
 
 /* ---- native layout helpers ------------------------------------------------------------------------ */
 size_t lq_native_bytes(const lq_ctx* ctx, int nrhs, int prec, int parity_only);
+/* Position of (site (x,y,z,t), right-hand side rhs, real j = 2*(3*spin+colour)+(re|im)) in a FULL-lattice native buffer of
+ * nrhs right-hand sides in precision prec: *elem_offset = index of the payload element counted in elements of that precision
+ * from the start of the site's parity block, *norm_offset = index of the fp32 norm counted in floats from the start of that
+ * block's norm array (LQ_HALF; else 0), *parity_block_byte = byte offset of the parity block in the buffer, *norm_array_byte
+ * = byte offset of the norm array inside the parity block (LQ_HALF; else 0).  Host-only arithmetic, no device work. */
+int lq_native_index(const lq_ctx* ctx, int nrhs, int prec, int x, int y, int z, int t, int rhs, int j,
+                    size_t* elem_offset, size_t* norm_offset, size_t* parity_block_byte, size_t* norm_array_byte);
 /* canonical (complex double, at loc) -> native (device, precision prec, full lattice) and back */
 int lq_pack(lq_ctx* ctx, void* native_out, const void* canonical_in, int nrhs, int prec, int loc);
 int lq_unpack(lq_ctx* ctx, void* canonical_out, const void* native_in, int nrhs, int prec, int loc);
@@ -155,8 +167,10 @@ typedef struct {
     int keep_direction;  /* 1: reliable updates (SURVEY 8(c.2) reading #11, 8(f) #3): after each fp64 residual refresh the
                             CG search direction is kept, p <- z_new + c (p - z_old), instead of restarting at p = z   */
     int algorithm;       /* inner solver: LQ_ALG_CGNR (0, default) or LQ_ALG_BICGSTAB (1): batched BiCGStab on Mhat
-                            itself with complex per-RHS scalars, 2 Mhat applications per iteration; no CUDA graph,
+                            itself with complex per-RHS scalars, 2 Mhat applications per iteration;
                             keep_direction ignored                                                       */
+    int use_x0;          /* 1: the even-site part of x on entry is the initial guess (SURVEY 8(b) solve row); 0: zero start,
+                            x is output only                                                             */
 } lq_solve_param;
 
 typedef struct {
@@ -166,13 +180,22 @@ typedef struct {
     int iters[LQ_MAX_RHS];             /* inner iteration count at which RHS k first met tol (estimate; parity unpinned) */
     double true_rel_residual[LQ_MAX_RHS]; /* ||bhat_e - Mhat x_e|| / ||b|| in fp64 = full-system residual   */
     double seconds;                    /* device time of the solve proper (CUDA events), excl. pack/unpack */
-    double dslash_applies;             /* single-parity stencil kernel launches (A or B), all precisions */
+    double dslash_applies;             /* single-parity stencil kernel launches (A or B) that did work, all precisions */
+    double model_bytes;                /* modelled (algorithmic) HBM bytes of the solve: every kernel's compulsory traffic,
+                                          SURVEY 8(d) byte model (stencil: spinor streams + links and clover once per launch;
+                                          block-BLAS: its streams)                                      */
+    double model_flops;                /* counted flops: 1320 hop + 504 clover (+48 xpay) per site per RHS per stencil launch,
+                                          plus the block-BLAS flops                                      */
 } lq_solve_info;
 
 /* Solves M x = b for nrhs independent right-hand sides (no block-Krylov coupling).  b, x: full-lattice
  * complex double, CANONICAL at `loc`, or NATIVE LQ_FP64 device buffers.  x is output only (zero start).
+ * CANONICAL host buffers are staged one right-hand side at a time (device staging = one canonical RHS, not the batch).
+ * x is output only unless param->use_x0.
  * Even-odd preconditioned CGNR (or, param->algorithm = LQ_ALG_BICGSTAB, batched BiCGStab on Mhat) in inner_prec inside an
- * fp64 defect correction.  Returns LQ_ENOTCONVERGED (x, info still valid) if any RHS misses tol. */
+ * fp64 defect correction.  The iteration body is replayed as a CUDA graph cached in the context;
+ * convergence is tested on the device and the host reads the flag one graph behind, so no launch waits for the host.
+ * Returns LQ_ENOTCONVERGED (x, info still valid) if any RHS misses tol. */
 int lq_solve(lq_ctx* ctx, void* x, const void* b, int nrhs, int loc, int layout, const lq_solve_param* param, lq_solve_info* info);
 
 /* ---- 3-d gauge-covariant Laplacian ------------------------
@@ -230,6 +253,13 @@ int lq_project(lq_ctx* ctx, void* P, const void* evecs, int n_ev, const void* so
  * must divide the group width), and
  * the L2 prefetch distance of the stencil kernels in 32-site blocks (0 = off, negative = library default). */
 int lq_set_tuning(lq_ctx* ctx, int dslash_variant, int dslash_rpt, int dslash_pfd);
+
+/* Plain FP32 ALU peak of this GPU measured with register-only FMA loops ("measure an FMA microbenchmark on
+ * the box and use that" as the denominator of the ALU roofline fraction).  mode 0: scalar FFMA, 1: packed FFMA2 with three
+ * distinct 64-bit operands, 2: packed FFMA2 whose first operand is shared by 4 consecutive instructions (the stencil kernels'
+ * pattern: one link element against 4 spinor reals).  Runs for about `ms` milliseconds on the context's stream, synchronises,
+ * and writes TFLOP/s (2 flops per FMA lane) to *tflops. */
+int lq_fma_peak(lq_ctx* ctx, int mode, double ms, double* tflops);
 
 /* Number of kernels this library has launched on this context since creation (for bench.py). */
 long long lq_kernel_launches(const lq_ctx* ctx);

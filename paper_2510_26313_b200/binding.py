@@ -26,14 +26,14 @@ PREC = {"fp64": LQ_FP64, "fp32": LQ_FP32, "half": LQ_HALF}
 
 EXPORTS = ["lq_create", "lq_destroy", "lq_last_error", "lq_set_allocator", "lq_load_gauge", "lq_fill_gauge_random",
            "lq_build_clover", "lq_apply", "lq_native_bytes", "lq_pack", "lq_unpack", "lq_fill_spinor_random", "lq_solve",
-           "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites",
+           "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites", "lq_native_index", "lq_fma_peak",
            "lq_laplacian", "lq_laplacian_native", "lq_cv_native_bytes", "lq_cv_fill_random", "lq_laph_eigensolve", "lq_project"]
 
 
 class SolveParam(ctypes.Structure):
     _fields_ = [("tol", ctypes.c_double), ("max_outer", ctypes.c_int), ("max_inner", ctypes.c_int), ("inner_prec", ctypes.c_int),
                 ("delta", ctypes.c_double), ("check_every", ctypes.c_int), ("use_graph", ctypes.c_int),
-                ("keep_direction", ctypes.c_int), ("algorithm", ctypes.c_int)]
+                ("keep_direction", ctypes.c_int), ("algorithm", ctypes.c_int), ("use_x0", ctypes.c_int)]
 
 
 class EigParam(ctypes.Structure):
@@ -49,7 +49,8 @@ class EigInfo(ctypes.Structure):
 class SolveInfo(ctypes.Structure):
     _fields_ = [("nrhs", ctypes.c_int), ("outer_cycles", ctypes.c_int), ("inner_iters", ctypes.c_int),
                 ("iters", ctypes.c_int * LQ_MAX_RHS), ("true_rel_residual", ctypes.c_double * LQ_MAX_RHS),
-                ("seconds", ctypes.c_double), ("dslash_applies", ctypes.c_double)]
+                ("seconds", ctypes.c_double), ("dslash_applies", ctypes.c_double), ("model_bytes", ctypes.c_double),
+                ("model_flops", ctypes.c_double)]
 
 
 ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
@@ -96,6 +97,9 @@ def load_library():
     lib.lq_project.argtypes = [vp, vp, vp, ci, vp, ci, ci, ci]
     lib.lq_laph_eigensolve.argtypes = [vp, vp, vp, ci, ctypes.POINTER(EigParam), ctypes.POINTER(EigInfo)]
     lib.lq_kernel_launches.argtypes = [vp]; lib.lq_kernel_launches.restype = ctypes.c_longlong
+    szp = ctypes.POINTER(ctypes.c_size_t)
+    lib.lq_native_index.argtypes = [vp, ci, ci, ci, ci, ci, ci, ci, ci, szp, szp, szp, szp]
+    lib.lq_fma_peak.argtypes = [vp, ci, cd, ctypes.POINTER(cd)]
     _lib = lib
     return lib
 
@@ -200,6 +204,22 @@ class Context:
     def native_empty(self, nrhs: int, prec: int, parity_only: bool = False):
         return self.torch.empty(self.native_bytes(nrhs, prec, parity_only), dtype=self.torch.uint8, device="cuda:%d" % self.device)
 
+    def native_index(self, nrhs: int, prec: int, site, rhs: int, j: int):
+        """(element offset in the parity block, norm offset, byte offset of the parity block, byte offset of the norm array)."""
+        o = [ctypes.c_size_t() for _ in range(4)]
+        x, y, z, t = (int(v) for v in site)
+        rc = self.lib.lq_native_index(self.h, nrhs, prec, x, y, z, t, rhs, j, *[ctypes.byref(v) for v in o])
+        if rc != 0:
+            raise LqError(rc, "lq_native_index: bad argument")
+        return tuple(int(v.value) for v in o)
+
+    def fma_peak(self, mode: int = 0, ms: float = 200.0) -> float:
+        """Measured FP32 FMA peak in TFLOP/s (mode 0 scalar FFMA, 1 FFMA2 with distinct operands, 2 FFMA2 with a shared operand)."""
+        self._enter()
+        out = ctypes.c_double()
+        self._check(self.lib.lq_fma_peak(self.h, mode, ms, ctypes.byref(out)))
+        return float(out.value)
+
     def pack(self, canonical, nrhs: int, prec: int):
         self._enter()
         out = self.native_empty(nrhs, prec)
@@ -301,11 +321,11 @@ class Context:
     # ------------------------------------------------------------------ solve
     def solve(self, b, tol: float, inner_prec: int = LQ_FP32, delta: float = 1e-3, max_outer: int = 50, max_inner: int = 2000,
               check_every: int = 10, use_graph: bool = False, x_out=None, native: bool = False, nrhs: int | None = None,
-              keep_direction: bool = True, algorithm: int = 0):
+              keep_direction: bool = True, algorithm: int = 0, use_x0: bool = False):
         """Solves M x = b.  b: canonical complex128 numpy / torch array (host or device), or a native fp64 device
-        buffer when native=True (then nrhs is required).  Returns (x, info dict)."""
+        buffer when native=True (then nrhs is required).  use_x0: x_out holds the initial guess.  Returns (x, info dict)."""
         self._enter()
-        prm = SolveParam(tol, max_outer, max_inner, inner_prec, delta, check_every, int(use_graph), int(keep_direction), int(algorithm))
+        prm = SolveParam(tol, max_outer, max_inner, inner_prec, delta, check_every, int(use_graph), int(keep_direction), int(algorithm), int(use_x0))
         info = SolveInfo()
         if native:
             x = x_out if x_out is not None else self.native_empty(nrhs, LQ_FP64)
@@ -325,5 +345,5 @@ class Context:
         self._check(rc, allow=(LQ_ENOTCONVERGED,))
         d = dict(converged=(rc == 0), nrhs=info.nrhs, outer_cycles=info.outer_cycles, inner_iters=info.inner_iters,
                  iters=list(info.iters)[:nrhs], true_rel_residual=list(info.true_rel_residual)[:nrhs], seconds=info.seconds,
-                 dslash_applies=info.dslash_applies)
+                 dslash_applies=info.dslash_applies, model_bytes=info.model_bytes, model_flops=info.model_flops)
         return x, d

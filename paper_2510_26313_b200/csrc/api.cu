@@ -3,8 +3,6 @@
 #include <string.h>
 #include "internal.cuh"
 
-void solver_forget(lq_ctx* c);
-int mhat_native(lq_ctx* c, int prec, int n, void* out_e, const void* in_e, int dagger);
 
 int set_err(lq_ctx* c, int code, const std::string& msg) {
     if (c) c->err = msg;
@@ -57,6 +55,7 @@ int lq_create(lq_ctx** out, const int dims[4], int device, void* cuda_stream) {
     c->alloc_fn = nullptr; c->free_fn = nullptr; c->alloc_user = nullptr;
     c->launches = 0; c->dslash_rpt = 0; c->dslash_variant = 0; c->dslash_pfd = LQ_DEFAULT_PFD; c->dslash_zc = 0;
     c->red_partials = nullptr; c->red_partials_elems = 0; c->red_counter = nullptr; c->h_scalars = nullptr; c->d_flag = nullptr;
+    c->ws = nullptr; c->loop_skip = nullptr; c->model_bytes = c->model_flops = 0.0; c->proj_scratch = nullptr; c->proj_scratch_bytes = 0;
     if (cudaMalloc(&c->red_counter, RED_COUNTER_BYTES) != cudaSuccess || cudaMemset(c->red_counter, 0, RED_COUNTER_BYTES) != cudaSuccess ||
         cudaMallocHost(&c->h_scalars, 8 * LQ_MAX_RHS * sizeof(double)) != cudaSuccess) { cudaGetLastError(); delete c; return LQ_ECUDA; }
     c->d_flag = (int*)(c->red_counter + 16);
@@ -68,7 +67,7 @@ int lq_destroy(lq_ctx* c) {
     if (!c) return LQ_EINVAL;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
-    solver_forget(c);
+    solver_release(c);
     std::vector<void*> owned = c->owned;
     for (void* p : owned) dev_free(c, p);
     cudaFree(c->red_counter);
@@ -161,28 +160,81 @@ static const void* stage_in(lq_ctx* c, const void* p, size_t bytes, int loc, voi
     return *staging;
 }
 
+// Host canonical arrays are staged through ONE device buffer of at most ~2 GiB, a few right-hand sides at a time: the device
+// never holds a canonical copy of the whole batch (configs[3]: 24.5 GB per field).  nk = right-hand sides per chunk.
+static int chunk_rhs(const lq_ctx* c, int nrhs) {
+    const size_t per = (size_t)c->g.V * 24 * sizeof(double);
+    size_t nk = ((size_t)2 << 30) / per;
+    if (nk < 1) nk = 1;
+    return nk > (size_t)nrhs ? nrhs : (int)nk;
+}
+// canonical complex double (host or device) -> native full-lattice batch
+static int pack_any(lq_ctx* c, void* native_out, const void* canonical_in, int nrhs, int prec, int loc) {
+    if (loc == LQ_DEVICE) return spinor_pack(c, native_out, canonical_in, nrhs, prec, LQ_FP64);
+    const size_t per = (size_t)c->g.V * 24 * sizeof(double);
+    const int nk = chunk_rhs(c, nrhs);
+    void* st = dev_alloc(c, per * nk);
+    if (!st) return LQ_ENOMEM;
+    int rc = 0;
+    for (int k0 = 0; k0 < nrhs && rc == 0; k0 += nk) {
+        const int m = nrhs - k0 < nk ? nrhs - k0 : nk;
+        if (cudaMemcpyAsync(st, (const char*)canonical_in + per * k0, per * m, cudaMemcpyHostToDevice, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "H2D copy failed");
+        if (rc == 0) rc = spinor_pack_part(c, native_out, st, nrhs, k0, m, prec, LQ_FP64);
+    }
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess && rc == 0) rc = set_err(c, LQ_ECUDA, "pack failed");
+    dev_free(c, st);
+    return rc;
+}
+static int unpack_any(lq_ctx* c, void* canonical_out, const void* native_in, int nrhs, int prec, int loc) {
+    if (loc == LQ_DEVICE) return spinor_unpack(c, canonical_out, native_in, nrhs, prec, LQ_FP64);
+    const size_t per = (size_t)c->g.V * 24 * sizeof(double);
+    const int nk = chunk_rhs(c, nrhs);
+    void* st = dev_alloc(c, per * nk);
+    if (!st) return LQ_ENOMEM;
+    int rc = 0;
+    for (int k0 = 0; k0 < nrhs && rc == 0; k0 += nk) {
+        const int m = nrhs - k0 < nk ? nrhs - k0 : nk;
+        rc = spinor_unpack_part(c, st, native_in, nrhs, k0, m, prec, LQ_FP64);
+        if (rc == 0 && cudaMemcpyAsync((char*)canonical_out + per * k0, st, per * m, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "D2H copy failed");
+    }
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess && rc == 0) rc = set_err(c, LQ_ECUDA, "unpack failed");
+    dev_free(c, st);
+    return rc;
+}
+
 int lq_pack(lq_ctx* c, void* native_out, const void* canonical_in, int nrhs, int prec, int loc) {
     if (!c || !native_out || !canonical_in || !nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "lq_pack: bad argument");
     cudaSetDevice(c->device);
-    const size_t bytes = (size_t)nrhs * c->g.V * 24 * sizeof(double);
-    void* st; const void* dev = stage_in(c, canonical_in, bytes, loc, &st);
-    if (!dev) return LQ_ENOMEM;
-    int rc = spinor_pack(c, native_out, dev, nrhs, prec, LQ_FP64);
+    int rc = pack_any(c, native_out, canonical_in, nrhs, prec, loc);
     if (rc == 0 && cudaStreamSynchronize(c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "pack failed");
-    if (st) dev_free(c, st);
     return rc;
 }
 int lq_unpack(lq_ctx* c, void* canonical_out, const void* native_in, int nrhs, int prec, int loc) {
     if (!c || !canonical_out || !native_in || !nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "lq_unpack: bad argument");
     cudaSetDevice(c->device);
-    const size_t bytes = (size_t)nrhs * c->g.V * 24 * sizeof(double);
-    void* dev = canonical_out; void* st = nullptr;
-    if (loc == LQ_HOST) { st = dev_alloc(c, bytes); if (!st) return LQ_ENOMEM; dev = st; }
-    int rc = spinor_unpack(c, dev, native_in, nrhs, prec, LQ_FP64);
-    if (rc == 0 && st && cudaMemcpyAsync(canonical_out, st, bytes, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "D2H copy failed");
+    int rc = unpack_any(c, canonical_out, native_in, nrhs, prec, loc);
     if (rc == 0 && cudaStreamSynchronize(c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "unpack failed");
-    if (st) dev_free(c, st);
     return rc;
+}
+
+int lq_native_index(const lq_ctx* c, int nrhs, int prec, int x, int y, int z, int t, int rhs, int j,
+                    size_t* elem_offset, size_t* norm_offset, size_t* parity_block_byte, size_t* norm_array_byte) {
+    if (!c || !nrhs_ok(nrhs) || rhs < 0 || rhs >= nrhs || j < 0 || j >= 24 || (prec != LQ_FP64 && prec != LQ_FP32 && prec != LQ_HALF)) return LQ_EINVAL;
+    const int xs[4] = {x, y, z, t};
+    for (int k = 0; k < 4; k++) if (xs[k] < 0 || xs[k] >= c->g.L[k]) return LQ_EINVAL;
+    int parity, cb;
+    coords_to_cb(c->g, x, y, z, t, parity, cb);
+    if (elem_offset) *elem_offset = sp_index(nrhs, cb, rhs, j);
+    if (norm_offset) *norm_offset = prec == LQ_HALF ? nrm_index(nrhs, cb, rhs) : 0;
+    if (parity_block_byte) *parity_block_byte = (size_t)parity * parity_bytes(c->g, nrhs, prec);
+    if (norm_array_byte) *norm_array_byte = prec == LQ_HALF ? round256((size_t)24 * c->g.NB * SB * nrhs * elem_bytes(prec)) : 0;
+    return 0;
+}
+
+int lq_fma_peak(lq_ctx* c, int mode, double ms, double* tflops) {
+    if (!c || !tflops || mode < 0 || mode > 2 || !(ms > 0)) return set_err(c, LQ_EINVAL, "lq_fma_peak: bad argument");
+    cudaSetDevice(c->device);
+    return fma_peak(c, mode, ms, tflops);
 }
 
 int lq_fill_spinor_random(lq_ctx* c, void* native_out, int nrhs, int prec, uint64_t seed, int parity_only, int parity) {
@@ -369,23 +421,16 @@ int lq_solve(lq_ctx* c, void* x, const void* b, int nrhs, int loc, int layout, c
         if (loc != LQ_DEVICE) return set_err(c, LQ_EINVAL, "native buffers must be device buffers");
         return solve_native(c, x, b, nrhs, param, info);
     }
-    const size_t cbytes = (size_t)nrhs * c->g.V * 24 * sizeof(double);
     const size_t pb = parity_bytes(c->g, nrhs, LQ_FP64);
-    void *st_b = nullptr, *st_x = nullptr;
     void *n_b = dev_alloc(c, 2 * pb), *n_x = dev_alloc(c, 2 * pb);
     int rc = (!n_b || !n_x) ? LQ_ENOMEM : 0;
-    const void* d_b = nullptr;
-    if (rc == 0) { d_b = stage_in(c, b, cbytes, loc, &st_b); if (!d_b) rc = LQ_ENOMEM; }
-    if (rc == 0) rc = spinor_pack(c, n_b, d_b, nrhs, LQ_FP64, LQ_FP64);
-    if (st_b && rc == 0) { cudaStreamSynchronize(c->stream); dev_free(c, st_b); st_b = nullptr; }
+    if (rc == 0) rc = pack_any(c, n_b, b, nrhs, LQ_FP64, loc);
+    if (rc == 0 && param->use_x0) rc = pack_any(c, n_x, x, nrhs, LQ_FP64, loc);
     int src = 0;
     if (rc == 0) { src = solve_native(c, n_x, n_b, nrhs, param, info); if (src != 0 && src != LQ_ENOTCONVERGED) rc = src; }
-    void* d_x = x;
-    if (rc == 0 && loc == LQ_HOST) { st_x = dev_alloc(c, cbytes); if (!st_x) rc = LQ_ENOMEM; d_x = st_x; }
-    if (rc == 0) rc = spinor_unpack(c, d_x, n_x, nrhs, LQ_FP64, LQ_FP64);
-    if (rc == 0 && st_x && cudaMemcpyAsync(x, st_x, cbytes, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "D2H copy failed");
+    if (rc == 0) rc = unpack_any(c, x, n_x, nrhs, LQ_FP64, loc);
     if (cudaStreamSynchronize(c->stream) != cudaSuccess && rc == 0) rc = set_err(c, LQ_ECUDA, std::string("lq_solve: ") + cudaGetErrorString(cudaGetLastError()));
-    void* tofree[] = {st_b, st_x, n_b, n_x};
+    void* tofree[] = {n_b, n_x};
     for (void* p : tofree) if (p) dev_free(c, p);
     return rc ? rc : src;
 }

@@ -28,10 +28,12 @@ template <int VW, int R> struct BlasIdx {
     }
 };
 
-struct BlasGeom { Geom g; int N, G; };
+struct BlasGeom { Geom g; int N, G; const int* skip; };   // skip: see lq_ctx::loop_skip
+#define LQ_BLAS_SKIP(bg) do { if ((bg).skip != nullptr && *(volatile const int*)(bg).skip) return; } while (0)
 
 template <class S, int VW, int R>
 __global__ void norm2_kernel(BlasGeom bg, SView<S> x, double* partials, unsigned int* counter, double* out) {
+    LQ_BLAS_SKIP(bg);
     using T = typename S::comp_t;
     BlasIdx<VW, R> ix(bg.g, bg.G);
     double part[VW];
@@ -52,6 +54,7 @@ __global__ void norm2_kernel(BlasGeom bg, SView<S> x, double* partials, unsigned
 template <class S, int VW, int R>
 __global__ void cg_update_ep_kernel(BlasGeom bg, SView<S> e, SView<S> p, SView<S> z, const double* __restrict__ rr, const double* __restrict__ pAp,
                                     const double* __restrict__ rr_new) {
+    LQ_BLAS_SKIP(bg);
     using T = typename S::comp_t;
     BlasIdx<VW, R> ix(bg.g, bg.G);
     if (!ix.valid) return;
@@ -78,9 +81,10 @@ __global__ void cg_update_ep_kernel(BlasGeom bg, SView<S> e, SView<S> p, SView<S
     store_site_regs<S, VW, R>(p.d + ix.own, S::has_norm ? p.n + ix.own_n : nullptr, b);
 }
 
-// p <- z_new + c (p - z_old)
+// p <- z_new + c (p - z_old) ; z_old <- z_new  (the vector buffers keep their roles, so the cached iteration graph stays valid)
 template <class S, int VW, int R>
 __global__ void keep_direction_kernel(BlasGeom bg, SView<S> p, SView<S> zo, SView<S> zn, const double* __restrict__ cs) {
+    LQ_BLAS_SKIP(bg);
     using T = typename S::comp_t;
     BlasIdx<VW, R> ix(bg.g, bg.G);
     if (!ix.valid) return;
@@ -95,6 +99,7 @@ __global__ void keep_direction_kernel(BlasGeom bg, SView<S> p, SView<S> zo, SVie
 #pragma unroll
         for (int k = 0; k < VW; k++) a[j][k] = cf[k] * (a[j][k] - b[j][k]);
     load_site_regs<S, VW, R>(zn.d + ix.own, S::has_norm ? zn.n + ix.own_n : nullptr, b);
+    store_site_regs<S, VW, R>(zo.d + ix.own, S::has_norm ? zo.n + ix.own_n : nullptr, b);
 #pragma unroll
     for (int j = 0; j < 24; j++)
 #pragma unroll
@@ -105,6 +110,7 @@ __global__ void keep_direction_kernel(BlasGeom bg, SView<S> p, SView<S> zo, SVie
 // y (fp64) += s_k * e
 template <class S, int VW, int R>
 __global__ void axpy_mixed_kernel(BlasGeom bg, double* __restrict__ y, SView<S> ev, const double* __restrict__ scale) {
+    LQ_BLAS_SKIP(bg);
     using T = typename S::comp_t;
     BlasIdx<VW, R> ix(bg.g, bg.G);
     if (!ix.valid) return;
@@ -120,6 +126,7 @@ __global__ void axpy_mixed_kernel(BlasGeom bg, double* __restrict__ y, SView<S> 
 template <int VW, int R>
 __global__ void residual_kernel(BlasGeom bg, double* __restrict__ r, const double* __restrict__ b, const double* __restrict__ tv,
                                 double* partials, unsigned int* counter, double* out) {
+    LQ_BLAS_SKIP(bg);
     BlasIdx<VW, R> ix(bg.g, bg.G);
     double part[VW];
 #pragma unroll
@@ -139,10 +146,12 @@ __global__ void residual_kernel(BlasGeom bg, double* __restrict__ r, const doubl
 
 // ---- host side -----------------------------------------------------------------------------------------------------
 struct Launch { BlasGeom bg; int R, vw, block, grid; size_t smem; };
+// modelled work of a block-BLAS launch: `streams` passes over a parity batch in precision prec, `fl` flops per site per RHS
+#define BLAS_MODEL(c, prec, nrhs, streams, fl) LQ_MODEL(c, (streams) * stream_bytes((c)->g, nrhs, prec), (double)(fl) * (c)->g.Vh * (nrhs))
 static int plan(lq_ctx* c, int nrhs, int maxvw, Launch& L) {
     const int R = group_width(nrhs);
     L.R = R; L.vw = R < maxvw ? R : maxvw;
-    L.bg.g = c->g; L.bg.N = nrhs; L.bg.G = nrhs / R;
+    L.bg.g = c->g; L.bg.N = nrhs; L.bg.G = nrhs / R; L.bg.skip = c->loop_skip;
     L.block = 128;
     const long long threads = (long long)c->g.NB * L.bg.G * SB * (R / L.vw);
     L.grid = (int)((threads + L.block - 1) / L.block);
@@ -164,6 +173,7 @@ template <class S> static int norm2_t(lq_ctx* c, int nrhs, const void* x, double
     SView<S> vx = make_view<S>(c->g, const_cast<void*>(x), nrhs, 0);
     VW_DISPATCH(L, S, norm2_kernel, L.smem, L.bg, vx, c->red_partials, c->red_counter, d_out);
     LQ_LAUNCHED(c);
+    BLAS_MODEL(c, S::prec, nrhs, 1, 48);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
@@ -178,6 +188,7 @@ template <class S> static int ep_t(lq_ctx* c, int nrhs, void* e, void* p, const 
     SView<S> ve = make_view<S>(c->g, e, nrhs, 0), vp = make_view<S>(c->g, p, nrhs, 0), vz = make_view<S>(c->g, const_cast<void*>(z), nrhs, 0);
     VW_DISPATCH(L, S, cg_update_ep_kernel, 0, L.bg, ve, vp, vz, rr, pAp, rrn);
     LQ_LAUNCHED(c);
+    BLAS_MODEL(c, S::prec, nrhs, 5, 96);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
@@ -187,15 +198,16 @@ int blas_cg_update_ep(lq_ctx* c, int prec, int nrhs, void* e, void* p, const voi
     return ep_t<H16>(c, nrhs, e, p, z, d_rr, d_pAp, d_rr_new);
 }
 
-template <class S> static int keep_t(lq_ctx* c, int nrhs, void* p, const void* zo, const void* zn, const double* cs) {
+template <class S> static int keep_t(lq_ctx* c, int nrhs, void* p, void* zo, const void* zn, const double* cs) {
     Launch L; LQ_TRY(plan(c, nrhs, S::prec == LQ_FP64 ? 2 : 4, L));
-    SView<S> vp = make_view<S>(c->g, p, nrhs, 0), vo = make_view<S>(c->g, const_cast<void*>(zo), nrhs, 0), vn = make_view<S>(c->g, const_cast<void*>(zn), nrhs, 0);
+    SView<S> vp = make_view<S>(c->g, p, nrhs, 0), vo = make_view<S>(c->g, zo, nrhs, 0), vn = make_view<S>(c->g, const_cast<void*>(zn), nrhs, 0);
     VW_DISPATCH(L, S, keep_direction_kernel, 0, L.bg, vp, vo, vn, cs);
     LQ_LAUNCHED(c);
+    BLAS_MODEL(c, S::prec, nrhs, 5, 96);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
-int blas_keep_direction(lq_ctx* c, int prec, int nrhs, void* p, const void* z_old, const void* z_new, const double* d_c) {
+int blas_keep_direction(lq_ctx* c, int prec, int nrhs, void* p, void* z_old, const void* z_new, const double* d_c) {
     if (prec == LQ_FP64) return keep_t<F64>(c, nrhs, p, z_old, z_new, d_c);
     if (prec == LQ_FP32) return keep_t<F32>(c, nrhs, p, z_old, z_new, d_c);
     return keep_t<H16>(c, nrhs, p, z_old, z_new, d_c);
@@ -206,6 +218,7 @@ template <class S> static int axpy_t(lq_ctx* c, int nrhs, void* y, const void* e
     SView<S> ve = make_view<S>(c->g, const_cast<void*>(e), nrhs, 0);
     VW_DISPATCH(L, S, axpy_mixed_kernel, 0, L.bg, (double*)y, ve, s);
     LQ_LAUNCHED(c);
+    BLAS_MODEL(c, S::prec, nrhs, 1, 48); BLAS_MODEL(c, LQ_FP64, nrhs, 2, 0);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
@@ -222,12 +235,14 @@ int blas_residual(lq_ctx* c, int nrhs, void* r, const void* b, const void* t, do
     else if (L.R == 2) residual_kernel<2, 2><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, rp, bp, tp, c->red_partials, c->red_counter, d_out);
     else residual_kernel<1, 1><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, rp, bp, tp, c->red_partials, c->red_counter, d_out);
     LQ_LAUNCHED(c);
+    BLAS_MODEL(c, LQ_FP64, nrhs, 3, 72);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
 
 int blas_copy(lq_ctx* c, int prec, int nrhs, void* dst, const void* src) {
     LQ_CUDA(c, cudaMemcpyAsync(dst, src, parity_bytes(c->g, nrhs, prec), cudaMemcpyDeviceToDevice, c->stream));
+    BLAS_MODEL(c, prec, nrhs, 2, 0);
     return 0;
 }
 
@@ -266,6 +281,7 @@ __device__ __forceinline__ void caxpy_regs(const T (&sr)[VW], const T (&si)[VW],
 // out = (Re <a, b>, Im <a, b>, ||a||^2) per RHS, <a, b> = sum conj(a) b
 template <class S, int VW, int R>
 __global__ void cdot3_kernel(BlasGeom bg, SView<S> a, SView<S> b, double* partials, unsigned int* counter, double* out) {
+    LQ_BLAS_SKIP(bg);
     using T = typename S::comp_t;
     BlasIdx<VW, R> ix(bg.g, bg.G);
     double part[3][VW];
@@ -291,6 +307,7 @@ __global__ void cdot3_kernel(BlasGeom bg, SView<S> a, SView<S> b, double* partia
 // s = r - alpha v
 template <class S, int VW, int R>
 __global__ void bicg_s_kernel(BlasGeom bg, SView<S> s, SView<S> r, SView<S> v, const double* __restrict__ rho, const double* __restrict__ c1) {
+    LQ_BLAS_SKIP(bg);
     using T = typename S::comp_t;
     BlasIdx<VW, R> ix(bg.g, bg.G);
     if (!ix.valid) return;
@@ -309,6 +326,7 @@ template <class S, int VW, int R>
 __global__ void bicg_xr_kernel(BlasGeom bg, SView<S> e, SView<S> r, SView<S> p, SView<S> s, SView<S> tv, SView<S> rhat,
                                const double* __restrict__ rho, const double* __restrict__ c1, const double* __restrict__ d2,
                                double* partials, unsigned int* counter, double* out) {
+    LQ_BLAS_SKIP(bg);
     using T = typename S::comp_t;
     BlasIdx<VW, R> ix(bg.g, bg.G);
     double part[3][VW];
@@ -349,6 +367,7 @@ __global__ void bicg_xr_kernel(BlasGeom bg, SView<S> e, SView<S> r, SView<S> p, 
 template <class S, int VW, int R>
 __global__ void bicg_p_kernel(BlasGeom bg, SView<S> p, SView<S> r, SView<S> v, const double* __restrict__ rho, const double* __restrict__ rho_new,
                               const double* __restrict__ c1, const double* __restrict__ d2) {
+    LQ_BLAS_SKIP(bg);
     using T = typename S::comp_t;
     BlasIdx<VW, R> ix(bg.g, bg.G);
     if (!ix.valid) return;
@@ -390,6 +409,7 @@ template <class S> static int cdot3_t(lq_ctx* c, int nrhs, const void* a, const 
     SView<S> va = make_view<S>(c->g, const_cast<void*>(a), nrhs, 0), vb = make_view<S>(c->g, const_cast<void*>(b), nrhs, 0);
     VW2_DISPATCH(L, S, cdot3_kernel, L.smem, L.bg, va, vb, c->red_partials, c->red_counter, d_out);
     LQ_LAUNCHED(c);
+    BLAS_MODEL(c, S::prec, nrhs, 2, 144);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
@@ -400,6 +420,7 @@ template <class S> static int bicg_s_t(lq_ctx* c, int nrhs, void* s, const void*
     SView<S> vs = make_view<S>(c->g, s, nrhs, 0), vr = make_view<S>(c->g, const_cast<void*>(r), nrhs, 0), vv = make_view<S>(c->g, const_cast<void*>(v), nrhs, 0);
     VW2_DISPATCH(L, S, bicg_s_kernel, 0, L.bg, vs, vr, vv, rho, c1);
     LQ_LAUNCHED(c);
+    BLAS_MODEL(c, S::prec, nrhs, 3, 96);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
@@ -414,6 +435,7 @@ template <class S> static int bicg_xr_t(lq_ctx* c, int nrhs, void* e, void* r, c
              vh = make_view<S>(c->g, const_cast<void*>(rhat), nrhs, 0);
     VW2_DISPATCH(L, S, bicg_xr_kernel, L.smem, L.bg, ve, vr, vp, vs, vt, vh, rho, c1, d2, c->red_partials, c->red_counter, d_out);
     LQ_LAUNCHED(c);
+    BLAS_MODEL(c, S::prec, nrhs, 7, 432);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
@@ -428,6 +450,7 @@ template <class S> static int bicg_p_t(lq_ctx* c, int nrhs, void* p, const void*
     SView<S> vp = make_view<S>(c->g, p, nrhs, 0), vr = make_view<S>(c->g, const_cast<void*>(r), nrhs, 0), vv = make_view<S>(c->g, const_cast<void*>(v), nrhs, 0);
     VW2_DISPATCH(L, S, bicg_p_kernel, 0, L.bg, vp, vr, vv, rho, rho_new, c1, d2);
     LQ_LAUNCHED(c);
+    BLAS_MODEL(c, S::prec, nrhs, 4, 192);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }

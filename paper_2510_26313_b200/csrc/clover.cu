@@ -167,6 +167,7 @@ int clover_build(lq_ctx* c, double kappa, double csw) {
         c->clov32 = (float*)dev_alloc(c, n * 4); c->clovinv32 = (float*)dev_alloc(c, n * 4);
         if (!c->clov64 || !c->clovinv64 || !c->clov32 || !c->clovinv32) return LQ_ENOMEM;
     }
+    c->has_clover = false;      // the stored blocks are overwritten below: valid again only if every block is positive definite
     LQ_CUDA(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int), c->stream));
     const int threads = 2 * c->g.Vh;
     clover_build_kernel<<<(threads + 63) / 64, 64, 0, c->stream>>>(c->g, c->gauge64, kappa * csw, c->clov64, c->clovinv64, c->d_flag);

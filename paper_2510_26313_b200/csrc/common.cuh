@@ -92,6 +92,8 @@ inline size_t parity_bytes(const Geom& g, int nrhs, int prec) {
     if (prec == LQ_HALF) pay += round256((size_t)g.NB * SB * nrhs * sizeof(float));
     return pay;
 }
+// algorithmic bytes of one pass over one parity of a batch (payload + norms)
+inline double stream_bytes(const Geom& g, int nrhs, int prec) { return (double)g.Vh * nrhs * (24.0 * elem_bytes(prec) + (prec == LQ_HALF ? 4.0 : 0.0)); }
 template <class S> inline SView<S> make_view(const Geom& g, void* base, int nrhs, int parity_block) {
     char* p = (char*)base + (size_t)parity_block * parity_bytes(g, nrhs, S::prec);
     SView<S> v;
@@ -179,6 +181,15 @@ struct lq_ctx {
     unsigned int* red_counter;
     double* h_scalars;              // pinned host, 8*LQ_MAX_RHS doubles
     int* d_flag;                    // device error flag
+    // solver state (solver.cu): workspace with the cached iteration graph, owned by the context
+    struct SolverWorkspace* ws;
+    // while the solver enqueues the body of an inner iteration: device flag that makes every kernel of the body return
+    // at once when set (the inner solve has converged; launches already queued behind the flag become no-ops)
+    const int* loop_skip;
+    // modelled work of everything launched so far (SURVEY 8(d) byte / flop model; lq_solve_info)
+    double model_bytes, model_flops;
+    // projection scratch kept between calls (project_tc.cu)
+    void* proj_scratch; size_t proj_scratch_bytes;
 };
 
 int set_err(lq_ctx* c, int code, const std::string& msg);
@@ -199,4 +210,6 @@ int ensure_partials(lq_ctx* c, size_t elems);      // reduction scratch of at le
     } while (0)
 #define LQ_TRY(x) do { int r_ = (x); if (r_ != 0) return r_; } while (0)
 #define LQ_LAUNCHED(ctx) do { (ctx)->launches++; } while (0)
+// modelled (algorithmic) bytes and counted flops of one launch
+#define LQ_MODEL(ctx, bytes, flops) do { (ctx)->model_bytes += (double)(bytes); (ctx)->model_flops += (double)(flops); } while (0)
 

@@ -46,6 +46,7 @@ template <class S> struct DslashArgs {
     double* epi_out;                   // per-RHS sums (device); EPI_CDOT: 3 x LQ_MAX_RHS
     SView<S> epi_v; int epi_conj;      // EPI_CDOT: h (on `parity`), conjugate the inner product
     double* red_partials; unsigned int* red_counter;   // reduction scratch of the context
+    const int* skip;       // device flag or nullptr: when set the launch is a no-op (lq_ctx::loop_skip, solver.cu)
 };
 
 __device__ __forceinline__ float fm(float a, float b, float c) { return fmaf(a, b, c); }

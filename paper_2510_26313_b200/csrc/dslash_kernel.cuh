@@ -159,6 +159,7 @@ template <class S, int RPT, int R, int RECON, int FORM, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S> a) {
     using T = typename S::comp_t;
     using ST = typename S::store_t;
+    if (a.skip != nullptr && *(volatile const int*)a.skip) return;      // the inner solve has converged (grid-uniform)
     constexpr int TPG = R / RPT;            // lanes per (site, group)
     constexpr int UT = SB * TPG;            // threads per unit
     constexpr int US = 24 * SB * R;         // payload elements per unit

@@ -27,6 +27,9 @@ int gauge_ingest(lq_ctx* c, const void* dev_canonical, int in_prec);            
 int gauge_make_fp32(lq_ctx* c, int recon);                                       // native fp64 -> native fp32 (18 or 12)
 int spinor_pack(lq_ctx* c, void* native_full, const void* dev_canonical, int nrhs, int prec, int in_prec);
 int spinor_unpack(lq_ctx* c, void* dev_canonical, const void* native_full, int nrhs, int prec, int out_prec);
+// the same for right-hand sides k0 .. k0+nk-1 only: dev_canonical holds just those nk fields (host buffers are staged in such chunks)
+int spinor_pack_part(lq_ctx* c, void* native_full, const void* dev_canonical, int nrhs, int k0, int nk, int prec, int in_prec);
+int spinor_unpack_part(lq_ctx* c, void* dev_canonical, const void* native_full, int nrhs, int k0, int nk, int prec, int out_prec);
 int spinor_convert(lq_ctx* c, void* dst, int dst_prec, const void* src, int src_prec, int nrhs, const double* d_scale /*per rhs, multiplies*/, int invert_scale);
 int spinor_zero_parity(lq_ctx* c, void* parity_block, int nrhs, int prec);
 int spinor_gather_sites(lq_ctx* c, double* dev_out, const void* parity_block, int nrhs, int prec, long long nsites, const int* dev_sites);
@@ -40,8 +43,8 @@ int blas_norm2(lq_ctx* c, int prec, int nrhs, const void* x, double* d_out);    
 // y (fp64) += s_k * e (prec)       (defect-correction accumulate)
 // fused CG vector update: alpha_k = rr_k / pAp_k, beta_k = rr_new_k / rr_k;  e += alpha p;  p = z + beta p
 int blas_cg_update_ep(lq_ctx* c, int prec, int nrhs, void* e, void* p, const void* z, const double* d_rr, const double* d_pAp, const double* d_rr_new);
-// reliable update of the search direction: p_k <- z_new_k + c_k (p_k - z_old_k), c per RHS on the device
-int blas_keep_direction(lq_ctx* c, int prec, int nrhs, void* p, const void* z_old, const void* z_new, const double* d_c);
+// reliable update of the search direction: p_k <- z_new_k + c_k (p_k - z_old_k), then z_old <- z_new; c per RHS on the device
+int blas_keep_direction(lq_ctx* c, int prec, int nrhs, void* p, void* z_old, const void* z_new, const double* d_c);
 int blas_axpy_mixed(lq_ctx* c, int prec, int nrhs, void* y64, const void* e, const double* d_scale);
 // r = b - t (fp64), d_out[k] = ||r_k||^2
 int blas_residual(lq_ctx* c, int nrhs, void* r, const void* b, const void* t, double* d_out);
@@ -58,7 +61,12 @@ int blas_bicg_p(lq_ctx* c, int prec, int nrhs, void* p, const void* r, const voi
 int fill_gauge(lq_ctx* c, uint64_t seed, double eps);
 int fill_spinor(lq_ctx* c, void* native, int nrhs, int prec, uint64_t seed, int parity_only, int parity);
 
+// fmapeak.cu
+int fma_peak(lq_ctx* c, int mode, double ms, double* tflops);
+
 // solver.cu
+void solver_release(lq_ctx* c);
+int mhat_native(lq_ctx* c, int prec, int n, void* out_e, const void* in_e, int dagger);
 int solve_native(lq_ctx* c, void* x_full64, const void* b_full64, int nrhs, const lq_solve_param* p, lq_solve_info* info);
 
 // laplace.cu : batched 3-d gauge-covariant Laplacian on native colour-vector fields

@@ -15,11 +15,22 @@ static DslashArgs<S> base_args(lq_ctx* c, int nrhs, int out_parity, void* out, c
     a.coef = T(1); a.tsign = T(c->t_bc); a.dsign = dagger ? T(-1) : T(1);
     a.epi = EPI_NONE; a.epi_num = a.epi_den = nullptr; a.epi_out = nullptr; a.red_partials = nullptr; a.red_counter = nullptr;
     a.epi_v = a.out; a.epi_conj = 0;
+    a.skip = c->loop_skip;
     return a;
 }
 
 template <class S, int FORM>
 static int run_form(lq_ctx* c, DslashArgs<S> a) {
+    {   // SURVEY 8(d) model: every input site read once, output written once, 8 links + the clover block once per launch
+        const int recon = S::prec == LQ_FP64 ? 18 : c->recon32;
+        const double cb = S::prec == LQ_FP64 ? 8.0 : 4.0;      // bytes per link / clover real
+        int streams = FORM == FORM_B ? 3 : 2;
+        if (FORM == FORM_B && (a.epi == EPI_XMAY || a.epi == EPI_CDOT)) streams++;
+        const double bytes = streams * stream_bytes(c->g, a.N, S::prec) + (double)c->g.Vh * (8.0 * recon + (a.clover ? 72.0 : 0.0)) * cb;
+        const double flops = (double)c->g.Vh * a.N * (1320.0 + (a.clover ? 504.0 : 0.0) + (FORM == FORM_B ? 48.0 : 0.0) +
+                                                      (FORM == FORM_B && a.epi != EPI_NONE ? 48.0 : 0.0) + (FORM == FORM_B && a.epi == EPI_CDOT ? 96.0 : 0.0));
+        LQ_MODEL(c, bytes, flops);
+    }
     if constexpr (S::prec == LQ_FP64) return launch_dslash<S, 18, FORM>(c, a, c->dslash_rpt, c->dslash_variant);
     else {
         if (c->recon32 == 12) return launch_dslash<S, 12, FORM>(c, a, c->dslash_rpt, c->dslash_variant);
@@ -118,6 +129,7 @@ template <class S> static int clover_t(lq_ctx* c, int nrhs, int parity, void* ou
         clover_apply_kernel<S, 1, 1><<<grid, block, 0, c->stream>>>(c->g, G, vo, vx, cl);
     }
     LQ_LAUNCHED(c);
+    LQ_MODEL(c, 2 * stream_bytes(c->g, nrhs, S::prec) + (double)c->g.Vh * 72.0 * (S::prec == LQ_FP64 ? 8.0 : 4.0), 504.0 * c->g.Vh * nrhs);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }

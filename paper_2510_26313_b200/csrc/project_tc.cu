@@ -199,8 +199,9 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
 #pragma unroll
     for (int st = 0; st < RING; st++) fetch_stage(st);
     for (int i = 0; i < nst; i++) {
-        if (!wait_bar(full + i % RING, (uint32_t)((i / RING) & 1))) { ok = false; break; }       // raw stage i has landed (all threads' copies)
-        if (i > 0 && !wait_mma((uint32_t)((i - 1) & 1))) { ok = false; break; }   // operand tiles released by the MMAs of stage i-1
+        bool arrived = wait_bar(full + i % RING, (uint32_t)((i / RING) & 1));                   // raw stage i has landed (all threads' copies)
+        if (arrived && i > 0) arrived = wait_mma((uint32_t)((i - 1) & 1));                       // operand tiles released by the MMAs of stage i-1
+        if (__syncthreads_or(!arrived)) { ok = false; break; }                                   // a timeout anywhere ends the loop for the whole CTA
         const unsigned char* slot = raw + (size_t)(i % RING) * Sh::RAW;
 #pragma unroll
         for (int k = 0; k < NTK; k++) {
@@ -293,11 +294,18 @@ int project_tc_run(lq_ctx* c, int Lt, int S3, int n_ev, int n_sol, const double*
     const int nchunk = (S3 + spc - 1) / spc;
     const size_t smem = TcShape<TN, SPB, RING>::SMEM;
     static_assert(TcShape<TN, SPB, RING>::SMEM <= 232448, "shared memory per CTA");
-    static bool configured = false;
-    if (!configured) { LQ_CUDA(c, cudaFuncSetAttribute(project_tc_kernel<TN, SPB, RING>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); configured = true; }
-    float* partial = (float*)dev_alloc(c, sizeof(float) * (size_t)Lt * nchunk * TM * TN);
-    int* d_err = (int*)dev_alloc(c, sizeof(int));
-    if (!partial || !d_err) { if (partial) dev_free(c, partial); if (d_err) dev_free(c, d_err); return LQ_ENOMEM; }
+    // the attribute is per device: set it on every call (cheap) rather than once per process
+    LQ_CUDA(c, cudaFuncSetAttribute(project_tc_kernel<TN, SPB, RING>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    // scratch (error word + split-K partials) lives in the context between calls
+    const size_t need = 256 + sizeof(float) * (size_t)Lt * nchunk * TM * TN;
+    if (c->proj_scratch_bytes < need) {
+        if (c->proj_scratch) dev_free(c, c->proj_scratch);
+        c->proj_scratch = dev_alloc(c, need);
+        c->proj_scratch_bytes = c->proj_scratch ? need : 0;
+        if (!c->proj_scratch) return LQ_ENOMEM;
+    }
+    int* d_err = (int*)c->proj_scratch;
+    float* partial = (float*)((char*)c->proj_scratch + 256);
     cudaMemsetAsync(d_err, 0, sizeof(int), c->stream);
     int rc = 0;
     for (int j0 = 0; j0 < n_ev && rc == 0; j0 += TM)
@@ -312,7 +320,6 @@ int project_tc_run(lq_ctx* c, int Lt, int S3, int n_ev, int n_sol, const double*
     if (rc == 0 && (cudaMemcpyAsync(&herr, d_err, sizeof(int), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess || cudaStreamSynchronize(c->stream) != cudaSuccess))
         rc = set_err(c, LQ_ECUDA, "lq_project: tensor-core kernel failed");
     if (rc == 0 && herr) rc = set_err(c, LQ_ECUDA, "lq_project: tcgen05 completion barrier timed out");
-    dev_free(c, partial); dev_free(c, d_err);
     return rc;
 }
 }  // namespace

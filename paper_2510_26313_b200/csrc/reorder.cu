@@ -79,17 +79,18 @@ __device__ __forceinline__ void store_site(const SView<S>& v, int N, int cb, int
 }
 
 // ---- spinor pack / unpack ---------------------------------------------------------------------------------------------
+// `canon` holds right-hand sides k0 .. k0+nk-1 of the batch of N (canonical [rhs][site][24]); the native buffer holds all N.
 template <class S, typename Tc, bool PACK>
-__global__ void spinor_reorder_kernel(Geom g, int N, SView<S> even, SView<S> odd, Tc* canon) {
+__global__ void spinor_reorder_kernel(Geom g, int N, int k0, int nk, SView<S> even, SView<S> odd, Tc* canon) {
     const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (tid >= 2LL * g.Vh * N) return;
-    const int k = (int)(tid % N);
-    const long long r = tid / N;
+    if (tid >= 2LL * g.Vh * nk) return;
+    const int kl = (int)(tid % nk), k = k0 + kl;
+    const long long r = tid / nk;
     const int cb = (int)(r % g.Vh), parity = (int)(r / g.Vh);
     int xh, y, z, t, odd_;
     cb_coords(g, parity, cb, xh, y, z, t, odd_);
     const long long site = (2 * xh + odd_) + (long long)g.L[0] * (y + (long long)g.L[1] * (z + (long long)g.L[2] * t));
-    Tc* p = canon + ((long long)k * g.V + site) * 24;
+    Tc* p = canon + ((long long)kl * g.V + site) * 24;
     const SView<S>& v = parity ? odd : even;
     double o[24];
     if constexpr (PACK) {
@@ -103,27 +104,33 @@ __global__ void spinor_reorder_kernel(Geom g, int N, SView<S> even, SView<S> odd
     }
 }
 template <class S, bool PACK>
-static int reorder_t(lq_ctx* c, void* native_full, void* canon, int nrhs, int cprec) {
+static int reorder_t(lq_ctx* c, void* native_full, void* canon, int nrhs, int k0, int nk, int cprec) {
     SView<S> e = make_view<S>(c->g, native_full, nrhs, 0), o = make_view<S>(c->g, native_full, nrhs, 1);
-    const long long threads = 2LL * c->g.Vh * nrhs;
+    const long long threads = 2LL * c->g.Vh * nk;
     const int block = 128; const int grid = (int)((threads + block - 1) / block);
-    if (cprec == LQ_FP64) spinor_reorder_kernel<S, double, PACK><<<grid, block, 0, c->stream>>>(c->g, nrhs, e, o, (double*)canon);
-    else spinor_reorder_kernel<S, float, PACK><<<grid, block, 0, c->stream>>>(c->g, nrhs, e, o, (float*)canon);
+    if (cprec == LQ_FP64) spinor_reorder_kernel<S, double, PACK><<<grid, block, 0, c->stream>>>(c->g, nrhs, k0, nk, e, o, (double*)canon);
+    else spinor_reorder_kernel<S, float, PACK><<<grid, block, 0, c->stream>>>(c->g, nrhs, k0, nk, e, o, (float*)canon);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
-int spinor_pack(lq_ctx* c, void* native_full, const void* dev_canonical, int nrhs, int prec, int in_prec) {
+int spinor_pack_part(lq_ctx* c, void* native_full, const void* dev_canonical, int nrhs, int k0, int nk, int prec, int in_prec) {
     void* cn = const_cast<void*>(dev_canonical);
-    if (prec == LQ_FP64) return reorder_t<F64, true>(c, native_full, cn, nrhs, in_prec);
-    if (prec == LQ_FP32) return reorder_t<F32, true>(c, native_full, cn, nrhs, in_prec);
-    return reorder_t<H16, true>(c, native_full, cn, nrhs, in_prec);
+    if (prec == LQ_FP64) return reorder_t<F64, true>(c, native_full, cn, nrhs, k0, nk, in_prec);
+    if (prec == LQ_FP32) return reorder_t<F32, true>(c, native_full, cn, nrhs, k0, nk, in_prec);
+    return reorder_t<H16, true>(c, native_full, cn, nrhs, k0, nk, in_prec);
+}
+int spinor_unpack_part(lq_ctx* c, void* dev_canonical, const void* native_full, int nrhs, int k0, int nk, int prec, int out_prec) {
+    void* nf = const_cast<void*>(native_full);
+    if (prec == LQ_FP64) return reorder_t<F64, false>(c, nf, dev_canonical, nrhs, k0, nk, out_prec);
+    if (prec == LQ_FP32) return reorder_t<F32, false>(c, nf, dev_canonical, nrhs, k0, nk, out_prec);
+    return reorder_t<H16, false>(c, nf, dev_canonical, nrhs, k0, nk, out_prec);
+}
+int spinor_pack(lq_ctx* c, void* native_full, const void* dev_canonical, int nrhs, int prec, int in_prec) {
+    return spinor_pack_part(c, native_full, dev_canonical, nrhs, 0, nrhs, prec, in_prec);
 }
 int spinor_unpack(lq_ctx* c, void* dev_canonical, const void* native_full, int nrhs, int prec, int out_prec) {
-    void* nf = const_cast<void*>(native_full);
-    if (prec == LQ_FP64) return reorder_t<F64, false>(c, nf, dev_canonical, nrhs, out_prec);
-    if (prec == LQ_FP32) return reorder_t<F32, false>(c, nf, dev_canonical, nrhs, out_prec);
-    return reorder_t<H16, false>(c, nf, dev_canonical, nrhs, out_prec);
+    return spinor_unpack_part(c, dev_canonical, native_full, nrhs, 0, nrhs, prec, out_prec);
 }
 
 // ---- precision conversion of one parity block, with an optional per-RHS scale ----------------------------------------------
@@ -150,6 +157,7 @@ static int convert_t(lq_ctx* c, void* dst, const void* src, int nrhs, const doub
     const int block = 128; const int grid = (int)((threads + block - 1) / block);
     convert_kernel<SD, SS><<<grid, block, 0, c->stream>>>(c->g.Vh, nrhs, d, s, d_scale, invert);
     LQ_LAUNCHED(c);
+    LQ_MODEL(c, stream_bytes(c->g, nrhs, SD::prec) + stream_bytes(c->g, nrhs, SS::prec), 24.0 * c->g.Vh * nrhs);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }

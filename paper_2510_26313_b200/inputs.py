@@ -94,7 +94,7 @@ def gaussian_spinors(dims, nrhs: int, seed: int) -> np.ndarray:
     return cgauss(seed, STREAM_SPINOR, idx).reshape(nrhs, Lt, Lz, Ly, Lx, 4, 3)
 
 
-def laph_sources(dims, nrhs: int, n_t: int, seed: int) -> np.ndarray:
+def laph_sources(dims, nrhs: int, n_t: int, seed: int, out: np.ndarray | None = None) -> np.ndarray:
     """LapH-style time/spin-diluted sources (step 10, reading #17).
 
     RHS k -> (t0 = (k // 4) * Lt / n_t, spin alpha = k % 4); one complex-Gaussian colour-vector field
@@ -102,7 +102,11 @@ def laph_sources(dims, nrhs: int, n_t: int, seed: int) -> np.ndarray:
     """
     Lx, Ly, Lz, Lt = dims
     Vs = Lx * Ly * Lz
-    b = np.zeros((nrhs, Lt, Lz, Ly, Lx, 4, 3), dtype=np.complex128)
+    if out is None:
+        b = np.zeros((nrhs, Lt, Lz, Ly, Lx, 4, 3), dtype=np.complex128)
+    else:                                         # caller-provided storage (e.g. pinned host memory), same shape
+        b = out.reshape(nrhs, Lt, Lz, Ly, Lx, 4, 3)
+        b[...] = 0
     for k in range(nrhs):
         n = (k // 4) % n_t
         t0 = n * Lt // n_t

@@ -25,11 +25,32 @@ def test_library_builds_and_exports_every_declared_symbol():
     assert sorted(binding.EXPORTS) == syms
 
 
-def test_struct_layouts_match_header():
-    # lq_solve_param: double,int,int,int,(pad),double,int,int,int,int ; lq_solve_info as declared
-    assert ctypes.sizeof(binding.SolveParam) == 48
-    assert ctypes.sizeof(binding.SolveInfo) == 4 * 3 + 4 * 16 + 4 + 8 * 16 + 8 + 8
-    assert binding.LQ_MAX_RHS == 16
+def test_struct_layouts_match_header(tmp_path):
+    """sizeof / offsetof of every struct of the header, as a C compiler sees them, against the ctypes mirrors."""
+    import subprocess
+    structs = {"lq_solve_param": (binding.SolveParam, ["tol", "max_outer", "max_inner", "inner_prec", "delta", "check_every", "use_graph",
+                                                       "keep_direction", "algorithm", "use_x0"]),
+               "lq_solve_info": (binding.SolveInfo, ["nrhs", "outer_cycles", "inner_iters", "iters", "true_rel_residual", "seconds", "dslash_applies",
+                                                     "model_bytes", "model_flops"]),
+               "lq_eig_param": (binding.EigParam, ["n_ev", "m", "cheb_degree", "max_restarts", "cheb_a", "cheb_b", "tol", "seed"]),
+               "lq_eig_info": (binding.EigInfo, ["restarts", "converged", "lap_applies", "max_ritz_residual", "max_true_residual", "seconds"])}
+    lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "lqcd_b200.h"', 'int main(void) {']
+    for name, (_, fields) in structs.items():
+        lines.append('printf("%s %%zu\\n", sizeof(%s));' % (name, name))
+        for f in fields:
+            lines.append('printf("%s.%s %%zu\\n", offsetof(%s, %s));' % (name, f, name, f))
+    lines.append('printf("LQ_MAX_RHS %d\\n", LQ_MAX_RHS); return 0; }')
+    src = tmp_path / "layout.c"
+    src.write_text("\n".join(lines))
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), "-o", str(exe), str(src)], check=True)
+    got = dict(l.split() for l in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.splitlines())
+    assert int(got["LQ_MAX_RHS"]) == binding.LQ_MAX_RHS == 16
+    for name, (cls, fields) in structs.items():
+        assert ctypes.sizeof(cls) == int(got[name]), name
+        assert [f for f, _ in cls._fields_] == fields, name
+        for f in fields:
+            assert getattr(cls, f).offset == int(got[name + "." + f]), (name, f)
 
 
 def test_bad_arguments_fail_without_a_gpu():

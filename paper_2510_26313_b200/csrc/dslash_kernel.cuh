@@ -219,6 +219,13 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
                 if constexpr (FORM == FORM_B) {
                     const char* qx = (const char*)(a.x.d + ((size_t)pb * G + grp) * US);
                     LQ_PF_LINES(qx, (int)(US * sizeof(ST) / LINE))
+                    if (a.epi == EPI_XMAY) {          // the epilogue reads the vector it updates
+                        const char* qz = (const char*)(a.out.d + ((size_t)pb * G + grp) * US);
+                        LQ_PF_LINES(qz, (int)(US * sizeof(ST) / LINE))
+                    } else if (a.epi == EPI_CDOT) {
+                        const char* qh = (const char*)(a.epi_v.d + ((size_t)pb * G + grp) * US);
+                        LQ_PF_LINES(qh, (int)(US * sizeof(ST) / LINE))
+                    }
                 }
                 constexpr int GL = 4 * RECON * SB * sizeof(T) / LINE;     // lines of one (parity, block) link slab
                 constexpr int CL = 72 * SB * sizeof(T) / LINE;            // lines of one clover block

@@ -48,7 +48,7 @@ static int launch_rpt(lq_ctx* c, DslashArgs<S> a, int variant) {
     a.dG = make_fastdiv(a.G);
     a.pfd = c->dslash_pfd;
     plan_sweep<S>(c, a);
-    if constexpr (S::prec == LQ_FP32) {
+    if constexpr (S::prec != LQ_FP64) {
         constexpr int ALT = RPT == 4 ? 3 : (RPT == 2 ? 4 : 5);
         if (variant == 1) return launch_one<S, RPT, R, RECON, FORM, ALT>(c, a);
     }

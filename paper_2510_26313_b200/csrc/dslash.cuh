@@ -243,40 +243,9 @@ __device__ __forceinline__ void hop_mulacc_f2(const float (&h)[2][3][2][RPT], co
 }
 #endif
 
-// ---- one of the eight hopping terms -------------------------------------------------------------------
-// acc[j][k] += cu * (1 - sigma*gamma_MU) W psi(nb),  W = U (FWD) or U^dag (backward), sigma = +-1.
-// `nb` points at real 0 of the neighbour's RPT right-hand sides; real j is at nb + j*SB*R.
-template <class S, int RPT, int R, int RECON, int MU, bool FWD>
-__device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ nb, const float* __restrict__ nb_norm,
-                                        const typename S::comp_t* __restrict__ link_blk, int link_s,
-                                        typename S::comp_t cu, typename S::comp_t sigma, typename S::comp_t (&acc)[24][RPT]) {
-    using T = typename S::comp_t;
-    constexpr int PL = SB * R;   // elements between consecutive reals of a site
-    T u[18];
-    load_link<T, RECON>(link_blk, link_s, u);
-
-    T cuk[RPT], clk[RPT];
-    if constexpr (S::has_norm) {
-        float nrm[RPT];
-        load_norm<RPT>(nb_norm, nrm);
-#pragma unroll
-        for (int k = 0; k < RPT; k++) cuk[k] = cu * nrm[k] * (1.0f / 32767.0f);
-    } else {
-#pragma unroll
-        for (int k = 0; k < RPT; k++) cuk[k] = cu;
-    }
-#pragma unroll
-    for (int k = 0; k < RPT; k++) clk[k] = sigma * cuk[k];
-
-    // projected half spinor h[s][c][ri][k]
-    T h[2][3][2][RPT];
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-        T p[4][2][RPT];
-#pragma unroll
-        for (int s = 0; s < 4; s++)
-#pragma unroll
-            for (int ri = 0; ri < 2; ri++) load_comp<S, RPT>(nb + (2 * (3 * s + c) + ri) * PL, p[s][ri]);
+// ---- spin projection of one colour: h[s][c] = rows of (1 - sigma gamma_MU) p, DeGrand-Rossi rank-2 structure ------------------
+template <typename T, int RPT, int MU>
+__device__ __forceinline__ void project_half(const T (&p)[4][2][RPT], T sigma, int c, T (&h)[2][3][2][RPT]) {
 #ifdef LQ_USE_FFMA2
         if constexpr (sizeof(T) == 4 && RPT % 2 == 0) {
 #pragma unroll
@@ -320,6 +289,43 @@ __device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ 
             }
         }
         }
+}
+
+// ---- one of the eight hopping terms -------------------------------------------------------------------
+// acc[j][k] += cu * (1 - sigma*gamma_MU) W psi(nb),  W = U (FWD) or U^dag (backward), sigma = +-1.
+// `nb` points at real 0 of the neighbour's RPT right-hand sides; real j is at nb + j*SB*R.
+template <class S, int RPT, int R, int RECON, int MU, bool FWD>
+__device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ nb, const float* __restrict__ nb_norm,
+                                        const typename S::comp_t* __restrict__ link_blk, int link_s,
+                                        typename S::comp_t cu, typename S::comp_t sigma, typename S::comp_t (&acc)[24][RPT]) {
+    using T = typename S::comp_t;
+    constexpr int PL = SB * R;   // elements between consecutive reals of a site
+    T u[18];
+    load_link<T, RECON>(link_blk, link_s, u);
+
+    T cuk[RPT], clk[RPT];
+    if constexpr (S::has_norm) {
+        float nrm[RPT];
+        load_norm<RPT>(nb_norm, nrm);
+#pragma unroll
+        for (int k = 0; k < RPT; k++) cuk[k] = cu * nrm[k] * (1.0f / 32767.0f);
+    } else {
+#pragma unroll
+        for (int k = 0; k < RPT; k++) cuk[k] = cu;
+    }
+#pragma unroll
+    for (int k = 0; k < RPT; k++) clk[k] = sigma * cuk[k];
+
+    // projected half spinor h[s][c][ri][k]
+    T h[2][3][2][RPT];
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        T p[4][2][RPT];
+#pragma unroll
+        for (int s = 0; s < 4; s++)
+#pragma unroll
+            for (int ri = 0; ri < 2; ri++) load_comp<S, RPT>(nb + (2 * (3 * s + c) + ri) * PL, p[s][ri]);
+        project_half<T, RPT, MU>(p, sigma, c, h);
     }
 #ifdef LQ_USE_FFMA2
     if constexpr (sizeof(T) == 4 && RPT % 2 == 0) { hop_mulacc_f2<RPT, MU, FWD>(h, u, cuk, clk, acc); return; }

@@ -155,7 +155,9 @@ template <class S> __device__ __forceinline__ int sweep_block(const DslashArgs<S
     return yb + a.nby * ((zch * a.zc + zi) + a.g.L[2] * t);
 }
 
-template <class S, int RPT, int R, int RECON, int FORM, int BLOCK, int MINB>
+// EPI: the fused block-BLAS epilogue of kernel B, a template parameter so that every launch carries only the code it runs
+// (one kernel with all three epilogues was 90 KB of instructions for half storage: instruction-fetch stalls)
+template <class S, int RPT, int R, int RECON, int FORM, int BLOCK, int MINB, int EPI = EPI_NONE>
 __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S> a) {
     using T = typename S::comp_t;
     using ST = typename S::store_t;
@@ -219,10 +221,10 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
                 if constexpr (FORM == FORM_B) {
                     const char* qx = (const char*)(a.x.d + ((size_t)pb * G + grp) * US);
                     LQ_PF_LINES(qx, (int)(US * sizeof(ST) / LINE))
-                    if (a.epi == EPI_XMAY) {          // the epilogue reads the vector it updates
+                    if constexpr (EPI == EPI_XMAY) {          // the epilogue reads the vector it updates
                         const char* qz = (const char*)(a.out.d + ((size_t)pb * G + grp) * US);
                         LQ_PF_LINES(qz, (int)(US * sizeof(ST) / LINE))
-                    } else if (a.epi == EPI_CDOT) {
+                    } else if constexpr (EPI == EPI_CDOT) {
                         const char* qh = (const char*)(a.epi_v.d + ((size_t)pb * G + grp) * US);
                         LQ_PF_LINES(qh, (int)(US * sizeof(ST) / LINE))
                     }
@@ -277,7 +279,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
 
     // ---- fused block-BLAS epilogues of kernel B and store ---------------------------------
     if constexpr (FORM == FORM_B) {
-        if (a.epi == EPI_XMAY) {
+        if constexpr (EPI == EPI_XMAY) {
             // out <- out - alpha_k acc  (the CG residual update z -= alpha q without ever storing q), alpha = rr / pAp
             T zv[24][RPT], al[RPT];
             load_site_regs<S, RPT, R>(a.out.d + own, S::has_norm ? a.out.n + own_n : nullptr, zv);
@@ -288,7 +290,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
 #pragma unroll
                 for (int k = 0; k < RPT; k++) acc[j][k] = zv[j][k] - al[k] * acc[j][k];
         }
-        if (a.epi == EPI_CDOT) {
+        if constexpr (EPI == EPI_CDOT) {
             // <h, out> for the 12 complex components, summed in the compute type per site like the norms below
             T hv[24][RPT], pr[RPT], pi[RPT];
             load_site_regs<S, RPT, R>(a.epi_v.d + own, S::has_norm ? a.epi_v.n + own_n : nullptr, hv);
@@ -304,7 +306,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
 #pragma unroll
             for (int k = 0; k < RPT; k++) { part_c[0][k] = (double)pr[k]; part_c[1][k] = a.epi_conj ? -(double)pi[k] : (double)pi[k]; }
         }
-        if (a.epi != EPI_NONE) {
+        if constexpr (EPI != EPI_NONE) {
             // the 24 squares of one site are summed in the compute type (relative error ~1e-7 in fp32, far below the
             // solver's use of these norms); sites are summed in fp64 by the reduction
             T ps[RPT];
@@ -321,12 +323,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
     store_site_regs<S, RPT, R>(a.out.d + own, S::has_norm ? a.out.n + own_n : nullptr, acc);
     }   // valid
     if constexpr (FORM == FORM_B) {
-        if (a.epi == EPI_CDOT) {
+        if constexpr (EPI == EPI_CDOT) {
             double p3[3][RPT];
 #pragma unroll
             for (int k = 0; k < RPT; k++) { p3[0][k] = part_c[0][k]; p3[1][k] = part_c[1][k]; p3[2][k] = part[k]; }
             reduce_multi<3, RPT, R>(p3, a.N, G, a.red_partials, a.red_counter, a.epi_out);
-        } else if (a.epi != EPI_NONE) reduce_per_rhs<RPT, R>(part, a.N, G, a.red_partials, a.red_counter, a.epi_out);
+        } else if constexpr (EPI != EPI_NONE) reduce_per_rhs<RPT, R>(part, a.N, G, a.red_partials, a.red_counter, a.epi_out);
     }
 }
 

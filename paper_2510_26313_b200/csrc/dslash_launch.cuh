@@ -11,7 +11,17 @@ static int launch_one(lq_ctx* c, DslashArgs<S> a) {
         LQ_TRY(ensure_partials(c, (size_t)grid * a.N * (a.epi == EPI_CDOT ? 3 : 1)));
         a.red_partials = c->red_partials; a.red_counter = c->red_counter;
     }
-    dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB><<<grid, BLOCK, FORM == FORM_B ? BLOCK * sizeof(double) : 0, c->stream>>>(a);
+    if constexpr (FORM == FORM_B) {
+        const size_t smem = BLOCK * sizeof(double);
+        switch (a.epi) {
+        case EPI_NORM: dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, EPI_NORM><<<grid, BLOCK, smem, c->stream>>>(a); break;
+        case EPI_XMAY: dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, EPI_XMAY><<<grid, BLOCK, smem, c->stream>>>(a); break;
+        case EPI_CDOT: dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, EPI_CDOT><<<grid, BLOCK, smem, c->stream>>>(a); break;
+        default: dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, EPI_NONE><<<grid, BLOCK, 0, c->stream>>>(a); break;
+        }
+    } else {
+        dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, EPI_NONE><<<grid, BLOCK, 0, c->stream>>>(a);
+    }
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;

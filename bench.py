@@ -53,7 +53,7 @@ def bytes_per_site_rhs(kind: str, prec: str, nrhs: int, recon: int) -> float:
     s = {"fp64": 8.0, "fp32": 4.0, "half": 2.0}[prec]
     g = 8.0 if prec == "fp64" else 4.0
     spinor = 24 * s + (4.0 if prec == "half" else 0.0)
-    per_batch = 8 * recon * g + (0.0 if kind == "hop" else 72 * g)
+    per_batch = 8 * recon * g + (0.0 if kind == "hop" else 72 * g)      # "probe" moves kernel A's bytes
     streams = 3 if kind == "B" else 2
     return streams * spinor + per_batch / nrhs
 
@@ -120,7 +120,7 @@ def time_dslash(ctx, B, kind: str, prec: str, nrhs: int, recon: int, iters: int 
         for j, b in enumerate(bufs[1:]):
             ctx.fill_spinor_random(b, nrhs, P, 7000 + 10 * i + j, parity_only=True, parity=(0 if (kind == "B" and j == 0) else (0 if kind != "B" else 1)))
         sets.append(bufs)
-    op = {"A": B.LQ_OP_KERNEL_A, "B": B.LQ_OP_KERNEL_B, "hop": B.LQ_OP_HOP_OE}[kind]
+    op = {"A": B.LQ_OP_KERNEL_A, "B": B.LQ_OP_KERNEL_B, "hop": B.LQ_OP_HOP_OE, "probe": B.LQ_OP_PROBE_LOADS}[kind]
 
     def launch(i):
         s = sets[i % nsets]
@@ -141,7 +141,7 @@ def time_dslash(ctx, B, kind: str, prec: str, nrhs: int, recon: int, iters: int 
     sec = e0.elapsed_time(e1) * 1e-3 / iters
     Vh = ctx.V // 2
     bps = bytes_per_site_rhs(kind, prec, nrhs, recon)
-    flop = {"A": FLOP_A, "B": FLOP_B, "hop": FLOP_HOP}[kind]
+    flop = {"A": FLOP_A, "B": FLOP_B, "hop": FLOP_HOP, "probe": 0.0}[kind]
     del sets
     return dict(kind=kind, prec=prec, nrhs=nrhs, recon=recon, seconds=sec, bytes_per_site_rhs=bps,
                 gbs=bps * Vh * nrhs / sec * 1e-9, gflops=flop * Vh * nrhs / sec * 1e-9, nsets=nsets)
@@ -190,7 +190,7 @@ def time_laplacian(ctx, B, nvec, prec="fp32", iters=20, warmup=3):
 
 # FP32 instruction slots (one FMA, multiply or add each) per output site per RHS when every complex product is written as fused
 # multiply-adds: hop 8 x (12 project + 72 SU(3) + 24 accumulate) = 864, clover 2 x 6 x 22 = 264
-FP_SLOTS = {"A": 1128.0, "B": 1128.0, "hop": 864.0}
+FP_SLOTS = {"A": 1128.0, "B": 1128.0, "hop": 864.0, "probe": 0.0}
 
 
 def roofline_entry(r, peak, peak_src, traffic=None, fma=None, lattice=None):
@@ -205,7 +205,7 @@ def roofline_entry(r, peak, peak_src, traffic=None, fma=None, lattice=None):
     if lattice:
         e["lattice"] = lattice
     if fma:
-        flop = {"A": FLOP_A, "B": FLOP_B, "hop": FLOP_HOP}[r["kind"]]
+        flop = {"A": FLOP_A, "B": FLOP_B, "hop": FLOP_HOP, "probe": 1.0}[r["kind"]]
         e["alu_peak_tflops"] = fma["scalar_ffma"]
         e["alu_frac"] = round(r["gflops"] * 1e-3 / fma["scalar_ffma"], 4)
         e["alu_issue_frac"] = round(r["gflops"] * 1e-3 * (2.0 * FP_SLOTS[r["kind"]] / flop) / fma["scalar_ffma"], 4)
@@ -217,7 +217,8 @@ def measure_fma_peak(ctx):
     """FP32 FMA peak through the C ABI (lq_fma_peak): scalar FFMA, packed FFMA2 with three distinct operands, packed FFMA2 with
     one operand shared by 4 consecutive instructions (the stencil's pattern).  TFLOP/s, 2 flops per FMA lane."""
     return {"scalar_ffma": round(ctx.fma_peak(0, 150.0), 2), "ffma2_distinct_operands": round(ctx.fma_peak(1, 150.0), 2),
-            "ffma2_shared_operand": round(ctx.fma_peak(2, 150.0), 2), "unit": "TFLOP/s", "nominal_1965MHz": 74.4,
+            "ffma2_shared_operand": round(ctx.fma_peak(2, 150.0), 2), "ffma2_register_scalar_operand": round(ctx.fma_peak(3, 150.0), 2),
+            "unit": "TFLOP/s", "nominal_1965MHz": 74.4,
             "how": "register-only FMA loops, 16 chains per thread, 8 CTAs x 256 threads per SM, ~150 ms each (csrc/fmapeak.cu)"}
 
 
@@ -530,7 +531,7 @@ def main():
     ap.add_argument("--delta", type=float, default=0.0, help="inner CG reduction per cycle (0 = the workload default)")
     ap.add_argument("--algorithm", choices=("cg", "bicgstab"), default="cg", help="inner solver of the timed step (default cg = the metric of BASELINE.json; bicgstab = the solver variant)")
     ap.add_argument("--op", default=None, metavar="CFG:KIND:PREC:N",
-                    help="time ONE stencil kernel only, e.g. cfg2:A:fp32:8 (lattice and links of configs[CFG]; KIND A|B|hop|lap|proj; "
+                    help="time ONE stencil kernel only, e.g. cfg2:A:fp32:8 (lattice and links of configs[CFG]; KIND A|B|hop|probe|lap|proj; "
                          "PREC fp64|fp32|half); optional :variant:rpt:pfd tuning suffix.  Prints its own JSON line (used for ncu captures)")
     ap.add_argument("--op-iters", type=int, default=20)
     args = ap.parse_args()

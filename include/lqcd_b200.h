@@ -89,7 +89,10 @@ typedef enum {
     LQ_OP_MHAT = 7,       /* parity: out_e = A_ee in_e - kappa^2 D_eo A_oo^{-1} D_oe in_e (step 8) */
     LQ_OP_MHAT_DAG = 8,   /* parity: out_e = g5 Mhat g5 in_e                                       */
     LQ_OP_KERNEL_A = 9,   /* parity: out_o = A_oo^{-1} D_oe in_e   */
-    LQ_OP_KERNEL_B = 10   /* parity: out_e = A_ee in_e - kappa^2 D_eo in2_o   */
+    LQ_OP_KERNEL_B = 10,  /* parity: out_e = A_ee in_e - kappa^2 D_eo in2_o   */
+    LQ_OP_PROBE_LOADS = 11 /* bench only (NATIVE layout, fp32 or half, 18-real links): kernel A's loads, prefetches and stores
+                              with one multiply-add per loaded value instead of its arithmetic; the output is meaningless, the
+                              time is the floor the memory path sets for kernel A's access pattern                        */
 } lq_op;
 
 /* ---- context --------------------------------------------------------------------------------- */
@@ -257,9 +260,16 @@ int lq_set_tuning(lq_ctx* ctx, int dslash_variant, int dslash_rpt, int dslash_pf
 /* Plain FP32 ALU peak of this GPU measured with register-only FMA loops ("measure an FMA microbenchmark on
  * the box and use that" as the denominator of the ALU roofline fraction).  mode 0: scalar FFMA, 1: packed FFMA2 with three
  * distinct 64-bit operands, 2: packed FFMA2 whose first operand is shared by 4 consecutive instructions (the stencil kernels'
- * pattern: one link element against 4 spinor reals).  Runs for about `ms` milliseconds on the context's stream, synchronises,
+ * pattern: one link element against 4 spinor reals), 3: packed FFMA2 whose first operand is one 32-bit register broadcast to
+ * both halves (the operand form the compiler emits for those products: it issues every 3rd cycle).  Runs for about `ms` milliseconds on the context's stream, synchronises,
  * and writes TFLOP/s (2 flops per FMA lane) to *tflops. */
 int lq_fma_peak(lq_ctx* ctx, int mode, double ms, double* tflops);
+
+/* Read bandwidth of the memory path measured with a streaming kernel (16-byte loads that bypass L1, 8 in flight per thread, 8 CTAs of
+ * 256 threads per SM).  mode 0: a buffer of `mbytes` MB (choose several times the L2 size) read 4 times: HBM; mode 1: a buffer that
+ * fits in L2 (e.g. 48 MB) read 200 times: the L2 -> SM bandwidth, the second memory-side bound of the stencil kernels (every compulsory
+ * byte crosses L2 -> SM about 3 times because the 8 neighbour reads of a site meet in L2).  Writes GB/s to *gbs. */
+int lq_mem_peak(lq_ctx* ctx, int mode, double mbytes, double* gbs);
 
 /* Number of kernels this library has launched on this context since creation (for bench.py). */
 long long lq_kernel_launches(const lq_ctx* ctx);

@@ -20,13 +20,13 @@ LQ_HOST, LQ_DEVICE = 0, 1
 LQ_CANONICAL, LQ_NATIVE = 0, 1
 LQ_MAX_RHS = 16
 (LQ_OP_HOP, LQ_OP_M, LQ_OP_MDAG, LQ_OP_CLOVER, LQ_OP_CLOVER_INV, LQ_OP_HOP_EO, LQ_OP_HOP_OE, LQ_OP_MHAT, LQ_OP_MHAT_DAG,
- LQ_OP_KERNEL_A, LQ_OP_KERNEL_B) = range(11)
+ LQ_OP_KERNEL_A, LQ_OP_KERNEL_B, LQ_OP_PROBE_LOADS) = range(12)
 LQ_OK, LQ_EINVAL, LQ_ESTATE, LQ_ENOMEM, LQ_ECUDA, LQ_ENOTCONVERGED, LQ_ESINGULAR = 0, -1, -2, -3, -4, -5, -6
 PREC = {"fp64": LQ_FP64, "fp32": LQ_FP32, "half": LQ_HALF}
 
 EXPORTS = ["lq_create", "lq_destroy", "lq_last_error", "lq_set_allocator", "lq_load_gauge", "lq_fill_gauge_random",
            "lq_build_clover", "lq_apply", "lq_native_bytes", "lq_pack", "lq_unpack", "lq_fill_spinor_random", "lq_solve",
-           "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites", "lq_native_index", "lq_fma_peak",
+           "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites", "lq_native_index", "lq_fma_peak", "lq_mem_peak",
            "lq_laplacian", "lq_laplacian_native", "lq_cv_native_bytes", "lq_cv_fill_random", "lq_laph_eigensolve", "lq_project"]
 
 
@@ -100,6 +100,7 @@ def load_library():
     szp = ctypes.POINTER(ctypes.c_size_t)
     lib.lq_native_index.argtypes = [vp, ci, ci, ci, ci, ci, ci, ci, ci, szp, szp, szp, szp]
     lib.lq_fma_peak.argtypes = [vp, ci, cd, ctypes.POINTER(cd)]
+    lib.lq_mem_peak.argtypes = [vp, ci, cd, ctypes.POINTER(cd)]
     _lib = lib
     return lib
 
@@ -218,6 +219,13 @@ class Context:
         self._enter()
         out = ctypes.c_double()
         self._check(self.lib.lq_fma_peak(self.h, mode, ms, ctypes.byref(out)))
+        return float(out.value)
+
+    def mem_peak(self, mode: int, mbytes: float) -> float:
+        """Measured read bandwidth in GB/s: mode 0 HBM (buffer much larger than L2), mode 1 L2 -> SM (buffer inside L2)."""
+        self._enter()
+        out = ctypes.c_double()
+        self._check(self.lib.lq_mem_peak(self.h, mode, mbytes, ctypes.byref(out)))
         return float(out.value)
 
     def pack(self, canonical, nrhs: int, prec: int):

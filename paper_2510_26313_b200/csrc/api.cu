@@ -26,9 +26,9 @@ void dev_free(lq_ctx* c, void* p) {
 }
 
 int ensure_partials(lq_ctx* c, size_t elems) {
-    if (elems + elems / 16 + 64 * LQ_MAX_RHS <= c->red_partials_elems) return 0;
+    if (elems + 256 * 3 * LQ_MAX_RHS <= c->red_partials_elems) return 0;
     if (c->red_partials) dev_free(c, c->red_partials);
-    c->red_partials_elems = elems * 2 + elems / 8 + 64 * LQ_MAX_RHS;   // rows of every level of the reduction tree (reduce.cuh)
+    c->red_partials_elems = elems + elems / 8 + 256 * 3 * LQ_MAX_RHS;   // the block rows and the rows of the second stage (reduce.cuh)
     c->red_partials = (double*)dev_alloc(c, c->red_partials_elems * sizeof(double));
     if (!c->red_partials) { c->red_partials_elems = 0; return LQ_ENOMEM; }
     return 0;
@@ -231,8 +231,14 @@ int lq_native_index(const lq_ctx* c, int nrhs, int prec, int x, int y, int z, in
     return 0;
 }
 
+int lq_mem_peak(lq_ctx* c, int mode, double mbytes, double* gbs) {
+    if (!c || !gbs || mode < 0 || mode > 1 || !(mbytes > 0)) return set_err(c, LQ_EINVAL, "lq_mem_peak: bad argument");
+    cudaSetDevice(c->device);
+    return mem_peak(c, mode, mbytes, gbs);
+}
+
 int lq_fma_peak(lq_ctx* c, int mode, double ms, double* tflops) {
-    if (!c || !tflops || mode < 0 || mode > 2 || !(ms > 0)) return set_err(c, LQ_EINVAL, "lq_fma_peak: bad argument");
+    if (!c || !tflops || mode < 0 || mode > 3 || !(ms > 0)) return set_err(c, LQ_EINVAL, "lq_fma_peak: bad argument");
     cudaSetDevice(c->device);
     return fma_peak(c, mode, ms, tflops);
 }
@@ -362,6 +368,7 @@ static int apply_native(lq_ctx* c, int op, void* out, const void* in, const void
     case LQ_OP_MHAT_DAG: return mhat_native(c, prec, n, out, in, 1);
     case LQ_OP_KERNEL_A: return op_kernel_a(c, prec, n, 1, out, in, 0);
     case LQ_OP_KERNEL_B: return op_kernel_b(c, prec, n, 0, out, in, in2, -k * k, 1, 0);
+    case LQ_OP_PROBE_LOADS: return op_probe_loads(c, prec, n, 1, out, in);
     default: return set_err(c, LQ_EINVAL, "unknown operator");
     }
 }
@@ -370,7 +377,8 @@ int lq_apply(lq_ctx* c, int op, void* out, const void* in, const void* in2, int 
     if (!c || !out || !in) return set_err(c, LQ_EINVAL, "lq_apply: null argument");
     if (!nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "nrhs must be one of 1,2,4,8,12,16");
     if (prec != LQ_FP64 && prec != LQ_FP32 && prec != LQ_HALF) return set_err(c, LQ_EINVAL, "bad precision");
-    if (op < 0 || op > LQ_OP_KERNEL_B) return set_err(c, LQ_EINVAL, "unknown operator");
+    if (op < 0 || op > LQ_OP_PROBE_LOADS) return set_err(c, LQ_EINVAL, "unknown operator");
+    if (op == LQ_OP_PROBE_LOADS && layout != LQ_NATIVE) return set_err(c, LQ_EINVAL, "LQ_OP_PROBE_LOADS is a native-layout bench probe");
     if (op == LQ_OP_KERNEL_B && !in2) return set_err(c, LQ_EINVAL, "LQ_OP_KERNEL_B needs in2");
     if (out == in || out == in2) return set_err(c, LQ_EINVAL, "out must not alias an input");
     if (!c->has_gauge) return set_err(c, LQ_ESTATE, "gauge field not loaded");

@@ -32,7 +32,7 @@ struct BlasGeom { Geom g; int N, G; const int* skip; };   // skip: see lq_ctx::l
 #define LQ_BLAS_SKIP(bg) do { if ((bg).skip != nullptr && *(volatile const int*)(bg).skip) return; } while (0)
 
 template <class S, int VW, int R>
-__global__ void norm2_kernel(BlasGeom bg, SView<S> x, double* partials, unsigned int* counter, double* out) {
+__global__ void norm2_kernel(BlasGeom bg, SView<S> x, double* partials) {
     LQ_BLAS_SKIP(bg);
     using T = typename S::comp_t;
     BlasIdx<VW, R> ix(bg.g, bg.G);
@@ -47,7 +47,7 @@ __global__ void norm2_kernel(BlasGeom bg, SView<S> x, double* partials, unsigned
 #pragma unroll
             for (int k = 0; k < VW; k++) part[k] += (double)a[j][k] * (double)a[j][k];
     }
-    reduce_per_rhs<VW, R>(part, bg.N, bg.G, partials, counter, out);
+    reduce_per_rhs<VW, R>(part, bg.N, bg.G, partials);
 }
 
 // e += alpha p ; p = z + beta p   (alpha = rr / pAp, beta = rr_new / rr)
@@ -125,7 +125,7 @@ __global__ void axpy_mixed_kernel(BlasGeom bg, double* __restrict__ y, SView<S> 
 // r = b - t (fp64), per-RHS ||r||^2
 template <int VW, int R>
 __global__ void residual_kernel(BlasGeom bg, double* __restrict__ r, const double* __restrict__ b, const double* __restrict__ tv,
-                                double* partials, unsigned int* counter, double* out) {
+                                double* partials) {
     LQ_BLAS_SKIP(bg);
     BlasIdx<VW, R> ix(bg.g, bg.G);
     double part[VW];
@@ -141,7 +141,55 @@ __global__ void residual_kernel(BlasGeom bg, double* __restrict__ r, const doubl
                 r[i] = d; part[k] += d * d;
             }
     }
-    reduce_per_rhs<VW, R>(part, bg.N, bg.G, partials, counter, out);
+    reduce_per_rhs<VW, R>(part, bg.N, bg.G, partials);
+}
+
+// ---- second stage of every per-RHS reduction (reduce.cuh): rows[nrows][NC] -> out[(col / N1) * LQ_MAX_RHS + col % N1] ----------
+// <= 256 blocks, each over a contiguous range of rows (thread = column x row slice, fixed order, shared-memory tree over the
+// slices), then the last block to finish adds the block rows in index order.  The only fence / atomic of the whole reduction.
+constexpr int RF_THREADS = 256, RF_MAXB = 256;
+__global__ void __launch_bounds__(RF_THREADS) reduce_finish_kernel(const double* __restrict__ rows, int nrows, int NC, int N1, double* stage2,
+                                                                   unsigned int* counter, double* __restrict__ out, const int* skip) {
+    if (skip != nullptr && *(volatile const int*)skip) return;
+    __shared__ double sm[RF_THREADS];
+    __shared__ bool last;
+    const int t = threadIdx.x;
+    int Q = 1;                                   // row slices per block: largest power of two with NC * Q <= RF_THREADS
+    while (NC * Q * 2 <= RF_THREADS) Q <<= 1;
+    const int col = t % NC, q = t / NC;
+    const int per = (nrows + gridDim.x - 1) / gridDim.x;
+    const int r0 = blockIdx.x * per, r1 = min(nrows, r0 + per);
+    double s = 0.0;
+    if (q < Q) for (int r = r0 + q; r < r1; r += Q) s += __ldcg(rows + (size_t)r * NC + col);
+    if (q < Q) sm[t] = s;
+    __syncthreads();
+    for (int stride = Q >> 1; stride >= 1; stride >>= 1) {
+        if (q < stride) sm[t] += sm[t + stride * NC];
+        __syncthreads();
+    }
+    if (t < NC) stage2[(size_t)blockIdx.x * NC + t] = sm[t];
+    __threadfence();
+    __syncthreads();
+    if (t == 0) last = (atomicInc(counter, gridDim.x - 1) == gridDim.x - 1);
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    if (t < NC) {
+        double f = 0.0;
+        for (unsigned b = 0; b < gridDim.x; b++) f += __ldcg(stage2 + (size_t)b * NC + t);
+        out[(t / N1) * LQ_MAX_RHS + (t % N1)] = f;
+    }
+}
+int reduce_finish(lq_ctx* c, int nrows, int nq, int n1, double* d_out) {
+    const int NC = nq * n1;
+    int P = nrows / 64;
+    if (P < 1) P = 1;
+    if (P > RF_MAXB) P = RF_MAXB;
+    reduce_finish_kernel<<<P, RF_THREADS, 0, c->stream>>>(c->red_partials, nrows, NC, n1, c->red_partials + (size_t)nrows * NC,
+                                                          c->red_counter + RED_COUNTER_BASE, d_out, c->loop_skip);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
 }
 
 // ---- host side -----------------------------------------------------------------------------------------------------
@@ -171,8 +219,9 @@ static int plan(lq_ctx* c, int nrhs, int maxvw, Launch& L) {
 template <class S> static int norm2_t(lq_ctx* c, int nrhs, const void* x, double* d_out) {
     Launch L; LQ_TRY(plan(c, nrhs, S::prec == LQ_FP64 ? 2 : 4, L));
     SView<S> vx = make_view<S>(c->g, const_cast<void*>(x), nrhs, 0);
-    VW_DISPATCH(L, S, norm2_kernel, L.smem, L.bg, vx, c->red_partials, c->red_counter, d_out);
+    VW_DISPATCH(L, S, norm2_kernel, L.smem, L.bg, vx, c->red_partials);
     LQ_LAUNCHED(c);
+    LQ_TRY(reduce_finish(c, L.grid, 1, nrhs, d_out));
     BLAS_MODEL(c, S::prec, nrhs, 1, 48);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
@@ -231,10 +280,11 @@ int blas_axpy_mixed(lq_ctx* c, int prec, int nrhs, void* y64, const void* e, con
 int blas_residual(lq_ctx* c, int nrhs, void* r, const void* b, const void* t, double* d_out) {
     Launch L; LQ_TRY(plan(c, nrhs, 2, L));
     double* rp = (double*)r; const double* bp = (const double*)b; const double* tp = (const double*)t;
-    if (L.R == 4) residual_kernel<2, 4><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, rp, bp, tp, c->red_partials, c->red_counter, d_out);
-    else if (L.R == 2) residual_kernel<2, 2><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, rp, bp, tp, c->red_partials, c->red_counter, d_out);
-    else residual_kernel<1, 1><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, rp, bp, tp, c->red_partials, c->red_counter, d_out);
+    if (L.R == 4) residual_kernel<2, 4><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, rp, bp, tp, c->red_partials);
+    else if (L.R == 2) residual_kernel<2, 2><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, rp, bp, tp, c->red_partials);
+    else residual_kernel<1, 1><<<L.grid, L.block, L.smem, c->stream>>>(L.bg, rp, bp, tp, c->red_partials);
     LQ_LAUNCHED(c);
+    LQ_TRY(reduce_finish(c, L.grid, 1, nrhs, d_out));
     BLAS_MODEL(c, LQ_FP64, nrhs, 3, 72);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
@@ -280,7 +330,7 @@ __device__ __forceinline__ void caxpy_regs(const T (&sr)[VW], const T (&si)[VW],
 
 // out = (Re <a, b>, Im <a, b>, ||a||^2) per RHS, <a, b> = sum conj(a) b
 template <class S, int VW, int R>
-__global__ void cdot3_kernel(BlasGeom bg, SView<S> a, SView<S> b, double* partials, unsigned int* counter, double* out) {
+__global__ void cdot3_kernel(BlasGeom bg, SView<S> a, SView<S> b, double* partials) {
     LQ_BLAS_SKIP(bg);
     using T = typename S::comp_t;
     BlasIdx<VW, R> ix(bg.g, bg.G);
@@ -301,7 +351,7 @@ __global__ void cdot3_kernel(BlasGeom bg, SView<S> a, SView<S> b, double* partia
                 part[0][k] += ar * br + ai * bi; part[1][k] += ar * bi - ai * br; part[2][k] += ar * ar + ai * ai;
             }
     }
-    reduce_multi<3, VW, R>(part, bg.N, bg.G, partials, counter, out);
+    reduce_multi<3, VW, R>(part, bg.N, bg.G, partials);
 }
 
 // s = r - alpha v
@@ -325,7 +375,7 @@ __global__ void bicg_s_kernel(BlasGeom bg, SView<S> s, SView<S> r, SView<S> v, c
 template <class S, int VW, int R>
 __global__ void bicg_xr_kernel(BlasGeom bg, SView<S> e, SView<S> r, SView<S> p, SView<S> s, SView<S> tv, SView<S> rhat,
                                const double* __restrict__ rho, const double* __restrict__ c1, const double* __restrict__ d2,
-                               double* partials, unsigned int* counter, double* out) {
+                               double* partials) {
     LQ_BLAS_SKIP(bg);
     using T = typename S::comp_t;
     BlasIdx<VW, R> ix(bg.g, bg.G);
@@ -360,7 +410,7 @@ __global__ void bicg_xr_kernel(BlasGeom bg, SView<S> e, SView<S> r, SView<S> p, 
                 part[0][k] += hr * rr + hi * ri; part[1][k] += hr * ri - hi * rr; part[2][k] += rr * rr + ri * ri;
             }
     }
-    reduce_multi<3, VW, R>(part, bg.N, bg.G, partials, counter, out);
+    reduce_multi<3, VW, R>(part, bg.N, bg.G, partials);
 }
 
 // p = r + beta (p - omega v), beta = (rho_new / rho)(alpha / omega)
@@ -407,8 +457,9 @@ template <class S> static int cdot3_t(lq_ctx* c, int nrhs, const void* a, const 
     Launch L; LQ_TRY(plan(c, nrhs, 2, L));
     LQ_TRY(ensure_partials(c, (size_t)L.grid * nrhs * 3));
     SView<S> va = make_view<S>(c->g, const_cast<void*>(a), nrhs, 0), vb = make_view<S>(c->g, const_cast<void*>(b), nrhs, 0);
-    VW2_DISPATCH(L, S, cdot3_kernel, L.smem, L.bg, va, vb, c->red_partials, c->red_counter, d_out);
+    VW2_DISPATCH(L, S, cdot3_kernel, L.smem, L.bg, va, vb, c->red_partials);
     LQ_LAUNCHED(c);
+    LQ_TRY(reduce_finish(c, L.grid, 3, nrhs, d_out));
     BLAS_MODEL(c, S::prec, nrhs, 2, 144);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
@@ -433,8 +484,9 @@ template <class S> static int bicg_xr_t(lq_ctx* c, int nrhs, void* e, void* r, c
     SView<S> ve = make_view<S>(c->g, e, nrhs, 0), vr = make_view<S>(c->g, r, nrhs, 0), vp = make_view<S>(c->g, const_cast<void*>(p), nrhs, 0),
              vs = make_view<S>(c->g, const_cast<void*>(s), nrhs, 0), vt = make_view<S>(c->g, const_cast<void*>(t), nrhs, 0),
              vh = make_view<S>(c->g, const_cast<void*>(rhat), nrhs, 0);
-    VW2_DISPATCH(L, S, bicg_xr_kernel, L.smem, L.bg, ve, vr, vp, vs, vt, vh, rho, c1, d2, c->red_partials, c->red_counter, d_out);
+    VW2_DISPATCH(L, S, bicg_xr_kernel, L.smem, L.bg, ve, vr, vp, vs, vt, vh, rho, c1, d2, c->red_partials);
     LQ_LAUNCHED(c);
+    LQ_TRY(reduce_finish(c, L.grid, 3, nrhs, d_out));
     BLAS_MODEL(c, S::prec, nrhs, 7, 432);
     LQ_CUDA(c, cudaGetLastError());
     return 0;

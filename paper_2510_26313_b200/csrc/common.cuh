@@ -113,7 +113,8 @@ template <typename T> struct VecOf;
 template <> struct VecOf<float>  { using v_t = float4;  static constexpr int VL = 4; };
 template <> struct VecOf<double> { using v_t = double2; static constexpr int VL = 2; };
 
-template <typename T, int R>
+// SMEM: blockbase points into shared memory (a staged copy of the block, same plane layout): plain loads instead of ld.global.nc
+template <typename T, int R, bool SMEM = false>
 __device__ __forceinline__ void load_planes(const T* __restrict__ blockbase, int s, T* out) {
     constexpr int VL = VecOf<T>::VL;
     constexpr int NF = R / VL;
@@ -121,15 +122,21 @@ __device__ __forceinline__ void load_planes(const T* __restrict__ blockbase, int
 #pragma unroll
     for (int q = 0; q < NF; q++) {
         if constexpr (VL == 4) {
-            float4 v = __ldg(reinterpret_cast<const float4*>(blockbase + q * 4 * SB) + s);
+            const float4* p = reinterpret_cast<const float4*>(blockbase + q * 4 * SB) + s;
+            float4 v;
+            if constexpr (SMEM) v = *p; else v = __ldg(p);
             out[4 * q] = v.x; out[4 * q + 1] = v.y; out[4 * q + 2] = v.z; out[4 * q + 3] = v.w;
         } else {
-            double2 v = __ldg(reinterpret_cast<const double2*>(blockbase + q * 2 * SB) + s);
+            const double2* p = reinterpret_cast<const double2*>(blockbase + q * 2 * SB) + s;
+            double2 v;
+            if constexpr (SMEM) v = *p; else v = __ldg(p);
             out[2 * q] = v.x; out[2 * q + 1] = v.y;
         }
     }
     if constexpr (REM == 2) {
-        float2 v = __ldg(reinterpret_cast<const float2*>(blockbase + NF * VL * SB) + s);
+        const float2* p = reinterpret_cast<const float2*>(blockbase + NF * VL * SB) + s;
+        float2 v;
+        if constexpr (SMEM) v = *p; else v = __ldg(p);
         out[NF * VL] = v.x; out[NF * VL + 1] = v.y;
     }
 }
@@ -195,12 +202,10 @@ struct lq_ctx {
 int set_err(lq_ctx* c, int code, const std::string& msg);
 void* dev_alloc(lq_ctx* c, size_t bytes);          // nullptr on failure (error recorded)
 void dev_free(lq_ctx* c, void* p);
-// deterministic reduction tree (reduce.cuh): fan-in, where its counters start in lq_ctx::red_counter (the first 64 words are
-// flags) and how many there are (enough for 4M blocks)
-constexpr int RED_FAN = 32;
+// second stage of the deterministic reductions (reduce.cuh, blas.cu): its one self-resetting counter sits behind the first 64
+// words of lq_ctx::red_counter (flags)
 constexpr int RED_COUNTER_BASE = 64;
-constexpr int RED_COUNTERS = 1 << 17;
-constexpr size_t RED_COUNTER_BYTES = (size_t)(RED_COUNTER_BASE + RED_COUNTERS) * sizeof(unsigned int);
+constexpr size_t RED_COUNTER_BYTES = (size_t)(RED_COUNTER_BASE + 64) * sizeof(unsigned int);
 int ensure_partials(lq_ctx* c, size_t elems);      // reduction scratch of at least `elems` doubles
 
 #define LQ_CUDA(ctx, call)                                                                     \

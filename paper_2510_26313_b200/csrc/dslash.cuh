@@ -20,7 +20,7 @@
 #pragma once
 #include "common.cuh"
 
-enum { FORM_HOP = 0, FORM_A = 1, FORM_B = 2 };
+enum { FORM_HOP = 0, FORM_A = 1, FORM_B = 2, FORM_PROBE = 3 };   // FORM_PROBE: kernel A's memory accesses with trivial arithmetic (bench only)
 // fused epilogues of kernel B: per-RHS ||out||^2, or out <- out - (num/den)_k * result with per-RHS ||out||^2
 // or (EPI_CDOT, BiCGStab) the complex inner product of a vector h with the result: (Re, Im <h, out>, ||out||^2), Im negated if epi_conj
 enum { EPI_NONE = 0, EPI_NORM = 1, EPI_XMAY = 2, EPI_CDOT = 3 };
@@ -109,9 +109,9 @@ __device__ __forceinline__ void store_comp(typename S::store_t* __restrict__ p, 
 }
 
 // ---- link load (+ 12-real reconstruction: third row = conj(row0 x row1)) -----------------------------
-template <typename T, int RECON>
+template <typename T, int RECON, bool SMEM = false>
 __device__ __forceinline__ void load_link(const T* __restrict__ blockbase, int s, T* u) {
-    load_planes<T, RECON>(blockbase, s, u);
+    load_planes<T, RECON, SMEM>(blockbase, s, u);
     if constexpr (RECON == 12) {
 #pragma unroll
         for (int c = 0; c < 3; c++) {
@@ -294,14 +294,14 @@ __device__ __forceinline__ void project_half(const T (&p)[4][2][RPT], T sigma, i
 // ---- one of the eight hopping terms -------------------------------------------------------------------
 // acc[j][k] += cu * (1 - sigma*gamma_MU) W psi(nb),  W = U (FWD) or U^dag (backward), sigma = +-1.
 // `nb` points at real 0 of the neighbour's RPT right-hand sides; real j is at nb + j*SB*R.
-template <class S, int RPT, int R, int RECON, int MU, bool FWD>
+template <class S, int RPT, int R, int RECON, int MU, bool FWD, bool SMLINK = false>
 __device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ nb, const float* __restrict__ nb_norm,
                                         const typename S::comp_t* __restrict__ link_blk, int link_s,
                                         typename S::comp_t cu, typename S::comp_t sigma, typename S::comp_t (&acc)[24][RPT]) {
     using T = typename S::comp_t;
     constexpr int PL = SB * R;   // elements between consecutive reals of a site
     T u[18];
-    load_link<T, RECON>(link_blk, link_s, u);
+    load_link<T, RECON, SMLINK>(link_blk, link_s, u);
 
     T cuk[RPT], clk[RPT];
     if constexpr (S::has_norm) {
@@ -332,3 +332,35 @@ __device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ 
 #endif
     hop_mulacc<T, RPT, MU, FWD>(h, u, cuk, clk, acc);
 }
+
+// ---- bench-only probe: the loads of one hopping term (link, 24 rows of the neighbour, norm) with ONE multiply-add per loaded
+// value.  Kernel FORM_PROBE = kernel A's address stream, prefetches and stores without its arithmetic: its time is the floor
+// that the memory path (L1 misses in flight, L2 -> SM transfers, HBM) sets for this access pattern (bench.py --op cfgN:probe:...).
+template <class S, int RPT, int R, int RECON, bool SMLINK = false>
+__device__ __forceinline__ void hop_dir_probe(const typename S::store_t* __restrict__ nb, const float* __restrict__ nb_norm,
+                                              const typename S::comp_t* __restrict__ link_blk, int link_s, typename S::comp_t (&acc)[24][RPT]) {
+    using T = typename S::comp_t;
+    constexpr int PL = SB * R;
+    T u[18];
+    load_planes<T, RECON, SMLINK>(link_blk, link_s, u);
+    if constexpr (RECON == 12) {
+#pragma unroll
+        for (int i = 12; i < 18; i++) u[i] = u[i - 12];
+    }
+    T sc[RPT];
+    if constexpr (S::has_norm) { float nrm[RPT]; load_norm<RPT>(nb_norm, nrm);
+#pragma unroll
+        for (int k = 0; k < RPT; k++) sc[k] = nrm[k];
+    } else {
+#pragma unroll
+        for (int k = 0; k < RPT; k++) sc[k] = T(1);
+    }
+#pragma unroll
+    for (int j = 0; j < 24; j++) {
+        T p[RPT];
+        load_comp<S, RPT>(nb + j * PL, p);
+#pragma unroll
+        for (int k = 0; k < RPT; k++) acc[j][k] = fm(p[k] * sc[k], u[j % 18], acc[j][k]);
+    }
+}
+

@@ -56,12 +56,12 @@ __device__ __forceinline__ void clover_block_mul(const T* cl, const T (&v)[6][2]
 }
 
 // acc (24 reals x RPT) <- C acc, one chirality block at a time
-template <typename T, int RPT>
+template <typename T, int RPT, bool SMEM = false>
 __device__ __forceinline__ void clover_apply_regs(const T* __restrict__ clov_blk, int s, T (&acc)[24][RPT]) {
 #pragma unroll
     for (int b = 0; b < 2; b++) {
         T cl[36], v[6][2][RPT], o[6][2][RPT];
-        load_planes<T, 36>(clov_blk + b * 36 * SB, s, cl);
+        load_planes<T, 36, SMEM>(clov_blk + b * 36 * SB, s, cl);
 #pragma unroll
         for (int i = 0; i < 6; i++)
 #pragma unroll
@@ -265,7 +265,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
     const T cp = (sc.t + 1 == sc.Lt) ? c0 * a.tsign : c0;     // boundary sign on the wrapped t terms
     const T cm = (sc.t == 0) ? c0 * a.tsign : c0;
 #define LQ_HOP(D) { const int nb_ = neighbour<D>(sc); \
-        hop_dir<S, RPT, R, RECON, ((D) >> 1), (((D) & 1) == 0)>(LQ_NB_PTR(nb_), LQ_NB_NRM(nb_), LQ_LINK(D, nb_), LQ_LINK_S(D, nb_), \
+        if constexpr (FORM == FORM_PROBE) hop_dir_probe<S, RPT, R, RECON>(LQ_NB_PTR(nb_), LQ_NB_NRM(nb_), LQ_LINK(D, nb_), LQ_LINK_S(D, nb_), acc); \
+        else hop_dir<S, RPT, R, RECON, ((D) >> 1), (((D) & 1) == 0)>(LQ_NB_PTR(nb_), LQ_NB_NRM(nb_), LQ_LINK(D, nb_), LQ_LINK_S(D, nb_), \
                 (D) == 6 ? cp : ((D) == 7 ? cm : c0), ((D) & 1) ? -a.dsign : a.dsign, acc); }
     LQ_HOP(0) LQ_HOP(1) LQ_HOP(2) LQ_HOP(3) LQ_HOP(4) LQ_HOP(5) LQ_HOP(6) LQ_HOP(7)
 #undef LQ_HOP
@@ -276,6 +277,14 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
 
     // ---- epilogue (FORM_A): acc <- C acc -----------------------------------------------------------------
     if constexpr (FORM == FORM_A) clover_apply_regs<T, RPT>(a.clover + (size_t)blk * (72 * SB), s, acc);
+    if constexpr (FORM == FORM_PROBE) {       // the clover block's loads, one multiply-add per loaded value
+        T cl[72];
+        load_planes<T, 72>(a.clover + (size_t)blk * (72 * SB), s, cl);
+#pragma unroll
+        for (int j = 0; j < 72; j++)
+#pragma unroll
+            for (int k = 0; k < RPT; k++) acc[j % 24][k] = fm(cl[j], T(0.5), acc[j % 24][k]);
+    }
 
     // ---- fused block-BLAS epilogues of kernel B and store ---------------------------------
     if constexpr (FORM == FORM_B) {
@@ -327,8 +336,8 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
             double p3[3][RPT];
 #pragma unroll
             for (int k = 0; k < RPT; k++) { p3[0][k] = part_c[0][k]; p3[1][k] = part_c[1][k]; p3[2][k] = part[k]; }
-            reduce_multi<3, RPT, R>(p3, a.N, G, a.red_partials, a.red_counter, a.epi_out);
-        } else if constexpr (EPI != EPI_NONE) reduce_per_rhs<RPT, R>(part, a.N, G, a.red_partials, a.red_counter, a.epi_out);
+            reduce_multi<3, RPT, R>(p3, a.N, G, a.red_partials);
+        } else if constexpr (EPI != EPI_NONE) reduce_per_rhs<RPT, R>(part, a.N, G, a.red_partials);
     }
 }
 

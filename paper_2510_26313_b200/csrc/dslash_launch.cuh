@@ -11,19 +11,20 @@ static int launch_one(lq_ctx* c, DslashArgs<S> a) {
         LQ_TRY(ensure_partials(c, (size_t)grid * a.N * (a.epi == EPI_CDOT ? 3 : 1)));
         a.red_partials = c->red_partials; a.red_counter = c->red_counter;
     }
+    const size_t smem = FORM == FORM_B ? BLOCK * sizeof(double) : 0;      // scratch of the fused reduction
     if constexpr (FORM == FORM_B) {
-        const size_t smem = BLOCK * sizeof(double);
         switch (a.epi) {
         case EPI_NORM: dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, EPI_NORM><<<grid, BLOCK, smem, c->stream>>>(a); break;
         case EPI_XMAY: dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, EPI_XMAY><<<grid, BLOCK, smem, c->stream>>>(a); break;
         case EPI_CDOT: dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, EPI_CDOT><<<grid, BLOCK, smem, c->stream>>>(a); break;
-        default: dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, EPI_NONE><<<grid, BLOCK, 0, c->stream>>>(a); break;
+        default: dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, EPI_NONE><<<grid, BLOCK, smem, c->stream>>>(a); break;
         }
     } else {
-        dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, EPI_NONE><<<grid, BLOCK, 0, c->stream>>>(a);
+        dslash_kernel<S, RPT, R, RECON, FORM, BLOCK, MINB, EPI_NONE><<<grid, BLOCK, smem, c->stream>>>(a);
     }
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
+    if (FORM == FORM_B && a.epi != EPI_NONE) LQ_TRY(reduce_finish(c, grid, a.epi == EPI_CDOT ? 3 : 1, a.N, a.epi_out));
     return 0;
 }
 
@@ -60,7 +61,7 @@ static int launch_rpt(lq_ctx* c, DslashArgs<S> a, int variant) {
     plan_sweep<S>(c, a);
     if constexpr (S::prec != LQ_FP64) {
         constexpr int ALT = RPT == 4 ? 3 : (RPT == 2 ? 4 : 5);
-        if (variant == 1) return launch_one<S, RPT, R, RECON, FORM, ALT>(c, a);
+        if ((variant & 1) == 1) return launch_one<S, RPT, R, RECON, FORM, ALT>(c, a);
     }
     return launch_one<S, RPT, R, RECON, FORM, DEF>(c, a);
 }

@@ -7,7 +7,10 @@
 // mode 0: x_i = fma(x_i, b, c)                    scalar FFMA, 3 distinct source registers
 // mode 1: X_i = ffma2(X_i, B, C)                  packed FFMA2, 3 distinct 64-bit sources
 // mode 2: X_i = ffma2(A_q, Y_i, X_i), q = i / 4   packed FFMA2, the first source shared by 4 consecutive instructions
-//                                                 (the stencil's pattern: one duplicated link element times 4 spinor reals)
+// mode 3: X_i = ffma2((s_q, s_q), Y_i, X_i)         packed FFMA2 whose first source is ONE 32-bit register broadcast to both halves
+//                                                 (SASS "R.F32" operand form): what the compiler emits for the stencil's
+//                                                 link-element x spinor-pair products; three register sources hit one register
+//                                                 bank three times, so the instruction issues every 3rd cycle instead of every 2nd
 template <int MODE>
 __global__ void __launch_bounds__(256) fma_peak_kernel(float* out, int iters, float b, float c0) {
     constexpr int NACC = 16;
@@ -32,8 +35,9 @@ __global__ void __launch_bounds__(256) fma_peak_kernel(float* out, int iters, fl
         for (int i = 0; i < NACC; i++) x[i] = make_float2(seed + i, seed - i);
         const float2 b2 = make_float2(b, b * 0.999f), c2 = make_float2(c0, c0 * 1.001f);
         float2 a[4], y[NACC];
+        float sc[4];
 #pragma unroll
-        for (int q = 0; q < 4; q++) a[q] = make_float2(b * (1.f + 0.01f * q), b * (1.f - 0.01f * q));
+        for (int q = 0; q < 4; q++) { a[q] = make_float2(b * (1.f + 0.01f * q), b * (1.f - 0.01f * q)); sc[q] = b * (1.f + 0.02f * q) + seed * 1e-3f; }
 #pragma unroll
         for (int i = 0; i < NACC; i++) y[i] = make_float2(c0 + 0.01f * i, c0 - 0.01f * i);
         for (int it = 0; it < iters; it++) {
@@ -42,12 +46,13 @@ __global__ void __launch_bounds__(256) fma_peak_kernel(float* out, int iters, fl
 #pragma unroll
                 for (int i = 0; i < NACC; i++) {
                     if constexpr (MODE == 1) x[i] = __ffma2_rn(x[i], b2, c2);
-                    else x[i] = __ffma2_rn(a[i >> 2], y[i], x[i]);
+                    else if constexpr (MODE == 2) x[i] = __ffma2_rn(a[i >> 2], y[i], x[i]);
+                    else x[i] = __ffma2_rn(make_float2(sc[i >> 2], sc[i >> 2]), y[i], x[i]);
                 }
             }
-            if constexpr (MODE == 2) {      // keep the operands loop-variant so nothing is hoisted or folded
+            if constexpr (MODE >= 2) {      // keep the operands loop-variant so nothing is hoisted or folded
 #pragma unroll
-                for (int q = 0; q < 4; q++) a[q].x = -a[q].x;
+                for (int q = 0; q < 4; q++) { a[q].x = -a[q].x; sc[q] = -sc[q]; }
             }
         }
         float s = 0.f;
@@ -72,7 +77,8 @@ int fma_peak(lq_ctx* c, int mode, double ms, double* tflops) {
         const float b = 0.9999f, c0 = 1e-4f;      // |x| stays bounded: x <- 0.9999 x + 1e-4
         if (mode == 0) fma_peak_kernel<0><<<grid, block, 0, c->stream>>>(out, iters, b, c0);
         else if (mode == 1) fma_peak_kernel<1><<<grid, block, 0, c->stream>>>(out, iters, b, c0);
-        else fma_peak_kernel<2><<<grid, block, 0, c->stream>>>(out, iters, 1e-6f, c0);
+        else if (mode == 2) fma_peak_kernel<2><<<grid, block, 0, c->stream>>>(out, iters, 1e-6f, c0);
+        else fma_peak_kernel<3><<<grid, block, 0, c->stream>>>(out, iters, 1e-6f, c0);
         LQ_LAUNCHED(c);
         cudaEventRecord(e1, c->stream);
         if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) return set_err(c, LQ_ECUDA, "fma_peak kernel failed");
@@ -99,3 +105,56 @@ int fma_peak(lq_ctx* c, int mode, double ms, double* tflops) {
     dev_free(c, out);
     return rc;
 }
+
+// ---- L2 -> SM read bandwidth ------------------------------------------------------------------------------------------------
+// Every thread streams 16-byte loads (ld.global.cg: no L1 allocation, 8 independent loads in flight) over a buffer that fits in
+// L2 (mode 1, re-read `passes` times) or exceeds it several times (mode 0: HBM).  The stencil kernels fetch every compulsory
+// byte ~3x from L2 (the 8 neighbour reads of a site meet in L2, not in L1), so next to HBM this is the second memory-side bound.
+__global__ void __launch_bounds__(256) mem_read_kernel(const float4* __restrict__ buf, size_t n16, int passes, float* out) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    float acc = 0.f;
+    for (int p = 0; p < passes; p++) {
+        size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+        for (; i + 7 * stride < n16; i += 8 * stride) {
+            float4 v[8];
+#pragma unroll
+            for (int u = 0; u < 8; u++) v[u] = __ldcg(buf + i + u * stride);
+#pragma unroll
+            for (int u = 0; u < 8; u++) acc += v[u].x + v[u].y + v[u].z + v[u].w;
+        }
+        for (; i < n16; i += stride) { const float4 v = __ldcg(buf + i); acc += v.x + v.y + v.z + v.w; }
+    }
+    if (acc == 123.456f) out[0] = acc;
+}
+
+int mem_peak(lq_ctx* c, int mode, double mbytes, double* gbs) {
+    int dev = 0, sms = 0;
+    LQ_CUDA(c, cudaGetDevice(&dev));
+    LQ_CUDA(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const size_t bytes = ((size_t)(mbytes * 1e6) / 4096) * 4096;
+    if (bytes < 4096) return set_err(c, LQ_EINVAL, "lq_mem_peak: buffer too small");
+    float* buf = (float*)dev_alloc(c, bytes + 256);
+    if (!buf) return LQ_ENOMEM;
+    int rc = 0;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (cudaMemsetAsync(buf, 0, bytes + 256, c->stream) != cudaSuccess || cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess)
+        rc = set_err(c, LQ_ECUDA, "lq_mem_peak: setup failed");
+    const int passes = mode == 1 ? 200 : 4;
+    const int grid = sms * 8;
+    float ms = 0.f;
+    if (rc == 0) {
+        mem_read_kernel<<<grid, 256, 0, c->stream>>>((const float4*)buf, bytes / 16, 2, buf + bytes / 4);       // warm-up (fills L2 in mode 1)
+        cudaEventRecord(e0, c->stream);
+        mem_read_kernel<<<grid, 256, 0, c->stream>>>((const float4*)buf, bytes / 16, passes, buf + bytes / 4);
+        cudaEventRecord(e1, c->stream);
+        c->launches += 2;
+        if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = set_err(c, LQ_ECUDA, "lq_mem_peak: kernel failed");
+        else cudaEventElapsedTime(&ms, e0, e1);
+    }
+    if (rc == 0) *gbs = (double)bytes * passes / (ms * 1e-3) * 1e-9;
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    dev_free(c, buf);
+    return rc;
+}
+

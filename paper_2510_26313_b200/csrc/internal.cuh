@@ -11,6 +11,8 @@ int launch_dslash(lq_ctx* c, DslashArgs<S> a, int rpt, int variant);
 // out(parity) = [C] D in(1-parity) ; form A uses A^{-1}, form HOP nothing
 int op_hop(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* in, int dagger);
 int op_kernel_a(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* in, int dagger);
+// bench only: kernel A's memory accesses with trivial arithmetic (fp32 / half storage, 18-real links)
+int op_probe_loads(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* in);
 // out(parity) = C x + coef D in ; use_clover: 1 -> A(parity), 0 -> identity
 int op_kernel_b(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger);
 // kernel B with a fused block-BLAS epilogue: EPI_NORM: epi_out[k] = ||out_k||^2 ; EPI_XMAY: out_k <- out_k - (num_k/den_k) (C x + coef D in)_k
@@ -63,6 +65,7 @@ int fill_spinor(lq_ctx* c, void* native, int nrhs, int prec, uint64_t seed, int 
 
 // fmapeak.cu
 int fma_peak(lq_ctx* c, int mode, double ms, double* tflops);
+int mem_peak(lq_ctx* c, int mode, double mbytes, double* gbs);
 
 // solver.cu
 void solver_release(lq_ctx* c);

@@ -60,6 +60,18 @@ int op_kernel_a(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const 
     return kernel_a_t<H16>(c, nrhs, out_parity, out, in, dagger);
 }
 
+int op_probe_loads(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* in) {
+    if (c->recon32 != 18 || (prec != LQ_FP32 && prec != LQ_HALF)) return set_err(c, LQ_EINVAL, "LQ_OP_PROBE_LOADS: fp32 or half storage with 18-real links only");
+    if (prec == LQ_FP32) {
+        auto a = base_args<F32>(c, nrhs, out_parity, out, in, nullptr, 0);
+        a.clover = clover_ptr<F32>(c, out_parity, 1);
+        return launch_dslash<F32, 18, FORM_PROBE>(c, a, c->dslash_rpt, c->dslash_variant);
+    }
+    auto a = base_args<H16>(c, nrhs, out_parity, out, in, nullptr, 0);
+    a.clover = clover_ptr<H16>(c, out_parity, 1);
+    return launch_dslash<H16, 18, FORM_PROBE>(c, a, c->dslash_rpt, c->dslash_variant);
+}
+
 template <class S> static int kernel_b_t(lq_ctx* c, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger,
                                          int epi, const double* num, const double* den, double* epi_out) {
     auto a = base_args<S>(c, nrhs, out_parity, out, in, x, dagger);

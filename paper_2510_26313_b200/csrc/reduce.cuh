@@ -1,16 +1,28 @@
 // reduce.cuh -- deterministic per-RHS sums over a whole launch (used by the block-BLAS kernels and by the fused
 // epilogues of the stencil kernels).  Thread mapping assumed: unit u = global thread / (32 * TPG), RHS group = u % G,
 // lane % TPG selects the VW right-hand sides of the thread inside the group; a warp lies inside one unit.
+//
+// Two stages.  (1) Inside the producing kernel (reduce_multi below): fp64 per thread -> warp shuffle -> fixed-order sum over
+// the block's warps -> ONE ROW of partial sums per block, written with plain stores: no fence, no atomic, nothing that makes a
+// block wait for its own stores (the round-1 version ended every block with __threadfence + atomicInc to elect a "last block";
+// on the 248832-block stencil launches of configs[3] that tail cost ~1 ms of a 6 ms kernel, profiles/r02_launches_cfg3.md).
+// (2) reduce_finish (blas.cu): a small second launch sums the rows in a fixed order (<= 256 blocks over contiguous row ranges,
+// then the last of THOSE blocks -- the only place a fence and an atomic remain -- adds their rows in index order).
+// Bitwise reproducible: the order of every addition is fixed by the launch geometry alone.
 #pragma once
 #include "common.cuh"
 
+// second stage (blas.cu): sums the `nrows` block rows left in lq_ctx::red_partials (nq quantities x n1 right-hand sides) into
+// d_out[q * LQ_MAX_RHS + rhs]; enqueued right behind the kernel that produced the rows
+int reduce_finish(lq_ctx* c, int nrows, int nq, int n1, double* d_out);
+
 // part[q][VW] are this thread's sums of quantity q for right-hand sides rhs0 + k (NQ quantities reduced in one pass, e.g. the real
-// and imaginary part of an inner product and a norm).  Result: out[q * LQ_MAX_RHS + rhs].  Block size must be a multiple of 32
-// and at least NQ * N.
+// and imaginary part of an inner product and a norm).  Writes partials[blockIdx.x][q * N1 + rhs] (a dense row: zeros for the
+// right-hand sides of groups this block does not touch).  Block size must be a multiple of 32 and at least N1.
 template <int NQ, int VW, int R>
-__device__ void reduce_multi(double (&part)[NQ][VW], int N1, int G, double* partials, unsigned int* counter, double* out) {
+__device__ __forceinline__ void reduce_multi(double (&part)[NQ][VW], int N1, int G, double* __restrict__ partials) {
     constexpr int TPG = R / VW;
-    extern __shared__ double sm[];       // [max(nwarps * R, blockDim.x)]
+    extern __shared__ double sm[];       // [nwarps * R]
     const int t = threadIdx.x, nt = blockDim.x, lane = t & 31, w = t >> 5, nw = nt >> 5;
     const int N = NQ * N1;               // row width of the partial sums
 #pragma unroll
@@ -38,48 +50,13 @@ __device__ void reduce_multi(double (&part)[NQ][VW], int N1, int G, double* part
             partials[(size_t)blockIdx.x * N + qq * N1 + t] = s;
         }
     }
-    // Fan-in tree over the blocks (RED_FAN per node, fixed grouping and order: bitwise reproducible).  The last block to
-    // finish in a group of RED_FAN adds the group's rows and becomes the group's representative one level up; the tail that
-    // runs after all other blocks have retired is then a few short rounds instead of one block reading every partial.
-    // Level l rows live behind those of level l-1 in `partials`, its self-resetting counters behind those of level l-1.
-    __shared__ bool last;
-    int Q = 1;                             // thread t handles RHS t % N, row slice t / N; Q = largest power of two with N*Q <= nt
-    while (N * Q * 2 <= nt) Q <<= 1;
-    const int r = t % N, q = t / N;
-    unsigned idx = blockIdx.x, n = gridDim.x;
-    double* src = partials;
-    unsigned int* cnt = counter + RED_COUNTER_BASE;
-    for (;;) {
-        const unsigned grp = idx / RED_FAN, ngrp = (n + RED_FAN - 1) / RED_FAN;
-        const unsigned gsize = min((unsigned)RED_FAN, n - grp * RED_FAN);
-        __threadfence();
-        __syncthreads();
-        if (t == 0) last = (atomicInc(cnt + grp, gsize - 1) == gsize - 1);
-        __syncthreads();
-        if (!last) return;
-        __threadfence();
-        const double* rows = src + (size_t)grp * RED_FAN * N;
-        double s = 0.0;
-        if (q < Q) for (unsigned b = q; b < gsize; b += Q) s += __ldcg(rows + (size_t)b * N + r);
-        __syncthreads();
-        if (q < Q) sm[t] = s;
-        __syncthreads();
-        for (int stride = Q >> 1; stride >= 1; stride >>= 1) {
-            if (q < stride) sm[t] += sm[t + stride * N];
-            __syncthreads();
-        }
-        if (ngrp == 1) { if (t < N) out[(t / N1) * LQ_MAX_RHS + (t % N1)] = sm[t]; return; }
-        double* dst = src + (size_t)n * N;
-        if (t < N) dst[(size_t)grp * N + t] = sm[t];
-        src = dst; cnt += ngrp; idx = grp; n = ngrp;
-    }
 }
 
-// part[VW] are this thread's sums for right-hand sides rhs0 + k; out[rhs]
+// part[VW] are this thread's sums for right-hand sides rhs0 + k
 template <int VW, int R>
-__device__ __forceinline__ void reduce_per_rhs(double (&part)[VW], int N, int G, double* partials, unsigned int* counter, double* out) {
+__device__ __forceinline__ void reduce_per_rhs(double (&part)[VW], int N, int G, double* __restrict__ partials) {
     double p1[1][VW];
 #pragma unroll
     for (int k = 0; k < VW; k++) p1[0][k] = part[k];
-    reduce_multi<1, VW, R>(p1, N, G, partials, counter, out);
+    reduce_multi<1, VW, R>(p1, N, G, partials);
 }

@@ -325,7 +325,7 @@ def time_eigensolve(B, device):
         kw = dict(n_ev=n_ev, m=m, cheb_degree=24, cheb_a=cut, cheb_b=12.5, tol=1e-9, max_restarts=50, want_vectors=False)
         ctx.laph_eigensolve(**kw)
         ev, _, info = ctx.laph_eigensolve(**kw)
-        out["cases"].append({"n_ev": n_ev, "krylov": m, "cheb_degree": 24, "seconds": round(info["seconds"], 4), "restarts": info["restarts"],
+        out["cases"].append({"n_ev": n_ev, "krylov": m, "cheb_degree": 24, "seconds": round(info["seconds"], 4), "seconds_ritz": round(info["seconds_ritz"], 4), "seconds_ortho": round(info["seconds_ortho"], 4), "restarts": info["restarts"],
                              "laplacian_applies": info["lap_applies"], "converged": info["converged"],
                              "max_true_residual": info["max_true_residual"], "eigenvalue_range": [float(ev.min()), float(ev.max())]})
     ctx.close()

@@ -233,6 +233,8 @@ typedef struct {
     double max_ritz_residual;  /* the convergence measure above, worst pair and slice                   */
     double max_true_residual;  /* max over pairs and slices of ||A v - lambda v||_2 of the returned vectors (||v|| = 1) */
     double seconds;
+    double seconds_ritz;       /* part of `seconds` spent in the Ritz step (projected eigenproblems of all slices + basis rotation) */
+    double seconds_ortho;      /* part spent in the Gram-Schmidt passes against the Krylov basis                              */
 } lq_eig_info;
 /* evals: HOST array [Lt][n_ev] (ascending per slice); evecs: canonical [n_ev][t][z][y][x][colour] complex double at
  * `loc`, or NULL.  Each returned vector has unit norm on every time-slice.  Returns LQ_ENOTCONVERGED (outputs still

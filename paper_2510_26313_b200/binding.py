@@ -43,7 +43,8 @@ class EigParam(ctypes.Structure):
 
 class EigInfo(ctypes.Structure):
     _fields_ = [("restarts", ctypes.c_int), ("converged", ctypes.c_int), ("lap_applies", ctypes.c_double),
-                ("max_ritz_residual", ctypes.c_double), ("max_true_residual", ctypes.c_double), ("seconds", ctypes.c_double)]
+                ("max_ritz_residual", ctypes.c_double), ("max_true_residual", ctypes.c_double), ("seconds", ctypes.c_double),
+                ("seconds_ritz", ctypes.c_double), ("seconds_ortho", ctypes.c_double)]
 
 
 class SolveInfo(ctypes.Structure):
@@ -277,7 +278,7 @@ class Context:
                                          LQ_HOST, ctypes.byref(prm), ctypes.byref(info))
         self._check(rc, allow=(LQ_ENOTCONVERGED,))
         d = dict(converged=bool(info.converged), restarts=info.restarts, lap_applies=info.lap_applies, max_ritz_residual=info.max_ritz_residual,
-                 max_true_residual=info.max_true_residual, seconds=info.seconds)
+                 max_true_residual=info.max_true_residual, seconds=info.seconds, seconds_ritz=info.seconds_ritz, seconds_ortho=info.seconds_ortho)
         return evals, evecs, d
 
     def project(self, evecs, sols, prec: int = LQ_FP64):

@@ -5,13 +5,13 @@
 // norms, projected matrices, Ritz rotations) exists once per slice.  The operator handed to Lanczos is the Chebyshev
 // polynomial B = T_d((2A - (a+b)) / (b-a)) of A = -Laplacian: eigenvalues of A below the cut `a` are mapped to the
 // largest |eigenvalues| of B, which Lanczos finds first.  The Krylov basis is kept fully orthogonal (two classical
-// Gram-Schmidt passes per step), so the projected matrix T = V^dag B V is real symmetric and is simply re-diagonalised
-// (host, m x m per slice, slices shared among host threads: cyclic Jacobi up to m = 64, Householder + implicit QL beyond) at every restart; the k best Ritz vectors and the residual vector seed the
-// next sweep (thick restart).  Eigenvalues of A are returned as Rayleigh quotients <v, A v> of the final Ritz vectors.
+// Gram-Schmidt passes per step), so the projected matrix T = V^dag B V is real symmetric and is simply re-diagonalised at every
+// restart ON THE DEVICE (ritz_jacobi_kernel: one CTA per time-slice, parallel two-sided Jacobi, all slices in one launch); the k
+// best Ritz vectors and the residual vector seed the next sweep (thick restart).  Eigenvalues of A are returned as Rayleigh quotients <v, A v> of the final Ritz vectors.
 #include <math.h>
 #include <algorithm>
 #include <vector>
-#include <thread>
+#include <chrono>
 #include "internal.cuh"
 #include "eigen_kernels.cuh"
 
@@ -63,128 +63,6 @@ int chebyshev(Eig& e, double* out, const double* v, int degree, double a, double
     return 0;
 }
 
-// cyclic Jacobi for a real symmetric n x n matrix (row-major a, destroyed); eigenvalues d, eigenvectors columns of q
-void jacobi(int n, std::vector<double>& a, std::vector<double>& d, std::vector<double>& q) {
-    q.assign((size_t)n * n, 0.0);
-    for (int i = 0; i < n; i++) q[(size_t)i * n + i] = 1.0;
-    for (int sweep = 0; sweep < 60; sweep++) {
-        double offd = 0.0;
-        for (int i = 0; i < n; i++) for (int j = i + 1; j < n; j++) offd += a[(size_t)i * n + j] * a[(size_t)i * n + j];
-        if (offd < 1e-300) break;
-        for (int p = 0; p < n; p++)
-            for (int r = p + 1; r < n; r++) {
-                const double apr = a[(size_t)p * n + r];
-                if (fabs(apr) < 1e-300) continue;
-                const double theta = (a[(size_t)r * n + r] - a[(size_t)p * n + p]) / (2.0 * apr);
-                const double tt = (theta >= 0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
-                const double cs = 1.0 / sqrt(tt * tt + 1.0), sn = tt * cs;
-                for (int k = 0; k < n; k++) {
-                    const double akp = a[(size_t)k * n + p], akr = a[(size_t)k * n + r];
-                    a[(size_t)k * n + p] = cs * akp - sn * akr; a[(size_t)k * n + r] = sn * akp + cs * akr;
-                }
-                for (int k = 0; k < n; k++) {
-                    const double apk = a[(size_t)p * n + k], ark = a[(size_t)r * n + k];
-                    a[(size_t)p * n + k] = cs * apk - sn * ark; a[(size_t)r * n + k] = sn * apk + cs * ark;
-                }
-                for (int k = 0; k < n; k++) {
-                    const double qkp = q[(size_t)k * n + p], qkr = q[(size_t)k * n + r];
-                    q[(size_t)k * n + p] = cs * qkp - sn * qkr; q[(size_t)k * n + r] = sn * qkp + cs * qkr;
-                }
-            }
-    }
-    d.resize(n);
-    for (int i = 0; i < n; i++) d[i] = a[(size_t)i * n + i];
-}
-
-// Householder tridiagonalisation followed by implicit-shift QL (the textbook dense symmetric eigensolver, ~5 n^3 flops
-// against ~30 n^3 for cyclic Jacobi): used for Krylov spaces beyond 64.  Row-major a (destroyed); eigenvalues d,
-// eigenvectors = columns of q.  Returns false if QL fails to converge in 60 iterations for one eigenvalue.
-bool tridiag_ql(int n, std::vector<double>& a, std::vector<double>& d, std::vector<double>& q) {
-    std::vector<double> e(n, 0.0);
-    d.assign(n, 0.0);
-#define A_(i, j) a[(size_t)(i) * n + (j)]
-    // reduction to tridiagonal form, accumulating the transformation in a
-    for (int i = n - 1; i > 0; i--) {
-        const int l = i - 1;
-        double h = 0.0, scale = 0.0;
-        if (l > 0) {
-            for (int k = 0; k <= l; k++) scale += fabs(A_(i, k));
-            if (scale == 0.0) e[i] = A_(i, l);
-            else {
-                for (int k = 0; k <= l; k++) { A_(i, k) /= scale; h += A_(i, k) * A_(i, k); }
-                double f = A_(i, l);
-                double g = f >= 0.0 ? -sqrt(h) : sqrt(h);
-                e[i] = scale * g; h -= f * g; A_(i, l) = f - g; f = 0.0;
-                for (int j = 0; j <= l; j++) {
-                    A_(j, i) = A_(i, j) / h;
-                    g = 0.0;
-                    for (int k = 0; k <= j; k++) g += A_(j, k) * A_(i, k);
-                    for (int k = j + 1; k <= l; k++) g += A_(k, j) * A_(i, k);
-                    e[j] = g / h; f += e[j] * A_(i, j);
-                }
-                const double hh = f / (h + h);
-                for (int j = 0; j <= l; j++) {
-                    f = A_(i, j); e[j] = g = e[j] - hh * f;
-                    for (int k = 0; k <= j; k++) A_(j, k) -= f * e[k] + g * A_(i, k);
-                }
-            }
-        } else e[i] = A_(i, l);
-        d[i] = h;
-    }
-    d[0] = 0.0; e[0] = 0.0;
-    for (int i = 0; i < n; i++) {
-        const int l = i - 1;
-        if (d[i] != 0.0) {
-            for (int j = 0; j <= l; j++) {
-                double g = 0.0;
-                for (int k = 0; k <= l; k++) g += A_(i, k) * A_(k, j);
-                for (int k = 0; k <= l; k++) A_(k, j) -= g * A_(k, i);
-            }
-        }
-        d[i] = A_(i, i); A_(i, i) = 1.0;
-        for (int j = 0; j <= l; j++) A_(j, i) = A_(i, j) = 0.0;
-    }
-    // implicit QL on (d, e), rotating the columns of a
-    for (int i = 1; i < n; i++) e[i - 1] = e[i];
-    e[n - 1] = 0.0;
-    for (int l = 0; l < n; l++) {
-        int iter = 0, mm;
-        do {
-            for (mm = l; mm < n - 1; mm++) {
-                const double dd = fabs(d[mm]) + fabs(d[mm + 1]);
-                if (fabs(e[mm]) <= 2.3e-16 * dd) break;
-            }
-            if (mm != l) {
-                if (iter++ == 60) return false;
-                double g = (d[l + 1] - d[l]) / (2.0 * e[l]);
-                double r = hypot(g, 1.0);
-                g = d[mm] - d[l] + e[l] / (g + (g >= 0.0 ? fabs(r) : -fabs(r)));
-                double sn = 1.0, cs = 1.0, pp = 0.0;
-                int i;
-                for (i = mm - 1; i >= l; i--) {
-                    double f = sn * e[i];
-                    const double b = cs * e[i];
-                    e[i + 1] = (r = hypot(f, g));
-                    if (r == 0.0) { d[i + 1] -= pp; e[mm] = 0.0; break; }
-                    sn = f / r; cs = g / r; g = d[i + 1] - pp;
-                    r = (d[i] - g) * sn + 2.0 * cs * b;
-                    d[i + 1] = g + (pp = sn * r); g = cs * r - b;
-                    for (int k = 0; k < n; k++) {
-                        f = A_(k, i + 1);
-                        A_(k, i + 1) = sn * A_(k, i) + cs * f;
-                        A_(k, i) = cs * A_(k, i) - sn * f;
-                    }
-                }
-                if (r == 0.0 && i >= l) continue;
-                d[l] -= pp; e[l] = g; e[mm] = 0.0;
-            }
-        } while (mm != l);
-    }
-#undef A_
-    q = a;
-    return true;
-}
-
 }  // namespace
 
 int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const lq_eig_param* p, lq_eig_info* info) {
@@ -211,23 +89,30 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
     e.d_partial = (double2*)alloc(sizeof(double2) * Lt * e.nchunk);
     e.d_H = (double2*)alloc(sizeof(double2) * (size_t)(2 * m + 4) * Lt);
     e.d_scale = (double*)alloc(sizeof(double) * 2 * Lt);
+    const int nT = (m + 1) & ~1;                                   // leading dimension of the projected matrices (even, for the Jacobi pairing)
     double* d_Q = (double*)alloc(sizeof(double) * (size_t)Lt * m * m);
+    double* d_T = (double*)alloc(sizeof(double) * (size_t)Lt * nT * nT);
+    double* d_QT = (double*)alloc(sizeof(double) * (size_t)Lt * nT * nT);
+    double* d_ritz = (double*)alloc(sizeof(double) * (size_t)Lt * (m + n_ev + 2));      // theta [Lt][m], residual estimates [Lt][n_ev], beta [Lt]
+    int* d_sweeps = (int*)alloc(sizeof(int) * Lt);
     double** d_ptr = (double**)alloc(sizeof(double*) * (size_t)(2 * m + 2));
     double2* d_mpart = (double2*)alloc(sizeof(double2) * (size_t)Lt * e.nchunk * (m + 1));
-    ok = ok && w && y0 && y1 && tmp && e.d_partial && e.d_H && e.d_scale && d_Q && d_ptr && d_mpart;
+    ok = ok && w && y0 && y1 && tmp && e.d_partial && e.d_H && e.d_scale && d_Q && d_ptr && d_mpart && d_T && d_QT && d_ritz && d_sweeps;
     if (!ok) { cleanup(); return LQ_ENOMEM; }
     const int grid = grid_sites(e);
-    cudaEvent_t ev0, ev1;
-    cudaEventCreate(&ev0); cudaEventCreate(&ev1);
+    cudaEvent_t ev0, ev1, evA, evB;
+    cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventCreate(&evA); cudaEventCreate(&evB);
     cudaEventRecord(ev0, c->stream);
+    double t_ortho = 0.0, t_ritz = 0.0;
 
     int rc = 0;
 #define EIG_TRY(x) do { rc = (x); if (rc) goto done; } while (0)
 #define EIG_CUDA(x) do { if ((x) != cudaSuccess) { rc = set_err(c, LQ_ECUDA, #x); goto done; } } while (0)
     {
-    std::vector<double> T((size_t)Lt * m * m, 0.0), beta_m(Lt, 0.0), hbuf;
+    std::vector<double> T((size_t)Lt * nT * nT, 0.0), beta_m(Lt, 0.0), hbuf;
     std::vector<double2> hH((size_t)(2 * m + 4) * Lt);
-    std::vector<double> hQ((size_t)Lt * m * m), theta((size_t)Lt * m);
+    std::vector<double> theta((size_t)Lt * m), hres((size_t)Lt * n_ev);
+    double* d_theta = d_ritz; double* d_res = d_ritz + (size_t)Lt * m; double* d_beta = d_res + (size_t)Lt * n_ev;
     int k = 0, restarts = 0; bool converged = false; double worst = 0.0;
     // v_0: pseudo-random, normalised on every slice; zero the padding first
     EIG_CUDA(cudaMemsetAsync(V[0], 0, e.fbytes, c->stream));
@@ -255,6 +140,7 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
         for (int j = k; j < m; j++) {
             EIG_TRY(chebyshev(e, w, V[j], p->cheb_degree, p->cheb_a, p->cheb_b, y0, y1, tmp));
             // two classical Gram-Schmidt passes against v_0 .. v_j; the coefficients are the column j of T
+            cudaEventRecord(evA, c->stream);
             for (int pass = 0; pass < 2; pass++) {
                 double2* H = e.d_H + (size_t)pass * (m + 1) * Lt;
                 const int nv = j + 1;
@@ -267,55 +153,40 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
             EIG_TRY(dot(e, w, w, e.d_H + (size_t)(2 * m + 2) * Lt));
             inv_norm_kernel<<<(Lt + 63) / 64, 64, 0, c->stream>>>(Lt, e.d_H + (size_t)(2 * m + 2) * Lt, e.d_scale, e.d_scale + Lt);
             slice_scale_kernel<<<grid, 128, 0, c->stream>>>(e.sg, V[j + 1], w, e.d_scale); c->launches += 2;
+            cudaEventRecord(evB, c->stream);
             hbuf.resize(Lt);
             EIG_CUDA(cudaMemcpyAsync(hbuf.data(), e.d_scale + Lt, sizeof(double) * Lt, cudaMemcpyDeviceToHost, c->stream));
             EIG_CUDA(cudaStreamSynchronize(c->stream));
+            { float tms = 0; cudaEventElapsedTime(&tms, evA, evB); t_ortho += tms * 1e-3; }
             for (int t = 0; t < Lt; t++) {
-                double* Tt = T.data() + (size_t)t * m * m;
+                double* Tt = T.data() + (size_t)t * nT * nT;
                 for (int i = 0; i <= j; i++) {
                     const double h = hH[(size_t)i * Lt + t].x + hH[(size_t)(m + 1 + i) * Lt + t].x;
-                    if (i >= k || j == k || i == j) { Tt[(size_t)i * m + j] = h; Tt[(size_t)j * m + i] = h; }
+                    if (i >= k || j == k || i == j) { Tt[(size_t)i * nT + j] = h; Tt[(size_t)j * nT + i] = h; }
                 }
-                if (j + 1 < m) { Tt[(size_t)(j + 1) * m + j] = hbuf[t]; Tt[(size_t)j * m + j + 1] = hbuf[t]; }
+                if (j + 1 < m) { Tt[(size_t)(j + 1) * nT + j] = hbuf[t]; Tt[(size_t)j * nT + j + 1] = hbuf[t]; }
                 else beta_m[t] = hbuf[t];
             }
         }
         // Ritz pairs of every slice
-        // (the slices are independent: host threads share them; every slice writes only its own rows)
+        const auto ritz_t0 = std::chrono::steady_clock::now();
         worst = 0.0; converged = true;
-        {
-            std::vector<double> worst_t(Lt, 0.0);
-            std::vector<char> conv_t(Lt, 1);
-            auto ritz = [&](int t) {
-                std::vector<double> a(T.begin() + (size_t)t * m * m, T.begin() + (size_t)(t + 1) * m * m), d, q;
-                if (m <= 64 || !tridiag_ql(m, a, d, q)) {          // QL failure (never seen): fall back to Jacobi on a fresh copy
-                    a.assign(T.begin() + (size_t)t * m * m, T.begin() + (size_t)(t + 1) * m * m);
-                    jacobi(m, a, d, q);
-                }
-                std::vector<int> ord(m);
-                for (int i = 0; i < m; i++) ord[i] = i;
-                std::sort(ord.begin(), ord.end(), [&](int x, int y) { return fabs(d[x]) > fabs(d[y]); });   // T_d(x < -1) is negative for odd d
-                for (int cidx = 0; cidx < m; cidx++) theta[(size_t)t * m + cidx] = d[ord[cidx]];
-                for (int cidx = 0; cidx < keep; cidx++)
-                    for (int i = 0; i < m; i++) hQ[((size_t)t * m + i) * keep + cidx] = q[(size_t)i * m + ord[cidx]];
-                for (int cidx = 0; cidx < n_ev; cidx++) {
-                    const double res = fabs(beta_m[t] * q[(size_t)(m - 1) * m + ord[cidx]]);
-                    const double rel = res / fmax(fabs(d[ord[0]]), 1e-300);
-                    worst_t[t] = fmax(worst_t[t], rel);
-                    if (!(rel <= p->tol)) conv_t[t] = 0;
-                }
-            };
-            const int nthr = (int)std::max(1u, std::min({std::thread::hardware_concurrency(), 16u, (unsigned)Lt}));
-            if (nthr == 1 || m <= 32) { for (int t = 0; t < Lt; t++) ritz(t); }
-            else {
-                std::vector<std::thread> pool;
-                for (int w0 = 0; w0 < nthr; w0++) pool.emplace_back([&, w0]() { for (int t = w0; t < Lt; t += nthr) ritz(t); });
-                for (auto& th : pool) th.join();
+        // all Lt projected eigenproblems in one launch; the kernel leaves the sorted eigenvalues, the residual estimates and the
+        // first `keep` eigenvectors (d_Q, the layout slice_rotate_kernel reads) on the device
+        EIG_CUDA(cudaMemcpyAsync(d_T, T.data(), sizeof(double) * (size_t)Lt * nT * nT, cudaMemcpyHostToDevice, c->stream));
+        EIG_CUDA(cudaMemcpyAsync(d_beta, beta_m.data(), sizeof(double) * Lt, cudaMemcpyHostToDevice, c->stream));
+        ritz_jacobi_kernel<<<Lt, RITZ_THREADS, 0, c->stream>>>(m, keep, n_ev, d_T, d_QT, d_beta, d_theta, d_Q, d_res, d_sweeps); c->launches++;
+        EIG_CUDA(cudaGetLastError());
+        EIG_CUDA(cudaMemcpyAsync(theta.data(), d_theta, sizeof(double) * (size_t)Lt * m, cudaMemcpyDeviceToHost, c->stream));
+        EIG_CUDA(cudaMemcpyAsync(hres.data(), d_res, sizeof(double) * (size_t)Lt * n_ev, cudaMemcpyDeviceToHost, c->stream));
+        EIG_CUDA(cudaStreamSynchronize(c->stream));
+        for (int t = 0; t < Lt; t++)
+            for (int cidx = 0; cidx < n_ev; cidx++) {
+                const double rel = hres[(size_t)t * n_ev + cidx];
+                worst = fmax(worst, rel);
+                if (!(rel <= p->tol)) converged = false;
             }
-            for (int t = 0; t < Lt; t++) { worst = fmax(worst, worst_t[t]); if (!conv_t[t]) converged = false; }
-        }
         // thick restart: V[0..keep) <- V Q[:, 0..keep), V[keep] <- v_m, T <- diag(theta) (the arrow is rebuilt by the sweep)
-        EIG_CUDA(cudaMemcpyAsync(d_Q, hQ.data(), sizeof(double) * (size_t)Lt * m * keep, cudaMemcpyHostToDevice, c->stream));
         {
             std::vector<double*> ptrs(2 * m + 2);
             for (int i = 0; i < m; i++) ptrs[i] = V[i];
@@ -326,8 +197,9 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
             for (int i = 0; i < keep; i++) std::swap(V[i], W[i]);
             std::swap(V[keep], V[m]);
         }
+        t_ritz += std::chrono::duration<double>(std::chrono::steady_clock::now() - ritz_t0).count();
         std::fill(T.begin(), T.end(), 0.0);
-        for (int t = 0; t < Lt; t++) for (int i = 0; i < keep; i++) T[(size_t)t * m * m + (size_t)i * m + i] = theta[(size_t)t * m + i];
+        for (int t = 0; t < Lt; t++) for (int i = 0; i < keep; i++) T[(size_t)t * nT * nT + (size_t)i * nT + i] = theta[(size_t)t * m + i];
         k = keep;
         if (converged) { restarts++; break; }
     }
@@ -354,11 +226,12 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
     float ms = 0; cudaEventElapsedTime(&ms, ev0, ev1);
     info->restarts = restarts; info->converged = converged ? 1 : 0; info->lap_applies = (double)e.lap_applies;
     info->max_ritz_residual = worst; info->max_true_residual = maxres; info->seconds = ms * 1e-3;
+    info->seconds_ritz = t_ritz; info->seconds_ortho = t_ortho;
     if (!converged) rc = LQ_ENOTCONVERGED;
     }
 done:
     cudaStreamSynchronize(c->stream);
-    cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+    cudaEventDestroy(ev0); cudaEventDestroy(ev1); cudaEventDestroy(evA); cudaEventDestroy(evB);
     cleanup();
     return rc;
 #undef EIG_TRY

@@ -386,7 +386,7 @@ def dslash_report(B, device, peak, peak_src, quick=False):
             fma = measure_fma_peak(ctx)
         ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=c["recon"])
         ctx.build_clover(c["kappa"], c["csw"])
-        ns = (1, 2, 4, 8, 12, 16) if cfg_id == 2 else (c["nrhs"],)
+        ns = (1, 2, 4, 8, 12, 16, 32) if cfg_id == 2 else (c["nrhs"],)
         for n in ns:
             for kind in ("A", "B", "hop"):
                 if quick and (kind == "hop" or n in (1, 2)):

@@ -57,7 +57,7 @@
 extern "C" {
 #endif
 
-#define LQ_MAX_RHS 16
+#define LQ_MAX_RHS 32
 
 typedef struct lq_ctx lq_ctx;
 
@@ -126,7 +126,8 @@ int lq_build_clover(lq_ctx* ctx, double kappa, double csw);
 
 /* ---- operator application (rows a3, a4, a5) ----------------------------------------------------- */
 /* out = op(in [, in2]) for nrhs right-hand sides in precision `prec`.
- * nrhs in {1,2,4,8,12,16}.  CANONICAL: complex double (LQ_FP64) or complex float (LQ_FP32) arrays
+ * nrhs in {1,2,4,8,12,16,20,24,28,32}: batches beyond 16 are further link-reuse tiles of the same launch (RHS groups of 4 that
+ * share every link and clover load through L1; SURVEY 8(f) #3 "larger N").  CANONICAL: complex double (LQ_FP64) or complex float (LQ_FP32) arrays
  * psi[rhs][t][z][y][x][4][3] at `loc`, reordered internally (LQ_HALF: canonical arrays are complex
  * float and are quantised to int16+norm on the way in -- the operator then sees what the half-storage
  * solver sees).  NATIVE: device buffers in the native layout (loc must be LQ_DEVICE).
@@ -203,7 +204,7 @@ int lq_solve(lq_ctx* ctx, void* x, const void* b, int nrhs, int loc, int layout,
 
 /* ---- 3-d gauge-covariant Laplacian ------------------------
  * (Lap v)(x) = sum_{i=x,y,z} [ U_i(x) v(x+i) + U_i(x-i)^dag v(x-i) ] - 6 v(x) on every time-slice independently,
- * periodic in space, for nvec colour-vector fields at once (nvec in {1,2,4,8,12,16}); uses the loaded gauge field
+ * periodic in space, for nvec colour-vector fields at once (nvec in {1,2,4,8,12,16,20,24,28,32}); uses the loaded gauge field
  * (fp64 links for LQ_FP64, the fp32 18- or 12-real links for LQ_FP32; LQ_HALF is not supported).
  * lq_laplacian: in/out canonical [vec][t][z][y][x][colour] complex double at `loc`; out must not alias in.
  * lq_laplacian_native: device buffers of lq_cv_native_bytes() bytes in the library's blocked even/odd layout

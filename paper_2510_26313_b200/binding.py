@@ -18,7 +18,7 @@ LQ_ALG_CGNR, LQ_ALG_BICGSTAB = 0, 1
 LQ_FP64, LQ_FP32, LQ_HALF = 0, 1, 2
 LQ_HOST, LQ_DEVICE = 0, 1
 LQ_CANONICAL, LQ_NATIVE = 0, 1
-LQ_MAX_RHS = 16
+LQ_MAX_RHS = 32
 (LQ_OP_HOP, LQ_OP_M, LQ_OP_MDAG, LQ_OP_CLOVER, LQ_OP_CLOVER_INV, LQ_OP_HOP_EO, LQ_OP_HOP_OE, LQ_OP_MHAT, LQ_OP_MHAT_DAG,
  LQ_OP_KERNEL_A, LQ_OP_KERNEL_B, LQ_OP_PROBE_LOADS) = range(12)
 LQ_OK, LQ_EINVAL, LQ_ESTATE, LQ_ENOMEM, LQ_ECUDA, LQ_ENOTCONVERGED, LQ_ESINGULAR = 0, -1, -2, -3, -4, -5, -6

@@ -33,7 +33,7 @@ int ensure_partials(lq_ctx* c, size_t elems) {
     if (!c->red_partials) { c->red_partials_elems = 0; return LQ_ENOMEM; }
     return 0;
 }
-static bool nrhs_ok(int n) { return n == 1 || n == 2 || n == 4 || n == 8 || n == 12 || n == 16; }
+static bool nrhs_ok(int n) { return n == 1 || n == 2 || (n >= 4 && n <= LQ_MAX_RHS && n % 4 == 0); }
 
 extern "C" {
 
@@ -375,7 +375,7 @@ static int apply_native(lq_ctx* c, int op, void* out, const void* in, const void
 
 int lq_apply(lq_ctx* c, int op, void* out, const void* in, const void* in2, int nrhs, int prec, int loc, int layout) {
     if (!c || !out || !in) return set_err(c, LQ_EINVAL, "lq_apply: null argument");
-    if (!nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "nrhs must be one of 1,2,4,8,12,16");
+    if (!nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "nrhs must be 1, 2 or a multiple of 4 up to 32");
     if (prec != LQ_FP64 && prec != LQ_FP32 && prec != LQ_HALF) return set_err(c, LQ_EINVAL, "bad precision");
     if (op < 0 || op > LQ_OP_PROBE_LOADS) return set_err(c, LQ_EINVAL, "unknown operator");
     if (op == LQ_OP_PROBE_LOADS && layout != LQ_NATIVE) return set_err(c, LQ_EINVAL, "LQ_OP_PROBE_LOADS is a native-layout bench probe");
@@ -422,7 +422,7 @@ int lq_apply(lq_ctx* c, int op, void* out, const void* in, const void* in2, int 
 
 int lq_solve(lq_ctx* c, void* x, const void* b, int nrhs, int loc, int layout, const lq_solve_param* param, lq_solve_info* info) {
     if (!c || !x || !b || !param || !info) return set_err(c, LQ_EINVAL, "lq_solve: null argument");
-    if (!nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "nrhs must be one of 1,2,4,8,12,16");
+    if (!nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "nrhs must be 1, 2 or a multiple of 4 up to 32");
     if (!(param->tol > 0) || param->max_outer < 1 || param->max_inner < 1) return set_err(c, LQ_EINVAL, "bad solve parameters");
     cudaSetDevice(c->device);
     if (layout == LQ_NATIVE) {

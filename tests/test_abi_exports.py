@@ -45,7 +45,7 @@ def test_struct_layouts_match_header(tmp_path):
     exe = tmp_path / "layout"
     subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), "-o", str(exe), str(src)], check=True)
     got = dict(l.split() for l in subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.splitlines())
-    assert int(got["LQ_MAX_RHS"]) == binding.LQ_MAX_RHS == 16
+    assert int(got["LQ_MAX_RHS"]) == binding.LQ_MAX_RHS == 32
     for name, (cls, fields) in structs.items():
         assert ctypes.sizeof(cls) == int(got[name]), name
         assert [f for f, _ in cls._fields_] == fields, name

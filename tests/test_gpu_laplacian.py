@@ -20,7 +20,7 @@ def rel(a, b):
 
 
 @pytest.mark.parametrize("dims", [(8, 4, 4, 6), (6, 6, 2, 6), (2, 2, 2, 2), (16, 4, 8, 4)])
-@pytest.mark.parametrize("nvec", [1, 2, 4, 8, 12, 16])
+@pytest.mark.parametrize("nvec", [1, 2, 4, 8, 12, 16, 32])
 def test_laplacian_matches_oracle(dims, nvec):
     U = inputs.make_links(dims, 61, 0.3)
     v = fields(dims, nvec, 62)

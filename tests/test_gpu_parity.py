@@ -54,7 +54,7 @@ def test_config0_all_operators_fp64():
     ctx.close()
 
 
-@pytest.mark.parametrize("nrhs", [1, 2, 4, 8, 12, 16])
+@pytest.mark.parametrize("nrhs", [1, 2, 4, 8, 12, 16, 24, 32])
 @pytest.mark.parametrize("prec", [B.LQ_FP64, B.LQ_FP32, B.LQ_HALF])
 def test_multi_rhs_ragged_lattice(nrhs, prec):
     """Unequal extents (Lxh = 3: x-lines do not fill a warp; several tiles and a ragged tail), every supported N."""

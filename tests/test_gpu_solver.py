@@ -126,7 +126,7 @@ def test_solve_is_bitwise_reproducible(inner):
     ctx.close()
 
 
-@pytest.mark.parametrize("nrhs", [1, 2, 12, 16])
+@pytest.mark.parametrize("nrhs", [1, 2, 12, 16, 20, 32])
 def test_every_batch_width_solves(nrhs):
     """RHS group widths 1, 2 and 4 and 1, 3 and 4 groups per site block through the fused CG iteration (fp32 inner)."""
     dims = (6, 6, 4, 8)          # Vh = 432: 13.5 site blocks, the last one half padding

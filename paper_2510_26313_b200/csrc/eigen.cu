@@ -45,17 +45,15 @@ __global__ void inv_norm_kernel(int Lt, const double2* nn, double* inv, double* 
 // w <- B w0 = T_d(L) w0, L = (2A - (a+b))/(b-a), A = -Laplacian; y0, y1, tmp are scratch fields
 int chebyshev(Eig& e, double* out, const double* v, int degree, double a, double b, double* y0, double* y1, double* tmp) {
     const double c1 = -2.0 / (b - a), c0 = -(b + a) / (b - a);
-    const int grid = grid_sites(e);
-    LQ_TRY(laplacian_native(e.c, tmp, v, 1, LQ_FP64)); e.lap_applies++;
-    // y1 = L v
-    cv_axpbypcz_kernel<<<grid, 128, 0, e.c->stream>>>(e.sg, y1, c1, tmp, c0, v, 0.0); e.c->launches++;
+    (void)tmp;
+    // y1 = L v = c1 Lap v + c0 v  (A = -Lap): the recurrence rides in the Laplacian kernel's epilogue
+    LQ_TRY(laplacian_native_axpby(e.c, y1, v, 1, LQ_FP64, c1, c0, 0.0, nullptr)); e.lap_applies++;
     if (degree == 1) { LQ_CUDA(e.c, cudaMemcpyAsync(out, y1, e.fbytes, cudaMemcpyDeviceToDevice, e.c->stream)); return 0; }
     LQ_CUDA(e.c, cudaMemcpyAsync(y0, v, e.fbytes, cudaMemcpyDeviceToDevice, e.c->stream));
     double *prev = y0, *cur = y1;
     for (int n = 1; n < degree; n++) {
-        LQ_TRY(laplacian_native(e.c, tmp, cur, 1, LQ_FP64)); e.lap_applies++;
         // prev <- 2 L cur - prev
-        cv_axpbypcz_kernel<<<grid, 128, 0, e.c->stream>>>(e.sg, prev, 2.0 * c1, tmp, 2.0 * c0, cur, -1.0); e.c->launches++;
+        LQ_TRY(laplacian_native_axpby(e.c, prev, cur, 1, LQ_FP64, 2.0 * c1, 2.0 * c0, -1.0, prev)); e.lap_applies++;
         std::swap(prev, cur);
     }
     LQ_CUDA(e.c, cudaMemcpyAsync(out, cur, e.fbytes, cudaMemcpyDeviceToDevice, e.c->stream));
@@ -141,13 +139,20 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
             EIG_TRY(chebyshev(e, w, V[j], p->cheb_degree, p->cheb_a, p->cheb_b, y0, y1, tmp));
             // two classical Gram-Schmidt passes against v_0 .. v_j; the coefficients are the column j of T
             cudaEventRecord(evA, c->stream);
+            // pass 0 is LOCAL: against v_{j-1}, v_j only (the three-term recurrence carries all of the weight there), except on the
+            // first step after a restart, where the arrow couples w to every kept Ritz vector; pass 1 is the full reorthogonalisation
+            // against v_0 .. v_j.  After pass 0 the components left along the older vectors are rounding-level, so one full classical
+            // Gram-Schmidt pass restores orthogonality to working precision at half the basis traffic of two full passes.
             for (int pass = 0; pass < 2; pass++) {
-                double2* H = e.d_H + (size_t)pass * (m + 1) * Lt;
-                const int nv = j + 1;
-                slice_multidot_kernel<<<dim3(Lt * e.nchunk, (nv + 7) / 8), 256, 0, c->stream>>>(e.sg, e.nchunk, nv, d_ptr, w, d_mpart);
+                const int first = (pass == 0 && j > k) ? j - 1 : 0;
+                const int nv = j + 1 - first;
+                double2* H = e.d_H + (size_t)pass * (m + 1) * Lt + (size_t)first * Lt;
+                double2* hHp = hH.data() + (size_t)pass * (m + 1) * Lt;
+                for (size_t q = 0; q < (size_t)first * Lt; q++) hHp[q] = make_double2(0.0, 0.0);
+                slice_multidot_kernel<<<dim3(Lt * e.nchunk, (nv + 7) / 8), 256, 0, c->stream>>>(e.sg, e.nchunk, nv, d_ptr + first, w, d_mpart);
                 slice_multidot_final_kernel<<<(Lt * nv + 127) / 128, 128, 0, c->stream>>>(Lt, e.nchunk, nv, d_mpart, H);
-                EIG_CUDA(cudaMemcpyAsync(hH.data() + (size_t)pass * (m + 1) * Lt, H, sizeof(double2) * (size_t)nv * Lt, cudaMemcpyDeviceToHost, c->stream));
-                slice_multiaxpy_kernel<<<grid, 128, 0, c->stream>>>(e.sg, nv, w, d_ptr, H);
+                EIG_CUDA(cudaMemcpyAsync(hHp + (size_t)first * Lt, H, sizeof(double2) * (size_t)nv * Lt, cudaMemcpyDeviceToHost, c->stream));
+                slice_multiaxpy_kernel<<<grid, 128, 0, c->stream>>>(e.sg, nv, w, d_ptr + first, H);
                 c->launches += 3;
             }
             EIG_TRY(dot(e, w, w, e.d_H + (size_t)(2 * m + 2) * Lt));
@@ -175,7 +180,7 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
         // first `keep` eigenvectors (d_Q, the layout slice_rotate_kernel reads) on the device
         EIG_CUDA(cudaMemcpyAsync(d_T, T.data(), sizeof(double) * (size_t)Lt * nT * nT, cudaMemcpyHostToDevice, c->stream));
         EIG_CUDA(cudaMemcpyAsync(d_beta, beta_m.data(), sizeof(double) * Lt, cudaMemcpyHostToDevice, c->stream));
-        ritz_jacobi_kernel<<<Lt, RITZ_THREADS, 0, c->stream>>>(m, keep, n_ev, d_T, d_QT, d_beta, d_theta, d_Q, d_res, d_sweeps); c->launches++;
+        ritz_jacobi_kernel<<<Lt * RITZ_CLUSTER, RITZ_THREADS, 0, c->stream>>>(m, keep, n_ev, d_T, d_QT, d_beta, d_theta, d_Q, d_res, d_sweeps); c->launches++;
         EIG_CUDA(cudaGetLastError());
         EIG_CUDA(cudaMemcpyAsync(theta.data(), d_theta, sizeof(double) * (size_t)Lt * m, cudaMemcpyDeviceToHost, c->stream));
         EIG_CUDA(cudaMemcpyAsync(hres.data(), d_res, sizeof(double) * (size_t)Lt * n_ev, cudaMemcpyDeviceToHost, c->stream));

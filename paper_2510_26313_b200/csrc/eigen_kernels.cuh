@@ -3,6 +3,7 @@
 // with N = 1 (common layout of laplace.cu): element (parity, cb, j) at parity*pbe + ((cb/32)*6 + j)*32 + cb%32, fp64.
 // Every kernel takes per-slice coefficients: the Lt time-slices are independent eigenproblems advancing in lockstep.
 #pragma once
+#include <cooperative_groups.h>
 #include "common.cuh"
 
 struct SliceGeom { int Vh, S3h, Lt; size_t pbe; FastDiv dS3h; };   // S3h = sites of one time-slice per parity
@@ -187,31 +188,39 @@ __global__ void slice_multiaxpy_kernel(SliceGeom g, int nv, double* __restrict__
 // rotations from the current 2x2 diagonal blocks; the matrix then splits into (n/2)^2 independent 2x2 blocks B(P,Q) that become
 // R_P^T B R_Q in place (each element belongs to exactly one block), and rows p, q of Q^T are rotated.  n - 1 steps = one sweep;
 // sweeps repeat until the off-diagonal Frobenius norm is below 1e-14 of the matrix norm.  A and Q^T live in global memory (they
-// stay in L2: 2 x 8 n^2 bytes per slice).  Afterwards the eigenvalues are ranked by |theta| descending (the Chebyshev map sends
+// stay in L2: 2 x 8 n^2 bytes per slice).  A slice is worked on by a CLUSTER of RITZ_CLUSTER thread blocks (one CTA alone is bound by
+// its SM's L1 bandwidth: 0.13 s for m = 288): every CTA derives the same rotations, takes every RITZ_CLUSTER-th chunk of the block
+// updates and meets the others at a cluster barrier (which also invalidates L1) once per step.  Afterwards the eigenvalues are ranked by |theta| descending (the Chebyshev map sends
 // the wanted end of the spectrum to the largest |T_d|) and the first `keep` eigenvectors, the Ritz residual estimates
 // |beta_m q_{m-1,i}| / |theta_0| and the sorted eigenvalues are written in the layouts the restart needs.
 constexpr int RITZ_THREADS = 1024;
 constexpr int RITZ_MAXN = 512;
+constexpr int RITZ_CLUSTER = 4;
 
-__global__ void __launch_bounds__(RITZ_THREADS) ritz_jacobi_kernel(int m, int keep, int n_ev, double* __restrict__ Aall /*[Lt][n][n], n = m rounded up to even*/,
+__global__ void __cluster_dims__(RITZ_CLUSTER, 1, 1) __launch_bounds__(RITZ_THREADS) ritz_jacobi_kernel(int m, int keep, int n_ev, double* __restrict__ Aall /*[Lt][n][n], n = m rounded up to even*/,
                                                                    double* __restrict__ QTall /*[Lt][n][n]*/, const double* __restrict__ beta /*[Lt]*/,
                                                                    double* __restrict__ theta /*[Lt][m]*/, double* __restrict__ Qk /*[Lt][m][keep]*/,
                                                                    double* __restrict__ res /*[Lt][n_ev]*/, int* __restrict__ sweeps_out /*[Lt]*/) {
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (int)cluster.block_rank();
     const int n = (m + 1) & ~1, half = n / 2;
-    const int t = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
+    const int t = blockIdx.x / RITZ_CLUSTER, tid = threadIdx.x, nt = blockDim.x;
+    const int gtid = rank * nt + tid, gnt = RITZ_CLUSTER * nt;      // thread index / count within the cluster
     double* A = Aall + (size_t)t * n * n;
     double* QT = QTall + (size_t)t * n * n;
     __shared__ double s_c[RITZ_MAXN / 2], s_s[RITZ_MAXN / 2];
     __shared__ int s_p[RITZ_MAXN / 2], s_q[RITZ_MAXN / 2];
     __shared__ double s_red[RITZ_THREADS / 32];
     __shared__ double s_off, s_tot;
-    for (int i = tid; i < n * n; i += nt) QT[i] = (i / n == i % n) ? 1.0 : 0.0;
-    __syncthreads();
+    for (int i = gtid; i < n * n; i += gnt) QT[i] = (i / n == i % n) ? 1.0 : 0.0;
+    __threadfence();
+    cluster.sync();
     int sweep = 0;
     for (; sweep < 40; sweep++) {
         // convergence: off-diagonal norm against the whole norm (fixed-order block reduction)
         double off = 0.0, tot = 0.0;
-        for (int i = tid; i < n * n; i += nt) { const double v = A[i]; tot += v * v; if (i / n != i % n) off += v * v; }
+        for (int i = tid; i < n * n; i += nt) { const double v = __ldcg(A + i); tot += v * v; if (i / n != i % n) off += v * v; }
         for (int pass = 0; pass < 2; pass++) {
             double v = pass == 0 ? off : tot;
             for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -227,7 +236,7 @@ __global__ void __launch_bounds__(RITZ_THREADS) ritz_jacobi_kernel(int m, int ke
                 int p, q;
                 if (tid == 0) { p = n - 1; q = step; }
                 else { p = (step + tid) % (n - 1); q = (step - tid + (n - 1)) % (n - 1); }
-                const double apq = A[(size_t)p * n + q], app = A[(size_t)p * n + p], aqq = A[(size_t)q * n + q];
+                const double apq = __ldcg(A + (size_t)p * n + q), app = __ldcg(A + (size_t)p * n + p), aqq = __ldcg(A + (size_t)q * n + q);
                 double cs = 1.0, sn = 0.0;
                 if (fabs(apq) > 1e-300) {
                     const double th = (aqq - app) / (2.0 * apq);
@@ -238,44 +247,46 @@ __global__ void __launch_bounds__(RITZ_THREADS) ritz_jacobi_kernel(int m, int ke
             }
             __syncthreads();
             // A <- J^T A J by independent 2x2 blocks; Q^T rows
-            for (int b = tid; b < half * half; b += nt) {
+            for (int b = gtid; b < half * half; b += gnt) {
                 const int k1 = b / half, k2 = b - k1 * half;
                 const int p1 = s_p[k1], q1 = s_q[k1], p2 = s_p[k2], q2 = s_q[k2];
                 const double c1 = s_c[k1], s1 = s_s[k1], c2 = s_c[k2], s2 = s_s[k2];
-                const double bpp = A[(size_t)p1 * n + p2], bpq = A[(size_t)p1 * n + q2], bqp = A[(size_t)q1 * n + p2], bqq = A[(size_t)q1 * n + q2];
+                const double bpp = __ldcg(A + (size_t)p1 * n + p2), bpq = __ldcg(A + (size_t)p1 * n + q2), bqp = __ldcg(A + (size_t)q1 * n + p2), bqq = __ldcg(A + (size_t)q1 * n + q2);
                 const double tpp = c2 * bpp - s2 * bpq, tpq = s2 * bpp + c2 * bpq, tqp = c2 * bqp - s2 * bqq, tqq = s2 * bqp + c2 * bqq;
                 double opp = c1 * tpp - s1 * tqp, opq = c1 * tpq - s1 * tqq, oqp = s1 * tpp + c1 * tqp, oqq = s1 * tpq + c1 * tqq;
                 if (k1 == k2) { opq = 0.0; oqp = 0.0; }
                 A[(size_t)p1 * n + p2] = opp; A[(size_t)p1 * n + q2] = opq; A[(size_t)q1 * n + p2] = oqp; A[(size_t)q1 * n + q2] = oqq;
             }
-            for (int b = tid; b < half * n; b += nt) {
+            for (int b = gtid; b < half * n; b += gnt) {
                 const int k = b / n, j = b - k * n;
                 const int p = s_p[k], q = s_q[k];
                 const double cs = s_c[k], sn = s_s[k];
-                const double vp = QT[(size_t)p * n + j], vq = QT[(size_t)q * n + j];
+                const double vp = __ldcg(QT + (size_t)p * n + j), vq = __ldcg(QT + (size_t)q * n + j);
                 QT[(size_t)p * n + j] = cs * vp - sn * vq; QT[(size_t)q * n + j] = sn * vp + cs * vq;
             }
-            __syncthreads();
+            __threadfence();
+            cluster.sync();          // the other CTAs' updates are visible (and the barrier drops this SM's stale L1 lines)
         }
     }
+    if (rank != 0) return;           // ranking and output by the first CTA of the cluster
     if (tid == 0) sweeps_out[t] = sweep;
     // rank by |theta| descending (ties by index): rank_i = number of eigenvalues that come before i
     __shared__ int s_ord[RITZ_MAXN];
     for (int i = tid; i < RITZ_MAXN; i += nt) s_ord[i] = 0;       // a NaN in the matrix must not leave an index unset
     __syncthreads();
     for (int i = tid; i < m; i += nt) {
-        const double di = fabs(A[(size_t)i * n + i]);
+        const double di = fabs(__ldcg(A + (size_t)i * n + i));
         int r = 0;
-        for (int j = 0; j < m; j++) { const double dj = fabs(A[(size_t)j * n + j]); if (dj > di || (dj == di && j < i)) r++; }
+        for (int j = 0; j < m; j++) { const double dj = fabs(__ldcg(A + (size_t)j * n + j)); if (dj > di || (dj == di && j < i)) r++; }
         s_ord[r] = i;
-        theta[(size_t)t * m + r] = A[(size_t)i * n + i];
+        theta[(size_t)t * m + r] = __ldcg(A + (size_t)i * n + i);
     }
     __syncthreads();
-    const double th0 = fmax(fabs(A[(size_t)s_ord[0] * n + s_ord[0]]), 1e-300);
+    const double th0 = fmax(fabs(__ldcg(A + (size_t)s_ord[0] * n + s_ord[0])), 1e-300);
     for (int b = tid; b < m * keep; b += nt) {
         const int i = b / keep, cidx = b - i * keep;
-        Qk[((size_t)t * m + i) * keep + cidx] = QT[(size_t)s_ord[cidx] * n + i];
+        Qk[((size_t)t * m + i) * keep + cidx] = __ldcg(QT + (size_t)s_ord[cidx] * n + i);
     }
-    for (int cidx = tid; cidx < n_ev; cidx += nt) res[(size_t)t * n_ev + cidx] = fabs(beta[t] * QT[(size_t)s_ord[cidx] * n + (m - 1)]) / th0;
+    for (int cidx = tid; cidx < n_ev; cidx += nt) res[(size_t)t * n_ev + cidx] = fabs(beta[t] * __ldcg(QT + (size_t)s_ord[cidx] * n + (m - 1))) / th0;
 }
 

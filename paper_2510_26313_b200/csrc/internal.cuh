@@ -74,6 +74,8 @@ int solve_native(lq_ctx* c, void* x_full64, const void* b_full64, int nrhs, cons
 
 // laplace.cu : batched 3-d gauge-covariant Laplacian on native colour-vector fields
 int laplacian_native(lq_ctx* c, void* out, const void* in, int nvec, int prec);
+// out = ca * Lap(in) + cb * in + cc * y, y = nullptr or any field (may be `out`); out must not alias in
+int laplacian_native_axpby(lq_ctx* c, void* out, const void* in, int nvec, int prec, double ca, double cb, double cc, const void* y);
 size_t cv_native_bytes(const lq_ctx* c, int nvec, int prec);
 int cv_pack(lq_ctx* c, void* native, const double* dev_canon, int nvec, int prec);
 int cv_unpack(lq_ctx* c, double* dev_canon, const void* native, int nvec, int prec);

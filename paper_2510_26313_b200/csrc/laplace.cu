@@ -20,8 +20,11 @@ template <> struct StoreOf<float> { using S = F32; };
 template <> struct StoreOf<double> { using S = F64; };
 
 template <typename T, int RPT, int R, int RECON>
-__global__ void __launch_bounds__(128) laplace_kernel(Geom g, int G, FastDiv d2G, int pfd, T* __restrict__ out_full, const T* __restrict__ in_full,
-                                                      size_t pb_elems, const T* __restrict__ gauge) {
+// Fused epilogue (the three-term Chebyshev recurrence of the Lanczos filter without a separate vector kernel and without
+// storing Lap v): out = ca * (Lap in) + cb * in + cc * y, y optional (may be `out` itself: every thread reads its own site of y
+// before it writes it); ca = 1, cb = cc = 0 is the plain operator.  out must not alias in.
+__global__ void __launch_bounds__(128) laplace_kernel(Geom g, int G, FastDiv d2G, int pfd, T* out_full, const T* __restrict__ in_full,
+                                                      size_t pb_elems, const T* __restrict__ gauge, T ca, T cb, T cc, const T* y_full) {
     using S = typename StoreOf<T>::S;
     constexpr int TPG = R / RPT, UT = SB * TPG, US = 6 * SB * R, PL = SB * R;
     const int tid = blockIdx.x * 128 + threadIdx.x;
@@ -67,12 +70,12 @@ __global__ void __launch_bounds__(128) laplace_kernel(Geom g, int G, FastDiv d2G
         if (grp == 1 % G) { const char* l = (const char*)(gauge + ((size_t)((1 - parity) * g.NB + pb) * 4) * (RECON * SB)); LQ_PF_LINES(l, GL) }
 #undef LQ_PF_LINES
     }
-    T acc[6][RPT];
+    T acc[6][RPT], vown[6][RPT];
 #pragma unroll
     for (int j = 0; j < 6; j++) {
-        load_comp<S, RPT>(in_own + own + j * PL, acc[j]);
+        load_comp<S, RPT>(in_own + own + j * PL, vown[j]);
 #pragma unroll
-        for (int k = 0; k < RPT; k++) acc[j][k] *= T(-6);
+        for (int k = 0; k < RPT; k++) acc[j][k] = vown[j][k] * T(-6);
     }
 #define LQ_LAP(D) { const int nb_ = neighbour<D>(sc); constexpr bool FWD_ = ((D) & 1) == 0; \
         const T* p_ = inb + (size_t)(nb_ >> 5) * bstride + (nb_ & 31) * R; \
@@ -87,12 +90,31 @@ __global__ void __launch_bounds__(128) laplace_kernel(Geom g, int G, FastDiv d2G
                 acc[2 * r + 1][k] = fm(ur_, v_[2 * c + 1][k], acc[2 * r + 1][k]); acc[2 * r + 1][k] = fm(ui_, v_[2 * c][k], acc[2 * r + 1][k]); } } }
     LQ_LAP(0) LQ_LAP(1) LQ_LAP(2) LQ_LAP(3) LQ_LAP(4) LQ_LAP(5)
 #undef LQ_LAP
+    if (ca != T(1) || cb != T(0) || y_full != nullptr) {
+        const T* y = y_full != nullptr ? y_full + (size_t)parity * pb_elems : nullptr;
+#pragma unroll
+        for (int j = 0; j < 6; j++) {
+            T yv[RPT];
+            if (y != nullptr) {
+                // plain loads: y may be the buffer this thread is about to overwrite
+                if constexpr (RPT == 1) yv[0] = y[own + j * PL];
+                else {
+#pragma unroll
+                    for (int k = 0; k < RPT; k++) yv[k] = y[own + j * PL + k];
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < RPT; k++) acc[j][k] = ca * acc[j][k] + cb * vown[j][k] + (y != nullptr ? cc * yv[k] : T(0));
+        }
+    }
 #pragma unroll
     for (int j = 0; j < 6; j++) store_comp<S, RPT>(out + own + j * PL, acc[j]);
 }
 
 template <typename T, int RECON>
-static int launch_laplace(lq_ctx* c, int nvec, T* out, const T* in, const T* gauge, int prec) {
+static int launch_laplace(lq_ctx* c, int nvec, T* out, const T* in, const T* gauge, int prec, double a, double b, double cc_, const void* yv) {
+    const T ca = (T)a, cb = (T)b, cc = (T)cc_;
+    const T* y = (const T*)yv;
     const int R = group_width(nvec), G = nvec / R;
     constexpr int MAXRPT = sizeof(T) == 8 ? 2 : 4;
     const int rpt = R < MAXRPT ? R : MAXRPT;
@@ -101,20 +123,24 @@ static int launch_laplace(lq_ctx* c, int nvec, T* out, const T* in, const T* gau
     const FastDiv d2G = make_fastdiv(2 * G);
     const size_t pbe = cv_parity_bytes(c->g, nvec, prec) / sizeof(T);
     const int pfd = c->dslash_pfd;
-    if (R == 4 && rpt == 4) { if constexpr (MAXRPT == 4) laplace_kernel<T, 4, 4, RECON><<<grid, 128, 0, c->stream>>>(c->g, G, d2G, pfd, out, in, pbe, gauge); }
-    else if (R == 4) laplace_kernel<T, 2, 4, RECON><<<grid, 128, 0, c->stream>>>(c->g, G, d2G, pfd, out, in, pbe, gauge);
-    else if (R == 2) laplace_kernel<T, 2, 2, RECON><<<grid, 128, 0, c->stream>>>(c->g, G, d2G, pfd, out, in, pbe, gauge);
-    else laplace_kernel<T, 1, 1, RECON><<<grid, 128, 0, c->stream>>>(c->g, G, d2G, pfd, out, in, pbe, gauge);
+    if (R == 4 && rpt == 4) { if constexpr (MAXRPT == 4) laplace_kernel<T, 4, 4, RECON><<<grid, 128, 0, c->stream>>>(c->g, G, d2G, pfd, out, in, pbe, gauge, ca, cb, cc, y); }
+    else if (R == 4) laplace_kernel<T, 2, 4, RECON><<<grid, 128, 0, c->stream>>>(c->g, G, d2G, pfd, out, in, pbe, gauge, ca, cb, cc, y);
+    else if (R == 2) laplace_kernel<T, 2, 2, RECON><<<grid, 128, 0, c->stream>>>(c->g, G, d2G, pfd, out, in, pbe, gauge, ca, cb, cc, y);
+    else laplace_kernel<T, 1, 1, RECON><<<grid, 128, 0, c->stream>>>(c->g, G, d2G, pfd, out, in, pbe, gauge, ca, cb, cc, y);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
 }
 
 // out, in: native full colour-vector fields (even block then odd block)
+// out = ca * Lap(in) + cb * in + cc * y  (y may be nullptr or `out`)
+int laplacian_native_axpby(lq_ctx* c, void* out, const void* in, int nvec, int prec, double ca, double cb, double cc, const void* y) {
+    if (prec == LQ_FP64) return launch_laplace<double, 18>(c, nvec, (double*)out, (const double*)in, c->gauge64, prec, ca, cb, cc, y);
+    if (c->recon32 == 12) return launch_laplace<float, 12>(c, nvec, (float*)out, (const float*)in, c->gauge32, prec, ca, cb, cc, y);
+    return launch_laplace<float, 18>(c, nvec, (float*)out, (const float*)in, c->gauge32, prec, ca, cb, cc, y);
+}
 int laplacian_native(lq_ctx* c, void* out, const void* in, int nvec, int prec) {
-    if (prec == LQ_FP64) return launch_laplace<double, 18>(c, nvec, (double*)out, (const double*)in, c->gauge64, prec);
-    if (c->recon32 == 12) return launch_laplace<float, 12>(c, nvec, (float*)out, (const float*)in, c->gauge32, prec);
-    return launch_laplace<float, 18>(c, nvec, (float*)out, (const float*)in, c->gauge32, prec);
+    return laplacian_native_axpby(c, out, in, nvec, prec, 1.0, 0.0, 0.0, nullptr);
 }
 size_t cv_native_bytes(const lq_ctx* c, int nvec, int prec) { return 2 * cv_parity_bytes(c->g, nvec, prec); }
 

@@ -606,7 +606,8 @@ def main():
     t_dev, t_e2e = max_over_ranks([t_dev, t_e2e], device="cuda")
     h2d, d2h = b_host.numel() * 16, x_host.numel() * 16
     del x_host
-    variant = None
+    inner = wl["inner"]
+    variant, variant_hl = None, None
     if not args.no_extras and world == 1 and args.algorithm == "cg":
         # solver variant, same sources, device resident: batched BiCGStab instead of CGNR (not the headline metric)
         kb = solve_kwargs(B, wl, c, "bicgstab", use_graph=not args.no_graph)
@@ -617,6 +618,15 @@ def main():
         variant = {"algorithm": "batched BiCGStab on Mhat, complex per-RHS scalars, same defect correction", "seconds_per_rhs": ib["seconds"] / nrhs,
                    "ms_per_step": ib["seconds"] * 1e3, "inner_iters": ib["inner_iters"], "outer_cycles": ib["outer_cycles"],
                    "dslash_applies_per_step": ib["dslash_applies"], "true_rel_residual_max": max(ib["true_rel_residual"]), "converged": ib["converged"]}
+        # solver variant: int16 fixed-point links in the half-storage kernels (reading #13), CG as in the headline step
+        if inner == "half":
+            ctx.set_half_links(True)
+            ctx.solve(nb, x_out=nx, native=True, nrhs=nrhs, **kw)
+            _, ih = ctx.solve(nb, x_out=nx, native=True, nrhs=nrhs, **kw)
+            ctx.set_half_links(False)
+            variant_hl = {"variant": "int16 links (36 instead of 72 bytes per link) in the int16+norm kernels", "seconds_per_rhs": ih["seconds"] / nrhs,
+                          "ms_per_step": ih["seconds"] * 1e3, "inner_iters": ih["inner_iters"], "outer_cycles": ih["outer_cycles"],
+                          "true_rel_residual_max": max(ih["true_rel_residual"]), "converged": ih["converged"]}
         del nb, nx
     del b_host
     torch.cuda.empty_cache()
@@ -640,6 +650,8 @@ def main():
         extras["cpu_dslash_baseline"] = cpu_dslash_baseline()
         if variant is not None:
             extras["solver_variant_bicgstab"] = variant
+        if variant_hl is not None:
+            extras["solver_variant_int16_links"] = variant_hl
         extras["laph_eigensolve"] = time_eigensolve(B, local)
         extras["projection"] = time_projection(B, local, peak)
     t_step = t_dev / args.steps

@@ -119,6 +119,10 @@ int lq_load_gauge(lq_ctx* ctx, const void* links, int in_prec, int loc, int reco
  * third row conj(a x b)) of 1 + eps*G, G_ij ~ CN(0,1) from the counter-based generator documented
  * in paper_2510_26313_b200/inputs.py (same stream / index convention). */
 int lq_fill_gauge_random(lq_ctx* ctx, uint64_t seed, double eps, int recon, int t_bc);
+/* Solver variant (SURVEY 8(f) #3, 8(c.2) reading #13; PAPER.md L116 mixed precision): with enable != 0 the LQ_HALF stencil kernels read
+ * the links as int16 fixed point (q = rint(32767 u), always 18 reals: 36 instead of 72 bytes per link); the fp64 / fp32 kernels and the
+ * fp64 defect correction are unaffected, so lq_solve still converges to the full-precision solution.  Needs a loaded gauge field. */
+int lq_set_half_links(lq_ctx* ctx, int enable);
 /* Computes A and A^{-1} (two 6x6 Hermitian blocks per site, both parities) on the device in fp64
  * from the 4-leaf field strength, keeps fp64 and fp32 copies.  LQ_ESINGULAR if a block is not
  * positive definite. */

@@ -26,7 +26,7 @@ PREC = {"fp64": LQ_FP64, "fp32": LQ_FP32, "half": LQ_HALF}
 
 EXPORTS = ["lq_create", "lq_destroy", "lq_last_error", "lq_set_allocator", "lq_load_gauge", "lq_fill_gauge_random",
            "lq_build_clover", "lq_apply", "lq_native_bytes", "lq_pack", "lq_unpack", "lq_fill_spinor_random", "lq_solve",
-           "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites", "lq_native_index", "lq_fma_peak", "lq_mem_peak",
+           "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites", "lq_native_index", "lq_fma_peak", "lq_mem_peak", "lq_set_half_links",
            "lq_laplacian", "lq_laplacian_native", "lq_cv_native_bytes", "lq_cv_fill_random", "lq_laph_eigensolve", "lq_project"]
 
 
@@ -82,6 +82,7 @@ def load_library():
     lib.lq_load_gauge.argtypes = [vp, vp, ci, ci, ci, ci]
     lib.lq_fill_gauge_random.argtypes = [vp, u64, cd, ci, ci]
     lib.lq_build_clover.argtypes = [vp, cd, cd]
+    lib.lq_set_half_links.argtypes = [vp, ci]
     lib.lq_apply.argtypes = [vp, ci, vp, vp, vp, ci, ci, ci, ci]
     lib.lq_native_bytes.argtypes = [vp, ci, ci, ci]; lib.lq_native_bytes.restype = ctypes.c_size_t
     lib.lq_pack.argtypes = [vp, vp, vp, ci, ci, ci]
@@ -195,6 +196,10 @@ class Context:
 
     def fill_gauge_random(self, seed: int, eps: float, recon: int = 18, t_bc: int = -1):
         self._check(self.lib.lq_fill_gauge_random(self.h, seed, eps, recon, t_bc))
+
+    def set_half_links(self, enable: bool = True):
+        """int16 fixed-point links in the LQ_HALF stencil kernels (solver variant, SURVEY 8(f) #3)."""
+        self._check(self.lib.lq_set_half_links(self.h, int(enable)))
 
     def build_clover(self, kappa: float, csw: float):
         self._check(self.lib.lq_build_clover(self.h, kappa, csw))

@@ -49,7 +49,7 @@ int lq_create(lq_ctx** out, const int dims[4], int device, void* cuda_stream) {
     c->g.Lxh = dims[0] / 2; c->g.V = V; c->g.Vh = (int)(V / 2); c->g.NB = (c->g.Vh + SB - 1) / SB;
     c->g.dLxh = make_fastdiv(c->g.Lxh); c->g.dLy = make_fastdiv(dims[1]); c->g.dLz = make_fastdiv(dims[2]);
     c->device = device; c->stream = (cudaStream_t)cuda_stream; c->t_bc = -1;
-    c->gauge64 = nullptr; c->gauge32 = nullptr; c->recon32 = 18;
+    c->gauge64 = nullptr; c->gauge32 = nullptr; c->recon32 = 18; c->gauge16 = nullptr; c->half_links = false;
     c->clov64 = c->clovinv64 = nullptr; c->clov32 = c->clovinv32 = nullptr;
     c->kappa = c->csw = 0; c->has_gauge = c->has_clover = false;
     c->alloc_fn = nullptr; c->free_fn = nullptr; c->alloc_user = nullptr;
@@ -119,6 +119,7 @@ int lq_load_gauge(lq_ctx* c, const void* links, int in_prec, int loc, int recon,
     }
     int rc = gauge_ingest(c, dev, in_prec);
     if (rc == 0) rc = gauge_make_fp32(c, recon);
+    if (rc == 0 && c->half_links) rc = gauge_make_int16(c);
     if (rc == 0 && cudaStreamSynchronize(c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "gauge ingest failed");
     if (staging) dev_free(c, staging);
     if (rc) return rc;
@@ -133,8 +134,21 @@ int lq_fill_gauge_random(lq_ctx* c, uint64_t seed, double eps, int recon, int t_
     LQ_TRY(ensure_gauge_storage(c, recon));
     LQ_TRY(fill_gauge(c, seed, eps));
     LQ_TRY(gauge_make_fp32(c, recon));
+    if (c->half_links) LQ_TRY(gauge_make_int16(c));
     LQ_CUDA(c, cudaStreamSynchronize(c->stream));
     c->t_bc = t_bc; c->has_gauge = true; c->has_clover = false;
+    return 0;
+}
+
+int lq_set_half_links(lq_ctx* c, int enable) {
+    if (!c) return LQ_EINVAL;
+    cudaSetDevice(c->device);
+    if (enable) {
+        if (!c->has_gauge) return set_err(c, LQ_ESTATE, "load the gauge field before lq_set_half_links");
+        LQ_TRY(gauge_make_int16(c));
+        LQ_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+    c->half_links = enable != 0;
     return 0;
 }
 

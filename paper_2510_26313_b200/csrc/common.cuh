@@ -53,9 +53,13 @@ __host__ __device__ inline void coords_to_cb(const Geom& g, int x, int y, int z,
 }
 
 // ------------------------------------------------------------------ storage traits
-struct F64 { using store_t = double; using comp_t = double; static constexpr int prec = LQ_FP64; static constexpr bool has_norm = false; };
-struct F32 { using store_t = float;  using comp_t = float;  static constexpr int prec = LQ_FP32; static constexpr bool has_norm = false; };
-struct H16 { using store_t = short;  using comp_t = float;  static constexpr int prec = LQ_HALF; static constexpr bool has_norm = true; };
+// link_t: storage type of the gauge links the stencil kernels read
+struct F64 { using store_t = double; using comp_t = double; using link_t = double; static constexpr int prec = LQ_FP64; static constexpr bool has_norm = false; };
+struct F32 { using store_t = float;  using comp_t = float;  using link_t = float;  static constexpr int prec = LQ_FP32; static constexpr bool has_norm = false; };
+struct H16 { using store_t = short;  using comp_t = float;  using link_t = float;  static constexpr int prec = LQ_HALF; static constexpr bool has_norm = true; };
+// half-storage spinors AND int16 fixed-point links (SURVEY 8(f) #3, 8(c.2) reading #13: entries of an SU(3) matrix lie in [-1, 1],
+// q = rint(32767 u), no norm needed): 36 instead of 72 bytes per link
+struct H16L { using store_t = short; using comp_t = float;  using link_t = short;  static constexpr int prec = LQ_HALF; static constexpr bool has_norm = true; };
 
 // ------------------------------------------------------------------ native spinor layout (one parity, N right-hand sides)
 // The batch is cut into G = N/R groups of R = 4 (N % 4 == 0), 2 (N even) or 1 consecutive right-hand sides and the
@@ -170,6 +174,8 @@ struct lq_ctx {
     double* gauge64;  // R = 18
     float* gauge32;   // R = recon32
     int recon32;
+    short* gauge16;   // int16 copy of the 18-real links (lq_set_half_links), or nullptr
+    bool half_links;  // LQ_HALF stencil kernels read gauge16
     // clover: [parity][blk] blocks of 72*SB reals; A and A^{-1}
     double *clov64, *clovinv64;
     float *clov32, *clovinv32;

@@ -32,7 +32,7 @@ template <class S> struct DslashArgs {
     int N, G;              // right-hand sides, RHS groups (N / R)
     FastDiv dG;            // division by G
     SView<S> out, in, x;   // out / x on `parity`, in on 1-parity
-    const T* gauge;        // [parity][blk][mu] blocks of RECON*SB reals
+    const typename S::link_t* gauge;   // [parity][blk][mu] blocks of RECON*SB reals (fp64 / fp32, or int16 fixed point for H16L)
     const T* clover;       // [blk] blocks of 72*SB reals of the output parity, or nullptr (identity)
     T coef;                // FORM_B
     T tsign;               // t_bc
@@ -128,6 +128,18 @@ __device__ __forceinline__ void load_link(const T* __restrict__ blockbase, int s
             u[12 + 2 * c] = re; u[12 + 2 * c + 1] = -im;
         }
     }
+}
+
+// int16 fixed-point links (H16L): the 18 values of a site are two 16-byte planes of 8 int16 and one 4-byte plane of 2
+__device__ __forceinline__ void load_link(const short* __restrict__ blockbase, int s, float* u) {
+    const uint4 a = __ldg(reinterpret_cast<const uint4*>(blockbase) + s);
+    const uint4 b = __ldg(reinterpret_cast<const uint4*>(blockbase + 8 * SB) + s);
+    const unsigned c = __ldg(reinterpret_cast<const unsigned*>(blockbase + 16 * SB) + s);
+    s16x2_to_f32(a.x, u[0], u[1]); s16x2_to_f32(a.y, u[2], u[3]); s16x2_to_f32(a.z, u[4], u[5]); s16x2_to_f32(a.w, u[6], u[7]);
+    s16x2_to_f32(b.x, u[8], u[9]); s16x2_to_f32(b.y, u[10], u[11]); s16x2_to_f32(b.z, u[12], u[13]); s16x2_to_f32(b.w, u[14], u[15]);
+    s16x2_to_f32(c, u[16], u[17]);
+#pragma unroll
+    for (int i = 0; i < 18; i++) u[i] *= (1.0f / 32767.0f);
 }
 
 // ---- SU(3) x projected half spinor, spin reconstruction and accumulation --------------------------------
@@ -296,12 +308,13 @@ __device__ __forceinline__ void project_half(const T (&p)[4][2][RPT], T sigma, i
 // `nb` points at real 0 of the neighbour's RPT right-hand sides; real j is at nb + j*SB*R.
 template <class S, int RPT, int R, int RECON, int MU, bool FWD, bool SMLINK = false>
 __device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ nb, const float* __restrict__ nb_norm,
-                                        const typename S::comp_t* __restrict__ link_blk, int link_s,
+                                        const typename S::link_t* __restrict__ link_blk, int link_s,
                                         typename S::comp_t cu, typename S::comp_t sigma, typename S::comp_t (&acc)[24][RPT]) {
     using T = typename S::comp_t;
     constexpr int PL = SB * R;   // elements between consecutive reals of a site
     T u[18];
-    load_link<T, RECON, SMLINK>(link_blk, link_s, u);
+    if constexpr (sizeof(typename S::link_t) == 2) load_link(link_blk, link_s, u);
+    else load_link<T, RECON, SMLINK>(link_blk, link_s, u);
 
     T cuk[RPT], clk[RPT];
     if constexpr (S::has_norm) {
@@ -338,14 +351,17 @@ __device__ __forceinline__ void hop_dir(const typename S::store_t* __restrict__ 
 // that the memory path (L1 misses in flight, L2 -> SM transfers, HBM) sets for this access pattern (bench.py --op cfgN:probe:...).
 template <class S, int RPT, int R, int RECON, bool SMLINK = false>
 __device__ __forceinline__ void hop_dir_probe(const typename S::store_t* __restrict__ nb, const float* __restrict__ nb_norm,
-                                              const typename S::comp_t* __restrict__ link_blk, int link_s, typename S::comp_t (&acc)[24][RPT]) {
+                                              const typename S::link_t* __restrict__ link_blk, int link_s, typename S::comp_t (&acc)[24][RPT]) {
     using T = typename S::comp_t;
     constexpr int PL = SB * R;
     T u[18];
-    load_planes<T, RECON, SMLINK>(link_blk, link_s, u);
-    if constexpr (RECON == 12) {
+    if constexpr (sizeof(typename S::link_t) == 2) load_link(link_blk, link_s, u);
+    else {
+        load_planes<T, RECON, SMLINK>(link_blk, link_s, u);
+        if constexpr (RECON == 12) {
 #pragma unroll
-        for (int i = 12; i < 18; i++) u[i] = u[i - 12];
+            for (int i = 12; i < 18; i++) u[i] = u[i - 12];
+        }
     }
     T sc[RPT];
     if constexpr (S::has_norm) { float nrm[RPT]; load_norm<RPT>(nb_norm, nrm);

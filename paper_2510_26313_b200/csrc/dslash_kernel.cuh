@@ -189,8 +189,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
 
     const int NB = a.g.NB;
     // forward links live on the output site, backward links on the neighbour (other parity)
-    const T* gown = a.gauge + ((size_t)(a.parity * NB + blk) * 4) * (RECON * SB);
-    const T* gopp = a.gauge + ((size_t)((1 - a.parity) * NB) * 4) * (RECON * SB);
+    using LT = typename S::link_t;
+    const LT* gown = a.gauge + ((size_t)(a.parity * NB + blk) * 4) * (RECON * SB);
+    const LT* gopp = a.gauge + ((size_t)((1 - a.parity) * NB) * 4) * (RECON * SB);
     const ST* inb = a.in.d + (size_t)grp * US + hoff;
     const float* inn = S::has_norm ? a.in.n + (size_t)grp * UN + hoff : nullptr;
     const size_t bstride = (size_t)G * US, nstride = (size_t)G * UN;
@@ -229,7 +230,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<S>
                         LQ_PF_LINES(qh, (int)(US * sizeof(ST) / LINE))
                     }
                 }
-                constexpr int GL = 4 * RECON * SB * sizeof(T) / LINE;     // lines of one (parity, block) link slab
+                constexpr int GL = 4 * RECON * SB * sizeof(typename S::link_t) / LINE;     // lines of one (parity, block) link slab
                 constexpr int CL = 72 * SB * sizeof(T) / LINE;            // lines of one clover block
                 if (grp == 0 % G) {
                     const char* l = (const char*)(a.gauge + ((size_t)(a.parity * NB + pb) * 4) * (RECON * SB));

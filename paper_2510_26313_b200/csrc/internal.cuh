@@ -26,7 +26,8 @@ int op_clover(lq_ctx* c, int prec, int nrhs, int parity, void* out, const void* 
 
 // reorder.cu
 int gauge_ingest(lq_ctx* c, const void* dev_canonical, int in_prec);            // canonical (device) -> native fp64
-int gauge_make_fp32(lq_ctx* c, int recon);                                       // native fp64 -> native fp32 (18 or 12)
+int gauge_make_fp32(lq_ctx* c, int recon);
+int gauge_make_int16(lq_ctx* c);                                                  // native fp64 -> int16 fixed point (18 reals), for H16L                                       // native fp64 -> native fp32 (18 or 12)
 int spinor_pack(lq_ctx* c, void* native_full, const void* dev_canonical, int nrhs, int prec, int in_prec);
 int spinor_unpack(lq_ctx* c, void* dev_canonical, const void* native_full, int nrhs, int prec, int out_prec);
 // the same for right-hand sides k0 .. k0+nk-1 only: dev_canonical holds just those nk fields (host buffers are staged in such chunks)

@@ -10,7 +10,9 @@ static DslashArgs<S> base_args(lq_ctx* c, int nrhs, int out_parity, void* out, c
     a.out = make_view<S>(c->g, out, nrhs, 0);
     a.in = make_view<S>(c->g, const_cast<void*>(in), nrhs, 0);
     a.x = make_view<S>(c->g, const_cast<void*>(x), nrhs, 0);
-    if constexpr (S::prec == LQ_FP64) a.gauge = c->gauge64; else a.gauge = c->gauge32;
+    if constexpr (S::prec == LQ_FP64) a.gauge = c->gauge64;
+    else if constexpr (sizeof(typename S::link_t) == 2) a.gauge = c->gauge16;
+    else a.gauge = c->gauge32;
     a.clover = nullptr;
     a.coef = T(1); a.tsign = T(c->t_bc); a.dsign = dagger ? T(-1) : T(1);
     a.epi = EPI_NONE; a.epi_num = a.epi_den = nullptr; a.epi_out = nullptr; a.red_partials = nullptr; a.red_counter = nullptr;
@@ -22,16 +24,17 @@ static DslashArgs<S> base_args(lq_ctx* c, int nrhs, int out_parity, void* out, c
 template <class S, int FORM>
 static int run_form(lq_ctx* c, DslashArgs<S> a) {
     {   // SURVEY 8(d) model: every input site read once, output written once, 8 links + the clover block once per launch
-        const int recon = S::prec == LQ_FP64 ? 18 : c->recon32;
-        const double cb = S::prec == LQ_FP64 ? 8.0 : 4.0;      // bytes per link / clover real
+        const int recon = (S::prec == LQ_FP64 || sizeof(typename S::link_t) == 2) ? 18 : c->recon32;
+        const double cb = S::prec == LQ_FP64 ? 8.0 : 4.0;      // bytes per clover real
+        const double lb = (double)sizeof(typename S::link_t);   // bytes per link real
         int streams = FORM == FORM_B ? 3 : 2;
         if (FORM == FORM_B && (a.epi == EPI_XMAY || a.epi == EPI_CDOT)) streams++;
-        const double bytes = streams * stream_bytes(c->g, a.N, S::prec) + (double)c->g.Vh * (8.0 * recon + (a.clover ? 72.0 : 0.0)) * cb;
+        const double bytes = streams * stream_bytes(c->g, a.N, S::prec) + (double)c->g.Vh * (8.0 * recon * lb + (a.clover ? 72.0 : 0.0) * cb);
         const double flops = (double)c->g.Vh * a.N * (1320.0 + (a.clover ? 504.0 : 0.0) + (FORM == FORM_B ? 48.0 : 0.0) +
                                                       (FORM == FORM_B && a.epi != EPI_NONE ? 48.0 : 0.0) + (FORM == FORM_B && a.epi == EPI_CDOT ? 96.0 : 0.0));
         LQ_MODEL(c, bytes, flops);
     }
-    if constexpr (S::prec == LQ_FP64) return launch_dslash<S, 18, FORM>(c, a, c->dslash_rpt, c->dslash_variant);
+    if constexpr (S::prec == LQ_FP64 || sizeof(typename S::link_t) == 2) return launch_dslash<S, 18, FORM>(c, a, c->dslash_rpt, c->dslash_variant);
     else {
         if (c->recon32 == 12) return launch_dslash<S, 12, FORM>(c, a, c->dslash_rpt, c->dslash_variant);
         return launch_dslash<S, 18, FORM>(c, a, c->dslash_rpt, c->dslash_variant);
@@ -46,6 +49,7 @@ template <class S> static const typename S::comp_t* clover_ptr(lq_ctx* c, int pa
 int op_hop(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* in, int dagger) {
     if (prec == LQ_FP64) return run_form<F64, FORM_HOP>(c, base_args<F64>(c, nrhs, out_parity, out, in, nullptr, dagger));
     if (prec == LQ_FP32) return run_form<F32, FORM_HOP>(c, base_args<F32>(c, nrhs, out_parity, out, in, nullptr, dagger));
+    if (c->half_links) return run_form<H16L, FORM_HOP>(c, base_args<H16L>(c, nrhs, out_parity, out, in, nullptr, dagger));
     return run_form<H16, FORM_HOP>(c, base_args<H16>(c, nrhs, out_parity, out, in, nullptr, dagger));
 }
 
@@ -57,6 +61,7 @@ template <class S> static int kernel_a_t(lq_ctx* c, int nrhs, int out_parity, vo
 int op_kernel_a(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* in, int dagger) {
     if (prec == LQ_FP64) return kernel_a_t<F64>(c, nrhs, out_parity, out, in, dagger);
     if (prec == LQ_FP32) return kernel_a_t<F32>(c, nrhs, out_parity, out, in, dagger);
+    if (c->half_links) return kernel_a_t<H16L>(c, nrhs, out_parity, out, in, dagger);
     return kernel_a_t<H16>(c, nrhs, out_parity, out, in, dagger);
 }
 
@@ -84,6 +89,7 @@ int op_kernel_b_epi(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, co
                     int epi, const double* num, const double* den, double* epi_out) {
     if (prec == LQ_FP64) return kernel_b_t<F64>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, epi, num, den, epi_out);
     if (prec == LQ_FP32) return kernel_b_t<F32>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, epi, num, den, epi_out);
+    if (c->half_links) return kernel_b_t<H16L>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, epi, num, den, epi_out);
     return kernel_b_t<H16>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, epi, num, den, epi_out);
 }
 // kernel B with the fused complex inner product <h, out> (conj: <out, h>) and ||out||^2: epi_out = 3 x LQ_MAX_RHS doubles
@@ -100,6 +106,7 @@ int op_kernel_b_cdot(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, c
                      const void* h, int conj, double* epi_out) {
     if (prec == LQ_FP64) return kernel_b_cdot_t<F64>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, h, conj, epi_out);
     if (prec == LQ_FP32) return kernel_b_cdot_t<F32>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, h, conj, epi_out);
+    if (c->half_links) return kernel_b_cdot_t<H16L>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, h, conj, epi_out);
     return kernel_b_cdot_t<H16>(c, nrhs, out_parity, out, x, in, coef, use_clover, dagger, h, conj, epi_out);
 }
 int op_kernel_b(lq_ctx* c, int prec, int nrhs, int out_parity, void* out, const void* x, const void* in, double coef, int use_clover, int dagger) {

@@ -50,6 +50,33 @@ int gauge_make_fp32(lq_ctx* c, int recon) {
     return 0;
 }
 
+// int16 fixed-point copy of the 18-real links for the half-storage kernels (H16L): q = rint(32767 u), |u| <= 1
+__global__ void gauge_to_int16_kernel(int Vh, int NB, const double* __restrict__ src, short* __restrict__ dst) {
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= 8LL * Vh) return;
+    const int cb = (int)(tid % Vh), pm = (int)(tid / Vh);
+    double r[18];
+    load_planes<double, 18>(link_block(src, NB, 18, pm >> 2, cb / SB, pm & 3), cb % SB, r);
+    short* blk = dst + ((size_t)((pm >> 2) * NB + cb / SB) * 4 + (pm & 3)) * (size_t)(18 * SB);
+    const int s = cb % SB;
+#pragma unroll
+    for (int k = 0; k < 18; k++) {
+        const float q = rintf(fminf(fmaxf((float)r[k], -1.0f), 1.0f) * 32767.0f);
+        const int plane = k / 8, e = k % 8;
+        if (plane < 2) blk[plane * 8 * SB + s * 8 + e] = (short)q; else blk[16 * SB + s * 2 + e] = (short)q;
+    }
+}
+int gauge_make_int16(lq_ctx* c) {
+    if (!c->gauge16) { c->gauge16 = (short*)dev_alloc(c, (size_t)8 * 18 * c->g.NB * SB * sizeof(short)); if (!c->gauge16) return LQ_ENOMEM; }
+    LQ_CUDA(c, cudaMemsetAsync(c->gauge16, 0, (size_t)8 * 18 * c->g.NB * SB * sizeof(short), c->stream));
+    const long long threads = 8LL * c->g.Vh;
+    const int block = 128; const int grid = (int)((threads + block - 1) / block);
+    gauge_to_int16_kernel<<<grid, block, 0, c->stream>>>(c->g.Vh, c->g.NB, c->gauge64, c->gauge16);
+    LQ_LAUNCHED(c);
+    LQ_CUDA(c, cudaGetLastError());
+    return 0;
+}
+
 // ---- scalar element access of a native parity block ---------------------------------------------------------------
 template <class S>
 __device__ __forceinline__ void load_site(const SView<S>& v, int N, int cb, int k, double* o) {

@@ -192,7 +192,7 @@ static GraphKey make_key(lq_ctx* c, SolverWorkspace* w, int alg, int prec, int n
     GraphKey k;
     k.prec = prec; k.n = n; k.check_every = check_every; k.alg = alg; k.recon = c->recon32; k.rpt = c->dslash_rpt; k.variant = c->dslash_variant;
     k.pfd = c->dslash_pfd; k.zc = c->dslash_zc; k.t_bc = c->t_bc; k.kappa = c->kappa; k.partials = c->red_partials;
-    k.gauge = prec == LQ_FP64 ? (const void*)c->gauge64 : (const void*)c->gauge32;
+    k.gauge = prec == LQ_FP64 ? (const void*)c->gauge64 : ((prec == LQ_HALF && c->half_links) ? (const void*)c->gauge16 : (const void*)c->gauge32);
     k.clov = prec == LQ_FP64 ? (const void*)c->clov64 : (const void*)c->clov32;
     k.clovinv = prec == LQ_FP64 ? (const void*)c->clovinv64 : (const void*)c->clovinv32;
     k.gen = w->gen;

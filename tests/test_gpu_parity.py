@@ -218,3 +218,29 @@ def test_error_paths():
     assert ctx.apply(B.LQ_OP_M, psi, B.LQ_FP64).shape == psi.shape
     assert ctx.launches > 0
     ctx.close()
+
+
+@pytest.mark.parametrize("nrhs", [1, 2, 4, 8, 12, 16])
+def test_int16_links_in_the_half_kernels(nrhs):
+    """Solver variant of SURVEY 8(f) #3 (reading #13): LQ_HALF stencil kernels with int16 fixed-point links.  Against the oracle on
+    the UNQUANTISED links and spinors the half-storage tolerance holds; against the oracle on links quantised the same way
+    (q = rint(32767 u) / 32767) the difference is the spinor quantisation alone."""
+    dims = (8, 6, 4, 6)          # Vh = 576: 18 site blocks
+    ctx, orc = make_case(dims, 51, 0.3, 0.1235, 1.0)
+    ctx.set_half_links(True)
+    ops = [B.LQ_OP_HOP, B.LQ_OP_M, B.LQ_OP_MDAG, B.LQ_OP_MHAT, B.LQ_OP_MHAT_DAG, B.LQ_OP_KERNEL_A, B.LQ_OP_KERNEL_B]
+    worst = check_ops(ctx, orc, nrhs, B.LQ_HALF, ops=ops)
+    assert worst <= 3e-3
+    Uq = (np.rint(orc.U.view(np.float64) * 32767.0) / 32767.0).view(np.complex128)
+    orc_q = OracleCase(dims, Uq, 0.1235, 1.0)
+    orc_q.A, orc_q.Ainv = orc.A, orc.Ainv                      # the clover term is built from the full-precision links
+    psi = inputs.gaussian_spinors(dims, nrhs, 7)
+    got = ctx.apply(B.LQ_OP_HOP, psi, B.LQ_HALF).astype(np.complex128)
+    e_q = max(rel_err(got[r], orc_q.apply(B.LQ_OP_HOP, psi)[r]) for r in range(nrhs))
+    e_u = max(rel_err(got[r], orc.apply(B.LQ_OP_HOP, psi)[r]) for r in range(nrhs))
+    assert e_q <= 1e-4 and e_u <= 2e-4, (e_q, e_u)
+    # switching back restores the fp32 links
+    ctx.set_half_links(False)
+    got32 = ctx.apply(B.LQ_OP_HOP, psi, B.LQ_HALF).astype(np.complex128)
+    assert max(rel_err(got32[r], orc.apply(B.LQ_OP_HOP, psi)[r]) for r in range(nrhs)) <= 1e-4
+    ctx.close()

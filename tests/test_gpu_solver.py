@@ -197,3 +197,17 @@ def test_batched_bicgstab_variant(inner, delta, tol, nrhs):
     xo, _, _ = oracle.solve_eo(dims, orc.U, orc.A, orc.Ainv, 0.124, b[k], tol * 1e-2)
     assert rel_err(x[k], xo.reshape(x[k].shape)) <= 50 * tol
     assert info["dslash_applies"] < info_cg["dslash_applies"]
+
+
+@pytest.mark.parametrize("algorithm", [B.LQ_ALG_CGNR, B.LQ_ALG_BICGSTAB])
+def test_half_solver_with_int16_links(algorithm):
+    """the int16+norm inner solver with int16 links still converges to the fp64 solution (the defect correction
+    uses the full-precision operator); true residual by the oracle's M."""
+    dims = (8, 8, 8, 16)
+    ctx, orc = setup(dims, 1003, 0.3, 0.1235, 1.0)
+    ctx.set_half_links(True)
+    b = inputs.laph_sources(dims, 12, 3, 2003)
+    x, info = ctx.solve(b, tol=1e-9, inner_prec=B.LQ_HALF, delta=1e-2, check_every=2, use_graph=True, algorithm=algorithm)
+    assert info["converged"], info
+    assert np.all(true_residuals(orc, x, b) <= 1e-9)
+    ctx.close()

@@ -542,3 +542,17 @@ def test_projection_definition_and_invariants(oracle_lib):
     gv = np.einsum("tzyxab,jtzyxb->jtzyxa", g, v)
     gpsi = np.einsum("tzyxab,ktzyxsb->ktzyxsa", g, psi)
     assert np.abs(oracle.project(gv, gpsi) - P).max() < 1e-11
+
+
+def test_int16_link_quantisation_error_of_the_operator(oracle_lib):
+    """SURVEY 8(c.2) reading #13 (the oracle-side check of the int16-link solver variant): quantising every link entry to
+    q = rint(32767 u) / 32767 changes M psi by a few 1e-5 relative (survey scratch: 3.5e-5), far below the half-storage tolerance."""
+    dims = (4, 4, 4, 8)
+    U = inputs.make_links(dims, 1000, 0.3)
+    Uq = (np.rint(U.view(np.float64) * 32767.0) / 32767.0).view(np.complex128)
+    oracle = oracle_lib
+    A = oracle.clover(dims, U, 0.12, 1.0)
+    psi = inputs.gaussian_spinors(dims, 1, 2000)[0]
+    ref = oracle.M(dims, U, A, 0.12, psi)
+    err = np.linalg.norm(oracle.M(dims, Uq, A, 0.12, psi) - ref) / np.linalg.norm(ref)
+    assert 1e-7 < err < 1e-4, err

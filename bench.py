@@ -321,11 +321,12 @@ def time_eigensolve(B, device):
     ctx = B.Context(c["dims"], device=device)
     ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=18)
     out = {"lattice": "x".join(map(str, c["dims"])), "cases": []}
-    for n_ev, m, cut in ((16, 48, 0.5), (64, 144, 1.0), (128, 288, 1.6)):
-        kw = dict(n_ev=n_ev, m=m, cheb_degree=24, cheb_a=cut, cheb_b=12.5, tol=1e-9, max_restarts=50, want_vectors=False)
+    # (n_ev, Krylov space, cut, filter degree): the 128-eigenpair case from a sweep over m in 176..288 and degree 16 / 24 / 32
+    for n_ev, m, cut, deg in ((16, 48, 0.5, 24), (64, 144, 1.0, 24), (128, 224, 1.6, 32)):
+        kw = dict(n_ev=n_ev, m=m, cheb_degree=deg, cheb_a=cut, cheb_b=12.5, tol=1e-9, max_restarts=50, want_vectors=False)
         ctx.laph_eigensolve(**kw)
         ev, _, info = ctx.laph_eigensolve(**kw)
-        out["cases"].append({"n_ev": n_ev, "krylov": m, "cheb_degree": 24, "seconds": round(info["seconds"], 4), "seconds_ritz": round(info["seconds_ritz"], 4), "seconds_ortho": round(info["seconds_ortho"], 4), "restarts": info["restarts"],
+        out["cases"].append({"n_ev": n_ev, "krylov": m, "cheb_degree": deg, "seconds": round(info["seconds"], 4), "seconds_ritz": round(info["seconds_ritz"], 4), "seconds_ortho": round(info["seconds_ortho"], 4), "restarts": info["restarts"],
                              "laplacian_applies": info["lap_applies"], "converged": info["converged"],
                              "max_true_residual": info["max_true_residual"], "eigenvalue_range": [float(ev.min()), float(ev.max())]})
     ctx.close()

@@ -9,6 +9,7 @@
 // restart ON THE DEVICE (ritz_jacobi_kernel: one CTA per time-slice, parallel two-sided Jacobi, all slices in one launch); the k
 // best Ritz vectors and the residual vector seed the next sweep (thick restart).  Eigenvalues of A are returned as Rayleigh quotients <v, A v> of the final Ritz vectors.
 #include <math.h>
+#include <string.h>
 #include <algorithm>
 #include <vector>
 #include <chrono>

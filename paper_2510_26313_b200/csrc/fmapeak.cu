@@ -7,10 +7,11 @@
 // mode 0: x_i = fma(x_i, b, c)                    scalar FFMA, 3 distinct source registers
 // mode 1: X_i = ffma2(X_i, B, C)                  packed FFMA2, 3 distinct 64-bit sources
 // mode 2: X_i = ffma2(A_q, Y_i, X_i), q = i / 4   packed FFMA2, the first source shared by 4 consecutive instructions
-// mode 3: X_i = ffma2((s_q, s_q), Y_i, X_i)         packed FFMA2 whose first source is ONE 32-bit register broadcast to both halves
-//                                                 (SASS "R.F32" operand form): what the compiler emits for the stencil's
-//                                                 link-element x spinor-pair products; three register sources hit one register
-//                                                 bank three times, so the instruction issues every 3rd cycle instead of every 2nd
+// mode 3: X_i = ffma2((s_q, s_q), Y_i, X_i)       packed FFMA2 whose first source is ONE 32-bit register broadcast to both halves
+//                                                 (SASS "R.F32" operand form, what the compiler emits for the stencil's link-element x
+//                                                 spinor-pair products), 16 different scalars in rotation so that the operand-reuse
+//                                                 cache rarely helps: scalar + two fresh register pairs read one register bank three
+//                                                 times and the instruction issues every 3rd cycle instead of every 2nd
 template <int MODE>
 __global__ void __launch_bounds__(256) fma_peak_kernel(float* out, int iters, float b, float c0) {
     constexpr int NACC = 16;
@@ -35,9 +36,11 @@ __global__ void __launch_bounds__(256) fma_peak_kernel(float* out, int iters, fl
         for (int i = 0; i < NACC; i++) x[i] = make_float2(seed + i, seed - i);
         const float2 b2 = make_float2(b, b * 0.999f), c2 = make_float2(c0, c0 * 1.001f);
         float2 a[4], y[NACC];
-        float sc[4];
+        float sc[16];
 #pragma unroll
-        for (int q = 0; q < 4; q++) { a[q] = make_float2(b * (1.f + 0.01f * q), b * (1.f - 0.01f * q)); sc[q] = b * (1.f + 0.02f * q) + seed * 1e-3f; }
+        for (int q = 0; q < 4; q++) a[q] = make_float2(b * (1.f + 0.01f * q), b * (1.f - 0.01f * q));
+#pragma unroll
+        for (int q = 0; q < 16; q++) sc[q] = b * (1.f + 0.01f * q) + seed;
 #pragma unroll
         for (int i = 0; i < NACC; i++) y[i] = make_float2(c0 + 0.01f * i, c0 - 0.01f * i);
         for (int it = 0; it < iters; it++) {
@@ -47,12 +50,14 @@ __global__ void __launch_bounds__(256) fma_peak_kernel(float* out, int iters, fl
                 for (int i = 0; i < NACC; i++) {
                     if constexpr (MODE == 1) x[i] = __ffma2_rn(x[i], b2, c2);
                     else if constexpr (MODE == 2) x[i] = __ffma2_rn(a[i >> 2], y[i], x[i]);
-                    else x[i] = __ffma2_rn(make_float2(sc[i >> 2], sc[i >> 2]), y[i], x[i]);
+                    else { const float sq = sc[(i >> 2) + 4 * (r & 3)]; x[i] = __ffma2_rn(make_float2(sq, sq), y[i], x[i]); }
                 }
             }
             if constexpr (MODE >= 2) {      // keep the operands loop-variant so nothing is hoisted or folded
 #pragma unroll
-                for (int q = 0; q < 4; q++) { a[q].x = -a[q].x; sc[q] = -sc[q]; }
+                for (int q = 0; q < 4; q++) a[q].x = -a[q].x;
+#pragma unroll
+                for (int q = 0; q < 16; q++) sc[q] = -sc[q];
             }
         }
         float s = 0.f;

@@ -278,6 +278,68 @@ int lq_fma_peak(lq_ctx* ctx, int mode, double ms, double* tflops);
  * byte crosses L2 -> SM about 3 times because the 8 neighbour reads of a site meet in L2).  Writes GB/s to *gbs. */
 int lq_mem_peak(lq_ctx* ctx, int mode, double mbytes, double* gbs);
 
+/* ------------------------------------------------------------------ two-level adaptive multigrid
+ * PAPER.md L118 ("adaptive geometric multi-grid solver", ref. [19]), L164 ("mixed-precision multi-grid solver") and L137 (batching
+ * matters most on the coarse grids).  M x = b for the FULL operator M = A - kappa D (step 7) and N right-hand sides at once:
+ *   setup   N_v near-null vectors v_k -> aggregates (blocks of block[0] x block[1] x block[2] x block[3] sites) x chirality
+ *           (spin 0,1 | spin 2,3) -> prolongator P with orthonormal columns: column (a, chi, k) is v_k restricted to aggregate a and
+ *           chirality chi, Gram-Schmidt over k = 0, 1, ... (each column against the earlier ones, twice, then normalised) ->
+ *           Galerkin coarse operator A_c = P^dag M P, a 9-point stencil of dense (2 N_v) x (2 N_v) blocks
+ *   cycle   z ~ M^{-1} r: nu_pre smoother steps from z = 0, coarse correction z += P A_c^{-1} P^dag (r - M z) with A_c^{-1} by
+ *           coarse_iters iterations of GCR (restart length min(coarse_iters, 16)), nu_post smoother steps; fp32 throughout.
+ *           Smoother LQ_MG_SMOOTH_MR: minimal-residual steps on M itself (t = M res, w = <t,res>/<t,t>, z += w res, res -= w t).
+ *           Smoother LQ_MG_SMOOTH_EO: the correction delta ~ M^{-1} res is taken through the even-odd Schur system of steps 8-10,
+ *           rho_e = res_e + kappa D_eo A_oo^{-1} res_o, nu minimal-residual steps on Mhat delta_e = rho_e from zero,
+ *           delta_o = A_oo^{-1} (res_o + kappa D_oe delta_e); z += delta.  (Mhat has the spectrum lambda (2 - lambda) of M's: the
+ *           lambda ~ 2 modes, which minimal residual on M leaves as undamped as the low modes, are folded onto the low modes.)
+ *   solve   flexible GCR(restart) preconditioned by the cycle, in fp32, inside an fp64 defect correction (true residual b - M x)
+ * Coarse site of (x,y,z,t): a = ax + Lcx (ay + Lcy (az + Lcz at)), a_mu = x_mu / block_mu, Lc_mu = L_mu / block_mu.  Coarse vectors at
+ * this boundary are complex fp64 arrays [rhs][a][chi][k]; fine vectors are CANONICAL complex fp64 [rhs][t][z][y][x][spin][colour].
+ * Restrictions: L_mu % block_mu == 0, V % 64 == 0, n_vec in {1, 2, 4, 8, ..., 32 (multiples of 4)}.  The hierarchy belongs to the
+ * context, is rebuilt by the next setup call and released by lq_mg_free / lq_destroy; it is invalidated (LQ_ESTATE from the calls
+ * below) by lq_load_gauge, lq_fill_gauge_random and lq_build_clover. */
+enum { LQ_MG_SMOOTH_MR = 0, LQ_MG_SMOOTH_EO = 1 };
+typedef struct lq_mg_param {
+    int block[4];         /* aggregate extent per direction */
+    int n_vec;            /* N_v */
+    int nu_pre, nu_post;  /* smoother steps before / after the coarse correction (>= 0) */
+    int smoother;         /* LQ_MG_SMOOTH_MR or LQ_MG_SMOOTH_EO */
+    int coarse_iters;     /* GCR iterations of the coarse solve (>= 1) */
+    int restart;          /* restart length of the outer flexible GCR, 1 .. 16 */
+    double setup_tol;     /* lq_mg_setup: v_k = M^{-1} eta_k by lq_solve's mixed-precision CG to this relative residual (e.g. 1e-3) */
+    uint64_t seed;        /* lq_mg_setup: seed of the Gaussian eta_k (the generator of lq_fill_spinor_random) */
+} lq_mg_param;
+typedef struct lq_mg_info {
+    int coarse_dims[4];
+    long long coarse_dof;        /* Vc * 2 N_v */
+    int probes;                  /* applications of M that built A_c */
+    double seconds_vectors;      /* lq_mg_setup: the near-null vector solves */
+    double seconds_prolongator;  /* gather + block Gram-Schmidt */
+    double seconds_coarse_op;    /* probing */
+    size_t bytes;                /* device memory of P, A_c and the tables */
+} lq_mg_info;
+typedef struct lq_mg_solve_info {
+    int iters;                              /* outer FGCR iterations (= multigrid cycles) summed over the defect-correction cycles */
+    int outer_cycles;                       /* fp64 defect-correction cycles */
+    double true_rel_residual[LQ_MAX_RHS];   /* ||b - M x|| / ||b|| in fp64 */
+    double seconds;                         /* device time of the solve (CUDA events), staging excluded */
+    double m_applies;                       /* applications of the fine operator M, all precisions */
+} lq_mg_solve_info;
+/* Adaptive setup: v_k = M^{-1} eta_k with Gaussian eta_k, k < n_vec (one batched lq_solve).  `info` may be NULL. */
+int lq_mg_setup(lq_ctx* ctx, const lq_mg_param* param, lq_mg_info* info);
+/* Setup from given near-null vectors: vecs = n_vec CANONICAL complex fp64 fields at `loc` (read only). */
+int lq_mg_setup_from_vectors(lq_ctx* ctx, const lq_mg_param* param, const void* vecs, int loc, lq_mg_info* info);
+int lq_mg_free(lq_ctx* ctx);
+/* The pieces of the cycle, each on nrhs right-hand sides at `loc` (parity tests; also usable on their own):
+ * coarse_out = P^dag fine_in ; fine_out = P coarse_in ; out = A_c in ; z = cycle(r). */
+int lq_mg_restrict(lq_ctx* ctx, void* coarse_out, const void* fine_in, int nrhs, int loc);
+int lq_mg_prolong(lq_ctx* ctx, void* fine_out, const void* coarse_in, int nrhs, int loc);
+int lq_mg_coarse_apply(lq_ctx* ctx, void* coarse_out, const void* coarse_in, int nrhs, int loc);
+int lq_mg_vcycle(lq_ctx* ctx, void* z, const void* r, int nrhs, int loc);
+/* Solve M x = b (CANONICAL complex fp64 at `loc`, zero initial guess) to ||b - M x|| <= tol ||b|| per right-hand side, at most max_iter
+ * outer iterations.  Returns LQ_ENOTCONVERGED (x and info still filled) if a right-hand side misses tol. */
+int lq_mg_solve(lq_ctx* ctx, void* x, const void* b, int nrhs, int loc, double tol, int max_iter, lq_mg_solve_info* info);
+
 /* Number of kernels this library has launched on this context since creation (for bench.py). */
 long long lq_kernel_launches(const lq_ctx* ctx);
 

@@ -64,18 +64,42 @@ def coarse_operator(apply_M, P):
     return P.conj().T @ MP
 
 
-def two_grid_preconditioner(apply_M, P, Ac, r, smooth=4):
-    """z ~ M^-1 r: `smooth` minimal-residual sweeps, coarse-grid correction with an exact coarse solve, `smooth` sweeps."""
-    def mr(x, b, n):
-        for _ in range(n):
-            res = b - apply_M(x)
-            Mr = apply_M(res)
-            om = np.vdot(Mr, res) / np.vdot(Mr, Mr)
-            x = x + om * res
-        return x
-    z = mr(np.zeros_like(r), r, smooth)
+def mr_smoother(apply_M, res, steps):
+    """LQ_MG_SMOOTH_MR: delta ~ M^-1 res by `steps` minimal-residual steps on M from zero."""
+    x = np.zeros_like(res)
+    for _ in range(steps):
+        r = res - apply_M(x)
+        Mr = apply_M(r)
+        om = np.vdot(Mr, r) / np.vdot(Mr, Mr)
+        x = x + om * r
+    return x
+
+
+def schur_mr_smoother(dims, U, A, Ainv, kappa, res, steps, t_bc=-1):
+    """LQ_MG_SMOOTH_EO: delta ~ M^-1 res through the even-odd Schur system (steps 8-10 of the solver): Schur source, `steps`
+    minimal-residual steps on Mhat delta_e = rho_e from zero, reconstruction of the odd sites.  Uses the pinned oracle operators."""
+    import oracle
+    V = dims[0] * dims[1] * dims[2] * dims[3]
+    r = np.asarray(res, dtype=np.complex128).reshape(V, 12)
+    rho = oracle.schur_source(dims, U, Ainv, kappa, r, t_bc)
+    d = np.zeros_like(rho)
+    for _ in range(steps):
+        t = oracle.Mhat(dims, U, A, Ainv, kappa, rho, False, t_bc)
+        om = np.vdot(t, rho) / np.vdot(t, t)
+        d = d + om * rho
+        rho = rho - om * t
+    return oracle.schur_reconstruct(dims, U, Ainv, kappa, r, d, t_bc).reshape(-1)
+
+
+def two_grid_preconditioner(apply_M, P, Ac, r, smooth=4, smoother=None):
+    """z ~ M^-1 r: pre-smoothing from zero, coarse-grid correction with an exact coarse solve, post-smoothing of the residual
+    equation.  smoother(res) -> delta ~ M^-1 res; default: `smooth` minimal-residual steps on M (mr_smoother)."""
+    if smoother is None:
+        def smoother(res):
+            return mr_smoother(apply_M, res, smooth)
+    z = smoother(r)
     z = z + P @ np.linalg.solve(Ac, P.conj().T @ (r - apply_M(z)))
-    return mr(z, r, smooth)
+    return z + smoother(r - apply_M(z))
 
 
 def fgcr(apply_M, b, tol, precond=None, maxit=200, restart=16):

@@ -19,6 +19,7 @@ LQ_FP64, LQ_FP32, LQ_HALF = 0, 1, 2
 LQ_HOST, LQ_DEVICE = 0, 1
 LQ_CANONICAL, LQ_NATIVE = 0, 1
 LQ_MAX_RHS = 32
+LQ_MG_SMOOTH_MR, LQ_MG_SMOOTH_EO = 0, 1
 (LQ_OP_HOP, LQ_OP_M, LQ_OP_MDAG, LQ_OP_CLOVER, LQ_OP_CLOVER_INV, LQ_OP_HOP_EO, LQ_OP_HOP_OE, LQ_OP_MHAT, LQ_OP_MHAT_DAG,
  LQ_OP_KERNEL_A, LQ_OP_KERNEL_B, LQ_OP_PROBE_LOADS) = range(12)
 LQ_OK, LQ_EINVAL, LQ_ESTATE, LQ_ENOMEM, LQ_ECUDA, LQ_ENOTCONVERGED, LQ_ESINGULAR = 0, -1, -2, -3, -4, -5, -6
@@ -27,7 +28,9 @@ PREC = {"fp64": LQ_FP64, "fp32": LQ_FP32, "half": LQ_HALF}
 EXPORTS = ["lq_create", "lq_destroy", "lq_last_error", "lq_set_allocator", "lq_load_gauge", "lq_fill_gauge_random",
            "lq_build_clover", "lq_apply", "lq_native_bytes", "lq_pack", "lq_unpack", "lq_fill_spinor_random", "lq_solve",
            "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites", "lq_native_index", "lq_fma_peak", "lq_mem_peak", "lq_set_half_links",
-           "lq_laplacian", "lq_laplacian_native", "lq_cv_native_bytes", "lq_cv_fill_random", "lq_laph_eigensolve", "lq_project"]
+           "lq_laplacian", "lq_laplacian_native", "lq_cv_native_bytes", "lq_cv_fill_random", "lq_laph_eigensolve", "lq_project",
+           "lq_mg_setup", "lq_mg_setup_from_vectors", "lq_mg_free", "lq_mg_restrict", "lq_mg_prolong", "lq_mg_coarse_apply", "lq_mg_vcycle",
+           "lq_mg_solve"]
 
 
 class SolveParam(ctypes.Structure):
@@ -52,6 +55,22 @@ class SolveInfo(ctypes.Structure):
                 ("iters", ctypes.c_int * LQ_MAX_RHS), ("true_rel_residual", ctypes.c_double * LQ_MAX_RHS),
                 ("seconds", ctypes.c_double), ("dslash_applies", ctypes.c_double), ("model_bytes", ctypes.c_double),
                 ("model_flops", ctypes.c_double)]
+
+
+class MgParam(ctypes.Structure):
+    _fields_ = [("block", ctypes.c_int * 4), ("n_vec", ctypes.c_int), ("nu_pre", ctypes.c_int), ("nu_post", ctypes.c_int), ("smoother", ctypes.c_int),
+                ("coarse_iters", ctypes.c_int), ("restart", ctypes.c_int), ("setup_tol", ctypes.c_double), ("seed", ctypes.c_uint64)]
+
+
+class MgInfo(ctypes.Structure):
+    _fields_ = [("coarse_dims", ctypes.c_int * 4), ("coarse_dof", ctypes.c_longlong), ("probes", ctypes.c_int),
+                ("seconds_vectors", ctypes.c_double), ("seconds_prolongator", ctypes.c_double), ("seconds_coarse_op", ctypes.c_double),
+                ("bytes", ctypes.c_size_t)]
+
+
+class MgSolveInfo(ctypes.Structure):
+    _fields_ = [("iters", ctypes.c_int), ("outer_cycles", ctypes.c_int), ("true_rel_residual", ctypes.c_double * LQ_MAX_RHS),
+                ("seconds", ctypes.c_double), ("m_applies", ctypes.c_double)]
 
 
 ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
@@ -103,6 +122,12 @@ def load_library():
     lib.lq_native_index.argtypes = [vp, ci, ci, ci, ci, ci, ci, ci, ci, szp, szp, szp, szp]
     lib.lq_fma_peak.argtypes = [vp, ci, cd, ctypes.POINTER(cd)]
     lib.lq_mem_peak.argtypes = [vp, ci, cd, ctypes.POINTER(cd)]
+    lib.lq_mg_setup.argtypes = [vp, ctypes.POINTER(MgParam), ctypes.POINTER(MgInfo)]
+    lib.lq_mg_setup_from_vectors.argtypes = [vp, ctypes.POINTER(MgParam), vp, ci, ctypes.POINTER(MgInfo)]
+    lib.lq_mg_free.argtypes = [vp]
+    for f in (lib.lq_mg_restrict, lib.lq_mg_prolong, lib.lq_mg_coarse_apply, lib.lq_mg_vcycle):
+        f.argtypes = [vp, vp, vp, ci, ci]
+    lib.lq_mg_solve.argtypes = [vp, vp, vp, ci, ci, cd, ci, ctypes.POINTER(MgSolveInfo)]
     _lib = lib
     return lib
 
@@ -331,6 +356,72 @@ class Context:
         self._check(self.lib.lq_apply(self.h, op, ctypes.c_void_p(out.ctypes.data), ctypes.c_void_p(psi.ctypes.data), p2, nrhs, prec,
                                       LQ_HOST, LQ_CANONICAL))
         return out
+
+    # ------------------------------------------------------------------ two-level multigrid (lq_mg_*)
+    def mg_setup(self, block, n_vec: int, nu_pre: int = 2, nu_post: int = 2, coarse_iters: int = 8, restart: int = 8,
+                 setup_tol: float = 1e-3, seed: int = 1, vecs=None, smoother: int = 1) -> dict:
+        """Builds the hierarchy: adaptively (vecs=None) or from n_vec given canonical complex128 near-null vectors."""
+        self._enter()
+        prm = MgParam((ctypes.c_int * 4)(*block), n_vec, nu_pre, nu_post, smoother, coarse_iters, restart, setup_tol, seed)
+        info = MgInfo()
+        if vecs is None:
+            self._check(self.lib.lq_mg_setup(self.h, ctypes.byref(prm), ctypes.byref(info)))
+        else:
+            if isinstance(vecs, np.ndarray):
+                vecs = np.ascontiguousarray(vecs, dtype=np.complex128)
+            assert vecs.shape[0] == n_vec
+            pv, loc = _ptr(vecs)
+            self._check(self.lib.lq_mg_setup_from_vectors(self.h, ctypes.byref(prm), pv, loc, ctypes.byref(info)))
+        self._mg = dict(coarse_dims=tuple(info.coarse_dims), n_vec=n_vec)
+        return dict(coarse_dims=tuple(info.coarse_dims), coarse_dof=info.coarse_dof, probes=info.probes, seconds_vectors=info.seconds_vectors,
+                    seconds_prolongator=info.seconds_prolongator, seconds_coarse_op=info.seconds_coarse_op, bytes=info.bytes)
+
+    def mg_free(self):
+        self._enter()
+        self._check(self.lib.lq_mg_free(self.h))
+
+    def _mg_piece(self, fn, inp: np.ndarray, out_fine: bool) -> np.ndarray:
+        self._enter()
+        inp = np.ascontiguousarray(inp, dtype=np.complex128)
+        nrhs = inp.shape[0]
+        Lc = self._mg["coarse_dims"]
+        if out_fine:
+            out = np.empty((nrhs, self.dims[3], self.dims[2], self.dims[1], self.dims[0], 4, 3), dtype=np.complex128)
+        else:
+            out = np.empty((nrhs, int(np.prod(Lc)), 2, self._mg["n_vec"]), dtype=np.complex128)
+        self._check(fn(self.h, ctypes.c_void_p(out.ctypes.data), ctypes.c_void_p(inp.ctypes.data), nrhs, LQ_HOST))
+        return out
+
+    def mg_restrict(self, fine: np.ndarray) -> np.ndarray:
+        """coarse[rhs][a][chi][k] = P^dag fine (canonical complex128 fine vectors)."""
+        return self._mg_piece(self.lib.lq_mg_restrict, fine, False)
+
+    def mg_prolong(self, coarse: np.ndarray) -> np.ndarray:
+        return self._mg_piece(self.lib.lq_mg_prolong, coarse, True)
+
+    def mg_coarse_apply(self, coarse: np.ndarray) -> np.ndarray:
+        return self._mg_piece(self.lib.lq_mg_coarse_apply, coarse, False)
+
+    def mg_vcycle(self, r: np.ndarray) -> np.ndarray:
+        return self._mg_piece(self.lib.lq_mg_vcycle, r, True)
+
+    def mg_solve(self, b, tol: float, max_iter: int = 200, x_out=None):
+        """Solves M x = b with the multigrid-preconditioned flexible GCR.  b: canonical complex128 (numpy or torch, host or device)."""
+        self._enter()
+        if isinstance(b, np.ndarray):
+            b = np.ascontiguousarray(b, dtype=np.complex128)
+            x = x_out if x_out is not None else np.empty_like(b)
+        else:
+            x = x_out if x_out is not None else self.torch.empty_like(b)
+        nrhs = b.shape[0]
+        pb, loc = _ptr(b)
+        px, locx = _ptr(x)
+        assert loc == locx
+        info = MgSolveInfo()
+        rc = self.lib.lq_mg_solve(self.h, px, pb, nrhs, loc, tol, max_iter, ctypes.byref(info))
+        self._check(rc, allow=(LQ_ENOTCONVERGED,))
+        return x, dict(converged=(rc == 0), iters=info.iters, outer_cycles=info.outer_cycles, seconds=info.seconds, m_applies=info.m_applies,
+                       true_rel_residual=list(info.true_rel_residual)[:nrhs])
 
     # ------------------------------------------------------------------ solve
     def solve(self, b, tol: float, inner_prec: int = LQ_FP32, delta: float = 1e-3, max_outer: int = 50, max_inner: int = 2000,

@@ -55,7 +55,7 @@ int lq_create(lq_ctx** out, const int dims[4], int device, void* cuda_stream) {
     c->alloc_fn = nullptr; c->free_fn = nullptr; c->alloc_user = nullptr;
     c->launches = 0; c->dslash_rpt = 0; c->dslash_variant = 0; c->dslash_pfd = LQ_DEFAULT_PFD; c->dslash_zc = 0;
     c->red_partials = nullptr; c->red_partials_elems = 0; c->red_counter = nullptr; c->h_scalars = nullptr; c->d_flag = nullptr;
-    c->ws = nullptr; c->loop_skip = nullptr; c->model_bytes = c->model_flops = 0.0; c->proj_scratch = nullptr; c->proj_scratch_bytes = 0;
+    c->ws = nullptr; c->mg = nullptr; c->loop_skip = nullptr; c->model_bytes = c->model_flops = 0.0; c->proj_scratch = nullptr; c->proj_scratch_bytes = 0;
     if (cudaMalloc(&c->red_counter, RED_COUNTER_BYTES) != cudaSuccess || cudaMemset(c->red_counter, 0, RED_COUNTER_BYTES) != cudaSuccess ||
         cudaMallocHost(&c->h_scalars, 8 * LQ_MAX_RHS * sizeof(double)) != cudaSuccess) { cudaGetLastError(); delete c; return LQ_ECUDA; }
     c->d_flag = (int*)(c->red_counter + 16);
@@ -68,6 +68,7 @@ int lq_destroy(lq_ctx* c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     solver_release(c);
+    mg_release(c);
     std::vector<void*> owned = c->owned;
     for (void* p : owned) dev_free(c, p);
     cudaFree(c->red_counter);
@@ -124,6 +125,7 @@ int lq_load_gauge(lq_ctx* c, const void* links, int in_prec, int loc, int recon,
     if (staging) dev_free(c, staging);
     if (rc) return rc;
     c->t_bc = t_bc; c->has_gauge = true; c->has_clover = false;
+    mg_invalidate(c);
     return 0;
 }
 
@@ -137,6 +139,7 @@ int lq_fill_gauge_random(lq_ctx* c, uint64_t seed, double eps, int recon, int t_
     if (c->half_links) LQ_TRY(gauge_make_int16(c));
     LQ_CUDA(c, cudaStreamSynchronize(c->stream));
     c->t_bc = t_bc; c->has_gauge = true; c->has_clover = false;
+    mg_invalidate(c);
     return 0;
 }
 
@@ -156,6 +159,7 @@ int lq_build_clover(lq_ctx* c, double kappa, double csw) {
     if (!c) return LQ_EINVAL;
     if (!c->has_gauge) return set_err(c, LQ_ESTATE, "load the gauge field before building the clover term");
     cudaSetDevice(c->device);
+    mg_invalidate(c);
     return clover_build(c, kappa, csw);
 }
 
@@ -452,6 +456,77 @@ int lq_solve(lq_ctx* c, void* x, const void* b, int nrhs, int loc, int layout, c
     if (rc == 0) { src = solve_native(c, n_x, n_b, nrhs, param, info); if (src != 0 && src != LQ_ENOTCONVERGED) rc = src; }
     if (rc == 0) rc = unpack_any(c, x, n_x, nrhs, LQ_FP64, loc);
     if (cudaStreamSynchronize(c->stream) != cudaSuccess && rc == 0) rc = set_err(c, LQ_ECUDA, std::string("lq_solve: ") + cudaGetErrorString(cudaGetLastError()));
+    void* tofree[] = {n_b, n_x};
+    for (void* p : tofree) if (p) dev_free(c, p);
+    return rc ? rc : src;
+}
+
+// ---- two-level multigrid (multigrid.cu) ---------------------------------------------------------------------------------------
+int lq_mg_setup(lq_ctx* c, const lq_mg_param* param, lq_mg_info* info) {
+    if (!c) return LQ_EINVAL;
+    cudaSetDevice(c->device);
+    return mg_setup_adaptive(c, param, info);
+}
+int lq_mg_setup_from_vectors(lq_ctx* c, const lq_mg_param* param, const void* vecs, int loc, lq_mg_info* info) {
+    if (!c) return LQ_EINVAL;
+    if (!param || !vecs || param->n_vec < 1 || param->n_vec > LQ_MAX_RHS) return set_err(c, LQ_EINVAL, "lq_mg_setup_from_vectors: bad argument");
+    cudaSetDevice(c->device);
+    void* st = nullptr;
+    const void* d = stage_in(c, vecs, (size_t)param->n_vec * c->g.V * 24 * sizeof(double), loc, &st);
+    int rc = d ? mg_setup_vectors(c, param, d, info) : LQ_ENOMEM;
+    if (st) { cudaStreamSynchronize(c->stream); dev_free(c, st); }
+    return rc;
+}
+int lq_mg_free(lq_ctx* c) {
+    if (!c) return LQ_EINVAL;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    mg_release(c);
+    return 0;
+}
+// one of the four pieces: in / out are fine (canonical) or coarse arrays at `loc`
+static int mg_piece(lq_ctx* c, int which, void* out, const void* in, int nrhs, int loc) {
+    if (!c) return LQ_EINVAL;
+    if (!out || !in || out == in || !nrhs_ok(nrhs)) return set_err(c, LQ_EINVAL, "lq_mg_*: bad argument");
+    if (!c->mg) return set_err(c, LQ_ESTATE, "lq_mg_*: no multigrid hierarchy");
+    cudaSetDevice(c->device);
+    const size_t fb = (size_t)nrhs * c->g.V * 24 * sizeof(double), cb = mg_coarse_canonical_bytes(c, nrhs);
+    const bool in_fine = which == 0 || which == 3, out_fine = which == 1 || which == 3;
+    const size_t ib = in_fine ? fb : cb, ob = out_fine ? fb : cb;
+    void *st_in = nullptr, *st_out = nullptr;
+    const void* d_in = stage_in(c, in, ib, loc, &st_in);
+    int rc = d_in ? 0 : LQ_ENOMEM;
+    void* d_out = out;
+    if (rc == 0 && loc == LQ_HOST) { st_out = dev_alloc(c, ob); if (!st_out) rc = LQ_ENOMEM; d_out = st_out; }
+    if (rc == 0) {
+        if (which == 0) rc = mg_restrict_dev(c, (double*)d_out, d_in, nrhs);
+        else if (which == 1) rc = mg_prolong_dev(c, d_out, (const double*)d_in, nrhs);
+        else if (which == 2) rc = mg_coarse_apply_dev(c, (double*)d_out, (const double*)d_in, nrhs);
+        else rc = mg_vcycle_dev(c, d_out, d_in, nrhs);
+    }
+    if (rc == 0 && st_out && cudaMemcpyAsync(out, st_out, ob, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "D2H copy failed");
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess && rc == 0) rc = set_err(c, LQ_ECUDA, std::string("lq_mg_*: ") + cudaGetErrorString(cudaGetLastError()));
+    if (st_in) dev_free(c, st_in);
+    if (st_out) dev_free(c, st_out);
+    return rc;
+}
+int lq_mg_restrict(lq_ctx* c, void* coarse_out, const void* fine_in, int nrhs, int loc) { return mg_piece(c, 0, coarse_out, fine_in, nrhs, loc); }
+int lq_mg_prolong(lq_ctx* c, void* fine_out, const void* coarse_in, int nrhs, int loc) { return mg_piece(c, 1, fine_out, coarse_in, nrhs, loc); }
+int lq_mg_coarse_apply(lq_ctx* c, void* coarse_out, const void* coarse_in, int nrhs, int loc) { return mg_piece(c, 2, coarse_out, coarse_in, nrhs, loc); }
+int lq_mg_vcycle(lq_ctx* c, void* z, const void* r, int nrhs, int loc) { return mg_piece(c, 3, z, r, nrhs, loc); }
+
+int lq_mg_solve(lq_ctx* c, void* x, const void* b, int nrhs, int loc, double tol, int max_iter, lq_mg_solve_info* info) {
+    if (!c) return LQ_EINVAL;
+    if (!x || !b || !info || !nrhs_ok(nrhs) || !(tol > 0) || max_iter < 1) return set_err(c, LQ_EINVAL, "lq_mg_solve: bad argument");
+    cudaSetDevice(c->device);
+    const size_t pb = parity_bytes(c->g, nrhs, LQ_FP64);
+    void *n_b = dev_alloc(c, 2 * pb), *n_x = dev_alloc(c, 2 * pb);
+    int rc = (!n_b || !n_x) ? LQ_ENOMEM : 0;
+    if (rc == 0) rc = pack_any(c, n_b, b, nrhs, LQ_FP64, loc);
+    int src = 0;
+    if (rc == 0) { src = mg_solve_native(c, n_x, n_b, nrhs, tol, max_iter, info); if (src != 0 && src != LQ_ENOTCONVERGED) rc = src; }
+    if (rc == 0) rc = unpack_any(c, x, n_x, nrhs, LQ_FP64, loc);
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess && rc == 0) rc = set_err(c, LQ_ECUDA, std::string("lq_mg_solve: ") + cudaGetErrorString(cudaGetLastError()));
     void* tofree[] = {n_b, n_x};
     for (void* p : tofree) if (p) dev_free(c, p);
     return rc ? rc : src;

@@ -196,6 +196,8 @@ struct lq_ctx {
     int* d_flag;                    // device error flag
     // solver state (solver.cu): workspace with the cached iteration graph, owned by the context
     struct SolverWorkspace* ws;
+    // two-level multigrid hierarchy (multigrid.cu), or nullptr
+    struct MgState* mg;
     // while the solver enqueues the body of an inner iteration: device flag that makes every kernel of the body return
     // at once when set (the inner solve has converged; launches already queued behind the flag become no-ops)
     const int* loop_skip;

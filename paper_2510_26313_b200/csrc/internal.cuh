@@ -89,3 +89,15 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
 int project_device(lq_ctx* c, double* dev_P, const double* dev_V, int n_ev, const double* dev_X, int n_sol);
 // project_tc.cu : the same contraction on tcgen05 tensor cores (3xTF32, fp32 TMEM accumulator, fp64 split-K sum)
 int project_device_tc(lq_ctx* c, double* dev_P, const double* dev_V, int n_ev, const double* dev_X, int n_sol);
+
+// multigrid.cu : two-level adaptive multigrid; canonical / coarse arrays below are DEVICE arrays
+void mg_release(lq_ctx* c);
+void mg_invalidate(lq_ctx* c);
+int mg_setup_vectors(lq_ctx* c, const lq_mg_param* p, const void* dev_canonical64, lq_mg_info* info);
+int mg_setup_adaptive(lq_ctx* c, const lq_mg_param* p, lq_mg_info* info);
+size_t mg_coarse_canonical_bytes(const lq_ctx* c, int n);
+int mg_restrict_dev(lq_ctx* c, double* coarse64, const void* fine_canonical64, int n);
+int mg_prolong_dev(lq_ctx* c, void* fine_canonical64, const double* coarse64, int n);
+int mg_coarse_apply_dev(lq_ctx* c, double* out64, const double* in64, int n);
+int mg_vcycle_dev(lq_ctx* c, void* z_canonical64, const void* r_canonical64, int n);
+int mg_solve_native(lq_ctx* c, void* x64, const void* b64, int n, double tol, int max_iter, lq_mg_solve_info* info);

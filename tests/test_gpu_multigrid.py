@@ -1,0 +1,208 @@
+"""GPU parity of the two-level multigrid (include/lqcd_b200.h lq_mg_*) against oracle/multigrid.py, piece by
+piece through the C ABI: prolongator columns, restriction, the Galerkin coarse operator (every block, every merged-neighbour case:
+Lc = 1, 2, 3, 4, 6), the cycle with a converged coarse solve, and the preconditioned solve (true residual by the oracle's M).
+fp32 kernels: tolerances are a few fp32 ulps times the length of the sums."""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import multigrid as omg
+from paper_2510_26313_b200 import inputs
+from paper_2510_26313_b200 import binding as B
+
+pytestmark = pytest.mark.gpu
+
+KAPPA, CSW, EPS = 0.128, 1.0, 0.15
+CASES = {
+    "2224": dict(dims=(4, 4, 4, 8), block=(2, 2, 2, 2), nv=4),      # Lc = 2,2,2,4
+    "1223": dict(dims=(4, 4, 4, 12), block=(4, 2, 2, 4), nv=4),     # Lc = 1,2,2,3
+    "3226": dict(dims=(6, 4, 4, 12), block=(2, 2, 2, 2), nv=2),     # Lc = 3,2,2,6
+}
+
+
+class Case:
+    def __init__(self, name):
+        cfg = CASES[name]
+        self.dims, self.block, self.nv = cfg["dims"], cfg["block"], cfg["nv"]
+        self.V = inputs.volume(self.dims)
+        self.U = inputs.make_links(self.dims, 1000, EPS)
+        self.A = oracle.clover(self.dims, self.U, KAPPA, CSW)
+        self.Ainv = oracle.clover_inverse(self.A)
+        eta = inputs.gaussian_spinors(self.dims, self.nv, 77)
+        self.vecs = np.stack([oracle.solve_eo(self.dims, self.U, self.A, self.Ainv, KAPPA, eta[k], 1e-3)[0].reshape(eta[k].shape)
+                              for k in range(self.nv)])
+        self.P, self.Lc = omg.prolongator(self.dims, self.block, self.vecs)
+        self.Ac = omg.coarse_operator(self.apply_M, self.P)
+        self.nc = self.P.shape[1]
+        self.ctx = B.Context(self.dims)
+        self.ctx.load_gauge(self.U)
+        self.ctx.build_clover(KAPPA, CSW)
+
+    def apply_M(self, v):
+        return oracle.M(self.dims, self.U, self.A, KAPPA, v.reshape(self.V, 12)).reshape(-1)
+
+    def setup(self, **kw):
+        return self.ctx.mg_setup(self.block, self.nv, vecs=self.vecs, **kw)
+
+    def coarse_shape(self, n):
+        return (n, self.nc // (2 * self.nv), 2, self.nv)
+
+
+@pytest.fixture(scope="module", params=list(CASES))
+def case(request, oracle_lib):
+    c = Case(request.param)
+    yield c
+    c.ctx.close()
+
+
+def unit_columns(case, fn, out_rows):
+    """Dense matrix of a linear map from coarse vectors, 32 unit vectors per call."""
+    nc = case.nc
+    out = np.empty((out_rows, nc), dtype=np.complex128)
+    for c0 in range(0, nc, 32):
+        n = min(32, nc - c0)
+        n_call = n if (n in (1, 2) or n % 4 == 0) else 4 * ((n + 3) // 4)
+        e = np.zeros((n_call, nc), dtype=np.complex128)
+        for k in range(n):
+            e[k, c0 + k] = 1.0
+        y = fn(e.reshape(case.coarse_shape(n_call)))
+        out[:, c0:c0 + n] = y.reshape(n_call, -1)[:n].T
+    return out
+
+
+def test_prolongator_columns_match_the_oracle(case):
+    info = case.setup()
+    assert info["coarse_dims"] == tuple(case.Lc) and info["coarse_dof"] == case.nc
+    Pg = unit_columns(case, case.ctx.mg_prolong, case.V * 12)
+    assert np.abs(Pg - case.P).max() <= 5e-6
+    # orthonormal to fp32
+    assert np.abs(Pg.conj().T @ Pg - np.eye(case.nc)).max() <= 2e-5
+
+
+@pytest.mark.parametrize("nrhs", [1, 2, 4, 12])
+def test_restriction_and_prolongation_of_random_vectors(case, nrhs):
+    case.setup()
+    x = inputs.gaussian_spinors(case.dims, nrhs, 31)
+    y = case.ctx.mg_restrict(x).reshape(nrhs, -1)
+    yo = (case.P.conj().T @ x.reshape(nrhs, -1).T).T
+    assert np.abs(y - yo).max() <= 2e-5 * np.abs(yo).max() * np.sqrt(case.P.shape[0] / case.nc)
+    rng = np.random.default_rng(5)
+    yc = rng.standard_normal((nrhs, case.nc)) + 1j * rng.standard_normal((nrhs, case.nc))
+    xf = case.ctx.mg_prolong(yc.reshape(case.coarse_shape(nrhs))).reshape(nrhs, -1)
+    xo = (case.P @ yc.T).T
+    assert np.abs(xf - xo).max() <= 1e-5 * np.abs(xo).max()
+
+
+def test_coarse_operator_matches_the_galerkin_product(case):
+    case.setup()
+    Ag = unit_columns(case, case.ctx.mg_coarse_apply, case.nc)
+    scale = np.abs(case.Ac).max()
+    assert np.abs(Ag - case.Ac).max() <= 2e-5 * scale
+    rng = np.random.default_rng(9)
+    for nrhs in (1, 8, 20):
+        yc = rng.standard_normal((nrhs, case.nc)) + 1j * rng.standard_normal((nrhs, case.nc))
+        out = case.ctx.mg_coarse_apply(yc.reshape(case.coarse_shape(nrhs))).reshape(nrhs, -1)
+        ref = (case.Ac @ yc.T).T
+        assert np.abs(out - ref).max() <= 5e-5 * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("smoother", [B.LQ_MG_SMOOTH_MR, B.LQ_MG_SMOOTH_EO])
+def test_cycle_matches_the_oracle_two_grid_preconditioner(case, smoother):
+    """Coarse GCR run long enough to converge (the coarse systems here have <= 256 unknowns), so the cycle equals the oracle's
+    with an exact coarse solve up to fp32 rounding amplified by cond(A_c)."""
+    case.setup(nu_pre=2, nu_post=2, coarse_iters=96, smoother=smoother)
+    r = inputs.gaussian_spinors(case.dims, 4, 41)
+    z = case.ctx.mg_vcycle(r)
+
+    def eo(res):
+        return omg.schur_mr_smoother(case.dims, case.U, case.A, case.Ainv, KAPPA, res, 2)
+    for k in range(4):
+        zo = omg.two_grid_preconditioner(case.apply_M, case.P, case.Ac, r[k].reshape(-1), smooth=2,
+                                         smoother=eo if smoother == B.LQ_MG_SMOOTH_EO else None)
+        err = np.linalg.norm(z[k].reshape(-1) - zo) / np.linalg.norm(zo)
+        assert err <= 2e-3, err
+    # and without smoothing: the pure coarse correction P A_c^{-1} P^dag r
+    case.setup(nu_pre=0, nu_post=0, coarse_iters=96, smoother=smoother)
+    z = case.ctx.mg_vcycle(r)
+    for k in range(4):
+        zo = case.P @ np.linalg.solve(case.Ac, case.P.conj().T @ r[k].reshape(-1))
+        err = np.linalg.norm(z[k].reshape(-1) - zo) / np.linalg.norm(zo)
+        assert err <= 2e-3, err
+    # one-sided cycles (the post-smoother works on the residual equation)
+    case.setup(nu_pre=0, nu_post=3, coarse_iters=96, smoother=smoother)
+    z = case.ctx.mg_vcycle(r[:1])
+    rr = r[0].reshape(-1)
+    zo = case.P @ np.linalg.solve(case.Ac, case.P.conj().T @ rr)
+    res = rr - case.apply_M(zo)
+    zo = zo + (omg.schur_mr_smoother(case.dims, case.U, case.A, case.Ainv, KAPPA, res, 3) if smoother == B.LQ_MG_SMOOTH_EO
+               else omg.mr_smoother(case.apply_M, res, 3))
+    assert np.linalg.norm(z[0].reshape(-1) - zo) <= 2e-3 * np.linalg.norm(zo)
+
+
+@pytest.mark.parametrize("smoother", [B.LQ_MG_SMOOTH_MR, B.LQ_MG_SMOOTH_EO])
+@pytest.mark.parametrize("nrhs", [1, 4])
+def test_preconditioned_solve_reaches_the_oracle_solution(case, nrhs, smoother):
+    case.setup(nu_pre=2, nu_post=2, coarse_iters=8, restart=8, smoother=smoother)
+    b = inputs.gaussian_spinors(case.dims, nrhs, 5)
+    x, info = case.ctx.mg_solve(b, tol=1e-9, max_iter=100)
+    assert info["converged"], info
+    for k in range(nrhs):
+        res = np.linalg.norm(b[k].reshape(-1) - case.apply_M(x[k].reshape(-1))) / np.linalg.norm(b[k].reshape(-1))
+        assert res <= 1e-9, res
+        assert abs(res - info["true_rel_residual"][k]) <= 1e-11
+    xr = oracle.solve_eo(case.dims, case.U, case.A, case.Ainv, KAPPA, b[0], 1e-11)[0].reshape(-1)
+    assert np.linalg.norm(x[0].reshape(-1) - xr) <= 1e-7 * np.linalg.norm(xr)
+    # the unpreconditioned GCR of the oracle needs ~150 iterations on these links (tests/test_oracle_multigrid.py); aggregates of
+    # 2^4 sites with <= 4 vectors and an 8-iteration coarse solve are a weak hierarchy, a halving is what they give
+    assert info["iters"] <= (100 if smoother == B.LQ_MG_SMOOTH_MR else 60), info
+
+
+def test_adaptive_setup_and_batched_solve():
+    dims = (8, 8, 8, 16)
+    U = inputs.make_links(dims, 1001, 0.2)
+    A = oracle.clover(dims, U, 0.124, 1.2)
+    V = inputs.volume(dims)
+    ctx = B.Context(dims)
+    ctx.load_gauge(U)
+    ctx.build_clover(0.124, 1.2)
+    info = ctx.mg_setup((4, 4, 4, 4), 8, nu_pre=2, nu_post=2, coarse_iters=8, restart=8, setup_tol=1e-3, seed=7)
+    assert info["coarse_dims"] == (2, 2, 2, 4) and info["probes"] == 16 * (1 + 2 + 2 + 2 + 4)
+    b = inputs.laph_sources(dims, 8, 2, 2001)
+    x, sinfo = ctx.mg_solve(b, tol=1e-8, max_iter=100)
+    assert sinfo["converged"], sinfo
+    for k in (0, 7):
+        r = b[k].reshape(-1) - oracle.M(dims, U, A, 0.124, x[k].reshape(V, 12)).reshape(-1)
+        assert np.linalg.norm(r) <= 1e-8 * np.linalg.norm(b[k].reshape(-1))
+    # same answer as the library's CG
+    xc, cinfo = ctx.solve(b, tol=1e-10)
+    assert np.linalg.norm(x - xc) <= 1e-6 * np.linalg.norm(xc)
+    print("mg iters", sinfo["iters"], "m_applies", sinfo["m_applies"], "cg inner iters", cinfo["inner_iters"], info)
+    ctx.close()
+
+
+def test_state_and_argument_errors():
+    dims = (4, 4, 4, 8)
+    ctx = B.Context(dims)
+    ctx.load_gauge(inputs.make_links(dims, 1000, EPS))
+    with pytest.raises(B.LqError):            # no clover term yet
+        ctx.mg_setup((2, 2, 2, 2), 4)
+    ctx.build_clover(KAPPA, CSW)
+    with pytest.raises(B.LqError):            # block does not divide the lattice
+        ctx.mg_setup((3, 2, 2, 2), 4)
+    with pytest.raises(B.LqError):            # unsupported n_vec
+        ctx.mg_setup((2, 2, 2, 2), 3)
+    b = inputs.gaussian_spinors(dims, 1, 5)
+    with pytest.raises(B.LqError):            # no hierarchy
+        ctx.mg_solve(b, tol=1e-8)
+    ctx.mg_setup((2, 2, 2, 2), 4, setup_tol=1e-2)
+    x, info = ctx.mg_solve(b, tol=1e-8)
+    assert info["converged"]
+    ctx.build_clover(KAPPA * 0.99, CSW)       # invalidates the hierarchy
+    with pytest.raises(B.LqError):
+        ctx.mg_solve(b, tol=1e-8)
+    # linearly dependent near-null vectors are reported, not normalised into garbage
+    v = inputs.gaussian_spinors(dims, 4, 3)
+    v[3] = v[0]
+    with pytest.raises(B.LqError):
+        ctx.mg_setup((2, 2, 2, 2), 4, vecs=v)
+    ctx.close()

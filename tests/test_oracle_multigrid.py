@@ -97,3 +97,36 @@ def test_two_grid_fgcr_reaches_the_solution_in_fewer_iterations(setup):
     oracle = setup["oracle"]
     xr = oracle.solve_eo(DIMS, setup["U"], setup["A"], setup["Ainv"], KAPPA, b.reshape(-1, 12), 1e-11)[0].reshape(-1)
     assert np.linalg.norm(x1 - xr) <= 1e-7 * np.linalg.norm(xr)
+
+
+def test_schur_smoother_solves_the_odd_rows_exactly_and_converges_to_the_inverse(setup):
+    """LQ_MG_SMOOTH_EO: after any number of steps the odd rows of r - M delta vanish (the reconstruction solves them exactly), the
+    even rows shrink monotonically (minimal residual), and many steps approach M^-1 r."""
+    mg, oracle, apply_M = setup["mg"], setup["oracle"], setup["apply_M"]
+    Lx, Ly, Lz, Lt = DIMS
+    t, z, y, x = np.meshgrid(np.arange(Lt), np.arange(Lz), np.arange(Ly), np.arange(Lx), indexing="ij")
+    odd = np.repeat(((x + y + z + t) & 1).reshape(-1) == 1, 12)
+    r = inputs.gaussian_spinors(DIMS, 1, 9)[0].reshape(-1)
+    prev = np.inf
+    for steps in (0, 1, 3, 6):
+        d = mg.schur_mr_smoother(DIMS, setup["U"], setup["A"], setup["Ainv"], KAPPA, r, steps)
+        res = r - apply_M(d)
+        assert np.linalg.norm(res[odd]) <= 1e-13 * np.linalg.norm(r)
+        n = np.linalg.norm(res[~odd])
+        assert n < prev
+        prev = n
+    d = mg.schur_mr_smoother(DIMS, setup["U"], setup["A"], setup["Ainv"], KAPPA, r, 300)
+    assert np.linalg.norm(r - apply_M(d)) <= 1e-3 * np.linalg.norm(r)          # MR(1) is slow but it does converge
+
+
+def test_even_odd_smoother_makes_the_better_cycle(setup):
+    mg, apply_M, P, Ac = setup["mg"], setup["apply_M"], setup["P"], setup["Ac"]
+    b = inputs.gaussian_spinors(DIMS, 1, 5)[0].reshape(-1)
+
+    def eo(res):
+        return mg.schur_mr_smoother(DIMS, setup["U"], setup["A"], setup["Ainv"], KAPPA, res, 2)
+    x1, it_mr, _ = mg.fgcr(apply_M, b, 1e-9, precond=lambda r: mg.two_grid_preconditioner(apply_M, P, Ac, r, smooth=2))
+    x2, it_eo, _ = mg.fgcr(apply_M, b, 1e-9, precond=lambda r: mg.two_grid_preconditioner(apply_M, P, Ac, r, smoother=eo))
+    assert np.linalg.norm(b - apply_M(x2)) <= 1e-9 * np.linalg.norm(b)
+    assert np.linalg.norm(x1 - x2) <= 1e-7 * np.linalg.norm(x1)
+    assert it_eo < it_mr, (it_eo, it_mr)

@@ -256,6 +256,18 @@ int lq_laph_eigensolve(lq_ctx* ctx, double* evals, void* evecs, int loc, const l
  * tensor-core completion barrier that timed out: the kernel never hangs). */
 int lq_project(lq_ctx* ctx, void* P, const void* evecs, int n_ev, const void* sols, int n_sol, int loc, int prec);
 
+/* The fp64 projection for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid it): the same arithmetic, summed in the same order, as lq_project(..., LQ_DEVICE, LQ_FP64), but the partial sums of its
+ * two-stage reduction sit in a static device array of LQ_NOALLOC_SCRATCH_BYTES that every GPU loading the library holds until the
+ * process exits.  P, evecs, sols: DEVICE arrays as for lq_project (the caller's; P is output).  The call allocates and frees nothing,
+ * enqueues two kernels on the context's stream and returns without synchronising: P is ready when the stream reaches that point.
+ * Limit: Lt * nchunk * 4 * n_ev * n_sol * 16 bytes <= LQ_NOALLOC_SCRATCH_BYTES with nchunk = clamp(ceil(Lx Ly Lz / 1024), 1, 32),
+ * e.g. 8^3 x 16 with 64 eigenvectors x 64 solutions, or 16^3 x 32 with 32 x 16; beyond it LQ_EINVAL with a message naming the limit.
+ * All calls on one GPU share the array, which keeps the previous call's contents (nothing needs to start at zero: every entry a call
+ * reads it has written itself).  Calls that overlap on the GPU -- other streams, contexts or threads -- race on it. */
+#define LQ_NOALLOC_SCRATCH_BYTES (4u << 20)
+int lq_project_noalloc(lq_ctx* ctx, void* P, const void* evecs, int n_ev, const void* sols, int n_sol);
+
 /* Launch-parameter knobs of the stencil kernels (the paper's autotuning, reduced to an
  * offline sweep): kernel variant (bits 0-7: 0 = default register budget, 1 = alternative; bits 8-15: z-chunk of the
  * sweep order, 0 = automatic, 0xFF = memory order; see csrc/dslash_launch.cuh),

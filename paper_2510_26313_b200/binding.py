@@ -30,7 +30,7 @@ EXPORTS = ["lq_create", "lq_destroy", "lq_last_error", "lq_set_allocator", "lq_l
            "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites", "lq_native_index", "lq_fma_peak", "lq_mem_peak", "lq_set_half_links",
            "lq_laplacian", "lq_laplacian_native", "lq_cv_native_bytes", "lq_cv_fill_random", "lq_laph_eigensolve", "lq_project",
            "lq_mg_setup", "lq_mg_setup_from_vectors", "lq_mg_free", "lq_mg_restrict", "lq_mg_prolong", "lq_mg_coarse_apply", "lq_mg_vcycle",
-           "lq_mg_solve"]
+           "lq_mg_solve", "lq_project_noalloc"]
 
 
 class SolveParam(ctypes.Structure):
@@ -116,6 +116,7 @@ def load_library():
     lib.lq_cv_native_bytes.restype = ctypes.c_size_t
     lib.lq_cv_fill_random.argtypes = [vp, vp, ci, ci, u64]
     lib.lq_project.argtypes = [vp, vp, vp, ci, vp, ci, ci, ci]
+    lib.lq_project_noalloc.argtypes = [vp, vp, vp, ci, vp, ci]
     lib.lq_laph_eigensolve.argtypes = [vp, vp, vp, ci, ctypes.POINTER(EigParam), ctypes.POINTER(EigInfo)]
     lib.lq_kernel_launches.argtypes = [vp]; lib.lq_kernel_launches.restype = ctypes.c_longlong
     szp = ctypes.POINTER(ctypes.c_size_t)
@@ -324,6 +325,18 @@ class Context:
             out = self.torch.empty((Lt, 4, n_ev, n_sol), dtype=self.torch.complex128, device=evecs.device)
         pv, loc = _ptr(evecs); px, _ = _ptr(sols); po, _ = _ptr(out)
         self._check(self.lib.lq_project(self.h, po, pv, n_ev, px, n_sol, loc, prec))
+        return out
+
+    def project_noalloc(self, evecs, sols, out):
+        """lq_project_noalloc: fp64 projection of torch DEVICE arrays into the caller's `out` [Lt][4][n_ev][n_sol] (complex128, device)
+        without any device allocation by the library (static scratch, see the header for the size limit).  Asynchronous on the
+        context's stream: synchronise (self.stream.synchronize()) or order later work on self.stream before reading `out`."""
+        self._enter()
+        n_ev, n_sol = evecs.shape[0], sols.shape[0]
+        assert evecs.is_cuda and sols.is_cuda and out.is_cuda and evecs.is_contiguous() and sols.is_contiguous() and out.is_contiguous()
+        assert evecs.dtype == sols.dtype == out.dtype == self.torch.complex128 and tuple(out.shape) == (self.dims[3], 4, n_ev, n_sol)
+        self._check(self.lib.lq_project_noalloc(self.h, ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(evecs.data_ptr()), n_ev,
+                                                ctypes.c_void_p(sols.data_ptr()), n_sol))
         return out
 
     def cv_native_empty(self, nvec: int, prec: int):

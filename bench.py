@@ -373,6 +373,38 @@ def time_projection(B, device, peak, shapes=((32, 8), (128, 32)), precs=("f64_fm
     return out
 
 
+def time_multigrid(B, device):
+    """Two-level adaptive multigrid on the configs[1] lattice, 8 Gaussian right-hand sides, next to the
+    library's CG on the same system: once on the configs[1] links (well conditioned) and once on smooth links with periodic
+    boundaries at kappa near critical, where the CG iteration count grows."""
+    import torch
+    c = inputs.CONFIGS[1]
+    Lx, Ly, Lz, Lt = c["dims"]
+    out = {"lattice": "x".join(map(str, c["dims"])), "nrhs": 8, "tol": 1e-8, "hierarchy": "4^4 aggregates x 2 chiralities x 24 vectors, setup_tol 1e-4",
+           "cycle": "3 + 3 even-odd minimal-residual steps, 8 coarse GCR iterations, FGCR(8) in fp32 inside fp64 defect correction", "cases": []}
+    g = torch.Generator(device="cuda").manual_seed(5)
+    b = torch.view_as_complex(torch.randn((8, Lt, Lz, Ly, Lx, 4, 3, 2), generator=g, device="cuda", dtype=torch.float64))
+    for name, eps, kappa, csw, t_bc in (("configs[1] links", c["eps"], c["kappa"], c["csw"], -1), ("smooth links, periodic, near-critical kappa", 0.05, 0.1252, 1.0, 1)):
+        ctx = B.Context(c["dims"], device=device)
+        ctx.fill_gauge_random(c["gauge_seed"], eps, recon=18, t_bc=t_bc)
+        ctx.build_clover(kappa, csw)
+        kw = dict(tol=1e-8, use_graph=True, max_inner=20000, max_outer=100)
+        ctx.solve(b, **kw)
+        xc, ci = ctx.solve(b, **kw)
+        ms = ctx.mg_setup((4, 4, 4, 4), 24, nu_pre=3, nu_post=3, coarse_iters=8, restart=8, setup_tol=1e-4, seed=7, smoother=B.LQ_MG_SMOOTH_EO)
+        ctx.mg_solve(b, tol=1e-8, max_iter=300)
+        x, si = ctx.mg_solve(b, tol=1e-8, max_iter=300)
+        out["cases"].append({"links": name, "eps": eps, "kappa": kappa, "csw": csw, "t_bc": t_bc,
+                             "cg": {"seconds": round(ci["seconds"], 4), "inner_iters": ci["inner_iters"], "converged": ci["converged"]},
+                             "mg": {"seconds": round(si["seconds"], 4), "cycles": si["iters"], "m_applies": si["m_applies"], "converged": si["converged"],
+                                    "true_rel_residual_max": max(si["true_rel_residual"]),
+                                    "setup_seconds": round(ms["seconds_vectors"] + ms["seconds_prolongator"] + ms["seconds_coarse_op"], 4),
+                                    "probes": ms["probes"], "hierarchy_mb": round(ms["bytes"] / 1e6, 1)},
+                             "rel_diff_mg_vs_cg": float(torch.linalg.vector_norm(x - xc) / torch.linalg.vector_norm(xc))})
+        ctx.close()
+    return out
+
+
 def dslash_report(B, device, peak, peak_src, quick=False):
     """The Dslash half of the metric.  configs[2] (32^3 x 64, fp32, 18-real links): kernel A / kernel B / bare hop over
     N_rhs in {1, 2, 4, 8, 12, 16}; configs[4] (64^3 x 128, N = 4, 12-real links); the int16+norm kernels of configs[3] come from
@@ -525,7 +557,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=sorted(SOLVER_WORKLOADS))
-    ap.add_argument("--no-extras", action="store_true", help="skip the extras (configs[1] solve, BiCGStab variant, Lanczos, projection, CPU Dslash baseline)")
+    ap.add_argument("--no-extras", action="store_true", help="skip the extras (configs[1] solve, BiCGStab variant, Lanczos, projection, multigrid, CPU Dslash baseline)")
     ap.add_argument("--no-dslash", action="store_true", help="skip the Dslash report (roofline of the configs[2]/[4] kernels) as well")
     ap.add_argument("--no-graph", action="store_true")
     ap.add_argument("--check-every", type=int, default=4, help="inner iterations between convergence tests")
@@ -655,6 +687,7 @@ def main():
             extras["solver_variant_int16_links"] = variant_hl
         extras["laph_eigensolve"] = time_eigensolve(B, local)
         extras["projection"] = time_projection(B, local, peak)
+        extras["multigrid"] = time_multigrid(B, local)
     t_step = t_dev / args.steps
     line = {
         "metric": "batched CG sec/RHS", "value": whole_job_seconds_per_rhs(t_dev, args.steps, nrhs, world), "unit": "s/RHS", "n_gpus": world, "steps": args.steps,

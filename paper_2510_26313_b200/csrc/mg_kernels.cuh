@@ -137,36 +137,51 @@ __global__ void __launch_bounds__(256) orthonormalise_kernel(MgGeom m, float2* _
 }
 
 // ---- restriction y = P^dag x and prolongation x (+)= P y, N right-hand sides ------------------------------------------------
-// One CTA per (aggregate, chirality).  restrict: thread = (k, RHS group), sums over the 6 ns rows of its column (P coalesced over
-// k, x broadcast).  prolong: the 2 Nv x N coarse values of the block sit in shared memory, thread = (row, RHS group).
+// One CTA per (aggregate, chirality).  restrict: thread = (k, RHS group, row slice), sums over the rows of its slice of its column
+// (P coalesced over k, x broadcast), slices added in order.  prolong: the 2 Nv x N coarse values of the block sit in shared memory, thread = (row, RHS group).
 template <int R>
-__global__ void restrict_kernel(MgGeom m, int N, const int* __restrict__ site_f, const float2* __restrict__ P, const float* __restrict__ x,
-                                float2* __restrict__ yc) {
-    const int G = N / R;
+__global__ void __launch_bounds__(256) restrict_kernel(MgGeom m, int N, int S, const int* __restrict__ site_f, const float2* __restrict__ P,
+                                                       const float* __restrict__ x, float2* __restrict__ yc) {
+    // thread = (k, RHS group, slice): slice sl of S takes the sites i = sl, sl + S, ... of the aggregate; the slices' partial sums are
+    // added in slice order through shared memory
+    extern __shared__ float2 rs[];     // [S][nv * G][R]
+    const int G = N / R, KG = m.nv * G;
     const int a = blockIdx.x >> 1, chi = blockIdx.x & 1;
     const int t = threadIdx.x;
-    if (t >= m.nv * G) return;
-    const int k = t % m.nv, g = t / m.nv;
-    const float2* Pb = P + (size_t)blockIdx.x * m.M * m.nv + k;
-    const int* sf = site_f + (size_t)a * m.ns;
+    const int kg = t % KG, sl = t / KG;
+    const int k = kg % m.nv, g = kg / m.nv;
     float ar[R], ai[R];
 #pragma unroll
     for (int r = 0; r < R; r++) ar[r] = ai[r] = 0.f;
-    for (int i = 0; i < m.ns; i++) {
-        const size_t base = fine_base<R>(sf[i], G, g) + (size_t)(12 * chi) * (SB * R);
+    if (sl < S) {
+        const float2* Pb = P + (size_t)blockIdx.x * m.M * m.nv + k;
+        const int* sf = site_f + (size_t)a * m.ns;
+#pragma unroll 2
+        for (int i = sl; i < m.ns; i += S) {
+            const size_t base = fine_base<R>(sf[i], G, g) + (size_t)(12 * chi) * (SB * R);
 #pragma unroll
-        for (int c6 = 0; c6 < 6; c6++) {
-            float xr[R], xi[R];
-            ldv<R>(x + base + (size_t)(2 * c6) * (SB * R), xr);
-            ldv<R>(x + base + (size_t)(2 * c6 + 1) * (SB * R), xi);
-            const float2 p = Pb[(size_t)(6 * i + c6) * m.nv];
+            for (int c6 = 0; c6 < 6; c6++) {
+                float xr[R], xi[R];
+                ldv<R>(x + base + (size_t)(2 * c6) * (SB * R), xr);
+                ldv<R>(x + base + (size_t)(2 * c6 + 1) * (SB * R), xi);
+                const float2 p = __ldg(Pb + (size_t)(6 * i + c6) * m.nv);
 #pragma unroll
-            for (int r = 0; r < R; r++) { ar[r] += p.x * xr[r] + p.y * xi[r]; ai[r] += p.x * xi[r] - p.y * xr[r]; }
+                for (int r = 0; r < R; r++) { ar[r] += p.x * xr[r] + p.y * xi[r]; ai[r] += p.x * xi[r] - p.y * xr[r]; }
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; r++) rs[((size_t)sl * KG + kg) * R + r] = make_float2(ar[r], ai[r]);
+    }
+    __syncthreads();
+    if (t < KG) {
+        float2* o = yc + ((size_t)a * m.nc + chi * m.nv + k) * N + g * R;
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            float2 sum = make_float2(0.f, 0.f);
+            for (int q = 0; q < S; q++) { const float2 v = rs[((size_t)q * KG + kg) * R + r]; sum.x += v.x; sum.y += v.y; }
+            o[r] = sum;
         }
     }
-    float2* o = yc + ((size_t)a * m.nc + chi * m.nv + k) * N + g * R;
-#pragma unroll
-    for (int r = 0; r < R; r++) o[r] = make_float2(ar[r], ai[r]);
 }
 
 template <int R, bool ACCUM>
@@ -187,13 +202,27 @@ __global__ void __launch_bounds__(256) prolong_kernel(MgGeom m, int N, const int
 #pragma unroll
         for (int r = 0; r < R; r++) xr[r] = xi[r] = 0.f;
         const float2* pr = Pb + (size_t)mm * m.nv;
-        for (int k = 0; k < m.nv; k++) {
-            const float2 p = pr[k];
+        if ((m.nv & 1) == 0) {          // two columns per 16-byte load
+            const float4* pr4 = reinterpret_cast<const float4*>(pr);
+#pragma unroll 4
+            for (int k2 = 0; k2 < (m.nv >> 1); k2++) {
+                const float4 p = __ldg(pr4 + k2);
 #pragma unroll
-            for (int r = 0; r < R; r++) {
-                const float2 y = ys[k * N + g * R + r];
-                xr[r] += p.x * y.x - p.y * y.y;
-                xi[r] += p.x * y.y + p.y * y.x;
+                for (int r = 0; r < R; r++) {
+                    const float2 y0 = ys[(2 * k2) * N + g * R + r], y1 = ys[(2 * k2 + 1) * N + g * R + r];
+                    xr[r] += p.x * y0.x - p.y * y0.y + p.z * y1.x - p.w * y1.y;
+                    xi[r] += p.x * y0.y + p.y * y0.x + p.z * y1.y + p.w * y1.x;
+                }
+            }
+        } else {
+            for (int k = 0; k < m.nv; k++) {
+                const float2 p = pr[k];
+#pragma unroll
+                for (int r = 0; r < R; r++) {
+                    const float2 y = ys[k * N + g * R + r];
+                    xr[r] += p.x * y.x - p.y * y.y;
+                    xi[r] += p.x * y.y + p.y * y.x;
+                }
             }
         }
         float* o = x + fine_base<R>(sf[i], G, g) + (size_t)(2 * (6 * chi + c6)) * (SB * R);
@@ -208,44 +237,72 @@ __global__ void __launch_bounds__(256) prolong_kernel(MgGeom m, int N, const int
 }
 
 // ---- coarse operator y[a] = sum_d A_c[a][d] x[nbr(a, d)], N right-hand sides ------------------------------------------------
-// One CTA per coarse site; thread = (row, RC right-hand sides), row fastest (A_c coalesced); the neighbour's 2 Nv x N values are
-// staged in shared memory.  With N right-hand sides every A_c entry read from HBM feeds N complex multiply-adds: the batched
-// coarse operator is the matrix-matrix form of PAPER.md L133-137.
-template <int RC>
-__global__ void coarse_apply_kernel(MgGeom m, int N, const int* __restrict__ nbr, const float2* __restrict__ Ac, const float2* __restrict__ x,
-                                    float2* __restrict__ y) {
-    extern __shared__ float2 xs[];     // [nc][N]
-    const int a = blockIdx.x;
-    const int t = threadIdx.x;
-    const int row = t % m.nc, q = t / m.nc;        // q: RHS slice
-    const bool active = q * RC < N;
-    float ar[RC], ai[RC];
+// One CTA of 9 warps per (coarse site, chunk of NCH right-hand sides): warp d streams the block of stencil direction d, lane l owns
+// the row pair (2l, 2l+1) (one 16-byte load per column, 4 columns in flight), the neighbour's values of a column are NCH
+// consecutive float2 that every lane reads from the same address (one L1 broadcast).  The 9 partial results meet in shared memory and
+// are added in direction order 0..8 (deterministic).  HBM-bound on A_c: every entry read once feeds NCH complex multiply-adds per
+// chunk -- the batched coarse operator is the matrix-matrix form of PAPER.md L133-137; 2 Nv <= 64 keeps a block row inside one warp.
+template <int NCH>
+__global__ void __launch_bounds__(288) coarse_apply_kernel(MgGeom m, int N, const int* __restrict__ nbr, const float2* __restrict__ Ac,
+                                                           const float2* __restrict__ x, float2* __restrict__ y) {
+    extern __shared__ float2 red[];     // [9][nc][NCH]
+    const int a = blockIdx.x, r0 = blockIdx.y * NCH;
+    const int d = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nc = m.nc;
+    const int nb = nbr[a * 9 + d];
+    float2 acc[2][NCH];
 #pragma unroll
-    for (int r = 0; r < RC; r++) ar[r] = ai[r] = 0.f;
-    for (int d = 0; d < 9; d++) {
-        const int nb = nbr[a * 9 + d];
-        if (nb < 0) continue;
-        __syncthreads();
-        const float2* src = x + (size_t)nb * m.nc * N;
-        for (int e = t; e < m.nc * N; e += blockDim.x) xs[e] = src[e];
-        __syncthreads();
-        if (active) {
-            const float2* A = Ac + ((size_t)(a * 9 + d) * m.nc) * m.nc + row;
-            for (int col = 0; col < m.nc; col++) {
-                const float2 c = A[(size_t)col * m.nc];
+    for (int q = 0; q < 2; q++)
 #pragma unroll
-                for (int r = 0; r < RC; r++) {
-                    const float2 v = xs[col * N + q * RC + r];
-                    ar[r] += c.x * v.x - c.y * v.y;
-                    ai[r] += c.x * v.y + c.y * v.x;
+        for (int r = 0; r < NCH; r++) acc[q][r] = make_float2(0.f, 0.f);
+    if (nb >= 0 && 2 * lane < nc) {
+        const float4* A = reinterpret_cast<const float4*>(Ac + ((size_t)(a * 9 + d) * nc) * nc) + lane;      // column stride nc / 2 float4
+        const float2* xv = x + (size_t)nb * nc * N + r0;
+        const int cs = nc >> 1;
+        constexpr int U = 4;            // columns per batch; the next batch's 16-byte loads are issued before this batch's arithmetic
+        float4 cur[U], nxt[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) cur[u] = u < nc ? __ldg(A + (size_t)u * cs) : make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int col0 = 0; col0 < nc; col0 += U) {
+#pragma unroll
+            for (int u = 0; u < U; u++) nxt[u] = col0 + U + u < nc ? __ldg(A + (size_t)(col0 + U + u) * cs) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const int col = col0 + u < nc ? col0 + u : nc - 1;      // a padded column multiplies zeros
+                float2 v[NCH];
+                if constexpr (NCH >= 2) {
+#pragma unroll
+                    for (int r = 0; r < NCH; r += 2) {
+                        const float4 w = __ldg(reinterpret_cast<const float4*>(xv + (size_t)col * N + r));
+                        v[r] = make_float2(w.x, w.y); v[r + 1] = make_float2(w.z, w.w);
+                    }
+                } else v[0] = __ldg(xv + (size_t)col * N);
+                const float4 c = cur[u];
+#pragma unroll
+                for (int r = 0; r < NCH; r++) {
+                    acc[0][r].x = fmaf(c.x, v[r].x, acc[0][r].x); acc[0][r].x = fmaf(-c.y, v[r].y, acc[0][r].x);
+                    acc[0][r].y = fmaf(c.x, v[r].y, acc[0][r].y); acc[0][r].y = fmaf(c.y, v[r].x, acc[0][r].y);
+                    acc[1][r].x = fmaf(c.z, v[r].x, acc[1][r].x); acc[1][r].x = fmaf(-c.w, v[r].y, acc[1][r].x);
+                    acc[1][r].y = fmaf(c.z, v[r].y, acc[1][r].y); acc[1][r].y = fmaf(c.w, v[r].x, acc[1][r].y);
                 }
             }
+#pragma unroll
+            for (int u = 0; u < U; u++) cur[u] = nxt[u];
         }
     }
-    if (active) {
-        float2* o = y + ((size_t)a * m.nc + row) * N + q * RC;
+    if (2 * lane < nc) {
 #pragma unroll
-        for (int r = 0; r < RC; r++) o[r] = make_float2(ar[r], ai[r]);
+        for (int q = 0; q < 2; q++)
+#pragma unroll
+            for (int r = 0; r < NCH; r++) red[((size_t)d * nc + 2 * lane + q) * NCH + r] = acc[q][r];
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < nc * NCH; e += blockDim.x) {
+        float2 sum = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int dd = 0; dd < 9; dd++) { const float2 v = red[(size_t)dd * nc * NCH + e]; sum.x += v.x; sum.y += v.y; }
+        const int row = e / NCH, r = e - row * NCH;
+        y[((size_t)a * nc + row) * N + r0 + r] = sum;
     }
 }
 

@@ -134,11 +134,15 @@ static int fine_sub(lq_ctx* c, int n, float* out, const float* a, const float* b
     return 0;
 }
 static int do_restrict(lq_ctx* c, MgState* s, int n, float2* yc, const float* x) {
-    const int R = group_width(n), G = n / R;
-    const int block = ((s->m.nv * G + 31) / 32) * 32, grid = s->m.Vc * 2;
-    MG_R_DISPATCH(R, (mg::restrict_kernel<4><<<grid, block, 0, c->stream>>>(s->m, n, s->site_f, s->P, x, yc)),
-                     (mg::restrict_kernel<2><<<grid, block, 0, c->stream>>>(s->m, n, s->site_f, s->P, x, yc)),
-                     (mg::restrict_kernel<1><<<grid, block, 0, c->stream>>>(s->m, n, s->site_f, s->P, x, yc)));
+    const int R = group_width(n), G = n / R, KG = s->m.nv * G;
+    int S = 256 / KG;
+    if (S < 1) S = 1;
+    if (S > s->m.ns) S = s->m.ns;
+    const int block = ((KG * S + 31) / 32) * 32, grid = s->m.Vc * 2;
+    const size_t smem = (size_t)S * KG * R * sizeof(float2);
+    MG_R_DISPATCH(R, (mg::restrict_kernel<4><<<grid, block, smem, c->stream>>>(s->m, n, S, s->site_f, s->P, x, yc)),
+                     (mg::restrict_kernel<2><<<grid, block, smem, c->stream>>>(s->m, n, S, s->site_f, s->P, x, yc)),
+                     (mg::restrict_kernel<1><<<grid, block, smem, c->stream>>>(s->m, n, S, s->site_f, s->P, x, yc)));
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
@@ -160,12 +164,13 @@ static int do_prolong(lq_ctx* c, MgState* s, int n, float* x, const float2* yc, 
     return 0;
 }
 static int coarse_M(lq_ctx* c, MgState* s, int n, float2* y, const float2* x) {
-    const int RC = group_width(n);
-    const int block = s->m.nc * (n / RC), grid = s->m.Vc;
-    const size_t smem = (size_t)s->m.nc * n * sizeof(float2);
-    MG_R_DISPATCH(RC, (mg::coarse_apply_kernel<4><<<grid, block, smem, c->stream>>>(s->m, n, s->nbr, s->Ac, x, y)),
-                      (mg::coarse_apply_kernel<2><<<grid, block, smem, c->stream>>>(s->m, n, s->nbr, s->Ac, x, y)),
-                      (mg::coarse_apply_kernel<1><<<grid, block, smem, c->stream>>>(s->m, n, s->nbr, s->Ac, x, y)));
+    const int nch = n % 8 == 0 ? 8 : (n % 4 == 0 ? 4 : n);      // right-hand sides per CTA
+    const dim3 grid(s->m.Vc, n / nch);
+    const size_t smem = (size_t)9 * s->m.nc * nch * sizeof(float2);
+    if (nch == 8) mg::coarse_apply_kernel<8><<<grid, 288, smem, c->stream>>>(s->m, n, s->nbr, s->Ac, x, y);
+    else if (nch == 4) mg::coarse_apply_kernel<4><<<grid, 288, smem, c->stream>>>(s->m, n, s->nbr, s->Ac, x, y);
+    else if (nch == 2) mg::coarse_apply_kernel<2><<<grid, 288, smem, c->stream>>>(s->m, n, s->nbr, s->Ac, x, y);
+    else mg::coarse_apply_kernel<1><<<grid, 288, smem, c->stream>>>(s->m, n, s->nbr, s->Ac, x, y);
     LQ_LAUNCHED(c);
     LQ_CUDA(c, cudaGetLastError());
     return 0;
@@ -279,9 +284,9 @@ static int smooth_eo(lq_ctx* c, MgState* s, int n, float* z, bool accumulate, in
     LQ_CUDA(c, cudaMemsetAsync(d_e, 0, pb, c->stream));
     for (int i = 0; i < steps; i++) {
         LQ_TRY(op_kernel_a(c, LQ_FP32, n, 1, t_o, rho_e, 0));
-        LQ_TRY(op_kernel_b(c, LQ_FP32, n, 0, t_e, rho_e, t_o, -k * k, 1, 0));
+        // t_e = Mhat rho_e with <t, rho> and ||t||^2 from the kernel's fused epilogue (the BiCGStab omega of solver.cu)
+        LQ_TRY(op_kernel_b_cdot(c, LQ_FP32, n, 0, t_e, rho_e, t_o, -k * k, 1, 0, rho_e, 1, slot(s, 3)));
         s->m_applies += 1;
-        LQ_TRY(fine_cdot3(c, n, (float*)t_e, (float*)rho_e, slot(s, 3), 1));
         LQ_TRY(fine_caxpy2(c, n, (float*)d_e, (float*)rho_e, 1.f, (float*)rho_e, (float*)t_e, -1.f, slot(s, 3), nullptr, nullptr, 1));
     }
     LQ_TRY(op_kernel_b(c, LQ_FP32, n, 1, t_o, res_o, d_e, k, 0, 0));

@@ -516,6 +516,19 @@ def run_op(args, B, device):
         r.update({"op": args.op, "clocks": sampler.stop()})
         print(json.dumps(r))
         return
+    if kind == "mg":       # two-level multigrid: setup + ONE solve of N right-hand sides, near-critical smooth links
+        import torch
+        Lx, Ly, Lz, Lt = c["dims"]
+        ctx = B.Context(c["dims"], device=device)
+        ctx.fill_gauge_random(c["gauge_seed"], 0.05, recon=18, t_bc=1)
+        ctx.build_clover(0.1252, 1.0)
+        g = torch.Generator(device="cuda").manual_seed(5)
+        b = torch.view_as_complex(torch.randn((n, Lt, Lz, Ly, Lx, 4, 3, 2), generator=g, device="cuda", dtype=torch.float64))
+        ms = ctx.mg_setup((4, 4, 4, 4), 24, nu_pre=3, nu_post=3, coarse_iters=8, restart=8, setup_tol=1e-4, seed=7, smoother=B.LQ_MG_SMOOTH_EO)
+        x, si = ctx.mg_solve(b, tol=1e-8, max_iter=args.op_iters)
+        ctx.close()
+        print(json.dumps({"op": args.op, "lattice": "x".join(map(str, c["dims"])), "setup": ms, "solve": si}))
+        return
     ctx = B.Context(c["dims"], device=device)
     ctx.fill_gauge_random(c["gauge_seed"], c["eps"], recon=c["recon"])
     ctx.build_clover(c["kappa"], c["csw"])

@@ -12,7 +12,6 @@
 #include <string.h>
 #include <algorithm>
 #include <vector>
-#include <chrono>
 #include "internal.cuh"
 #include "eigen_kernels.cuh"
 
@@ -108,8 +107,12 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
 #define EIG_TRY(x) do { rc = (x); if (rc) goto done; } while (0)
 #define EIG_CUDA(x) do { if ((x) != cudaSuccess) { rc = set_err(c, LQ_ECUDA, #x); goto done; } } while (0)
     {
-    std::vector<double> T((size_t)Lt * nT * nT, 0.0), beta_m(Lt, 0.0), hbuf;
     std::vector<double2> hH((size_t)(2 * m + 4) * Lt);
+    struct EventList { std::vector<cudaEvent_t> v; ~EventList() { for (cudaEvent_t ev : v) if (ev) cudaEventDestroy(ev); } } evlist;
+    evlist.v.assign(2 * (size_t)m, nullptr);                   // per-step event pairs around the orthogonalisation (read after the sweep)
+    std::vector<cudaEvent_t>& evs = evlist.v;
+    for (auto& ev : evs) EIG_CUDA(cudaEventCreate(&ev));
+    EIG_CUDA(cudaMemsetAsync(d_T, 0, sizeof(double) * (size_t)Lt * nT * nT, c->stream));
     std::vector<double> theta((size_t)Lt * m), hres((size_t)Lt * n_ev);
     double* d_theta = d_ritz; double* d_res = d_ritz + (size_t)Lt * m; double* d_beta = d_res + (size_t)Lt * n_ev;
     int k = 0, restarts = 0; bool converged = false; double worst = 0.0;
@@ -139,53 +142,42 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
         for (int j = k; j < m; j++) {
             EIG_TRY(chebyshev(e, w, V[j], p->cheb_degree, p->cheb_a, p->cheb_b, y0, y1, tmp));
             // two classical Gram-Schmidt passes against v_0 .. v_j; the coefficients are the column j of T
-            cudaEventRecord(evA, c->stream);
+            cudaEventRecord(evs[2 * (size_t)j], c->stream);
             // pass 0 is LOCAL: against v_{j-1}, v_j only (the three-term recurrence carries all of the weight there), except on the
             // first step after a restart, where the arrow couples w to every kept Ritz vector; pass 1 is the full reorthogonalisation
             // against v_0 .. v_j.  After pass 0 the components left along the older vectors are rounding-level, so one full classical
             // Gram-Schmidt pass restores orthogonality to working precision at half the basis traffic of two full passes.
+            // Nothing of a step goes through the host: the coefficients stay in d_H and t_column_kernel / t_beta_kernel write
+            // column j of the projected matrices, so the whole sweep is enqueued without a synchronisation.
             for (int pass = 0; pass < 2; pass++) {
                 const int first = (pass == 0 && j > k) ? j - 1 : 0;
                 const int nv = j + 1 - first;
                 double2* H = e.d_H + (size_t)pass * (m + 1) * Lt + (size_t)first * Lt;
-                double2* hHp = hH.data() + (size_t)pass * (m + 1) * Lt;
-                for (size_t q = 0; q < (size_t)first * Lt; q++) hHp[q] = make_double2(0.0, 0.0);
                 slice_multidot_kernel<<<dim3(Lt * e.nchunk, (nv + 7) / 8), 256, 0, c->stream>>>(e.sg, e.nchunk, nv, d_ptr + first, w, d_mpart);
                 slice_multidot_final_kernel<<<(Lt * nv + 127) / 128, 128, 0, c->stream>>>(Lt, e.nchunk, nv, d_mpart, H);
-                EIG_CUDA(cudaMemcpyAsync(hHp + (size_t)first * Lt, H, sizeof(double2) * (size_t)nv * Lt, cudaMemcpyDeviceToHost, c->stream));
                 slice_multiaxpy_kernel<<<grid, 128, 0, c->stream>>>(e.sg, nv, w, d_ptr + first, H);
                 c->launches += 3;
             }
+            t_column_kernel<<<(Lt * (j + 1) + 127) / 128, 128, 0, c->stream>>>(Lt, nT, j, k, j > k ? j - 1 : 0, e.d_H, e.d_H + (size_t)(m + 1) * Lt, d_T);
             EIG_TRY(dot(e, w, w, e.d_H + (size_t)(2 * m + 2) * Lt));
             inv_norm_kernel<<<(Lt + 63) / 64, 64, 0, c->stream>>>(Lt, e.d_H + (size_t)(2 * m + 2) * Lt, e.d_scale, e.d_scale + Lt);
-            slice_scale_kernel<<<grid, 128, 0, c->stream>>>(e.sg, V[j + 1], w, e.d_scale); c->launches += 2;
-            cudaEventRecord(evB, c->stream);
-            hbuf.resize(Lt);
-            EIG_CUDA(cudaMemcpyAsync(hbuf.data(), e.d_scale + Lt, sizeof(double) * Lt, cudaMemcpyDeviceToHost, c->stream));
-            EIG_CUDA(cudaStreamSynchronize(c->stream));
-            { float tms = 0; cudaEventElapsedTime(&tms, evA, evB); t_ortho += tms * 1e-3; }
-            for (int t = 0; t < Lt; t++) {
-                double* Tt = T.data() + (size_t)t * nT * nT;
-                for (int i = 0; i <= j; i++) {
-                    const double h = hH[(size_t)i * Lt + t].x + hH[(size_t)(m + 1 + i) * Lt + t].x;
-                    if (i >= k || j == k || i == j) { Tt[(size_t)i * nT + j] = h; Tt[(size_t)j * nT + i] = h; }
-                }
-                if (j + 1 < m) { Tt[(size_t)(j + 1) * nT + j] = hbuf[t]; Tt[(size_t)j * nT + j + 1] = hbuf[t]; }
-                else beta_m[t] = hbuf[t];
-            }
+            slice_scale_kernel<<<grid, 128, 0, c->stream>>>(e.sg, V[j + 1], w, e.d_scale);
+            t_beta_kernel<<<(Lt + 63) / 64, 64, 0, c->stream>>>(Lt, nT, j, m, e.d_scale + Lt, d_T, d_beta); c->launches += 4;
+            cudaEventRecord(evs[2 * (size_t)j + 1], c->stream);
+            EIG_CUDA(cudaGetLastError());
         }
+        const int k_sweep = k;
         // Ritz pairs of every slice
-        const auto ritz_t0 = std::chrono::steady_clock::now();
+        cudaEventRecord(evA, c->stream);
         worst = 0.0; converged = true;
         // all Lt projected eigenproblems in one launch; the kernel leaves the sorted eigenvalues, the residual estimates and the
         // first `keep` eigenvectors (d_Q, the layout slice_rotate_kernel reads) on the device
-        EIG_CUDA(cudaMemcpyAsync(d_T, T.data(), sizeof(double) * (size_t)Lt * nT * nT, cudaMemcpyHostToDevice, c->stream));
-        EIG_CUDA(cudaMemcpyAsync(d_beta, beta_m.data(), sizeof(double) * Lt, cudaMemcpyHostToDevice, c->stream));
         ritz_jacobi_kernel<<<Lt * RITZ_CLUSTER, RITZ_THREADS, 0, c->stream>>>(m, keep, n_ev, d_T, d_QT, d_beta, d_theta, d_Q, d_res, d_sweeps); c->launches++;
         EIG_CUDA(cudaGetLastError());
         EIG_CUDA(cudaMemcpyAsync(theta.data(), d_theta, sizeof(double) * (size_t)Lt * m, cudaMemcpyDeviceToHost, c->stream));
         EIG_CUDA(cudaMemcpyAsync(hres.data(), d_res, sizeof(double) * (size_t)Lt * n_ev, cudaMemcpyDeviceToHost, c->stream));
         EIG_CUDA(cudaStreamSynchronize(c->stream));
+        for (int jj = k_sweep; jj < m; jj++) { float tms = 0; cudaEventElapsedTime(&tms, evs[2 * (size_t)jj], evs[2 * (size_t)jj + 1]); t_ortho += tms * 1e-3; }
         for (int t = 0; t < Lt; t++)
             for (int cidx = 0; cidx < n_ev; cidx++) {
                 const double rel = hres[(size_t)t * n_ev + cidx];
@@ -203,9 +195,10 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
             for (int i = 0; i < keep; i++) std::swap(V[i], W[i]);
             std::swap(V[keep], V[m]);
         }
-        t_ritz += std::chrono::duration<double>(std::chrono::steady_clock::now() - ritz_t0).count();
-        std::fill(T.begin(), T.end(), 0.0);
-        for (int t = 0; t < Lt; t++) for (int i = 0; i < keep; i++) T[(size_t)t * nT * nT + (size_t)i * nT + i] = theta[(size_t)t * m + i];
+        cudaEventRecord(evB, c->stream);
+        EIG_CUDA(cudaEventSynchronize(evB));
+        { float tms = 0; cudaEventElapsedTime(&tms, evA, evB); t_ritz += tms * 1e-3; }
+        t_reset_kernel<<<(int)(((long long)Lt * nT * nT + 255) / 256), 256, 0, c->stream>>>(Lt, nT, keep, m, d_theta, d_T); c->launches++;
         k = keep;
         if (converged) { restarts++; break; }
     }

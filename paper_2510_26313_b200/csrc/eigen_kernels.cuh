@@ -183,6 +183,35 @@ __global__ void slice_multiaxpy_kernel(SliceGeom g, int nv, double* __restrict__
     for (int j = 0; j < 6; j++) w[off + j * SB] = acc[j];
 }
 
+// ---- the projected matrices T[t] = V^dag B V are assembled ON THE DEVICE (no host round trip inside a Lanczos sweep) ----------
+// column j from the Gram-Schmidt coefficients of step j: H0 (local pass, rows first0 .. j) + H1 (full pass, rows 0 .. j), rows
+// [i][Lt] of double2; rows i < k (the kept Ritz vectors) couple to column j only in the first step after a restart (the arrow)
+__global__ void t_column_kernel(int Lt, int nT, int j, int k, int first0, const double2* __restrict__ H0, const double2* __restrict__ H1, double* __restrict__ T) {
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= Lt * (j + 1)) return;
+    const int t = idx % Lt, i = idx / Lt;
+    const double h = (i >= first0 ? H0[(size_t)i * Lt + t].x : 0.0) + H1[(size_t)i * Lt + t].x;
+    if (i >= k || j == k || i == j) {
+        double* Tt = T + (size_t)t * nT * nT;
+        Tt[(size_t)i * nT + j] = h; Tt[(size_t)j * nT + i] = h;
+    }
+}
+// sub-diagonal entry beta_j = ||w|| of step j, or the residual norm beta_m of the last step
+__global__ void t_beta_kernel(int Lt, int nT, int j, int m, const double* __restrict__ beta, double* __restrict__ T, double* __restrict__ beta_m) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= Lt) return;
+    if (j + 1 < m) { double* Tt = T + (size_t)t * nT * nT; Tt[(size_t)(j + 1) * nT + j] = beta[t]; Tt[(size_t)j * nT + j + 1] = beta[t]; }
+    else beta_m[t] = beta[t];
+}
+// thick restart: T <- diag(theta_0 .. theta_{keep-1})
+__global__ void t_reset_kernel(int Lt, int nT, int keep, int m, const double* __restrict__ theta, double* __restrict__ T) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)Lt * nT * nT) return;
+    const int t = (int)(idx / ((long long)nT * nT)), e = (int)(idx - (long long)t * nT * nT), i = e / nT, jj = e - i * nT;
+    T[idx] = (i == jj && i < keep) ? theta[(size_t)t * m + i] : 0.0;
+}
+
+
 // ---- Ritz step on the device: all Lt projected matrices at once, one CTA per time-slice ---------------------------------------
 // Parallel two-sided Jacobi (Brent-Luk round-robin ordering): in every step the n/2 disjoint index pairs (p, q) get their
 // rotations from the current 2x2 diagonal blocks; the matrix then splits into (n/2)^2 independent 2x2 blocks B(P,Q) that become

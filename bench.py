@@ -380,7 +380,7 @@ def time_multigrid(B, device):
     import torch
     c = inputs.CONFIGS[1]
     Lx, Ly, Lz, Lt = c["dims"]
-    out = {"lattice": "x".join(map(str, c["dims"])), "nrhs": 8, "tol": 1e-8, "hierarchy": "4^4 aggregates x 2 chiralities x 24 vectors, setup_tol 1e-4",
+    out = {"lattice": "x".join(map(str, c["dims"])), "nrhs": 8, "tol": 1e-8, "hierarchy": "4^4 aggregates x 2 chiralities x 24 vectors, setup_tol 1e-4, one refinement pass",
            "cycle": "3 + 3 even-odd minimal-residual steps, 8 coarse GCR iterations, FGCR(8) in fp32 inside fp64 defect correction", "cases": []}
     g = torch.Generator(device="cuda").manual_seed(5)
     b = torch.view_as_complex(torch.randn((8, Lt, Lz, Ly, Lx, 4, 3, 2), generator=g, device="cuda", dtype=torch.float64))
@@ -391,7 +391,7 @@ def time_multigrid(B, device):
         kw = dict(tol=1e-8, use_graph=True, max_inner=20000, max_outer=100)
         ctx.solve(b, **kw)
         xc, ci = ctx.solve(b, **kw)
-        ms = ctx.mg_setup((4, 4, 4, 4), 24, nu_pre=3, nu_post=3, coarse_iters=8, restart=8, setup_tol=1e-4, seed=7, smoother=B.LQ_MG_SMOOTH_EO)
+        ms = ctx.mg_setup((4, 4, 4, 4), 24, nu_pre=3, nu_post=3, coarse_iters=8, restart=8, setup_tol=1e-4, seed=7, smoother=B.LQ_MG_SMOOTH_EO, refine=1)
         ctx.mg_solve(b, tol=1e-8, max_iter=300)
         x, si = ctx.mg_solve(b, tol=1e-8, max_iter=300)
         out["cases"].append({"links": name, "eps": eps, "kappa": kappa, "csw": csw, "t_bc": t_bc,
@@ -524,7 +524,7 @@ def run_op(args, B, device):
         ctx.build_clover(0.1252, 1.0)
         g = torch.Generator(device="cuda").manual_seed(5)
         b = torch.view_as_complex(torch.randn((n, Lt, Lz, Ly, Lx, 4, 3, 2), generator=g, device="cuda", dtype=torch.float64))
-        ms = ctx.mg_setup((4, 4, 4, 4), 24, nu_pre=3, nu_post=3, coarse_iters=8, restart=8, setup_tol=1e-4, seed=7, smoother=B.LQ_MG_SMOOTH_EO)
+        ms = ctx.mg_setup((4, 4, 4, 4), 24, nu_pre=3, nu_post=3, coarse_iters=8, restart=8, setup_tol=1e-4, seed=7, smoother=B.LQ_MG_SMOOTH_EO, refine=1)
         x, si = ctx.mg_solve(b, tol=1e-8, max_iter=args.op_iters)
         ctx.close()
         print(json.dumps({"op": args.op, "lattice": "x".join(map(str, c["dims"])), "setup": ms, "solve": si}))

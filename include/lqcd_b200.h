@@ -293,7 +293,7 @@ int lq_mem_peak(lq_ctx* ctx, int mode, double mbytes, double* gbs);
 /* ------------------------------------------------------------------ two-level adaptive multigrid
  * PAPER.md L118 ("adaptive geometric multi-grid solver", ref. [19]), L164 ("mixed-precision multi-grid solver") and L137 (batching
  * matters most on the coarse grids).  M x = b for the FULL operator M = A - kappa D (step 7) and N right-hand sides at once:
- *   setup   N_v near-null vectors v_k -> aggregates (blocks of block[0] x block[1] x block[2] x block[3] sites) x chirality
+ *   setup   N_v near-null vectors v_k (adaptive: v_k = M^{-1} eta_k, then `refine` passes v_k <- v_k - cycle(M v_k)) -> aggregates (blocks of block[0] x block[1] x block[2] x block[3] sites) x chirality
  *           (spin 0,1 | spin 2,3) -> prolongator P with orthonormal columns: column (a, chi, k) is v_k restricted to aggregate a and
  *           chirality chi, Gram-Schmidt over k = 0, 1, ... (each column against the earlier ones, twice, then normalised) ->
  *           Galerkin coarse operator A_c = P^dag M P, a 9-point stencil of dense (2 N_v) x (2 N_v) blocks
@@ -320,6 +320,8 @@ typedef struct lq_mg_param {
     int restart;          /* restart length of the outer flexible GCR, 1 .. 16 */
     double setup_tol;     /* lq_mg_setup: v_k = M^{-1} eta_k by lq_solve's mixed-precision CG to this relative residual (e.g. 1e-3) */
     uint64_t seed;        /* lq_mg_setup: seed of the Gaussian eta_k (the generator of lq_fill_spinor_random) */
+    int refine;           /* lq_mg_setup: adaptive refinement passes (>= 0): with the hierarchy just built, v_k <- v_k - cycle(M v_k) for all
+                             k at once (the cycle removes from v_k what the hierarchy already represents badly), then P and A_c are rebuilt */
 } lq_mg_param;
 typedef struct lq_mg_info {
     int coarse_dims[4];

@@ -59,7 +59,7 @@ class SolveInfo(ctypes.Structure):
 
 class MgParam(ctypes.Structure):
     _fields_ = [("block", ctypes.c_int * 4), ("n_vec", ctypes.c_int), ("nu_pre", ctypes.c_int), ("nu_post", ctypes.c_int), ("smoother", ctypes.c_int),
-                ("coarse_iters", ctypes.c_int), ("restart", ctypes.c_int), ("setup_tol", ctypes.c_double), ("seed", ctypes.c_uint64)]
+                ("coarse_iters", ctypes.c_int), ("restart", ctypes.c_int), ("setup_tol", ctypes.c_double), ("seed", ctypes.c_uint64), ("refine", ctypes.c_int)]
 
 
 class MgInfo(ctypes.Structure):
@@ -372,10 +372,10 @@ class Context:
 
     # ------------------------------------------------------------------ two-level multigrid (lq_mg_*)
     def mg_setup(self, block, n_vec: int, nu_pre: int = 2, nu_post: int = 2, coarse_iters: int = 8, restart: int = 8,
-                 setup_tol: float = 1e-3, seed: int = 1, vecs=None, smoother: int = 1) -> dict:
+                 setup_tol: float = 1e-3, seed: int = 1, vecs=None, smoother: int = 1, refine: int = 0) -> dict:
         """Builds the hierarchy: adaptively (vecs=None) or from n_vec given canonical complex128 near-null vectors."""
         self._enter()
-        prm = MgParam((ctypes.c_int * 4)(*block), n_vec, nu_pre, nu_post, smoother, coarse_iters, restart, setup_tol, seed)
+        prm = MgParam((ctypes.c_int * 4)(*block), n_vec, nu_pre, nu_post, smoother, coarse_iters, restart, setup_tol, seed, refine)
         info = MgInfo()
         if vecs is None:
             self._check(self.lib.lq_mg_setup(self.h, ctypes.byref(prm), ctypes.byref(info)))

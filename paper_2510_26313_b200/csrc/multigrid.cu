@@ -487,6 +487,7 @@ int mg_setup_vectors(lq_ctx* c, const lq_mg_param* p, const void* dev_canonical6
 int mg_setup_adaptive(lq_ctx* c, const lq_mg_param* p, lq_mg_info* info) {
     LQ_TRY(check_param(c, p));
     if (!(p->setup_tol > 0) || !(p->setup_tol < 1)) return set_err(c, LQ_EINVAL, "lq_mg_setup: setup_tol must lie in (0, 1)");
+    if (p->refine < 0 || p->refine > 16) return set_err(c, LQ_EINVAL, "lq_mg_setup: refine must lie in 0 .. 16");
     if (info) memset(info, 0, sizeof(*info));
     const int nv = p->n_vec;
     const size_t pb64 = parity_bytes(c->g, nv, LQ_FP64), pb32 = parity_bytes(c->g, nv, LQ_FP32);
@@ -509,6 +510,24 @@ int mg_setup_adaptive(lq_ctx* c, const lq_mg_param* p, lq_mg_info* info) {
     if (rc == 0) rc = spinor_convert(c, v32, LQ_FP32, v64, LQ_FP64, nv, nullptr, 0);
     if (rc == 0) rc = spinor_convert(c, (char*)v32 + pb32, LQ_FP32, (char*)v64 + pb64, LQ_FP64, nv, nullptr, 0);
     if (rc == 0) rc = setup_from_native(c, p, v32, info);
+    // adaptive refinement: with the hierarchy just built, v <- v - cycle(M v) for all vectors at once, then rebuild P and A_c
+    double t_p = info ? info->seconds_prolongator : 0.0, t_a = info ? info->seconds_coarse_op : 0.0;
+    int probes = info ? info->probes : 0;
+    for (int pass = 0; pass < p->refine && rc == 0; pass++) {
+        MgState* s = c->mg;
+        rc = work_ensure(c, s, nv, false);
+        float* r = nullptr; float* z = nullptr;
+        if (rc == 0) { r = (float*)dev_alloc(c, 2 * pb32); z = (float*)dev_alloc(c, 2 * pb32); if (!r || !z) rc = LQ_ENOMEM; }
+        if (rc == 0) rc = fine_M(c, s, nv, r, v32);
+        if (rc == 0) rc = vcycle(c, s, nv, z, r);
+        if (rc == 0) rc = fine_sub(c, nv, v32, v32, z, -1.f);
+        if (cudaStreamSynchronize(c->stream) != cudaSuccess && rc == 0) rc = set_err(c, LQ_ECUDA, "lq_mg_setup: refinement failed");
+        if (r) dev_free(c, r);
+        if (z) dev_free(c, z);
+        if (rc == 0) rc = setup_from_native(c, p, v32, info);
+        if (rc == 0 && info) { t_p += info->seconds_prolongator; t_a += info->seconds_coarse_op; probes += info->probes; }
+    }
+    if (rc == 0 && info) { info->seconds_prolongator = t_p; info->seconds_coarse_op = t_a; info->probes = probes; }
     if (cudaStreamSynchronize(c->stream) != cudaSuccess && rc == 0) rc = set_err(c, LQ_ECUDA, "lq_mg_setup failed");
     void* tofree[] = {eta, v64, v32};
     for (void* q : tofree) if (q) dev_free(c, q);

@@ -33,7 +33,7 @@ def test_struct_layouts_match_header(tmp_path):
                "lq_solve_info": (binding.SolveInfo, ["nrhs", "outer_cycles", "inner_iters", "iters", "true_rel_residual", "seconds", "dslash_applies",
                                                      "model_bytes", "model_flops"]),
                "lq_eig_param": (binding.EigParam, ["n_ev", "m", "cheb_degree", "max_restarts", "cheb_a", "cheb_b", "tol", "seed"]),
-               "lq_mg_param": (binding.MgParam, ["block", "n_vec", "nu_pre", "nu_post", "smoother", "coarse_iters", "restart", "setup_tol", "seed"]),
+               "lq_mg_param": (binding.MgParam, ["block", "n_vec", "nu_pre", "nu_post", "smoother", "coarse_iters", "restart", "setup_tol", "seed", "refine"]),
                "lq_mg_info": (binding.MgInfo, ["coarse_dims", "coarse_dof", "probes", "seconds_vectors", "seconds_prolongator", "seconds_coarse_op", "bytes"]),
                "lq_mg_solve_info": (binding.MgSolveInfo, ["iters", "outer_cycles", "true_rel_residual", "seconds", "m_applies"]),
                "lq_eig_info": (binding.EigInfo, ["restarts", "converged", "lap_applies", "max_ritz_residual", "max_true_residual", "seconds", "seconds_ritz", "seconds_ortho"])}

@@ -180,6 +180,31 @@ def test_adaptive_setup_and_batched_solve():
     ctx.close()
 
 
+def test_refinement_pass_improves_the_hierarchy_and_twelve_right_hand_sides():
+    """Smooth links with periodic boundaries near the critical kappa (the regime the method is for): one adaptive refinement pass
+    v <- v - cycle(M v) lowers the cycle count; 12 right-hand sides (three groups of four) against the library's CG."""
+    import torch
+    dims = (8, 8, 8, 16)
+    ctx = B.Context(dims)
+    ctx.fill_gauge_random(1001, 0.05, t_bc=1)
+    ctx.build_clover(0.1252, 1.0)
+    g = torch.Generator(device="cuda").manual_seed(5)
+    b = torch.view_as_complex(torch.randn((12, 16, 8, 8, 8, 4, 3, 2), generator=g, device="cuda", dtype=torch.float64))
+    xc, cinfo = ctx.solve(b, tol=1e-10, max_inner=20000, max_outer=100)
+    assert cinfo["converged"]
+    cycles = []
+    for refine in (0, 1):
+        info = ctx.mg_setup((4, 4, 4, 4), 8, nu_pre=2, nu_post=2, coarse_iters=8, restart=8, setup_tol=1e-3, seed=7, refine=refine)
+        assert info["probes"] == (1 + refine) * 16 * (1 + 2 + 2 + 2 + 4)
+        x, sinfo = ctx.mg_solve(b, tol=1e-8, max_iter=300)
+        assert sinfo["converged"], sinfo
+        assert (torch.linalg.vector_norm(x - xc) / torch.linalg.vector_norm(xc)).item() <= 1e-5      # cond(M) is large here
+        assert max(sinfo["true_rel_residual"]) <= 1e-8
+        cycles.append(sinfo["iters"])
+    assert cycles[1] < cycles[0], cycles
+    ctx.close()
+
+
 def test_state_and_argument_errors():
     dims = (4, 4, 4, 8)
     ctx = B.Context(dims)
@@ -191,6 +216,14 @@ def test_state_and_argument_errors():
         ctx.mg_setup((3, 2, 2, 2), 4)
     with pytest.raises(B.LqError):            # unsupported n_vec
         ctx.mg_setup((2, 2, 2, 2), 3)
+    with pytest.raises(B.LqError):            # refine out of range
+        ctx.mg_setup((2, 2, 2, 2), 4, refine=-1)
+    odd = B.Context((6, 6, 6, 4))             # V / 2 = 432 sites is not a multiple of 32: padded site blocks, no multigrid
+    odd.load_gauge(inputs.make_links((6, 6, 6, 4), 1000, EPS))
+    odd.build_clover(KAPPA, CSW)
+    with pytest.raises(B.LqError):
+        odd.mg_setup((2, 2, 2, 2), 4)
+    odd.close()
     b = inputs.gaussian_spinors(dims, 1, 5)
     with pytest.raises(B.LqError):            # no hierarchy
         ctx.mg_solve(b, tol=1e-8)

@@ -96,42 +96,50 @@ __device__ __forceinline__ void block_sum(double (&v)[NQ], double* sm /* [NQ * 3
 }
 
 // Gram-Schmidt over k = 0, 1, ... inside every (aggregate, chirality) block: column k against the earlier columns, twice, then
-// normalised (the order of oracle/multigrid.py).  One CTA per block; the columns stay in global memory (L1 / L2 resident).
+// normalised.  One CTA of 8 warps per block; the columns stay in global memory (L1 / L2 resident).  Each of the two passes is
+// classical Gram-Schmidt in two phases -- all inner products <col_j, col_k>, j < k, at once (warp w takes j = w, w + 8, ..., its lanes
+// stride the rows, fp64 sums), then one update col_k -= sum_j d_j col_j -- instead of 2 k dependent dot / update rounds; two
+// classical passes give the Q factor of the oracle's (modified, twice) order to rounding: the factor is unique.
 // status[0] is set when a column has (nearly) no component left: linearly dependent near-null vectors.
 __global__ void __launch_bounds__(256) orthonormalise_kernel(MgGeom m, float2* __restrict__ P, int* __restrict__ status) {
     __shared__ double sm[2 * 32];
+    __shared__ float2 dj[LQ_MAX_RHS];
     float2* Pb = P + (size_t)blockIdx.x * m.M * m.nv;
-    const int t = threadIdx.x, nt = blockDim.x;
+    const int t = threadIdx.x, nt = blockDim.x, lane = t & 31, w = t >> 5, nw = nt >> 5;
     for (int k = 0; k < m.nv; k++) {
         double n0[1] = {0.0};
         for (int r = t; r < m.M; r += nt) { const float2 b = Pb[(size_t)r * m.nv + k]; n0[0] += (double)b.x * b.x + (double)b.y * b.y; }
         block_sum<1>(n0, sm);
-        for (int pass = 0; pass < 2; pass++) {
-            for (int j = 0; j < k; j++) {
-                double d[2] = {0.0, 0.0};
-                for (int r = t; r < m.M; r += nt) {
+        for (int pass = 0; pass < 2 && k > 0; pass++) {
+            for (int j = w; j < k; j += nw) {
+                double dr = 0.0, di = 0.0;
+                for (int r = lane; r < m.M; r += 32) {
                     const float2 a = Pb[(size_t)r * m.nv + j], b = Pb[(size_t)r * m.nv + k];
-                    d[0] += (double)a.x * b.x + (double)a.y * b.y;
-                    d[1] += (double)a.x * b.y - (double)a.y * b.x;
+                    dr += (double)a.x * b.x + (double)a.y * b.y;
+                    di += (double)a.x * b.y - (double)a.y * b.x;
                 }
-                block_sum<2>(d, sm);
-                const float dr = (float)d[0], di = (float)d[1];
-                for (int r = t; r < m.M; r += nt) {
-                    const float2 a = Pb[(size_t)r * m.nv + j];
-                    float2 b = Pb[(size_t)r * m.nv + k];
-                    b.x -= dr * a.x - di * a.y;
-                    b.y -= dr * a.y + di * a.x;
-                    Pb[(size_t)r * m.nv + k] = b;
-                }
-                __syncthreads();
+#pragma unroll
+                for (int off = 16; off >= 1; off >>= 1) { dr += __shfl_xor_sync(0xffffffffu, dr, off); di += __shfl_xor_sync(0xffffffffu, di, off); }
+                if (lane == 0) dj[j] = make_float2((float)dr, (float)di);
             }
+            __syncthreads();
+            for (int r = t; r < m.M; r += nt) {
+                float2 b = Pb[(size_t)r * m.nv + k];
+                for (int j = 0; j < k; j++) {
+                    const float2 a = Pb[(size_t)r * m.nv + j], d = dj[j];
+                    b.x -= d.x * a.x - d.y * a.y;
+                    b.y -= d.x * a.y + d.y * a.x;
+                }
+                Pb[(size_t)r * m.nv + k] = b;
+            }
+            __syncthreads();
         }
         double n[1] = {0.0};
         for (int r = t; r < m.M; r += nt) { const float2 b = Pb[(size_t)r * m.nv + k]; n[0] += (double)b.x * b.x + (double)b.y * b.y; }
         block_sum<1>(n, sm);
         if (!(n[0] > 1e-8 * n0[0])) { if (t == 0) atomicExch(status, 1); n[0] = 1.0; }    // less than 1e-4 of the column is new
-        const float s = (float)(1.0 / sqrt(n[0]));
-        for (int r = t; r < m.M; r += nt) { float2 b = Pb[(size_t)r * m.nv + k]; b.x *= s; b.y *= s; Pb[(size_t)r * m.nv + k] = b; }
+        const float sc = (float)(1.0 / sqrt(n[0]));
+        for (int r = t; r < m.M; r += nt) { float2 b = Pb[(size_t)r * m.nv + k]; b.x *= sc; b.y *= sc; Pb[(size_t)r * m.nv + k] = b; }
         __syncthreads();
     }
 }

@@ -366,7 +366,8 @@ static int setup_from_native(lq_ctx* c, const lq_mg_param* p, const float* vecs3
     s->Ac = (float2*)dev_alloc(c, Abytes);
     s->d_s = (double*)dev_alloc(c, (size_t)8 * 3 * LQ_MAX_RHS * sizeof(double));
     if (!s->site_f || !s->nbr || !s->status || !s->P || !s->Ac || !s->d_s) return LQ_ENOMEM;
-    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    struct Events { cudaEvent_t e[3] = {nullptr, nullptr, nullptr}; ~Events() { for (cudaEvent_t x : e) if (x) cudaEventDestroy(x); } } evs;   // also on the error returns
+    cudaEvent_t (&ev)[3] = evs.e;
     for (auto& e : ev) LQ_CUDA(c, cudaEventCreate(&e));
     LQ_CUDA(c, cudaEventRecord(ev[0], c->stream));
     // tables
@@ -467,7 +468,6 @@ static int setup_from_native(lq_ctx* c, const lq_mg_param* p, const float* vecs3
         info->seconds_coarse_op = ms_between(ev[1], ev[2]) * 1e-3;
         info->bytes = Pbytes + Abytes + (size_t)m.Vc * (m.ns + 9) * sizeof(int);
     }
-    for (auto& e : ev) cudaEventDestroy(e);
     return 0;
 }
 

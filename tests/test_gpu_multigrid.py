@@ -205,6 +205,41 @@ def test_refinement_pass_improves_the_hierarchy_and_twelve_right_hand_sides():
     ctx.close()
 
 
+def test_hierarchy_properties_and_solve_at_bench_size():
+    """The shape bench.py times (16^3 x 32, 4^4 aggregates, 24 vectors, one refinement pass): the dense oracle hierarchy does not fit
+    there, so what holds at any size is checked instead -- P^dag P = 1, the Galerkin identity A_c y = P^dag M P y with M applied in
+    fp64 through lq_apply (itself compared with the oracle at this size in test_gpu_fullsize.py), and the solve by recomputing
+    b - M x with the ORACLE's operator."""
+    import torch
+    cfg = inputs.CONFIGS[1]
+    dims = cfg["dims"]
+    V = inputs.volume(dims)
+    U = inputs.make_links(dims, cfg["gauge_seed"], cfg["eps"])
+    ctx = B.Context(dims)
+    ctx.load_gauge(U)
+    ctx.build_clover(cfg["kappa"], cfg["csw"])
+    info = ctx.mg_setup((4, 4, 4, 4), 24, nu_pre=3, nu_post=3, coarse_iters=8, restart=8, setup_tol=1e-4, seed=7, refine=1)
+    assert info["coarse_dims"] == (4, 4, 4, 8) and info["coarse_dof"] == 512 * 48
+    rng = np.random.default_rng(11)
+    y = rng.standard_normal((4, 512, 2, 24)) + 1j * rng.standard_normal((4, 512, 2, 24))
+    Py = ctx.mg_prolong(y)
+    back = ctx.mg_restrict(Py)
+    assert np.abs(back - y).max() <= 2e-5 * np.abs(y).max()                                  # orthonormal columns
+    MPy = ctx.apply(B.LQ_OP_M, Py, B.LQ_FP64)
+    galerkin = ctx.mg_restrict(MPy)
+    Ay = ctx.mg_coarse_apply(y)
+    assert np.abs(Ay - galerkin).max() <= 5e-5 * np.abs(galerkin).max()                      # A_c = P^dag M P (fp32 probing vs fp64 M)
+    b = inputs.laph_sources(dims, 8, 2, 2001)
+    x, sinfo = ctx.mg_solve(b, tol=1e-8, max_iter=100)
+    assert sinfo["converged"] and sinfo["iters"] <= 25, sinfo
+    A = oracle.clover(dims, U, cfg["kappa"], cfg["csw"])
+    for k in (0, 5):
+        r = b[k].reshape(-1) - oracle.M(dims, U, A, cfg["kappa"], x[k].reshape(V, 12)).reshape(-1)
+        res = np.linalg.norm(r) / np.linalg.norm(b[k].reshape(-1))
+        assert res <= 1e-8 and abs(res - sinfo["true_rel_residual"][k]) <= 1e-10, (res, sinfo["true_rel_residual"][k])
+    ctx.close()
+
+
 def test_state_and_argument_errors():
     dims = (4, 4, 4, 8)
     ctx = B.Context(dims)

@@ -367,6 +367,21 @@ def time_projection(B, device, peak, shapes=((32, 8), (128, 32)), precs=("f64_fm
                 ref = got
             elif ref is not None:
                 e[name]["max_rel_diff_vs_f64"] = float((got - ref).abs().max() / ref.abs().max())
+        if "tcgen05_3xtf32" in precs:      # the same kernel fed with complex64 fields (lq_project_c64): half the compulsory bytes
+            v32, x32 = vc.to(torch.complex64), xc.to(torch.complex64)
+            for _ in range(3):
+                got = ctx.project_c64(v32, x32)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(iters):
+                ctx.project_c64(v32, x32)
+            torch.cuda.synchronize()
+            sec = (time.perf_counter() - t0) / iters
+            e["tcgen05_3xtf32_c64_fields"] = {"us": round(sec * 1e6, 1), "compulsory_gbs": round(nbytes / 2 / sec * 1e-9, 1), "frac_measured_hbm": round(nbytes / 2 / sec * 1e-9 / peak, 4),
+                                              "gflops": round(flops / sec * 1e-9, 1)}
+            if ref is not None:
+                e["tcgen05_3xtf32_c64_fields"]["max_rel_diff_vs_f64_of_unrounded_fields"] = float((got - ref).abs().max() / ref.abs().max())
+            del v32, x32
         out["shapes"].append(e)
         del vc, xc
     ctx.close()

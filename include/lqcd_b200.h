@@ -256,6 +256,12 @@ int lq_laph_eigensolve(lq_ctx* ctx, double* evals, void* evecs, int loc, const l
  * tensor-core completion barrier that timed out: the kernel never hangs). */
 int lq_project(lq_ctx* ctx, void* P, const void* evecs, int n_ev, const void* sols, int n_sol, int loc, int prec);
 
+/* The same projection for SINGLE-PRECISION fields: evecs and sols are complex float arrays (8 bytes per number, same index order, 16-byte
+ * aligned) at `loc` -- what an fp32 inner solve and an fp32 eigenvector store hold; P is complex double as above.  Always the tensor-core
+ * kernel (3xTF32, error <= 4e-7 of max |P| relative to the exact projection of the given fp32 fields).  Half the compulsory bytes of
+ * lq_project, and the smaller raw stages leave shared memory for a second operand buffer, so conversion and MMAs overlap. */
+int lq_project_c64(lq_ctx* ctx, void* P, const void* evecs, int n_ev, const void* sols, int n_sol, int loc);
+
 /* The fp64 projection for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that
  * forbid it): the same arithmetic, summed in the same order, as lq_project(..., LQ_DEVICE, LQ_FP64), but the partial sums of its
  * two-stage reduction sit in a static device array of LQ_NOALLOC_SCRATCH_BYTES that every GPU loading the library holds until the

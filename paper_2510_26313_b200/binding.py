@@ -30,7 +30,7 @@ EXPORTS = ["lq_create", "lq_destroy", "lq_last_error", "lq_set_allocator", "lq_l
            "lq_set_tuning", "lq_kernel_launches", "lq_gather_sites", "lq_native_index", "lq_fma_peak", "lq_mem_peak", "lq_set_half_links",
            "lq_laplacian", "lq_laplacian_native", "lq_cv_native_bytes", "lq_cv_fill_random", "lq_laph_eigensolve", "lq_project",
            "lq_mg_setup", "lq_mg_setup_from_vectors", "lq_mg_free", "lq_mg_restrict", "lq_mg_prolong", "lq_mg_coarse_apply", "lq_mg_vcycle",
-           "lq_mg_solve", "lq_project_noalloc"]
+           "lq_mg_solve", "lq_project_noalloc", "lq_project_c64"]
 
 
 class SolveParam(ctypes.Structure):
@@ -117,6 +117,7 @@ def load_library():
     lib.lq_cv_fill_random.argtypes = [vp, vp, ci, ci, u64]
     lib.lq_project.argtypes = [vp, vp, vp, ci, vp, ci, ci, ci]
     lib.lq_project_noalloc.argtypes = [vp, vp, vp, ci, vp, ci]
+    lib.lq_project_c64.argtypes = [vp, vp, vp, ci, vp, ci, ci]
     lib.lq_laph_eigensolve.argtypes = [vp, vp, vp, ci, ctypes.POINTER(EigParam), ctypes.POINTER(EigInfo)]
     lib.lq_kernel_launches.argtypes = [vp]; lib.lq_kernel_launches.restype = ctypes.c_longlong
     szp = ctypes.POINTER(ctypes.c_size_t)
@@ -325,6 +326,22 @@ class Context:
             out = self.torch.empty((Lt, 4, n_ev, n_sol), dtype=self.torch.complex128, device=evecs.device)
         pv, loc = _ptr(evecs); px, _ = _ptr(sols); po, _ = _ptr(out)
         self._check(self.lib.lq_project(self.h, po, pv, n_ev, px, n_sol, loc, prec))
+        return out
+
+    def project_c64(self, evecs, sols):
+        """lq_project_c64: the tensor-core projection of complex64 fields (numpy host arrays or torch device arrays, shapes as for
+        project); returns complex128 [Lt][4][n_ev][n_sol] of the same kind."""
+        self._enter()
+        Lt = self.dims[3]
+        n_ev, n_sol = evecs.shape[0], sols.shape[0]
+        if isinstance(evecs, np.ndarray):
+            evecs = np.ascontiguousarray(evecs, dtype=np.complex64); sols = np.ascontiguousarray(sols, dtype=np.complex64)
+            out = np.empty((Lt, 4, n_ev, n_sol), dtype=np.complex128)
+        else:
+            assert evecs.dtype == sols.dtype == self.torch.complex64
+            out = self.torch.empty((Lt, 4, n_ev, n_sol), dtype=self.torch.complex128, device=evecs.device)
+        pv, loc = _ptr(evecs); px, _ = _ptr(sols); po, _ = _ptr(out)
+        self._check(self.lib.lq_project_c64(self.h, po, pv, n_ev, px, n_sol, loc))
         return out
 
     def project_noalloc(self, evecs, sols, out):

@@ -360,6 +360,26 @@ int lq_project(lq_ctx* c, void* P, const void* evecs, int n_ev, const void* sols
     for (void* q : tofree) if (q) dev_free(c, q);
     return rc;
 }
+int lq_project_c64(lq_ctx* c, void* P, const void* evecs, int n_ev, const void* sols, int n_sol, int loc) {
+    if (!c) return LQ_EINVAL;
+    if (!P || !evecs || !sols || n_ev < 1 || n_ev > 1024 || n_sol < 1 || n_sol > 64) return set_err(c, LQ_EINVAL, "lq_project_c64: bad argument");
+    cudaSetDevice(c->device);
+    const size_t vb = (size_t)n_ev * c->g.V * 3 * 2 * sizeof(float), xb = (size_t)n_sol * c->g.V * 12 * 2 * sizeof(float);
+    const size_t pb = (size_t)c->g.L[3] * 4 * n_ev * n_sol * 2 * sizeof(double);
+    void *st_v = nullptr, *st_x = nullptr, *st_p = nullptr;
+    const void* d_v = stage_in(c, evecs, vb, loc, &st_v);
+    const void* d_x = d_v ? stage_in(c, sols, xb, loc, &st_x) : nullptr;
+    int rc = (!d_v || !d_x) ? LQ_ENOMEM : 0;
+    void* d_p = P;
+    if (rc == 0 && loc == LQ_HOST) { st_p = dev_alloc(c, pb); if (!st_p) rc = LQ_ENOMEM; d_p = st_p; }
+    if (rc == 0) rc = project_device_tc32(c, (double*)d_p, (const float*)d_v, n_ev, (const float*)d_x, n_sol);
+    if (rc == 0 && st_p) {
+        if (cudaMemcpyAsync(P, st_p, pb, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess || cudaStreamSynchronize(c->stream) != cudaSuccess) rc = set_err(c, LQ_ECUDA, "D2H copy failed");
+    }
+    void* tofree[] = {st_v, st_x, st_p};
+    for (void* q : tofree) if (q) dev_free(c, q);
+    return rc;
+}
 // the operator on native buffers
 static int apply_native(lq_ctx* c, int op, void* out, const void* in, const void* in2, int n, int prec) {
     const size_t pb = parity_bytes(c->g, n, prec);

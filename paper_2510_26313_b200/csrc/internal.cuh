@@ -89,6 +89,8 @@ int laph_eigensolve(lq_ctx* c, double* h_evals, double* dev_canon_evecs, const l
 int project_device(lq_ctx* c, double* dev_P, const double* dev_V, int n_ev, const double* dev_X, int n_sol);
 // project_tc.cu : the same contraction on tcgen05 tensor cores (3xTF32, fp32 TMEM accumulator, fp64 split-K sum)
 int project_device_tc(lq_ctx* c, double* dev_P, const double* dev_V, int n_ev, const double* dev_X, int n_sol);
+// project_tc32.cu : the tensor-core kernel for complex-float fields (two operand buffers: conversion overlaps the MMAs)
+int project_device_tc32(lq_ctx* c, double* dev_P, const float* dev_V, int n_ev, const float* dev_X, int n_sol);
 
 // multigrid.cu : two-level adaptive multigrid; canonical / coarse arrays below are DEVICE arrays
 void mg_release(lq_ctx* c);

@@ -101,3 +101,35 @@ def test_laph_chain_eigensolve_solve_project():
     xo = np.stack([oracle.solve_eo(dims, U, A, Ainv, kappa, b[k], 1e-12)[0].reshape(b[k].shape) for k in range(4)])
     Po = oracle.project(vec, xo)
     assert np.abs(P - Po).max() <= 1e-8 * np.abs(Po).max()
+
+
+@pytest.mark.parametrize("dims,n_ev,n_sol", [((4, 4, 4, 4), 5, 3), ((6, 4, 2, 6), 8, 4), ((8, 8, 8, 2), 13, 1), ((2, 2, 2, 2), 1, 2), ((6, 6, 10, 2), 150, 11)])
+def test_single_precision_fields_match_einsum(dims, n_ev, n_sol):
+    """lq_project_c64: complex64 fields in, the oracle's einsum on exactly those (rounded) fields as the reference; tiles, padding,
+    ragged K chunks and both kernel shapes (n_sol <= 8: N = 64 with 8-site stages; more: N = 256 with 4-site stages)."""
+    Lx, Ly, Lz, Lt = dims
+    rng = np.random.default_rng(15)
+    v = (rng.normal(size=(n_ev, Lt, Lz, Ly, Lx, 3)) + 1j * rng.normal(size=(n_ev, Lt, Lz, Ly, Lx, 3))).astype(np.complex64)
+    psi = inputs.gaussian_spinors(dims, n_sol, 83).astype(np.complex64)
+    want = oracle.project(v.astype(np.complex128), psi.astype(np.complex128))
+    ctx = B.Context(dims)
+    got = ctx.project_c64(v, psi)
+    again = ctx.project_c64(v, psi)
+    ctx.close()
+    assert np.abs(got - want).max() <= 3e-6 * np.abs(want).max()
+    assert np.array_equal(got, again)                     # fixed summation order
+
+
+def test_single_precision_projection_bench_size():
+    """16^3 x 32, 128 x 32, device arrays: every output against the fp64 FMA kernel run on the same (rounded) fields."""
+    import torch
+    dims, n_ev, n_sol = inputs.CONFIGS[1]["dims"], 128, 32
+    Lx, Ly, Lz, Lt = dims
+    g = torch.Generator(device="cuda").manual_seed(9)
+    v = torch.view_as_complex(torch.randn((n_ev, Lt, Lz, Ly, Lx, 3, 2), generator=g, device="cuda", dtype=torch.float32))
+    x = torch.view_as_complex(torch.randn((n_sol, Lt, Lz, Ly, Lx, 4, 3, 2), generator=g, device="cuda", dtype=torch.float32))
+    ctx = B.Context(dims)
+    p32 = ctx.project_c64(v, x)
+    p64 = ctx.project(v.to(torch.complex128), x.to(torch.complex128))
+    ctx.close()
+    assert ((p32 - p64).abs().max() / p64.abs().max()).item() <= 3e-6

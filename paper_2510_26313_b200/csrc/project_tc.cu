@@ -227,13 +227,16 @@ __global__ void __launch_bounds__(NT) project_tc_kernel(int Lt, int S3, int nchu
         asm volatile("tcgen05.fence::after_thread_sync;");
         if (tid == NT - 32) {
             const uint32_t d = tmem + (i & 1) * TN;
-#pragma unroll 1
+            // descriptors of k-step 0; k-step s starts 2 s chunks further: the 14-bit start-address field (bytes >> 4) grows by a constant
+            // (the operand tiles lie below 72 KB, the field holds 256 KB: no carry into the next field)
+            uint64_t ah = smem_desc(s32(sAh), TM * 16, 128), al = smem_desc(s32(sAl), TM * 16, 128);
+            uint64_t bh = smem_desc(s32(sBh), TN * 16, 128), bl = smem_desc(s32(sBl), TN * 16, 128);
+#pragma unroll
             for (int s = 0; s < KB / 8; s++) {
-                const uint64_t ah = smem_desc(s32(sAh) + (2 * s) * (TM * 16), TM * 16, 128), al = smem_desc(s32(sAl) + (2 * s) * (TM * 16), TM * 16, 128);
-                const uint64_t bh = smem_desc(s32(sBh) + (2 * s) * (TN * 16), TN * 16, 128), bl = smem_desc(s32(sBl) + (2 * s) * (TN * 16), TN * 16, 128);
                 mma_tf32(d, al, bh, idesc, s == 0 ? 0u : 1u);
                 mma_tf32(d, ah, bl, idesc, 1u);
                 mma_tf32(d, ah, bh, idesc, 1u);
+                ah += (2 * TM * 16) >> 4; al += (2 * TM * 16) >> 4; bh += (2 * TN * 16) >> 4; bl += (2 * TN * 16) >> 4;
             }
             asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(s32(bar)) : "memory");
         }

@@ -114,12 +114,18 @@ __device__ __forceinline__ void store_site_regs(typename S::store_t* __restrict_
 #pragma unroll
         for (int k = 0; k < RPT; k++) inv[k] = mx[k] > 0.f ? 32767.0f / mx[k] : 0.f;
         store_norm<RPT>(pn, mx);
+        // q = round-to-nearest-even(v * 32767 / max) without the conversion unit: ONE fused multiply-add onto 1.5 * 2^23 leaves the rounded
+        // integer, as two's complement, in the low 16 bits of the result (|q| <= 32767 << 2^22; rounded once, where rintf(v * inv)
+        // rounds twice); a byte permute packs two of them.  (FRND + F2I, the straightforward form, run on the 16-lane unit.)
 #pragma unroll
         for (int j = 0; j < 24; j++) {
-            T q[RPT];
+            unsigned b[RPT];
 #pragma unroll
-            for (int k = 0; k < RPT; k++) q[k] = rintf(v[j][k] * inv[k]);
-            store_comp<S, RPT>(p + j * PL, q);
+            for (int k = 0; k < RPT; k++) b[k] = __float_as_uint(fmaf(v[j][k], inv[k], 12582912.0f));
+            short* q = p + j * PL;
+            if constexpr (RPT == 4) *(uint2*)q = make_uint2(__byte_perm(b[0], b[1], 0x5410), __byte_perm(b[2], b[3], 0x5410));
+            else if constexpr (RPT == 2) *(unsigned*)q = __byte_perm(b[0], b[1], 0x5410);
+            else *q = (short)(b[0] & 0xFFFFu);
         }
     } else {
 #pragma unroll
